@@ -1,0 +1,202 @@
+"""Seeded synthetic inputs for the BSE hot path (arXiv 2504.10096).
+
+This module serves BOTH the CPU oracle's tests and the CUDA path's tests/bench.  It holds
+none of the method's arithmetic (no apply, no orthogonalisation, no eigensolver): only
+  * a counter-based random number generator (splitmix64 finaliser + Box-Muller), so that any
+    matrix entry is a pure function of (seed, stream, i, j) -- the CUDA library implements the
+    same generator in `bse_fill_synthetic` so that 77 GB operands never cross PCIe;
+  * the "BSE-shaped" generator of BASELINE.json `configs` (R = diag(d_eps + sigma) + K, C complex
+    symmetric) standing in for the paper's CrI3 / TD-DFT matrices (Table 2), which
+    are not available;
+  * closed-form instances with a prescribed spectrum (Householder similarity), whose entries
+    are O(1) each to evaluate, used to pin eigenvalues at any size.
+
+Recipe (DESIGN.md section "Inputs"):
+  d_eps_i ~ U[1,10], sorted ascending inside each group of `group` consecutive indices
+            (group = N_v*N_c; 16 for configs 0-3, 64 for config 4)
+  i > j : K_ij = 0.1 (g1 + i g2) / (1 + |i-j|/64),  K_ji = conj(K_ij);  K_ii = 0.1 g1 (real)
+  R = diag(d_eps + sigma) + K
+  i >= j: C_ij = C_ji = 0.05 (g1 + i g2) / (1 + |i-j|/64)      (diagonal complex)
+  X     : i.i.d. complex standard normal (g1 + i g2)
+with (g1, g2) = Box-Muller(u1, u2), u from the hash of (seed, stream, i, j).
+"""
+from __future__ import annotations
+
+import numpy as np
+
+STREAM_EPS = 1
+STREAM_K = 2
+STREAM_C = 3
+STREAM_X = 4
+STREAM_AUX = 5
+
+_M1 = np.uint64(0xBF58476D1CE4E5B9)
+_M2 = np.uint64(0x94D049BB133111EB)
+_GOLD = np.uint64(0x9E3779B97F4A7C15)
+_CI = np.uint64(0xD1B54A32D192ED03)
+_CJ = np.uint64(0x8CB92BA72F3D8DD7)
+
+
+def _mix64(z: np.ndarray) -> np.ndarray:
+    z = z.astype(np.uint64, copy=True)
+    z ^= z >> np.uint64(30)
+    z *= _M1
+    z ^= z >> np.uint64(27)
+    z *= _M2
+    z ^= z >> np.uint64(31)
+    return z
+
+
+def hash2(seed: int, stream: int, i, j):
+    """Two 64-bit hashes per counter (i, j).  All arithmetic is modulo 2^64."""
+    i = np.asarray(i, dtype=np.uint64)
+    j = np.asarray(j, dtype=np.uint64)
+    with np.errstate(over="ignore"):
+        h0 = _mix64(np.asarray([np.uint64(seed) ^ (np.uint64(stream) * _GOLD)], dtype=np.uint64))[0]
+        h1 = _mix64(h0 + i * _CI)
+        h2 = _mix64(h1 ^ (j * _CJ))
+        h3 = _mix64(h2 + _GOLD)
+    return h2, h3
+
+
+def _u01(h: np.ndarray) -> np.ndarray:
+    """Uniform in (0,1): ((h >> 12) + 0.5) * 2^-52  (exact in binary64)."""
+    return ((h >> np.uint64(12)).astype(np.float64) + 0.5) * (2.0 ** -52)
+
+
+def uniforms(seed: int, stream: int, i, j):
+    h2, h3 = hash2(seed, stream, i, j)
+    return _u01(h2), _u01(h3)
+
+
+def normals(seed: int, stream: int, i, j):
+    """(g1, g2) i.i.d. N(0,1) by Box-Muller on the two uniforms of counter (i, j)."""
+    u1, u2 = uniforms(seed, stream, i, j)
+    r = np.sqrt(-2.0 * np.log(u1))
+    th = 2.0 * np.pi * u2
+    return r * np.cos(th), r * np.sin(th)
+
+
+def transition_energies(N: int, seed: int, group: int = 16) -> np.ndarray:
+    """d_eps ~ U[1,10], sorted ascending inside each group of `group` consecutive indices."""
+    idx = np.arange(N, dtype=np.uint64)
+    u1, _ = uniforms(seed, STREAM_EPS, idx, np.zeros_like(idx))
+    d = 1.0 + 9.0 * u1
+    assert N % group == 0
+    return np.sort(d.reshape(N // group, group), axis=1).reshape(N)
+
+
+def _decay(i: np.ndarray, j: np.ndarray) -> np.ndarray:
+    return 1.0 + np.abs(i.astype(np.float64) - j.astype(np.float64)) / 64.0
+
+
+def rows_R(N: int, seed: int, rows, sigma: float = 0.0, group: int = 16) -> np.ndarray:
+    """Full (unpacked) rows of the Hermitian R, shape (len(rows), N), complex128."""
+    rows = np.asarray(rows, dtype=np.int64)
+    i = rows[:, None] + np.zeros((1, N), dtype=np.int64)
+    j = np.arange(N, dtype=np.int64)[None, :] + np.zeros((len(rows), 1), dtype=np.int64)
+    hi = np.maximum(i, j)
+    lo = np.minimum(i, j)
+    g1, g2 = normals(seed, STREAM_K, hi, lo)
+    val = 0.1 * (g1 + 1j * g2) / _decay(hi, lo)
+    val = np.where(i >= j, val, np.conj(val))
+    d = transition_energies(N, seed, group)
+    on = i == j
+    val = np.where(on, 0.1 * g1 + d[np.minimum(i, N - 1)] + sigma, val)
+    return val.astype(np.complex128)
+
+
+def rows_C(N: int, seed: int, rows) -> np.ndarray:
+    """Full rows of the complex symmetric C (C = C^T)."""
+    rows = np.asarray(rows, dtype=np.int64)
+    i = rows[:, None] + np.zeros((1, N), dtype=np.int64)
+    j = np.arange(N, dtype=np.int64)[None, :] + np.zeros((len(rows), 1), dtype=np.int64)
+    hi = np.maximum(i, j)
+    lo = np.minimum(i, j)
+    g1, g2 = normals(seed, STREAM_C, hi, lo)
+    return (0.05 * (g1 + 1j * g2) / _decay(hi, lo)).astype(np.complex128)
+
+
+def dense_R(N: int, seed: int, sigma: float = 0.0, group: int = 16, chunk: int = 1024) -> np.ndarray:
+    out = np.empty((N, N), dtype=np.complex128)
+    for r0 in range(0, N, chunk):
+        r1 = min(N, r0 + chunk)
+        out[r0:r1] = rows_R(N, seed, np.arange(r0, r1), sigma, group)
+    return out
+
+
+def dense_C(N: int, seed: int, chunk: int = 1024) -> np.ndarray:
+    out = np.empty((N, N), dtype=np.complex128)
+    for r0 in range(0, N, chunk):
+        r1 = min(N, r0 + chunk)
+        out[r0:r1] = rows_C(N, seed, np.arange(r0, r1))
+    return out
+
+
+def block_X(n_rows: int, k: int, seed: int) -> np.ndarray:
+    """n_rows x k block of i.i.d. complex standard normals (column-major friendly: F order)."""
+    i = np.arange(n_rows, dtype=np.uint64)[:, None] + np.zeros((1, k), dtype=np.uint64)
+    j = np.arange(k, dtype=np.uint64)[None, :] + np.zeros((n_rows, 1), dtype=np.uint64)
+    g1, g2 = normals(seed, STREAM_X, i, j)
+    return np.asfortranarray(g1 + 1j * g2)
+
+
+# ---------------------------------------------------------------------------------------------
+# Closed-form instances with a prescribed spectrum.  Entry (i, j) costs O(1); the device fills
+# them tile by tile (bse_fill_closed_form) and the expected eigenvalues are the inputs below.
+# ---------------------------------------------------------------------------------------------
+
+def householder_u(N: int, seed: int, complex_u: bool = True) -> np.ndarray:
+    """Unit vector u defining the Householder reflector Q = I - 2 u u^H."""
+    idx = np.arange(N, dtype=np.uint64)
+    g1, g2 = normals(seed, STREAM_AUX, idx, np.zeros_like(idx))
+    u = g1 + 1j * g2 if complex_u else g1.astype(np.complex128)
+    return u / np.linalg.norm(u)
+
+
+def prescribed_spectrum(N: int, seed: int, lo: float = 1.0, hi: float = 10.0) -> np.ndarray:
+    """Distinct, strictly increasing values in [lo, hi]: a jittered grid (gaps >= 0.25 (hi-lo)/N)."""
+    idx = np.arange(N, dtype=np.uint64)
+    u1, _ = uniforms(seed, STREAM_AUX, idx, np.ones_like(idx))
+    return lo + (hi - lo) * (np.arange(N) + 0.25 + 0.5 * u1) / N
+
+
+def closed_form_tda_dense(lam: np.ndarray, u: np.ndarray) -> np.ndarray:
+    """R = Q diag(lam) Q^H with Q = I - 2 u u^H, written entrywise:
+       R_ij = lam_i d_ij - 2 u_i conj(u_j) (lam_i + lam_j) + 4 u_i conj(u_j) s,  s = sum_l lam_l |u_l|^2."""
+    s = float(np.sum(lam * np.abs(u) ** 2))
+    R = -2.0 * np.outer(u, np.conj(u)) * (lam[:, None] + lam[None, :]) + 4.0 * s * np.outer(u, np.conj(u))
+    R[np.diag_indices_from(R)] = (lam - 4.0 * lam * np.abs(u) ** 2 + 4.0 * s * np.abs(u) ** 2)
+    return R
+
+
+def closed_form_full_dense(d1: np.ndarray, d2: np.ndarray, u_real: np.ndarray, phi: np.ndarray):
+    """Pair (R, C) with omega_i = sqrt(d1_i d2_i) exactly (closed-form pair):
+       M+ = Q D1 Q^T, M- = Q D2 Q^T (real Householder Q), R0 = (M+ + M-)/2, C0 = (M+ - M-)/2,
+       R = U R0 U^H, C = U C0 U^T with U = diag(exp(i phi))."""
+    ur = np.real(u_real).astype(np.float64)
+    Mp = np.real(closed_form_tda_dense(d1, ur.astype(np.complex128)))
+    Mm = np.real(closed_form_tda_dense(d2, ur.astype(np.complex128)))
+    R0 = 0.5 * (Mp + Mm)
+    C0 = 0.5 * (Mp - Mm)
+    e = np.exp(1j * phi)
+    R = (e[:, None] * R0) * np.conj(e)[None, :]
+    C = (e[:, None] * C0) * e[None, :]
+    return R, C
+
+
+def phases(N: int, seed: int) -> np.ndarray:
+    idx = np.arange(N, dtype=np.uint64)
+    u1, _ = uniforms(seed, STREAM_AUX, idx, np.full_like(idx, 2))
+    return 2.0 * np.pi * u1
+
+
+# BASELINE.json configs (sigma: SURVEY.md 8(d) -- the literal constants give an indefinite problem,
+# full mode uses the documented shift sigma = 1.0).
+CONFIGS = {
+    0: dict(mode="tda", N=1024, group=16, nev=10, k=4, sigma=0.0),
+    1: dict(mode="full", N=2048, group=16, nev=20, k=4, sigma=1.0),
+    2: dict(mode="tda", N=16384, group=16, nev=100, k=4, sigma=0.0),
+    3: dict(mode="full", N=32768, group=16, nev=100, k=4, sigma=1.0),
+    4: dict(mode="tda", N=98304, group=64, nev=500, k=8, sigma=0.0),
+}

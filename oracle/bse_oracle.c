@@ -1,0 +1,557 @@
+/*
+ * oracle/bse_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, obviously-correct CPU implementation of what the hot path of arXiv 2504.10096
+ * computes (structured BSE operator x block of vectors, basis orthogonalisation, Lanczos
+ * eigenpairs).  Written from PAPER.md only; shares no code with the CUDA library.  Only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may call it.
+ *
+ * Conventions: all matrices are DENSE, ROW-MAJOR, complex128 (C99 `double complex`);
+ * vector blocks X, Y are ROW-MAJOR n_rows x k.  Accumulation is in `long double` so that the
+ * oracle's own rounding (~N 2^-64) is negligible against the 1e-12 parity budget.
+ *
+ * Pins (tests/test_oracle_*.py): identity / diagonal / unit-impulse operators, numpy matmul of
+ * the unpacked operator, the paper's identity Q^H H Q = -i J M_r (Eq. 2-3), prescribed spectra
+ * Q diag(lambda) Q^H, +-omega pairing, omega^2 = eig((R-C)(R+C)) for real R, C,
+ * sum omega^2 = |R|_F^2 - |C|_F^2, residuals.  The paper prints no eigenvalue, residual or
+ * vector of its own: parity against the paper's own outputs is UNPINNED.
+ */
+#include <complex.h>
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#include <stdint.h>
+
+typedef double complex zc;
+typedef long double ld;
+
+/* ------------------------------------------------------------------------------------------
+ * Operator entries.  PAPER.md:18 (Eq. 1): H = [[R, C], [-C^dagger, -A]], R = R^dagger.
+ * optical case A = R^*, C = C^T.  PAPER.md:24: TDA sets C = 0 => R x = w x.
+ * Only the LOWER triangle (j <= i) of the stored R and C is read; the rest follows from
+ * R_ij = conj(R_ji) and C_ij = C_ji.  The diagonal of R is real (imaginary part ignored).
+ * ------------------------------------------------------------------------------------------ */
+static inline zc R_at(const zc *R, int64_t N, int64_t i, int64_t j)
+{
+    if (i == j) return creal(R[i * N + i]);
+    return (j < i) ? R[i * N + j] : conj(R[j * N + i]);
+}
+static inline zc C_at(const zc *C, int64_t N, int64_t i, int64_t j)
+{
+    return (j <= i) ? C[i * N + j] : C[j * N + i];
+}
+/* entry (i, j) of the full 2N x 2N operator of Eq. (1) with A = R^*, C^dagger = conj(C^T) */
+static inline zc H_at(const zc *R, const zc *C, int64_t N, int64_t i, int64_t j)
+{
+    if (i < N) {
+        return (j < N) ? R_at(R, N, i, j) : C_at(C, N, i, j - N);
+    } else {
+        int64_t ii = i - N;
+        if (j < N) return -conj(C_at(C, N, j, ii));          /* -(C^dagger)_{ii,j} = -conj(C_{j,ii}) */
+        return -conj(R_at(R, N, ii, j - N));                  /* -A = -R^*                            */
+    }
+}
+
+/* Y = R X, rows r0 <= i < r1 of Y only (TDA).  Triple loop. */
+void orc_apply_tda_rows(int64_t N, int64_t k, const zc *R, const zc *X, zc *Y, int64_t r0, int64_t r1)
+{
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t i = r0; i < r1; ++i) {
+        for (int64_t c = 0; c < k; ++c) {
+            ld ar = 0.0L, ai = 0.0L;
+            for (int64_t j = 0; j < N; ++j) {
+                zc h = R_at(R, N, i, j);
+                zc x = X[j * k + c];
+                ar += (ld)creal(h) * (ld)creal(x) - (ld)cimag(h) * (ld)cimag(x);
+                ai += (ld)creal(h) * (ld)cimag(x) + (ld)cimag(h) * (ld)creal(x);
+            }
+            Y[i * k + c] = (double)ar + I * (double)ai;
+        }
+    }
+}
+void orc_apply_tda(int64_t N, int64_t k, const zc *R, const zc *X, zc *Y)
+{
+    orc_apply_tda_rows(N, k, R, X, Y, 0, N);
+}
+
+/* [Y1;Y2] = H [X1;X2], X and Y are 2N x k (Eq. 1).  Rows r0 <= i < r1 only. */
+void orc_apply_full_rows(int64_t N, int64_t k, const zc *R, const zc *C, const zc *X, zc *Y,
+                         int64_t r0, int64_t r1)
+{
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t i = r0; i < r1; ++i) {
+        for (int64_t c = 0; c < k; ++c) {
+            ld ar = 0.0L, ai = 0.0L;
+            for (int64_t j = 0; j < 2 * N; ++j) {
+                zc h = H_at(R, C, N, i, j);
+                zc x = X[j * k + c];
+                ar += (ld)creal(h) * (ld)creal(x) - (ld)cimag(h) * (ld)cimag(x);
+                ai += (ld)creal(h) * (ld)cimag(x) + (ld)cimag(h) * (ld)creal(x);
+            }
+            Y[i * k + c] = (double)ar + I * (double)ai;
+        }
+    }
+}
+void orc_apply_full(int64_t N, int64_t k, const zc *R, const zc *C, const zc *X, zc *Y)
+{
+    orc_apply_full_rows(N, k, R, C, X, Y, 0, 2 * N);
+}
+
+/* Structured half-apply (reading S4, derived from Eq. 1): for u = [x; sign*conj(x)],
+ * the upper half of H u is  R x + sign * C conj(x).  sign=+1: P(x); sign=-1: M(x). */
+void orc_apply_half(int64_t N, int64_t k, int sign, const zc *R, const zc *C, const zc *X, zc *Y)
+{
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t i = 0; i < N; ++i) {
+        for (int64_t c = 0; c < k; ++c) {
+            ld ar = 0.0L, ai = 0.0L;
+            for (int64_t j = 0; j < N; ++j) {
+                zc r = R_at(R, N, i, j);
+                zc cc = C_at(C, N, i, j);
+                zc x = X[j * k + c];
+                zc xc = conj(x);
+                ar += (ld)creal(r) * (ld)creal(x) - (ld)cimag(r) * (ld)cimag(x);
+                ai += (ld)creal(r) * (ld)cimag(x) + (ld)cimag(r) * (ld)creal(x);
+                ar += sign * ((ld)creal(cc) * (ld)creal(xc) - (ld)cimag(cc) * (ld)cimag(xc));
+                ai += sign * ((ld)creal(cc) * (ld)cimag(xc) + (ld)cimag(cc) * (ld)creal(xc));
+            }
+            Y[i * k + c] = (double)ar + I * (double)ai;
+        }
+    }
+}
+
+/* Generic dense row panel times block: Y (nr x k) = Hrows (nr x n) X (n x k).  Used for sampled-row
+ * parity at sizes where the dense operator does not fit the host (rows come from bse_inputs). */
+void orc_rows_times_block(int64_t nr, int64_t n, int64_t k, const zc *Hrows, const zc *X, zc *Y)
+{
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t i = 0; i < nr; ++i) {
+        for (int64_t c = 0; c < k; ++c) {
+            ld ar = 0.0L, ai = 0.0L;
+            for (int64_t j = 0; j < n; ++j) {
+                zc h = Hrows[i * n + j];
+                zc x = X[j * k + c];
+                ar += (ld)creal(h) * (ld)creal(x) - (ld)cimag(h) * (ld)cimag(x);
+                ai += (ld)creal(h) * (ld)cimag(x) + (ld)cimag(h) * (ld)creal(x);
+            }
+            Y[i * k + c] = (double)ar + I * (double)ai;
+        }
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Cyclic Jacobi for a Hermitian n x n matrix (textbook; north_star asks for it at tiny sizes).
+ * A (row-major) is overwritten; w gets the eigenvalues ascending, V (row-major, columns are
+ * eigenvectors) the eigenvectors.  Returns the number of sweeps, or -1 if not converged.
+ * Rotation: a_pq = |a_pq| e^{i phi}; U = D J, D = diag(1, e^{-i phi}), J = [[c, s], [-s, c]],
+ * t = sgn(th)/(|th| + sqrt(th^2+1)), th = (a_qq - a_pp) / (2 |a_pq|);  A <- U^H A U.
+ * ------------------------------------------------------------------------------------------ */
+int orc_jacobi_herm(int64_t n, zc *A, double *w, zc *V)
+{
+    for (int64_t i = 0; i < n; ++i)
+        for (int64_t j = 0; j < n; ++j) V[i * n + j] = (i == j) ? 1.0 : 0.0;
+    double fro = 0.0;
+    for (int64_t i = 0; i < n * n; ++i) fro += creal(A[i]) * creal(A[i]) + cimag(A[i]) * cimag(A[i]);
+    fro = sqrt(fro);
+    int sweep;
+    int converged = 0;
+    for (sweep = 0; sweep < 100; ++sweep) {
+        double off = 0.0;
+        for (int64_t i = 0; i < n; ++i)
+            for (int64_t j = 0; j < n; ++j)
+                if (i != j) off += creal(A[i * n + j]) * creal(A[i * n + j]) + cimag(A[i * n + j]) * cimag(A[i * n + j]);
+        if (sqrt(off) <= 1e-15 * fro || fro == 0.0) { converged = 1; break; }
+        for (int64_t p = 0; p < n - 1; ++p) {
+            for (int64_t q = p + 1; q < n; ++q) {
+                zc apq = A[p * n + q];
+                double g = cabs(apq);
+                if (g == 0.0) continue;
+                double app = creal(A[p * n + p]), aqq = creal(A[q * n + q]);
+                if (g < 1e-300) continue;
+                double th = (aqq - app) / (2.0 * g);
+                double t = ((th >= 0.0) ? 1.0 : -1.0) / (fabs(th) + sqrt(th * th + 1.0));
+                double c = 1.0 / sqrt(t * t + 1.0), s = t * c;
+                zc e = conj(apq) / g;                       /* e^{-i phi} */
+                zc Upp = c, Upq = s, Uqp = -s * e, Uqq = c * e;
+                for (int64_t r = 0; r < n; ++r) {           /* A <- A U */
+                    zc arp = A[r * n + p], arq = A[r * n + q];
+                    A[r * n + p] = arp * Upp + arq * Uqp;
+                    A[r * n + q] = arp * Upq + arq * Uqq;
+                }
+                for (int64_t r = 0; r < n; ++r) {           /* A <- U^H A */
+                    zc apr = A[p * n + r], aqr = A[q * n + r];
+                    A[p * n + r] = conj(Upp) * apr + conj(Uqp) * aqr;
+                    A[q * n + r] = conj(Upq) * apr + conj(Uqq) * aqr;
+                }
+                A[p * n + q] = 0.0; A[q * n + p] = 0.0;
+                A[p * n + p] = creal(A[p * n + p]); A[q * n + q] = creal(A[q * n + q]);
+                for (int64_t r = 0; r < n; ++r) {           /* V <- V U */
+                    zc vrp = V[r * n + p], vrq = V[r * n + q];
+                    V[r * n + p] = vrp * Upp + vrq * Uqp;
+                    V[r * n + q] = vrp * Upq + vrq * Uqq;
+                }
+            }
+        }
+    }
+    /* sort ascending (selection sort, swapping eigenvector columns) */
+    for (int64_t i = 0; i < n; ++i) w[i] = creal(A[i * n + i]);
+    for (int64_t i = 0; i < n - 1; ++i) {
+        int64_t m = i;
+        for (int64_t j = i + 1; j < n; ++j) if (w[j] < w[m]) m = j;
+        if (m != i) {
+            double tw = w[i]; w[i] = w[m]; w[m] = tw;
+            for (int64_t r = 0; r < n; ++r) { zc tv = V[r * n + i]; V[r * n + i] = V[r * n + m]; V[r * n + m] = tv; }
+        }
+    }
+    return converged ? sweep : -1;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * The paper's direct route for the full problem, PAPER.md:40-53 (section 2.1, Eq. 2-4):
+ *   M_r = [[Re(R+C), Im(R-C)], [-Im(R+C), Re(R-C)]]          (Eq. 3)
+ *   M_r = L L^T (real Cholesky; fails iff M_r -- equivalently Omega -- is not positive definite)
+ *   W = L^T J L,  J = [[0, I], [-I, 0]]  (Eq. 2);  -iW Hermitian with the eigenvalues of H
+ *   eigenvector of H:  v = Q L^-T z,   Q = (1/sqrt 2) [[I, -iI], [I, iI]]  (Eq. 2, reading S1)
+ * Outputs: Mr (2N x 2N real, row-major; may be NULL), omega (2N ascending: -w ... +w),
+ * V (2N x 2N complex row-major, columns = right eigenvectors of H; may be NULL).
+ * Returns 0, or 1 if the Cholesky factorisation met a non-positive pivot, or 2 if Jacobi failed.
+ * ------------------------------------------------------------------------------------------ */
+void orc_build_Mr(int64_t N, const zc *R, const zc *C, double *Mr)
+{
+    int64_t n2 = 2 * N;
+    for (int64_t i = 0; i < N; ++i)
+        for (int64_t j = 0; j < N; ++j) {
+            zc r = R_at(R, N, i, j), c = C_at(C, N, i, j);
+            Mr[i * n2 + j] = creal(r + c);
+            Mr[i * n2 + (j + N)] = cimag(r - c);
+            Mr[(i + N) * n2 + j] = -cimag(r + c);
+            Mr[(i + N) * n2 + (j + N)] = creal(r - c);
+        }
+}
+
+int orc_cholesky_real(int64_t n, const double *A, double *L)
+{
+    memset(L, 0, sizeof(double) * n * n);
+    for (int64_t j = 0; j < n; ++j) {
+        ld d = A[j * n + j];
+        for (int64_t p = 0; p < j; ++p) d -= (ld)L[j * n + p] * (ld)L[j * n + p];
+        if (!(d > 0.0L)) return 1;
+        double ljj = sqrt((double)d);
+        L[j * n + j] = ljj;
+        for (int64_t i = j + 1; i < n; ++i) {
+            ld s = A[i * n + j];
+            for (int64_t p = 0; p < j; ++p) s -= (ld)L[i * n + p] * (ld)L[j * n + p];
+            L[i * n + j] = (double)(s / ljj);
+        }
+    }
+    return 0;
+}
+
+int orc_bse_direct(int64_t N, const zc *R, const zc *C, double *Mr_out, double *omega, zc *V)
+{
+    int64_t n2 = 2 * N;
+    double *Mr = (double *)malloc(sizeof(double) * n2 * n2);
+    double *L = (double *)malloc(sizeof(double) * n2 * n2);
+    double *JL = (double *)malloc(sizeof(double) * n2 * n2);
+    zc *Hm = (zc *)malloc(sizeof(zc) * n2 * n2);
+    zc *Z = (zc *)malloc(sizeof(zc) * n2 * n2);
+    int rc = 0;
+    orc_build_Mr(N, R, C, Mr);
+    if (Mr_out) memcpy(Mr_out, Mr, sizeof(double) * n2 * n2);
+    if (orc_cholesky_real(n2, Mr, L)) { rc = 1; goto done; }
+    /* JL = J L : rows 0..N-1 of JL are rows N..2N-1 of L; rows N..2N-1 are minus rows 0..N-1 */
+    for (int64_t i = 0; i < N; ++i)
+        for (int64_t j = 0; j < n2; ++j) {
+            JL[i * n2 + j] = L[(i + N) * n2 + j];
+            JL[(i + N) * n2 + j] = -L[i * n2 + j];
+        }
+    /* W = L^T (J L);  Hm = -i W */
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n2; ++i)
+        for (int64_t j = 0; j < n2; ++j) {
+            ld s = 0.0L;
+            for (int64_t p = 0; p < n2; ++p) s += (ld)L[p * n2 + i] * (ld)JL[p * n2 + j];
+            Hm[i * n2 + j] = -I * (double)s;
+        }
+    /* enforce exact Hermitian symmetry of -iW against rounding (W is skew by construction) */
+    for (int64_t i = 0; i < n2; ++i) {
+        Hm[i * n2 + i] = 0.0;
+        for (int64_t j = i + 1; j < n2; ++j) {
+            zc a = 0.5 * (Hm[i * n2 + j] + conj(Hm[j * n2 + i]));
+            Hm[i * n2 + j] = a; Hm[j * n2 + i] = conj(a);
+        }
+    }
+    if (orc_jacobi_herm(n2, Hm, omega, Z) < 0) { rc = 2; goto done; }
+    if (V) {
+        /* vbar = L^-T z (back substitution with the upper triangular L^T), then v = Q vbar */
+        double isq2 = 1.0 / sqrt(2.0);
+        zc *vb = (zc *)malloc(sizeof(zc) * n2);
+        for (int64_t c = 0; c < n2; ++c) {
+            for (int64_t i = n2 - 1; i >= 0; --i) {
+                zc s = Z[i * n2 + c];
+                for (int64_t p = i + 1; p < n2; ++p) s -= L[p * n2 + i] * vb[p];
+                vb[i] = s / L[i * n2 + i];
+            }
+            for (int64_t i = 0; i < N; ++i) {
+                V[i * n2 + c] = isq2 * (vb[i] - I * vb[i + N]);
+                V[(i + N) * n2 + c] = isq2 * (vb[i] + I * vb[i + N]);
+            }
+        }
+        free(vb);
+    }
+done:
+    free(Mr); free(L); free(JL); free(Hm); free(Z);
+    return rc;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Block classical Gram-Schmidt with one reorthogonalisation (new vectors "have to
+ * be orthogonalized against the previous ones"), followed by a column-by-column QR of the block.
+ * In:  V (N x m, orthonormal columns, row-major), W (N x k row-major).
+ * Out: Q (N x k), h (m x k), B (k x k upper triangular, positive real diagonal) with
+ *      W = V h + Q B,  V^H Q = 0,  Q^H Q = I.  Returns the numerical rank of the block.
+ * ------------------------------------------------------------------------------------------ */
+static zc dotc_col(int64_t N, const zc *A, int64_t lda, int64_t ca, const zc *B, int64_t ldb, int64_t cb)
+{
+    ld sr = 0.0L, si = 0.0L;
+    for (int64_t i = 0; i < N; ++i) {
+        zc a = A[i * lda + ca], b = B[i * ldb + cb];
+        sr += (ld)creal(a) * (ld)creal(b) + (ld)cimag(a) * (ld)cimag(b);
+        si += (ld)creal(a) * (ld)cimag(b) - (ld)cimag(a) * (ld)creal(b);
+    }
+    return (double)sr + I * (double)si;
+}
+
+int orc_block_cgs2(int64_t N, int64_t m, int64_t k, const zc *V, const zc *W, zc *Q, zc *h, zc *B)
+{
+    memcpy(Q, W, sizeof(zc) * N * k);
+    for (int64_t i = 0; i < m * k; ++i) h[i] = 0.0;
+    for (int64_t i = 0; i < k * k; ++i) B[i] = 0.0;
+    zc *c = (zc *)malloc(sizeof(zc) * (m > k ? m : k) * k);
+    for (int pass = 0; pass < 2; ++pass) {
+        for (int64_t a = 0; a < m; ++a)
+            for (int64_t b = 0; b < k; ++b) c[a * k + b] = dotc_col(N, V, m, a, Q, k, b);   /* c = V^H Q */
+        for (int64_t i = 0; i < N; ++i)
+            for (int64_t b = 0; b < k; ++b) {
+                zc s = 0.0;
+                for (int64_t a = 0; a < m; ++a) s += V[i * m + a] * c[a * k + b];
+                Q[i * k + b] -= s;
+            }
+        for (int64_t i = 0; i < m * k; ++i) h[i] += c[i];
+    }
+    int rank = 0;
+    double scale = 0.0;
+    for (int64_t b = 0; b < k; ++b) { double nb = sqrt(creal(dotc_col(N, W, k, b, W, k, b))); if (nb > scale) scale = nb; }
+    for (int64_t b = 0; b < k; ++b) {
+        for (int pass = 0; pass < 2; ++pass)
+            for (int64_t a = 0; a < b; ++a) {
+                zc r = dotc_col(N, Q, k, a, Q, k, b);
+                for (int64_t i = 0; i < N; ++i) Q[i * k + b] -= Q[i * k + a] * r;
+                B[a * k + b] += r;
+            }
+        double nb = sqrt(creal(dotc_col(N, Q, k, b, Q, k, b)));
+        B[b * k + b] = nb;
+        if (nb > 1e-14 * scale && nb > 0.0) {
+            ++rank;
+            for (int64_t i = 0; i < N; ++i) Q[i * k + b] /= nb;
+        } else {
+            B[b * k + b] = 0.0;
+            for (int64_t i = 0; i < N; ++i) Q[i * k + b] = 0.0;
+        }
+    }
+    free(c);
+    return rank;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Textbook Lanczos, TDA (Hermitian R), single vector, full reorthogonalisation (classical
+ * Gram-Schmidt twice) -- PAPER.md:65-71: vectors generated one by one, each orthogonalised
+ * against the previous ones and stored.  No restart (the basis fits at the sizes the oracle runs).
+ * The projected tridiagonal T is diagonalised by the Jacobi routine above every `check` steps.
+ * Converged when the nev lowest Ritz pairs have |beta_{m+1} s_{m,i}| <= tol * max|theta|.
+ * Out: w (nev ascending), Vec (N x nev row-major), res (nev), returns number of steps (<0: failed).
+ * ------------------------------------------------------------------------------------------ */
+static double nrm2(int64_t n, const zc *x)
+{
+    ld s = 0.0L;
+    for (int64_t i = 0; i < n; ++i) s += (ld)creal(x[i]) * (ld)creal(x[i]) + (ld)cimag(x[i]) * (ld)cimag(x[i]);
+    return sqrt((double)s);
+}
+
+int orc_lanczos_tda(int64_t N, const zc *R, int nev, double tol, int maxit, int check, const zc *v0,
+                    double *w, zc *Vec, double *res)
+{
+    if (maxit > N) maxit = (int)N;
+    zc *Vb = (zc *)malloc(sizeof(zc) * (size_t)N * (maxit + 1));      /* basis, vector j at Vb + j*N */
+    double *alpha = (double *)calloc(maxit + 1, sizeof(double));
+    double *beta = (double *)calloc(maxit + 2, sizeof(double));        /* beta[j] couples j-1 and j */
+    zc *wv = (zc *)malloc(sizeof(zc) * N);
+    zc *T = NULL, *S = NULL; double *th = NULL;
+    int m = 0, result = -1;
+    double n0 = nrm2(N, v0);
+    for (int64_t i = 0; i < N; ++i) Vb[i] = v0[i] / n0;
+    for (int j = 0; j < maxit; ++j) {
+        orc_apply_tda(N, 1, R, Vb + (size_t)j * N, wv);                  /* w = R v_j */
+        ld a = 0.0L;
+        for (int64_t i = 0; i < N; ++i) {
+            zc v = Vb[(size_t)j * N + i];
+            a += (ld)creal(v) * (ld)creal(wv[i]) + (ld)cimag(v) * (ld)cimag(wv[i]);
+        }
+        alpha[j] = (double)a;
+        for (int pass = 0; pass < 2; ++pass)                              /* full reorthogonalisation */
+            for (int p = 0; p <= j; ++p) {
+                const zc *vp = Vb + (size_t)p * N;
+                ld sr = 0.0L, si = 0.0L;
+                for (int64_t i = 0; i < N; ++i) {
+                    sr += (ld)creal(vp[i]) * (ld)creal(wv[i]) + (ld)cimag(vp[i]) * (ld)cimag(wv[i]);
+                    si += (ld)creal(vp[i]) * (ld)cimag(wv[i]) - (ld)cimag(vp[i]) * (ld)creal(wv[i]);
+                }
+                zc cf = (double)sr + I * (double)si;
+                for (int64_t i = 0; i < N; ++i) wv[i] -= cf * vp[i];
+            }
+        double b = nrm2(N, wv);
+        beta[j + 1] = b;
+        m = j + 1;
+        int last = (m == maxit) || (b <= 1e-300);
+        if (b > 1e-300) for (int64_t i = 0; i < N; ++i) Vb[(size_t)(j + 1) * N + i] = wv[i] / b;
+        if (m >= nev && (m % check == 0 || last)) {
+            T = (zc *)realloc(T, sizeof(zc) * m * m); S = (zc *)realloc(S, sizeof(zc) * m * m);
+            th = (double *)realloc(th, sizeof(double) * m);
+            for (int i = 0; i < m * m; ++i) T[i] = 0.0;
+            for (int i = 0; i < m; ++i) {
+                T[i * m + i] = alpha[i];
+                if (i + 1 < m) { T[i * m + i + 1] = beta[i + 1]; T[(i + 1) * m + i] = beta[i + 1]; }
+            }
+            if (orc_jacobi_herm(m, T, th, S) < 0) break;
+            double hn = fmax(fabs(th[0]), fabs(th[m - 1]));
+            int ok = 1;
+            for (int i = 0; i < nev; ++i) {
+                res[i] = fabs(b) * cabs(S[(m - 1) * m + i]);
+                if (res[i] > tol * hn) ok = 0;
+            }
+            if (ok || last) {
+                for (int i = 0; i < nev; ++i) {
+                    w[i] = th[i];
+                    for (int64_t r = 0; r < N; ++r) {
+                        zc s = 0.0;
+                        for (int p = 0; p < m; ++p) s += Vb[(size_t)p * N + r] * S[p * m + i];
+                        Vec[r * nev + i] = s;
+                    }
+                }
+                result = ok ? m : -m;
+                break;
+            }
+        }
+        if (last) break;
+    }
+    free(Vb); free(alpha); free(beta); free(wv); free(T); free(S); free(th);
+    return result;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Textbook structure-preserving Lanczos, full mode -- DESIGN.md reading S4 of PAPER.md:65-69
+ * (basis with block structure from the start vector, lower blocks implicit, works on H^2, last
+ * step recovers +omega and eigenvectors).  With P(x) = R x + C conj(x), M(y) = R y - C conj(y):
+ *   x_1 random, p_1 = P(x_1), both scaled by 1/sqrt(Re(x_1^H p_1));
+ *   w = M(p_j); alpha_j = Re(p_j^H w); w -= X c, c = Re(PX^H w) (real, twice);
+ *   pw = P(w); beta_{j+1} = sqrt(Re(w^H pw)) (<= 0: Omega not positive definite, return -1000000);
+ *   x_{j+1} = w / beta, p_{j+1} = pw / beta.   T = tridiag(beta, alpha, beta) real symmetric,
+ *   theta_i, s_i its eigenpairs; omega_i = sqrt(theta_i); x = X s_i, y = (PX s_i)/omega_i;
+ *   v_i = [x + y; conj(x - y)] sqrt(omega_i)/2   (then v^H Sigma v = 1).
+ * Residual estimate |H v - omega v| = sqrt(2) beta_{m+1} |s_{m,i}| |x_{m+1}|_2 / omega * (sqrt(omega)/2).
+ * Out: omega (nev ascending), Vec (2N x nev row-major), res (nev).  Returns steps (<0: failed).
+ * ------------------------------------------------------------------------------------------ */
+int orc_lanczos_full(int64_t N, const zc *R, const zc *C, int nev, double tol, int maxit, int check,
+                     const zc *x0, double *omega, zc *Vec, double *res)
+{
+    if (maxit > 2 * N) maxit = (int)(2 * N);
+    zc *Xb = (zc *)malloc(sizeof(zc) * (size_t)N * (maxit + 1));
+    zc *Pb = (zc *)malloc(sizeof(zc) * (size_t)N * (maxit + 1));
+    double *alpha = (double *)calloc(maxit + 1, sizeof(double));
+    double *beta = (double *)calloc(maxit + 2, sizeof(double));
+    zc *wv = (zc *)malloc(sizeof(zc) * N), *pw = (zc *)malloc(sizeof(zc) * N);
+    zc *T = NULL, *S = NULL; double *th = NULL;
+    int m = 0, result = -1;
+    memcpy(Xb, x0, sizeof(zc) * N);
+    orc_apply_half(N, 1, +1, R, C, Xb, Pb);
+    {
+        ld s = 0.0L;
+        for (int64_t i = 0; i < N; ++i) s += (ld)creal(Xb[i]) * (ld)creal(Pb[i]) + (ld)cimag(Xb[i]) * (ld)cimag(Pb[i]);
+        if (!(s > 0.0L)) { result = -1000000; goto done; }
+        double sc = 1.0 / sqrt((double)s);
+        for (int64_t i = 0; i < N; ++i) { Xb[i] *= sc; Pb[i] *= sc; }
+    }
+    for (int j = 0; j < maxit; ++j) {
+        const zc *pj = Pb + (size_t)j * N;
+        orc_apply_half(N, 1, -1, R, C, pj, wv);                            /* w = M(p_j) */
+        ld a = 0.0L;
+        for (int64_t i = 0; i < N; ++i) a += (ld)creal(pj[i]) * (ld)creal(wv[i]) + (ld)cimag(pj[i]) * (ld)cimag(wv[i]);
+        alpha[j] = (double)a;
+        for (int pass = 0; pass < 2; ++pass)
+            for (int p = 0; p <= j; ++p) {
+                const zc *pp = Pb + (size_t)p * N; const zc *xp = Xb + (size_t)p * N;
+                ld s = 0.0L;
+                for (int64_t i = 0; i < N; ++i) s += (ld)creal(pp[i]) * (ld)creal(wv[i]) + (ld)cimag(pp[i]) * (ld)cimag(wv[i]);
+                double cf = (double)s;                                       /* real coefficient */
+                for (int64_t i = 0; i < N; ++i) wv[i] -= cf * xp[i];
+            }
+        orc_apply_half(N, 1, +1, R, C, wv, pw);                             /* pw = P(w) */
+        ld b2 = 0.0L;
+        for (int64_t i = 0; i < N; ++i) b2 += (ld)creal(wv[i]) * (ld)creal(pw[i]) + (ld)cimag(wv[i]) * (ld)cimag(pw[i]);
+        m = j + 1;
+        double xn1 = 0.0;
+        double b = 0.0;
+        int breakdown = 0;
+        if (b2 > 0.0L) {
+            b = sqrt((double)b2);
+            for (int64_t i = 0; i < N; ++i) { Xb[(size_t)(j + 1) * N + i] = wv[i] / b; Pb[(size_t)(j + 1) * N + i] = pw[i] / b; }
+            xn1 = nrm2(N, Xb + (size_t)(j + 1) * N);
+        } else if (nrm2(N, wv) > 1e-10) {
+            result = -1000000; break;                                         /* not positive definite */
+        } else breakdown = 1;
+        beta[j + 1] = b;
+        int last = (m == maxit) || breakdown;
+        if (m >= nev && (m % check == 0 || last)) {
+            T = (zc *)realloc(T, sizeof(zc) * m * m); S = (zc *)realloc(S, sizeof(zc) * m * m);
+            th = (double *)realloc(th, sizeof(double) * m);
+            for (int i = 0; i < m * m; ++i) T[i] = 0.0;
+            for (int i = 0; i < m; ++i) {
+                T[i * m + i] = alpha[i];
+                if (i + 1 < m) { T[i * m + i + 1] = beta[i + 1]; T[(i + 1) * m + i] = beta[i + 1]; }
+            }
+            if (orc_jacobi_herm(m, T, th, S) < 0) break;
+            if (!(th[0] > 0.0)) { result = -1000000; break; }
+            double hn = sqrt(fabs(th[m - 1]));
+            int ok = 1;
+            for (int i = 0; i < nev; ++i) {
+                double om = sqrt(th[i]);
+                res[i] = sqrt(2.0) * b * cabs(S[(m - 1) * m + i]) * xn1 / om * (sqrt(om) / 2.0);
+                if (res[i] > tol * hn) ok = 0;
+            }
+            if (ok || last) {
+                for (int i = 0; i < nev; ++i) {
+                    double om = sqrt(th[i]);
+                    omega[i] = om;
+                    double sc = sqrt(om) / 2.0;
+                    for (int64_t r = 0; r < N; ++r) {
+                        zc x = 0.0, y = 0.0;
+                        for (int p = 0; p < m; ++p) {
+                            double s = creal(S[p * m + i]);
+                            x += Xb[(size_t)p * N + r] * s;
+                            y += Pb[(size_t)p * N + r] * s;
+                        }
+                        y /= om;
+                        Vec[r * nev + i] = sc * (x + y);
+                        Vec[(r + N) * nev + i] = sc * conj(x - y);
+                    }
+                }
+                result = ok ? m : -m;
+                break;
+            }
+        }
+        if (last) break;
+    }
+done:
+    free(Xb); free(Pb); free(alpha); free(beta); free(wv); free(pw); free(T); free(S); free(th);
+    return result;
+}
