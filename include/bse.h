@@ -1,0 +1,174 @@
+/*
+ * bse.h -- C ABI of the B200-native BSE hot path (arXiv 2504.10096, iterative solution).
+ *
+ * What the library computes (citations are PAPER.md line + equation/section):
+ *   * the structured operator of Eq. (1) in the optical case A = R^*, C = C^T
+ *      applied to a block of k vectors -- "the most expensive step ... are the
+ *     matrix-vector products";  TDA: C = 0, Y = R X with R Hermitian;
+ *   * block classical Gram-Schmidt with reorthogonalisation of new vectors against the stored
+ *     Krylov basis;
+ *   * thick-restart Lanczos: Hermitian for TDA, structure-preserving (works on H^2 with the lower
+ *     blocks of matrix and basis implicit, final step recovers +omega and eigenvectors) for the
+ *     full case.
+ *
+ * Conventions
+ *   - every pointer named d* is a DEVICE pointer in the caller's current CUDA context, every pointer
+ *     named h* is a HOST pointer; complex128 = interleaved (re, im) doubles, 16-byte aligned;
+ *   - dense matrices and vector blocks are COLUMN-MAJOR with an explicit leading dimension
+ *     (in complex elements);  sizes are int64_t / int32_t;
+ *   - all device work is enqueued on the `stream` given to bse_create (a cudaStream_t passed as
+ *     void*; NULL = the legacy default stream).  bse_apply / bse_apply_half / bse_orth are
+ *     asynchronous with respect to the host; bse_solve and the *_host calls are synchronous;
+ *   - no call throws or exits; every call returns a bse_status_t;
+ *   - there is no CPU fallback: without a CUDA device every compute call returns BSE_ERR_CUDA.
+ *
+ * Packed triangular tile storage (north_star: "R lower triangle ... stored as packed triangular
+ * tiles").  With TB = 64 and nt = ceil(N / 64), a matrix is nt (nt + 1) / 2 tiles of 64 x 64
+ * complex128 (65536 bytes each, contiguous); tile (I, J), J <= I, is tile number I (I + 1) / 2 + J.
+ * Rows/columns >= N of the last tile row are zero.  Diagonal tiles are stored in full, the strictly
+ * upper part holding the Hermitian (R) or symmetric (C) mirror image; the diagonal of R is real.
+ * Inside a tile the 64 x 64 entries are ordered in 8 x 8 patches, patch (ib, jb) at byte
+ * (jb * 8 + ib) * 1024, entry (a, b) of a patch at slot
+ *     ((a>>2)<<2 | (b>>2)<<1 | (a>>1 & 1)) * 8 + ((a&1)<<2 | (b&1)<<1 | ((a>>1 ^ b>>1) & 1))
+ * of 16 bytes -- the order in which the FP64 tensor-core fragments of the apply kernel read it
+ * from shared memory without bank conflicts, both as T and as T^H.  The layout is opaque to
+ * callers: fill it with bse_pack_from_dense / bse_fill_synthetic / bse_fill_closed_form_*.
+ */
+#ifndef BSE_B200_H
+#define BSE_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bse_handle_s *bse_handle_t;
+
+typedef enum {
+    BSE_OK = 0,
+    BSE_ERR_INVALID_ARG = 1,
+    BSE_ERR_CUDA = 2,               /* a CUDA runtime call failed (or no device)                  */
+    BSE_ERR_ALLOC = 3,
+    BSE_ERR_NOT_CONVERGED = 4,      /* bse_solve: outputs hold the best estimates, see info.nconv */
+    BSE_ERR_NOT_POSITIVE_DEFINITE = 5, /* full mode: Re(w^H P(w)) <= 0 met (PAPER.md:49 precondition) */
+    BSE_ERR_INTERNAL = 6
+} bse_status_t;
+
+enum { BSE_MODE_TDA = 0, BSE_MODE_FULL = 1 };
+enum { BSE_MATRIX_R = 0, BSE_MATRIX_C = 1 };
+
+typedef struct {
+    int32_t n_apply;        /* operator applications (block applies; a full-mode step counts 2 half applies) */
+    int32_t n_restart;      /* thick restarts performed                                                   */
+    int32_t nconv;          /* wanted Ritz pairs that met the tolerance                                    */
+    int32_t ncv;            /* basis size used                                                              */
+    double  seconds_apply, seconds_orth, seconds_project, seconds_restart, seconds_total;
+    double  norm_est;       /* estimate of ||H|| (largest |Ritz value| seen; sqrt of it in full mode)      */
+} bse_info_t;
+
+const char *bse_status_string(bse_status_t s);
+
+/* Tile geometry for an N x N matrix: *tile = 64, *n_tiles = nt (nt+1)/2, *bytes = n_tiles * 65536.
+ * N < 1 -> BSE_ERR_INVALID_ARG.  Output pointers may be NULL. */
+bse_status_t bse_layout(int64_t N, int32_t *tile, int64_t *n_tiles, int64_t *bytes_per_matrix);
+
+/* dTiles <- lower triangle of the dense column-major N x N matrix dDense (leading dimension ld);
+ * which = BSE_MATRIX_R (Hermitian: mirror is the conjugate, diagonal imaginary part dropped) or
+ * BSE_MATRIX_C (symmetric: mirror is a copy).  Only entries (i, j) with j <= i are read. */
+bse_status_t bse_pack_from_dense(const void *dDense, int64_t ld, int64_t N, int32_t which,
+                                 void *dTiles, void *stream);
+
+/* dDense (column-major, ld) <- the full N x N matrix the tiles represent (both triangles). Test helper. */
+bse_status_t bse_unpack_to_dense(const void *dTiles, int64_t N, int32_t which,
+                                 void *dDense, int64_t ld, void *stream);
+
+/* The synthetic "BSE-shaped" generator of BASELINE.json, evaluated on the device
+ * with the same counter-based generator as bse_inputs/ (matches it to a few ulp):
+ *   R = diag(d_eps + sigma) + K,  K_ij = 0.1 (g1 + i g2) / (1 + |i-j|/64), d_eps ~ U[1,10] sorted in
+ *   groups of `group` indices;  C_ij = C_ji = 0.05 (g1 + i g2) / (1 + |i-j|/64).
+ * N % group != 0 -> BSE_ERR_INVALID_ARG (which = R only). */
+bse_status_t bse_fill_synthetic(void *dTiles, int64_t N, int32_t which, uint64_t seed, double sigma,
+                                int32_t group, void *stream);
+
+/* Closed-form instance with a prescribed spectrum: R = Q diag(lam) Q^H, Q = I - 2 u u^H,
+ *   R_ij = lam_i d_ij - 2 u_i conj(u_j) (lam_i + lam_j - 2 s),  s = sum_l lam_l |u_l|^2.
+ * dLam: N doubles (device), dU: N complex128 (device, unit 2-norm).  which=BSE_MATRIX_R only. */
+bse_status_t bse_fill_closed_form_tda(void *dTiles, int64_t N, const double *dLam, const void *dU,
+                                      double s, void *stream);
+
+/* Closed-form pair with omega_i = sqrt(d1_i d2_i): M+- = Q diag(d1|d2) Q^T (real Householder, dUr real
+ * unit vector), R = U (M+ + M-)/2 U^H, C = U (M+ - M-)/2 U^T, U = diag(exp(i phi)).
+ * All inputs are device arrays of N doubles; s1 = sum d1 u^2, s2 = sum d2 u^2. */
+bse_status_t bse_fill_closed_form_full(void *dRTiles, void *dCTiles, int64_t N, const double *dD1,
+                                       const double *dD2, const double *dUr, const double *dPhi,
+                                       double s1, double s2, void *stream);
+
+/* Creates a handle.  BORROWS dRTiles (and dCTiles in full mode): the caller keeps them alive and
+ * unmodified until bse_destroy.  mode = BSE_MODE_TDA (dCTiles ignored, may be NULL) or BSE_MODE_FULL
+ * (dCTiles required).  Does not verify Hermitian / symmetric / positive-definite structure.
+ * Workspace O(N k) is allocated lazily by later calls with cudaMalloc. */
+bse_status_t bse_create(bse_handle_t *h, int32_t mode, int64_t N, const void *dRTiles,
+                        const void *dCTiles, void *stream);
+bse_status_t bse_destroy(bse_handle_t h);
+
+/* Y = H X for a block of k >= 1 vectors.
+ *   TDA : X, Y are N x k;   Y = R X.
+ *   FULL: X, Y are 2N x k, rows [X1; X2];  Y1 = R X1 + C X2,  Y2 = -(C^H X1 + R^* X2).
+ * X and Y must not alias.  Asynchronous on the handle's stream.  Each stored tile of R (and C) is
+ * read from HBM once per group of 4 columns (TDA) / 2 columns (FULL). */
+bse_status_t bse_apply(bse_handle_t h, const void *dX, int64_t ldx, void *dY, int64_t ldy, int32_t k);
+
+/* FULL mode only, N-row half vectors:  Y = R X + sign * C conj(X),  sign = +1 (P) or -1 (M).
+ * This is the upper half of H [x; sign*conj(x)] -- "working implicitly with the lower blocks of the
+ * matrix and vector basis".  The structured solver uses only this call. */
+bse_status_t bse_apply_half(bse_handle_t h, int32_t sign, const void *dX, int64_t ldx, void *dY,
+                            int64_t ldy, int32_t k);
+
+/* Same as bse_apply with HOST buffers (pageable or pinned): copies X to the device, applies, copies
+ * Y back and synchronises the stream.  The end-to-end entry point measured by bench.py's "e2e". */
+bse_status_t bse_apply_host(bse_handle_t h, const void *hX, int64_t ldx, void *hY, int64_t ldy, int32_t k);
+
+/* Block classical Gram-Schmidt with one reorthogonalisation, then orthonormalises
+ * the block in place:   W_in = V hcoef + W_out Bfac,   <V, W_out> = 0,  <W_out, W_out> = I.
+ *   dV   : n x m basis (m >= 0), orthonormal in the inner product below; ldv
+ *   dBV  : NULL -> Euclidean complex inner product <x, y> = x^H y (TDA);
+ *          else the n x m block P(V) and the REAL inner product <x, y> = Re(x^H P(y)) with real
+ *          coefficients (full mode, reading S4); then dBW (n x k, = P(W) on entry) is
+ *          required and is updated consistently (dBW_out = P(W_out));
+ *   dW   : n x k block, overwritten with the orthonormalised block;
+ *   dHcoef: m x k (ld = m) device output, complex128 (imaginary parts 0 in the real case), nullable;
+ *   dBfac : k x k (ld = k) device output, upper triangular, positive real diagonal, nullable;
+ *   hRank : host int, numerical rank of the block; columns found dependent (diagonal of Bfac below
+ *           1e-13 * the largest column norm of W_in) are replaced by orthonormalised pseudo-random
+ *           vectors and their Bfac row/column entries set to 0.  Reading it synchronises the stream.
+ * n is N for both modes (half vectors in full mode). Returns BSE_ERR_NOT_POSITIVE_DEFINITE if a
+ * P-norm is not positive. */
+bse_status_t bse_orth(bse_handle_t h, const void *dV, int64_t ldv, int32_t m, const void *dBV,
+                      int64_t ldbv, void *dW, int64_t ldw, int32_t k, void *dBW, int64_t ldbw,
+                      void *dHcoef, void *dBfac, int32_t *hRank);
+
+/* Thick-restart block Lanczos.
+ *   TDA : the nev algebraically smallest eigenvalues of R, ascending, and orthonormal eigenvectors
+ *         (N x nev, column-major, ldvec) in dVec.
+ *   FULL: the nev smallest positive omega of H, ascending, and right eigenvectors [X_I; Y_I]
+ *         (2N x nev) normalised X^H X - Y^H Y = 1.  The -omega partner is [conj(Y); conj(X)].
+ *   k    : block size (>= 1; >= 2 recommended in full mode);  ncv: maximum basis
+ *          size, 0 -> default max(2 nev, nev + 15) (doubled in full mode), rounded up to a multiple of k;
+ *   tol  : a Ritz pair is converged when ||H v - w v||_2 <= tol * ||H||_est * ||v||_2;
+ *   hOmega: nev doubles (host);  hResid: nev doubles (host, nullable): the residual estimates;
+ *   info : nullable.
+ * Synchronous.  Errors: BSE_ERR_NOT_CONVERGED after max_restarts, BSE_ERR_NOT_POSITIVE_DEFINITE,
+ * BSE_ERR_INVALID_ARG (nev < 1, nev + k > N, ...), BSE_ERR_ALLOC, BSE_ERR_CUDA. */
+bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_t ncv, double tol,
+                       int32_t max_restarts, uint64_t seed, double *hOmega, void *dVec, int64_t ldvec,
+                       double *hResid, bse_info_t *info);
+
+/* Number of kernels this library has launched on the calling process's device since load (bench.py's
+ * "gpu_launches" claim). */
+int64_t bse_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BSE_B200_H */

@@ -1,0 +1,240 @@
+"""Thin Python binding of libbse_b200.so (include/bse.h).  Argument marshalling only: every step of the
+path runs in the library's CUDA kernels.  torch is used for device memory and streams, nothing else.
+
+The binding fails loudly if the CUDA library is missing or a call returns an error; there is no CPU
+fallback and this package never imports `oracle`.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBPATH = os.path.join(_HERE, "libbse_b200.so")
+_lib = None
+
+MODE_TDA, MODE_FULL = 0, 1
+MATRIX_R, MATRIX_C = 0, 1
+TILE = 64
+TILE_BYTES = 65536
+
+STATUS = {0: "BSE_OK", 1: "BSE_ERR_INVALID_ARG", 2: "BSE_ERR_CUDA", 3: "BSE_ERR_ALLOC", 4: "BSE_ERR_NOT_CONVERGED",
+          5: "BSE_ERR_NOT_POSITIVE_DEFINITE", 6: "BSE_ERR_INTERNAL"}
+
+
+class BseError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {STATUS.get(status, status)}")
+
+
+class _Info(ctypes.Structure):
+    _fields_ = [("n_apply", ctypes.c_int32), ("n_restart", ctypes.c_int32), ("nconv", ctypes.c_int32),
+                ("ncv", ctypes.c_int32), ("seconds_apply", ctypes.c_double), ("seconds_orth", ctypes.c_double),
+                ("seconds_project", ctypes.c_double), ("seconds_restart", ctypes.c_double),
+                ("seconds_total", ctypes.c_double), ("norm_est", ctypes.c_double)]
+
+
+_vp, _i64, _i32, _u64, _dbl = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_uint64, ctypes.c_double
+
+_SIGNATURES = {
+    "bse_layout": [_i64, ctypes.POINTER(_i32), ctypes.POINTER(_i64), ctypes.POINTER(_i64)],
+    "bse_pack_from_dense": [_vp, _i64, _i64, _i32, _vp, _vp],
+    "bse_unpack_to_dense": [_vp, _i64, _i32, _vp, _i64, _vp],
+    "bse_fill_synthetic": [_vp, _i64, _i32, _u64, _dbl, _i32, _vp],
+    "bse_fill_closed_form_tda": [_vp, _i64, _vp, _vp, _dbl, _vp],
+    "bse_fill_closed_form_full": [_vp, _vp, _i64, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp],
+    "bse_create": [ctypes.POINTER(_vp), _i32, _i64, _vp, _vp, _vp],
+    "bse_destroy": [_vp],
+    "bse_apply": [_vp, _vp, _i64, _vp, _i64, _i32],
+    "bse_apply_half": [_vp, _i32, _vp, _i64, _vp, _i64, _i32],
+    "bse_apply_host": [_vp, _vp, _i64, _vp, _i64, _i32],
+    "bse_orth": [_vp, _vp, _i64, _i32, _vp, _i64, _vp, _i64, _i32, _vp, _i64, _vp, _vp, ctypes.POINTER(_i32)],
+    "bse_solve": [_vp, _i32, _i32, _i32, _dbl, _i32, _u64, ctypes.POINTER(_dbl), _vp, _i64, ctypes.POINTER(_dbl),
+                  ctypes.POINTER(_Info)],
+}
+EXPORTS = sorted(list(_SIGNATURES) + ["bse_status_string", "bse_launch_count"])
+
+
+def lib():
+    """Loads the C-ABI library.  Raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIBPATH):
+            raise ImportError(f"{_LIBPATH} is missing: run `python -m paper_2504_10096_b200.build` "
+                              "(or __graft_entry__.build()); there is no CPU fallback")
+        L = ctypes.CDLL(_LIBPATH)
+        for name, args in _SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.argtypes = args
+            fn.restype = ctypes.c_int
+        L.bse_status_string.argtypes = [ctypes.c_int]
+        L.bse_status_string.restype = ctypes.c_char_p
+        L.bse_launch_count.argtypes = []
+        L.bse_launch_count.restype = ctypes.c_int64
+        _lib = L
+    return _lib
+
+
+def _check(st: int, where: str):
+    if st != 0:
+        raise BseError(st, where)
+
+
+def _stream_ptr():
+    import torch
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def bse_layout(N: int):
+    t, n, b = _i32(), _i64(), _i64()
+    _check(lib().bse_layout(N, ctypes.byref(t), ctypes.byref(n), ctypes.byref(b)), "bse_layout")
+    return t.value, n.value, b.value
+
+
+def alloc_tiles(N: int):
+    """Uninitialised device buffer for one packed matrix (torch uint8 tensor)."""
+    import torch
+    _, _, nbytes = bse_layout(N)
+    return torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+
+
+def _ld(t):
+    """Leading dimension (complex elements) of a column-major block held as a torch tensor.
+
+    Blocks are passed as torch complex128 tensors of shape (k, n) that are C-contiguous, i.e. the
+    memory is column-major n x k with ld = n (or 1-D tensors of n elements for k = 1)."""
+    assert t.is_cuda and t.dtype.is_complex and t.element_size() == 16 and t.is_contiguous()
+    return t.shape[-1]
+
+
+def bse_pack_from_dense(dense_cm, N: int, which: int, tiles=None):
+    """dense_cm: torch complex128 CUDA tensor of shape (N, N) holding the matrix COLUMN-major
+    (dense_cm[j, i] = A_ij), e.g. torch.from_numpy(A.T.copy()).cuda()."""
+    tiles = alloc_tiles(N) if tiles is None else tiles
+    _check(lib().bse_pack_from_dense(dense_cm.data_ptr(), N, N, which, tiles.data_ptr(), _stream_ptr()),
+           "bse_pack_from_dense")
+    return tiles
+
+
+def bse_unpack_to_dense(tiles, N: int, which: int):
+    import torch
+    out = torch.zeros((N, N), dtype=torch.complex128, device="cuda")
+    _check(lib().bse_unpack_to_dense(tiles.data_ptr(), N, which, out.data_ptr(), N, _stream_ptr()),
+           "bse_unpack_to_dense")
+    return out      # out[j, i] = A_ij
+
+
+def bse_fill_synthetic(N: int, which: int, seed: int, sigma: float = 0.0, group: int = 16, tiles=None):
+    tiles = alloc_tiles(N) if tiles is None else tiles
+    _check(lib().bse_fill_synthetic(tiles.data_ptr(), N, which, seed, sigma, group, _stream_ptr()),
+           "bse_fill_synthetic")
+    return tiles
+
+
+def bse_fill_closed_form_tda(N: int, lam, u, s: float, tiles=None):
+    tiles = alloc_tiles(N) if tiles is None else tiles
+    _check(lib().bse_fill_closed_form_tda(tiles.data_ptr(), N, lam.data_ptr(), u.data_ptr(), s, _stream_ptr()),
+           "bse_fill_closed_form_tda")
+    return tiles
+
+
+def bse_fill_closed_form_full(N: int, d1, d2, ur, phi, s1: float, s2: float):
+    rt, ct = alloc_tiles(N), alloc_tiles(N)
+    _check(lib().bse_fill_closed_form_full(rt.data_ptr(), ct.data_ptr(), N, d1.data_ptr(), d2.data_ptr(),
+                                           ur.data_ptr(), phi.data_ptr(), s1, s2, _stream_ptr()),
+           "bse_fill_closed_form_full")
+    return rt, ct
+
+
+@dataclass
+class SolveResult:
+    omega: "object"
+    vectors: "object"
+    resid: "object"
+    info: dict
+    status: int
+
+
+class Bse:
+    """Handle wrapper (bse_create / bse_destroy).  Keeps the borrowed tile buffers alive."""
+
+    def __init__(self, mode: int, N: int, r_tiles, c_tiles=None):
+        self.mode, self.N = mode, N
+        self._keep = (r_tiles, c_tiles)
+        self.n_op = 2 * N if mode == MODE_FULL else N
+        h = _vp()
+        _check(lib().bse_create(ctypes.byref(h), mode, N, r_tiles.data_ptr(),
+                                c_tiles.data_ptr() if c_tiles is not None else None, _stream_ptr()), "bse_create")
+        self._h = h
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().bse_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def apply(self, X, Y=None):
+        """Y = H X.  X: torch complex128 CUDA tensor of shape (k, n_op) (column-major n_op x k)."""
+        import torch
+        k = X.shape[0] if X.dim() == 2 else 1
+        Y = torch.empty_like(X) if Y is None else Y
+        _check(lib().bse_apply(self._h, X.data_ptr(), _ld(X), Y.data_ptr(), _ld(Y), k), "bse_apply")
+        return Y
+
+    def apply_half(self, X, sign: int, Y=None):
+        import torch
+        k = X.shape[0] if X.dim() == 2 else 1
+        Y = torch.empty_like(X) if Y is None else Y
+        _check(lib().bse_apply_half(self._h, sign, X.data_ptr(), _ld(X), Y.data_ptr(), _ld(Y), k), "bse_apply_half")
+        return Y
+
+    def apply_host(self, X_np, Y_np=None):
+        """Host entry point: X_np numpy complex128 of shape (k, n_op), C-contiguous."""
+        import numpy as np
+        assert X_np.dtype == np.complex128 and X_np.flags.c_contiguous
+        Y_np = np.empty_like(X_np) if Y_np is None else Y_np
+        k, n = X_np.shape
+        _check(lib().bse_apply_host(self._h, X_np.ctypes.data, n, Y_np.ctypes.data, n, k), "bse_apply_host")
+        return Y_np
+
+    def orth(self, V, W, BV=None, BW=None):
+        """Block CGS2 of W (k, n) against V (m, n) [+ P-images].  Returns (hcoef (k, m), Bfac (k, k), rank).
+        W (and BW) are overwritten.  hcoef/Bfac are column-major m x k / k x k viewed as torch (k, m)/(k, k)."""
+        import torch
+        m = 0 if V is None else V.shape[0]
+        k = W.shape[0]
+        hcoef = torch.zeros((k, max(m, 1)), dtype=torch.complex128, device="cuda")
+        bfac = torch.zeros((k, k), dtype=torch.complex128, device="cuda")
+        rank = _i32(0)
+        _check(lib().bse_orth(self._h, V.data_ptr() if m else None, _ld(V) if m else self.N, m,
+                              BV.data_ptr() if BV is not None else None, _ld(BV) if BV is not None else self.N,
+                              W.data_ptr(), _ld(W), k, BW.data_ptr() if BW is not None else None,
+                              _ld(BW) if BW is not None else self.N, hcoef.data_ptr(), bfac.data_ptr(),
+                              ctypes.byref(rank)), "bse_orth")
+        return hcoef[:, :m], bfac, rank.value
+
+    def solve(self, nev: int, k: int, ncv: int = 0, tol: float = 1e-8, max_restarts: int = 1000, seed: int = 1,
+              raise_on_error: bool = True):
+        import numpy as np
+        import torch
+        omega = np.zeros(nev)
+        resid = np.zeros(nev)
+        vec = torch.zeros((nev, self.n_op), dtype=torch.complex128, device="cuda")
+        info = _Info()
+        st = lib().bse_solve(self._h, nev, k, ncv, tol, max_restarts, seed,
+                             omega.ctypes.data_as(ctypes.POINTER(_dbl)), vec.data_ptr(), self.n_op,
+                             resid.ctypes.data_as(ctypes.POINTER(_dbl)), ctypes.byref(info))
+        if st != 0 and raise_on_error:
+            raise BseError(st, "bse_solve")
+        return SolveResult(omega, vec, resid, {f: getattr(info, f) for f, _ in _Info._fields_}, st)
+
+
+def launch_count() -> int:
+    return lib().bse_launch_count()

@@ -1,0 +1,252 @@
+// Structured block-matvec over the packed triangular tile store.
+//
+// One pass computes, for up to 4 columns of X,
+//     HERM :  Y += s * R X            (R Hermitian, lower triangle stored)
+//     SYMC :  Y += s * C conj(X)      (C complex symmetric, lower triangle stored)
+// Every stored tile T = T_IJ (I >= J) is brought from HBM exactly once by a TMA bulk copy
+// (cp.async.bulk -> UBLKCP) into a 3-stage shared-memory ring and used twice from there:
+//     P1:  Y_I += T   x_J            (HERM)      Y_I += T   conj(x_J)   (SYMC)
+//     P2:  Y_J += T^H x_I            (HERM)      Y_J += T^T conj(x_I)   (SYMC)       (skipped when I == J)
+// Both products run on the FP64 tensor cores (mma.sync m8n8k4 -> DMMA.8x8x4) in real arithmetic:
+// with N-dimension n = 2 c + part (c = column of X, part = re/im),
+//     [Yr|Yi] += Tr * Ba + Ti * Bb,   Ba, Bb = signed re/im selections of X (table in DESIGN.md).
+//
+// Work decomposition: a unit is a run of up to L consecutive tiles of one tile row I.  A CTA
+// (8 consumer warps + 1 producer warp, persistent, one per SM) walks its units; consumer warp w
+// owns tile columns 8w .. 8w+7 of every tile, i.e. for P1 a slice of the contraction (partial Y_I for
+// all 64 rows, accumulated in registers over the whole unit) and for P2 eight output rows of Y_J
+// (contraction over all 64 i, with the x_I fragments held in registers for the whole unit).
+// Partial results are added to Y with red.global.add.f64 (Y must be zero or hold the running sum).
+#pragma once
+#include "bse_common.cuh"
+
+namespace bse {
+
+constexpr int APPLY_STAGES = 3;
+constexpr int APPLY_CONSUMERS = 8;                       // consumer warps
+constexpr int APPLY_THREADS = (APPLY_CONSUMERS + 1) * 32;
+constexpr int XCOL_STRIDE = 1024 + 16;                   // bytes between the columns of an X panel in smem
+constexpr int XPAN_BYTES = 4224;                         // 4 columns, rounded up to 128 B
+constexpr int APPLY_SMEM = APPLY_STAGES * TILE_BYTES + APPLY_STAGES * XPAN_BYTES + 2 * XPAN_BYTES + 128;
+
+enum { PASS_HERM = 0, PASS_SYMC = 1 };
+
+struct ApplyParams {
+    const char *tiles;
+    const double2 *X;
+    int64_t ldx;
+    double *Y;          // complex128 viewed as doubles
+    int64_t ldy;
+    int64_t N;
+    int nt;             // tile rows
+    int kc;             // columns in this pass (1..4)
+    int pass;           // PASS_HERM / PASS_SYMC
+    double sign;        // s
+    int L;              // unit length in tiles
+    int64_t n_units;
+};
+
+__host__ __device__ __forceinline__ int64_t apply_num_units(int nt, int L)
+{
+    int64_t bf = nt / L, r = nt % L;
+    return (int64_t)L * bf * (bf + 1) / 2 + r * (bf + 1);
+}
+// unit u -> (I, J0, J1): rows I in [bL, (b+1)L) have b+1 units each.
+__device__ __forceinline__ void apply_decode_unit(int64_t u, int L, int &I, int &J0, int &J1)
+{
+    int64_t b = (int64_t)((sqrt(1.0 + 8.0 * (double)u / (double)L) - 1.0) * 0.5);
+    while ((int64_t)L * b * (b + 1) / 2 > u) --b;
+    while ((int64_t)L * (b + 1) * (b + 2) / 2 <= u) ++b;
+    int64_t rem = u - (int64_t)L * b * (b + 1) / 2;
+    int r = (int)(rem / (b + 1)), seg = (int)(rem % (b + 1));
+    I = (int)(b * L + r);
+    J0 = seg * L;
+    J1 = min(J0 + L, I + 1);
+}
+
+__global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const ApplyParams p)
+{
+    extern __shared__ __align__(1024) char smem[];
+    char *tile_s = smem;
+    char *xj_s = smem + APPLY_STAGES * TILE_BYTES;
+    char *xi_s = xj_s + APPLY_STAGES * XPAN_BYTES;
+    uint64_t *bars = reinterpret_cast<uint64_t *>(xi_s + 2 * XPAN_BYTES);
+    uint64_t *full = bars, *empty = bars + APPLY_STAGES, *xfull = bars + 2 * APPLY_STAGES, *xempty = xfull + 2;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    // zero the X panels once: rows beyond N of a ragged last panel are never written by the bulk copies
+    for (int i = threadIdx.x; i < (APPLY_STAGES + 2) * XPAN_BYTES / 16; i += APPLY_THREADS)
+        reinterpret_cast<double2 *>(xj_s)[i] = make_double2(0.0, 0.0);
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < APPLY_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], APPLY_CONSUMERS); }
+        for (int s = 0; s < 2; ++s) { mbar_init(&xfull[s], 1); mbar_init(&xempty[s], APPLY_CONSUMERS); }
+        fence_barrier_init();
+    }
+    fence_proxy_async();
+    __syncthreads();
+
+    const int kc = p.kc;
+    if (warp == APPLY_CONSUMERS) {
+        // ------------------------------ producer warp (one elected lane) ------------------------------
+        if (lane == 0) {
+            int st = 0, xs = 0;
+            uint32_t ph = 0, xph = 0;
+            for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
+                int I, J0, J1;
+                apply_decode_unit(u, p.L, I, J0, J1);
+                {
+                    int rows = (int)min((int64_t)TB, p.N - (int64_t)I * TB);
+                    mbar_wait(&xempty[xs], xph ^ 1);
+                    mbar_expect_tx(&xfull[xs], (uint32_t)(kc * rows * 16));
+                    for (int c = 0; c < kc; ++c)
+                        bulk_g2s(xi_s + xs * XPAN_BYTES + c * XCOL_STRIDE, p.X + (int64_t)I * TB + c * p.ldx,
+                                 (uint32_t)(rows * 16), &xfull[xs]);
+                    if (++xs == 2) { xs = 0; xph ^= 1; }
+                }
+                const char *src = p.tiles + tile_index(I, J0) * (int64_t)TILE_BYTES;
+                for (int J = J0; J < J1; ++J, src += TILE_BYTES) {
+                    int rows = (int)min((int64_t)TB, p.N - (int64_t)J * TB);
+                    mbar_wait(&empty[st], ph ^ 1);
+                    mbar_expect_tx(&full[st], (uint32_t)(TILE_BYTES + kc * rows * 16));
+                    bulk_g2s(tile_s + st * TILE_BYTES, src, TILE_BYTES, &full[st]);
+                    for (int c = 0; c < kc; ++c)
+                        bulk_g2s(xj_s + st * XPAN_BYTES + c * XCOL_STRIDE, p.X + (int64_t)J * TB + c * p.ldx,
+                                 (uint32_t)(rows * 16), &full[st]);
+                    if (++st == APPLY_STAGES) { st = 0; ph ^= 1; }
+                }
+            }
+        }
+        return;
+    }
+
+    // ------------------------------------ consumer warps ------------------------------------------
+    const int w = warp;
+    const int g = lane >> 2, t = lane & 3;
+    const int g2 = (g >> 2) & 1, g1 = (g >> 1) & 1, g0 = g & 1, t1 = (t >> 1) & 1, t0 = t & 1;
+    // fragment byte offsets inside a patch (see patch_slot): P1 reads (a = g, b = 4 s + t), P2 reads (a = 4 s + t, b = g)
+    const int offP1 = (((g2 << 2) | g1) * 8 + ((g0 << 2) | (t0 << 1) | (g1 ^ t1))) * 16;   // + s * 256
+    const int offP2 = (((g2 << 1) | t1) * 8 + ((t0 << 2) | (g0 << 1) | (t1 ^ g1))) * 16;   // + s * 512
+    // B fragments: lane supplies B[kk = t][n = g], n = 2 c + part
+    const int col = g >> 1, part = g & 1;
+    const bool colok = col < kc;
+    // Ba pairs with Re(T), Bb with Im(T); value = coef * (re or im of x):
+    //   HERM P1 (T x):        Ba = [xr, xi]   Bb = [-xi, xr]
+    //   HERM P2 (T^H x):      Ba = [xr, xi]   Bb = [ xi, -xr]
+    //   SYMC P1/P2 (T conj x): Ba = [xr, -xi]  Bb = [ xi, xr]
+    double ca1, cb1, ca2, cb2;
+    if (p.pass == PASS_HERM) {
+        ca1 = 1.0; cb1 = part ? 1.0 : -1.0;
+        ca2 = 1.0; cb2 = part ? -1.0 : 1.0;
+    } else {
+        ca1 = part ? -1.0 : 1.0; cb1 = 1.0;
+        ca2 = ca1; cb2 = 1.0;
+    }
+    if (!colok) { ca1 = cb1 = ca2 = cb2 = 0.0; }
+    ca1 *= p.sign; cb1 *= p.sign; ca2 *= p.sign; cb2 *= p.sign;
+    const int xoff = (colok ? col : 0) * XCOL_STRIDE;
+
+    int st = 0, xs = 0;
+    uint32_t ph = 0, xph = 0;
+    for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
+        int I, J0, J1;
+        apply_decode_unit(u, p.L, I, J0, J1);
+
+        // x_I fragments for P2, kept in registers for the whole unit
+        double BaI[8][2], BbI[8][2];
+        mbar_wait(&xfull[xs], xph);
+        {
+            const char *xp = xi_s + xs * XPAN_BYTES + xoff;
+#pragma unroll
+            for (int ib = 0; ib < 8; ++ib)
+#pragma unroll
+                for (int s = 0; s < 2; ++s) {
+                    double2 x = *reinterpret_cast<const double2 *>(xp + (ib * 8 + s * 4 + t) * 16);
+                    BaI[ib][s] = (part ? x.y : x.x) * ca2;
+                    BbI[ib][s] = (part ? x.x : x.y) * cb2;
+                }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&xempty[xs]);
+        if (++xs == 2) { xs = 0; xph ^= 1; }
+
+        double C1[8][2];
+#pragma unroll
+        for (int ib = 0; ib < 8; ++ib) C1[ib][0] = C1[ib][1] = 0.0;
+
+        for (int J = J0; J < J1; ++J) {
+            mbar_wait(&full[st], ph);
+            const char *tp = tile_s + st * TILE_BYTES + w * 8 * PATCH_BYTES;
+            double BaJ[2], BbJ[2];
+            {
+                const char *xp = xj_s + st * XPAN_BYTES + xoff;
+#pragma unroll
+                for (int s = 0; s < 2; ++s) {
+                    double2 x = *reinterpret_cast<const double2 *>(xp + (w * 8 + s * 4 + t) * 16);
+                    BaJ[s] = (part ? x.y : x.x) * ca1;
+                    BbJ[s] = (part ? x.x : x.y) * cb1;
+                }
+            }
+            if (I != J) {
+                double C2[4][2];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) C2[q][0] = C2[q][1] = 0.0;
+#pragma unroll
+                for (int ib = 0; ib < 8; ++ib) {
+                    const char *pp = tp + ib * PATCH_BYTES;
+                    double2 a0 = *reinterpret_cast<const double2 *>(pp + offP1);
+                    double2 a1 = *reinterpret_cast<const double2 *>(pp + offP1 + 256);
+                    double2 b0 = *reinterpret_cast<const double2 *>(pp + offP2);
+                    double2 b1 = *reinterpret_cast<const double2 *>(pp + offP2 + 512);
+                    dmma(C1[ib], a0.x, BaJ[0]);
+                    dmma(C2[ib & 3], b0.x, BaI[ib][0]);
+                    dmma(C1[ib], a0.y, BbJ[0]);
+                    dmma(C2[ib & 3], b0.y, BbI[ib][0]);
+                    dmma(C1[ib], a1.x, BaJ[1]);
+                    dmma(C2[ib & 3], b1.x, BaI[ib][1]);
+                    dmma(C1[ib], a1.y, BbJ[1]);
+                    dmma(C2[ib & 3], b1.y, BbI[ib][1]);
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[st]);
+                // flush Y_J rows 8w + g, column t
+                double yr = (C2[0][0] + C2[1][0]) + (C2[2][0] + C2[3][0]);
+                double yi = (C2[0][1] + C2[1][1]) + (C2[2][1] + C2[3][1]);
+                int64_t row = (int64_t)J * TB + w * 8 + g;
+                if (t < kc && row < p.N) {
+                    double *y = p.Y + 2 * (row + (int64_t)t * p.ldy);
+                    red_add(y, yr);
+                    red_add(y + 1, yi);
+                }
+            } else {
+#pragma unroll
+                for (int ib = 0; ib < 8; ++ib) {
+                    const char *pp = tp + ib * PATCH_BYTES;
+                    double2 a0 = *reinterpret_cast<const double2 *>(pp + offP1);
+                    double2 a1 = *reinterpret_cast<const double2 *>(pp + offP1 + 256);
+                    dmma(C1[ib], a0.x, BaJ[0]);
+                    dmma(C1[ib], a0.y, BbJ[0]);
+                    dmma(C1[ib], a1.x, BaJ[1]);
+                    dmma(C1[ib], a1.y, BbJ[1]);
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[st]);
+            }
+            if (++st == APPLY_STAGES) { st = 0; ph ^= 1; }
+        }
+        // flush this warp's partial Y_I (all 64 rows, column t)
+        if (t < kc) {
+#pragma unroll
+            for (int ib = 0; ib < 8; ++ib) {
+                int64_t row = (int64_t)I * TB + ib * 8 + g;
+                if (row < p.N) {
+                    double *y = p.Y + 2 * (row + (int64_t)t * p.ldy);
+                    red_add(y, C1[ib][0]);
+                    red_add(y + 1, C1[ib][1]);
+                }
+            }
+        }
+    }
+}
+
+}  // namespace bse

@@ -1,0 +1,244 @@
+// C-ABI entry points: layout, pack / generators, handle, apply.  (orth: bse_orth.cu, solve: bse_solve.cu)
+#include <cstdio>
+#include <cstdlib>
+#include <new>
+
+#include "apply_kernel.cuh"
+#include "bse_internal.h"
+#include "tile_layout.cuh"
+
+namespace bse {
+
+std::atomic<int64_t> g_launches{0};
+
+static bse_status_t grow(void **p, size_t *have, size_t want)
+{
+    if (*have >= want) return BSE_OK;
+    if (*p) cudaFree(*p);
+    *p = nullptr;
+    *have = 0;
+    if (cudaMalloc(p, want) != cudaSuccess) { cudaGetLastError(); return BSE_ERR_ALLOC; }
+    *have = want;
+    return BSE_OK;
+}
+bse_status_t ensure_ws(bse_handle_s *h, size_t bytes) { return grow(&h->ws, &h->ws_bytes, bytes); }
+bse_status_t ensure_ws2(bse_handle_s *h, size_t bytes) { return grow(&h->ws2, &h->ws2_bytes, bytes); }
+bse_status_t ensure_pin(bse_handle_s *h, size_t bytes)
+{
+    if (h->hpin_bytes >= bytes) return BSE_OK;
+    if (h->hpin) cudaFreeHost(h->hpin);
+    h->hpin = nullptr;
+    h->hpin_bytes = 0;
+    if (cudaMallocHost(&h->hpin, bytes) != cudaSuccess) { cudaGetLastError(); return BSE_ERR_ALLOC; }
+    h->hpin_bytes = bytes;
+    return BSE_OK;
+}
+
+static void tile_grid(int64_t n_tiles, dim3 &grid)
+{
+    int64_t gy = n_tiles < 32768 ? n_tiles : 32768;
+    int64_t gz = (n_tiles + gy - 1) / gy;
+    grid = dim3(TB * TB / 256, (unsigned)gy, (unsigned)gz);
+}
+
+bse_status_t zero_block(bse_handle_s *h, void *dY, int64_t ldy, int64_t rows, int32_t k)
+{
+    BSE_CUDA(cudaMemset2DAsync(dY, (size_t)ldy * 16, 0, (size_t)rows * 16, (size_t)k, h->stream));
+    return BSE_OK;
+}
+
+bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, double sign, const void *dX,
+                               int64_t ldx, void *dY, int64_t ldy, int32_t k)
+{
+    static bool attr_set = false;
+    if (!attr_set) {
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        attr_set = true;
+    }
+    ApplyParams p;
+    p.tiles = tiles;
+    p.N = h->N;
+    p.nt = h->nt;
+    p.pass = pass;
+    p.sign = sign;
+    p.ldx = ldx;
+    p.ldy = ldy;
+    int64_t total_tiles = (int64_t)h->nt * (h->nt + 1) / 2;
+    int64_t L = total_tiles / ((int64_t)h->num_sms * 12);
+    if (L < 1) L = 1;
+    if (L > 32) L = 32;
+    if (const char *e = getenv("BSE_APPLY_UNIT")) { int v = atoi(e); if (v >= 1 && v <= 4096) L = v; }
+    p.L = (int)L;
+    p.n_units = apply_num_units(h->nt, p.L);
+    int grid = (int)(p.n_units < h->num_sms ? p.n_units : h->num_sms);
+    for (int32_t c0 = 0; c0 < k; c0 += 4) {
+        p.kc = (k - c0) < 4 ? (k - c0) : 4;
+        p.X = reinterpret_cast<const double2 *>(dX) + (int64_t)c0 * ldx;
+        p.Y = reinterpret_cast<double *>(dY) + 2 * (int64_t)c0 * ldy;
+        apply_tiles_kernel<<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+        count_launch();
+    }
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}
+
+}  // namespace bse
+
+using namespace bse;
+
+extern "C" {
+
+const char *bse_status_string(bse_status_t s)
+{
+    switch (s) {
+        case BSE_OK: return "ok";
+        case BSE_ERR_INVALID_ARG: return "invalid argument";
+        case BSE_ERR_CUDA: return "CUDA error";
+        case BSE_ERR_ALLOC: return "allocation failed";
+        case BSE_ERR_NOT_CONVERGED: return "not converged";
+        case BSE_ERR_NOT_POSITIVE_DEFINITE: return "operator not positive definite";
+        default: return "internal error";
+    }
+}
+
+int64_t bse_launch_count(void) { return g_launches.load(); }
+
+bse_status_t bse_layout(int64_t N, int32_t *tile, int64_t *n_tiles, int64_t *bytes_per_matrix)
+{
+    if (N < 1) return BSE_ERR_INVALID_ARG;
+    int64_t nt = (N + TB - 1) / TB;
+    if (tile) *tile = TB;
+    if (n_tiles) *n_tiles = nt * (nt + 1) / 2;
+    if (bytes_per_matrix) *bytes_per_matrix = nt * (nt + 1) / 2 * (int64_t)TILE_BYTES;
+    return BSE_OK;
+}
+
+bse_status_t bse_pack_from_dense(const void *dDense, int64_t ld, int64_t N, int32_t which, void *dTiles, void *stream)
+{
+    if (!dDense || !dTiles || N < 1 || ld < N || (which != 0 && which != 1)) return BSE_ERR_INVALID_ARG;
+    int64_t n_tiles;
+    bse_layout(N, nullptr, &n_tiles, nullptr);
+    dim3 grid;
+    tile_grid(n_tiles, grid);
+    pack_from_dense_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((const double2 *)dDense, ld, N, which,
+                                                                   (char *)dTiles, n_tiles);
+    count_launch();
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}
+
+bse_status_t bse_unpack_to_dense(const void *dTiles, int64_t N, int32_t which, void *dDense, int64_t ld, void *stream)
+{
+    if (!dDense || !dTiles || N < 1 || ld < N || (which != 0 && which != 1)) return BSE_ERR_INVALID_ARG;
+    int64_t n_tiles;
+    bse_layout(N, nullptr, &n_tiles, nullptr);
+    dim3 grid;
+    tile_grid(n_tiles, grid);
+    unpack_to_dense_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((const char *)dTiles, N, which, (double2 *)dDense,
+                                                                   ld, n_tiles);
+    count_launch();
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}
+
+bse_status_t bse_fill_synthetic(void *dTiles, int64_t N, int32_t which, uint64_t seed, double sigma, int32_t group,
+                                void *stream)
+{
+    if (!dTiles || N < 1 || (which != 0 && which != 1)) return BSE_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    double *deps = nullptr;
+    if (which == 0) {
+        if (group < 1 || group > 64 || N % group) return BSE_ERR_INVALID_ARG;
+        if (cudaMallocAsync(&deps, sizeof(double) * N, s) != cudaSuccess) { cudaGetLastError(); return BSE_ERR_ALLOC; }
+        int64_t ngroups = N / group;
+        transition_energies_kernel<<<(unsigned)((ngroups + 127) / 128), 128, 0, s>>>(deps, N, group,
+                                                                                    stream_key(seed, 1));
+        count_launch();
+    }
+    int64_t n_tiles;
+    bse_layout(N, nullptr, &n_tiles, nullptr);
+    dim3 grid;
+    tile_grid(n_tiles, grid);
+    fill_synthetic_kernel<<<grid, 256, 0, s>>>((char *)dTiles, N, which, stream_key(seed, which == 0 ? 2 : 3), sigma,
+                                               deps, n_tiles);
+    count_launch();
+    if (deps) cudaFreeAsync(deps, s);
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}
+
+bse_status_t bse_fill_closed_form_tda(void *dTiles, int64_t N, const double *dLam, const void *dU, double s, void *stream)
+{
+    if (!dTiles || !dLam || !dU || N < 1) return BSE_ERR_INVALID_ARG;
+    int64_t n_tiles;
+    bse_layout(N, nullptr, &n_tiles, nullptr);
+    dim3 grid;
+    tile_grid(n_tiles, grid);
+    fill_closed_tda_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((char *)dTiles, N, dLam, (const double2 *)dU, s,
+                                                                   n_tiles);
+    count_launch();
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}
+
+bse_status_t bse_fill_closed_form_full(void *dRTiles, void *dCTiles, int64_t N, const double *dD1, const double *dD2,
+                                       const double *dUr, const double *dPhi, double s1, double s2, void *stream)
+{
+    if (!dRTiles || !dCTiles || !dD1 || !dD2 || !dUr || !dPhi || N < 1) return BSE_ERR_INVALID_ARG;
+    int64_t n_tiles;
+    bse_layout(N, nullptr, &n_tiles, nullptr);
+    dim3 grid;
+    tile_grid(n_tiles, grid);
+    fill_closed_full_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((char *)dRTiles, N, 0, dD1, dD2, dUr, dPhi, s1, s2,
+                                                                    n_tiles);
+    fill_closed_full_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((char *)dCTiles, N, 1, dD1, dD2, dUr, dPhi, s1, s2,
+                                                                    n_tiles);
+    count_launch(2);
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}
+
+bse_status_t bse_create(bse_handle_t *out, int32_t mode, int64_t N, const void *dRTiles, const void *dCTiles,
+                        void *stream)
+{
+    if (!out || !dRTiles || N < 1 || (mode != BSE_MODE_TDA && mode != BSE_MODE_FULL)) return BSE_ERR_INVALID_ARG;
+    if (mode == BSE_MODE_FULL && !dCTiles) return BSE_ERR_INVALID_ARG;
+    int dev = 0;
+    BSE_CUDA(cudaGetDevice(&dev));
+    int sms = 0;
+    BSE_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    bse_handle_s *h = new (std::nothrow) bse_handle_s();
+    if (!h) return BSE_ERR_ALLOC;
+    h->mode = mode;
+    h->N = N;
+    h->nt = (int)((N + TB - 1) / TB);
+    h->R = (const char *)dRTiles;
+    h->C = (mode == BSE_MODE_FULL) ? (const char *)dCTiles : nullptr;
+    h->stream = (cudaStream_t)stream;
+    h->num_sms = sms;
+    *out = h;
+    return BSE_OK;
+}
+
+bse_status_t bse_destroy(bse_handle_t h)
+{
+    if (!h) return BSE_ERR_INVALID_ARG;
+    if (h->ws) cudaFree(h->ws);
+    if (h->ws2) cudaFree(h->ws2);
+    if (h->hpin) cudaFreeHost(h->hpin);
+    delete h;
+    return BSE_OK;
+}
+
+bse_status_t bse_apply_half(bse_handle_t h, int32_t sign, const void *dX, int64_t ldx, void *dY, int64_t ldy, int32_t k)
+{
+    if (!h || !dX || !dY || k < 1 || ldx < h->N || ldy < h->N || (sign != 1 && sign != -1)) return BSE_ERR_INVALID_ARG;
+    if (h->mode != BSE_MODE_FULL) return BSE_ERR_INVALID_ARG;
+    bse_status_t st = zero_block(h, dY, ldy, h->N, k);
+    if (st) return st;
+    st = launch_apply_pass(h, h->R, PASS_HERM, 1.0, dX, ldx, dY, ldy, k);
+    if (st) return st;
+    return launch_apply_pass(h, h->C, PASS_SYMC, (double)sign, dX, ldx, dY, ldy, k);
+}
+
+}  // extern "C"

@@ -1,0 +1,81 @@
+// Common device helpers for the BSE hot-path kernels (sm_100a).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace bse {
+
+constexpr int TB = 64;                 // tile edge (complex elements)
+constexpr int TILE_BYTES = TB * TB * 16;
+constexpr int PATCH_BYTES = 8 * 8 * 16;
+
+// Slot (16-byte unit) of entry (a, b), 0 <= a, b < 8, inside an 8 x 8 patch.  Chosen so that both
+// DMMA fragment reads of the apply kernel -- lanes (g, t) reading (a = g, b = 4s + t) and
+// (a = 4s + t, b = g) -- touch 8 distinct 16-byte bank groups per quarter-warp (see include/bse.h).
+__host__ __device__ __forceinline__ int patch_slot(int a, int b)
+{
+    int r = ((a >> 2) << 2) | ((b >> 2) << 1) | ((a >> 1) & 1);
+    int c = ((a & 1) << 2) | ((b & 1) << 1) | (((a >> 1) ^ (b >> 1)) & 1);
+    return r * 8 + c;
+}
+// Byte offset of entry (il, jl), 0 <= il, jl < 64, inside a tile.
+__host__ __device__ __forceinline__ int tile_offset(int il, int jl)
+{
+    return ((jl >> 3) * 8 + (il >> 3)) * PATCH_BYTES + patch_slot(il & 7, jl & 7) * 16;
+}
+__host__ __device__ __forceinline__ int64_t tile_index(int64_t I, int64_t J) { return I * (I + 1) / 2 + J; }
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *b, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *b, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *b)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *b, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}" ::"r"(smem_u32(b)), "r"(parity) : "memory");
+}
+// TMA bulk copy global -> shared, completion signalled on an mbarrier (SASS: UBLKCP).
+__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+__device__ __forceinline__ double2 lds128(uint32_t addr)
+{
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+// FP64 tensor-core MMA, D(8x8) += A(8x4, row) * B(4x8, col).  SASS: DMMA.8x8x4.
+// Fragments: lane = 4 g + t;  a = A[g][t];  b = B[t][g];  c[0..1] = C[g][2t .. 2t+1].
+__device__ __forceinline__ void dmma(double (&c)[2], double a, double b)
+{
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+        : "+d"(c[0]), "+d"(c[1])
+        : "d"(a), "d"(b));
+}
+__device__ __forceinline__ void red_add(double *p, double v) { atomicAdd(p, v); }
+
+}  // namespace bse

@@ -1,0 +1,143 @@
+"""Parity of the CUDA apply path (through the C ABI) against the CPU oracle, element by element."""
+import numpy as np
+import pytest
+
+import bse_inputs as gen
+from gpu_util import pack, relerr, to_dev, to_host
+
+pytestmark = pytest.mark.gpu
+
+TOL_APPLY = 1e-12      # north_star: apply normwise relative error <= 1e-12
+
+
+def _herm(n, seed):
+    A = gen.block_X(n, n, seed)
+    A = (A + A.conj().T) / 2
+    A[np.diag_indices(n)] = A.diagonal().real
+    return A
+
+
+def _sym(n, seed):
+    A = gen.block_X(n, n, seed)
+    return (A + A.T) / 2
+
+
+@pytest.mark.parametrize("N", [1, 8, 64, 100, 257])
+@pytest.mark.parametrize("which", [0, 1])
+def test_pack_unpack_roundtrip(N, which):
+    import paper_2504_10096_b200 as b
+    A = _herm(N, 3) if which == 0 else _sym(N, 4)
+    junk = A.copy()
+    junk[np.triu_indices(N, 1)] = 1e30          # the strictly upper triangle must never be read
+    tiles = pack(junk, which)
+    back = to_host(b.bse_unpack_to_dense(tiles, N, which))
+    assert np.array_equal(back, A)
+
+
+def test_pack_drops_imaginary_diagonal_of_R():
+    import paper_2504_10096_b200 as b
+    N = 70
+    A = _herm(N, 5) + 1j * np.eye(N)
+    back = to_host(b.bse_unpack_to_dense(pack(A, 0), N, 0))
+    assert np.all(back.diagonal().imag == 0)
+
+
+@pytest.mark.parametrize("N,group", [(256, 16), (320, 64)])
+def test_device_generator_matches_cpu_generator(N, group):
+    import paper_2504_10096_b200 as b
+    R = gen.dense_R(N, 7, sigma=0.5, group=group)
+    C = gen.dense_C(N, 7)
+    Rd = to_host(b.bse_unpack_to_dense(b.bse_fill_synthetic(N, 0, 7, 0.5, group), N, 0))
+    Cd = to_host(b.bse_unpack_to_dense(b.bse_fill_synthetic(N, 1, 7), N, 1))
+    # same integer hash on both sides; log / sincos differ by a few ulp
+    assert np.max(np.abs(Rd - R)) < 1e-14
+    assert np.max(np.abs(Cd - C)) < 1e-14
+    assert np.array_equal(Rd, Rd.conj().T) and np.array_equal(Cd, Cd.T)
+
+
+def test_closed_form_fill_matches_cpu():
+    import torch
+    import paper_2504_10096_b200 as b
+    N = 200
+    lam = gen.prescribed_spectrum(N, 5); u = gen.householder_u(N, 5)
+    s = float(np.sum(lam * np.abs(u) ** 2))
+    t = b.bse_fill_closed_form_tda(N, torch.from_numpy(lam).cuda(), torch.from_numpy(u).cuda(), s)
+    Rd = to_host(b.bse_unpack_to_dense(t, N, 0))
+    assert np.max(np.abs(Rd - gen.closed_form_tda_dense(lam, u))) < 1e-13
+    d1 = gen.prescribed_spectrum(N, 7, 1.0, 9.0); d2 = gen.prescribed_spectrum(N, 8, 2.0, 5.0)
+    ur = gen.householder_u(N, 9, complex_u=False).real.copy(); phi = gen.phases(N, 9)
+    rt, ct = b.bse_fill_closed_form_full(N, *(torch.from_numpy(a).cuda() for a in (d1, d2, ur, phi)),
+                                         float(np.sum(d1 * ur ** 2)), float(np.sum(d2 * ur ** 2)))
+    R, C = gen.closed_form_full_dense(d1, d2, ur, phi)
+    assert np.max(np.abs(to_host(b.bse_unpack_to_dense(rt, N, 0)) - R)) < 1e-13
+    assert np.max(np.abs(to_host(b.bse_unpack_to_dense(ct, N, 1)) - C)) < 1e-13
+
+
+def test_identity_and_diagonal_exact():
+    import paper_2504_10096_b200 as b
+    N, k = 200, 3
+    X = gen.block_X(N, k, 5)
+    h = b.Bse(b.MODE_TDA, N, pack(np.eye(N, dtype=complex), 0))
+    assert np.array_equal(to_host(h.apply(to_dev(X))), X)
+    d = np.linspace(-2, 3, N)
+    h = b.Bse(b.MODE_TDA, N, pack(np.diag(d).astype(complex), 0))
+    assert np.array_equal(to_host(h.apply(to_dev(X))), d[:, None] * X)
+
+
+def test_unit_impulses_cover_tile_borders(orc):
+    # every stored entry class: inside a diagonal tile (both triangles), off-diagonal tile, tile borders
+    import paper_2504_10096_b200 as b
+    N, k = 136, 2
+    X = gen.block_X(N, k, 7)
+    Xd = to_dev(X)
+    for (i, j) in [(5, 2), (63, 0), (64, 63), (65, 64), (127, 64), (128, 0), (135, 127), (135, 135), (100, 37)]:
+        R = np.zeros((N, N), dtype=complex)
+        R[i, j] = 0.7 - 1.3j
+        Y = to_host(b.Bse(b.MODE_TDA, N, pack(R, 0)).apply(Xd))
+        assert np.allclose(Y, orc.apply_tda(R, X), rtol=0, atol=1e-15), (i, j)
+
+
+@pytest.mark.parametrize("N", [64, 100, 320, 1024])
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5, 8])
+def test_tda_apply_matches_oracle(orc, N, k):
+    import paper_2504_10096_b200 as b
+    R = _herm(N, 11) if N < 1024 else gen.dense_R(N, 1)
+    X = gen.block_X(N, k, 12)
+    Y = to_host(b.Bse(b.MODE_TDA, N, pack(R, 0)).apply(to_dev(X)))
+    assert relerr(Y, orc.apply_tda(R, X)) <= TOL_APPLY
+
+
+@pytest.mark.parametrize("N", [64, 200, 448])
+@pytest.mark.parametrize("k", [1, 4, 6])
+def test_full_apply_and_half_apply_match_oracle(orc, N, k):
+    import paper_2504_10096_b200 as b
+    R, C = _herm(N, 21), _sym(N, 22)
+    h = b.Bse(b.MODE_FULL, N, pack(R, 0), pack(C, 1))
+    X = gen.block_X(2 * N, k, 23)
+    assert relerr(to_host(h.apply(to_dev(X))), orc.apply_full(R, C, X)) <= TOL_APPLY
+    x = gen.block_X(N, k, 24)
+    for sign in (+1, -1):
+        assert relerr(to_host(h.apply_half(to_dev(x), sign)), orc.apply_half(R, C, x, sign)) <= TOL_APPLY
+
+
+def test_apply_host_entry_point(orc):
+    import paper_2504_10096_b200 as b
+    N, k = 320, 4
+    R = _herm(N, 31)
+    X = gen.block_X(N, k, 32)
+    h = b.Bse(b.MODE_TDA, N, pack(R, 0))
+    Y = h.apply_host(np.ascontiguousarray(X.T)).T
+    assert relerr(Y, orc.apply_tda(R, X)) <= TOL_APPLY
+
+
+def test_invalid_arguments():
+    import paper_2504_10096_b200 as b
+    with pytest.raises(b.BseError):
+        b.bse_layout(0)
+    N = 64
+    t = pack(np.eye(N, dtype=complex), 0)
+    with pytest.raises(b.BseError):
+        b.Bse(b.MODE_FULL, N, t, None)
+    h = b.Bse(b.MODE_TDA, N, t)
+    with pytest.raises(b.BseError):
+        h.apply_half(to_dev(np.ones((N, 1))), +1)      # half apply is full-mode only
