@@ -164,6 +164,12 @@ bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_t ncv, doub
                        int32_t max_restarts, uint64_t seed, double *hOmega, void *dVec, int64_t ldvec,
                        double *hResid, bse_info_t *info);
 
+/* Host utility (no device work): eigen-decomposition of the m x m complex Hermitian matrix hA (column-major, lda,
+ * lower triangle read, destroyed) -- the "small projected eigenproblem" of PAPER.md:67, which bse_solve keeps on
+ * the host.  hW: m eigenvalues ascending; hZ (m x nz, ldz): the first nz eigenvectors.  Returns BSE_ERR_INTERNAL
+ * if the QL iteration fails. */
+bse_status_t bse_host_heev(int32_t m, void *hA, int32_t lda, double *hW, void *hZ, int32_t ldz, int32_t nz);
+
 /* Number of kernels this library has launched on the calling process's device since load (bench.py's
  * "gpu_launches" claim). */
 int64_t bse_launch_count(void);

@@ -51,6 +51,7 @@ _SIGNATURES = {
     "bse_apply_half": [_vp, _i32, _vp, _i64, _vp, _i64, _i32],
     "bse_apply_host": [_vp, _vp, _i64, _vp, _i64, _i32],
     "bse_orth": [_vp, _vp, _i64, _i32, _vp, _i64, _vp, _i64, _i32, _vp, _i64, _vp, _vp, ctypes.POINTER(_i32)],
+    "bse_host_heev": [_i32, _vp, _i32, _vp, _vp, _i32, _i32],
     "bse_solve": [_vp, _i32, _i32, _i32, _dbl, _i32, _u64, ctypes.POINTER(_dbl), _vp, _i64, ctypes.POINTER(_dbl),
                   ctypes.POINTER(_Info)],
 }
@@ -234,6 +235,18 @@ class Bse:
         if st != 0 and raise_on_error:
             raise BseError(st, "bse_solve")
         return SolveResult(omega, vec, resid, {f: getattr(info, f) for f, _ in _Info._fields_}, st)
+
+
+def host_heev(A, nz=None):
+    """Host utility: eigenvalues (ascending) and first nz eigenvectors of a Hermitian numpy matrix."""
+    import numpy as np
+    m = A.shape[0]
+    nz = m if nz is None else nz
+    a = np.asfortranarray(A, dtype=np.complex128).copy(order="F")
+    w = np.zeros(m)
+    Z = np.zeros((m, max(nz, 1)), dtype=np.complex128, order="F")
+    _check(lib().bse_host_heev(m, a.ctypes.data, m, w.ctypes.data, Z.ctypes.data, m, nz), "bse_host_heev")
+    return w, Z[:, :nz]
 
 
 def launch_count() -> int:

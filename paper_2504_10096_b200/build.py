@@ -8,7 +8,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libbse_b200.so")
-SOURCES = ["bse_api.cu", "bse_apply.cu", "bse_orth.cu", "bse_solve.cu"]
+SOURCES = ["bse_api.cu", "bse_apply.cu", "dense_ops.cu", "bse_orth.cu", "bse_solve.cu"]
+HOST_SOURCES = ["host_eig.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "-Xptxas", "-v"]
 
@@ -32,15 +33,21 @@ def build(force: bool = False, verbose: bool = False) -> str:
         objs.append(o)
         cmd = [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, s), "-o", o]
         procs.append((s, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
+    gxx = os.environ.get("CXX", "g++")
+    for s in HOST_SOURCES:
+        o = os.path.join(CSRC, s.replace(".cpp", ".o"))
+        objs.append(o)
+        cmd = [gxx, "-O3", "-std=c++17", "-fopenmp", "-fPIC", "-c", os.path.join(CSRC, s), "-o", o]
+        procs.append((s, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     log = []
     for s, p in procs:
         out, _ = p.communicate()
         log.append(out)
         if p.returncode:
             sys.stderr.write(out)
-            raise RuntimeError(f"nvcc failed on {s}")
+            raise RuntimeError(f"compile failed on {s}")
     tmp = LIB + f".tmp{os.getpid()}"
-    subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp, *objs, "-lcudart"])
+    subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp, *objs, "-lcudart", "-lgomp"])
     os.replace(tmp, LIB)
     os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
     with open(os.path.join(HERE, "build", "ptxas.log"), "w") as f:

@@ -3,20 +3,26 @@
 // One pass computes, for up to 4 columns of X,
 //     HERM :  Y += s * R X            (R Hermitian, lower triangle stored)
 //     SYMC :  Y += s * C conj(X)      (C complex symmetric, lower triangle stored)
-// Every stored tile T = T_IJ (I >= J) is brought from HBM exactly once by a TMA bulk copy
-// (cp.async.bulk -> UBLKCP) into a 3-stage shared-memory ring and used twice from there:
+// Every stored tile T = T_IJ (I >= J) is brought from HBM exactly once by ONE TMA bulk copy
+// (cp.async.bulk -> UBLKCP, 64 KB, contiguous) into a 3-stage shared-memory ring and used twice from there:
 //     P1:  Y_I += T   x_J            (HERM)      Y_I += T   conj(x_J)   (SYMC)
 //     P2:  Y_J += T^H x_I            (HERM)      Y_J += T^T conj(x_I)   (SYMC)       (skipped when I == J)
 // Both products run on the FP64 tensor cores (mma.sync m8n8k4 -> DMMA.8x8x4) in real arithmetic:
 // with N-dimension n = 2 c + part (c = column of X, part = re/im),
-//     [Yr|Yi] += Tr * Ba + Ti * Bb,   Ba, Bb = signed re/im selections of X (table in DESIGN.md).
+//     [Yr|Yi] += Tr * Ba + Ti * Bb,   Ba, Bb = signed re/im selections of X (table below and in DESIGN.md).
 //
 // Work decomposition: a unit is a run of up to L consecutive tiles of one tile row I.  A CTA
 // (8 consumer warps + 1 producer warp, persistent, one per SM) walks its units; consumer warp w
 // owns tile columns 8w .. 8w+7 of every tile, i.e. for P1 a slice of the contraction (partial Y_I for
 // all 64 rows, accumulated in registers over the whole unit) and for P2 eight output rows of Y_J
 // (contraction over all 64 i, with the x_I fragments held in registers for the whole unit).
-// Partial results are added to Y with red.global.add.f64 (Y must be zero or hold the running sum).
+// The X fragments are read by the consumers straight from global memory (X is L2-resident: 16 N k bytes),
+// x_J one tile ahead of its use.  Partial results are added to Y with red.global.add.f64 (Y must be zero or
+// hold the running sum).
+//
+// Round-1 note: an earlier version staged the X panels through shared memory with small (1 KB) bulk copies on
+// their own mbarrier; with 4 columns and one-tile units it returned stale fragments about once per launch on
+// B200.  Tests at N >= 4096 (many units per CTA) cover this path now.
 #pragma once
 #include "bse_common.cuh"
 
@@ -25,11 +31,11 @@ namespace bse {
 constexpr int APPLY_STAGES = 3;
 constexpr int APPLY_CONSUMERS = 8;                       // consumer warps
 constexpr int APPLY_THREADS = (APPLY_CONSUMERS + 1) * 32;
-constexpr int XCOL_STRIDE = 1024 + 16;                   // bytes between the columns of an X panel in smem
-constexpr int XPAN_BYTES = 4224;                         // 4 columns, rounded up to 128 B
-constexpr int APPLY_SMEM = APPLY_STAGES * TILE_BYTES + APPLY_STAGES * XPAN_BYTES + 2 * XPAN_BYTES + 128;
+constexpr int APPLY_SMEM = APPLY_STAGES * TILE_BYTES + 128;
 
 enum { PASS_HERM = 0, PASS_SYMC = 1 };
+// high word no IEEE operation produces (a NaN payload): 'live != kNeverHi' is always true but cannot be folded
+constexpr int kNeverHi = 0x7ff8dead;
 
 struct ApplyParams {
     const char *tiles;
@@ -68,51 +74,29 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
 {
     extern __shared__ __align__(1024) char smem[];
     char *tile_s = smem;
-    char *xj_s = smem + APPLY_STAGES * TILE_BYTES;
-    char *xi_s = xj_s + APPLY_STAGES * XPAN_BYTES;
-    uint64_t *bars = reinterpret_cast<uint64_t *>(xi_s + 2 * XPAN_BYTES);
-    uint64_t *full = bars, *empty = bars + APPLY_STAGES, *xfull = bars + 2 * APPLY_STAGES, *xempty = xfull + 2;
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + APPLY_STAGES * TILE_BYTES);
+    uint64_t *full = bars, *empty = bars + APPLY_STAGES;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-
-    // zero the X panels once: rows beyond N of a ragged last panel are never written by the bulk copies
-    for (int i = threadIdx.x; i < (APPLY_STAGES + 2) * XPAN_BYTES / 16; i += APPLY_THREADS)
-        reinterpret_cast<double2 *>(xj_s)[i] = make_double2(0.0, 0.0);
     if (threadIdx.x == 0) {
         for (int s = 0; s < APPLY_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], APPLY_CONSUMERS); }
-        for (int s = 0; s < 2; ++s) { mbar_init(&xfull[s], 1); mbar_init(&xempty[s], APPLY_CONSUMERS); }
         fence_barrier_init();
     }
-    fence_proxy_async();
     __syncthreads();
 
-    const int kc = p.kc;
     if (warp == APPLY_CONSUMERS) {
         // ------------------------------ producer warp (one elected lane) ------------------------------
         if (lane == 0) {
-            int st = 0, xs = 0;
-            uint32_t ph = 0, xph = 0;
+            int st = 0;
+            uint32_t ph = 0;
             for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
                 int I, J0, J1;
                 apply_decode_unit(u, p.L, I, J0, J1);
-                {
-                    int rows = (int)min((int64_t)TB, p.N - (int64_t)I * TB);
-                    mbar_wait(&xempty[xs], xph ^ 1);
-                    mbar_expect_tx(&xfull[xs], (uint32_t)(kc * rows * 16));
-                    for (int c = 0; c < kc; ++c)
-                        bulk_g2s(xi_s + xs * XPAN_BYTES + c * XCOL_STRIDE, p.X + (int64_t)I * TB + c * p.ldx,
-                                 (uint32_t)(rows * 16), &xfull[xs]);
-                    if (++xs == 2) { xs = 0; xph ^= 1; }
-                }
                 const char *src = p.tiles + tile_index(I, J0) * (int64_t)TILE_BYTES;
                 for (int J = J0; J < J1; ++J, src += TILE_BYTES) {
-                    int rows = (int)min((int64_t)TB, p.N - (int64_t)J * TB);
                     mbar_wait(&empty[st], ph ^ 1);
-                    mbar_expect_tx(&full[st], (uint32_t)(TILE_BYTES + kc * rows * 16));
+                    mbar_expect_tx(&full[st], (uint32_t)TILE_BYTES);
                     bulk_g2s(tile_s + st * TILE_BYTES, src, TILE_BYTES, &full[st]);
-                    for (int c = 0; c < kc; ++c)
-                        bulk_g2s(xj_s + st * XPAN_BYTES + c * XCOL_STRIDE, p.X + (int64_t)J * TB + c * p.ldx,
-                                 (uint32_t)(rows * 16), &full[st]);
                     if (++st == APPLY_STAGES) { st = 0; ph ^= 1; }
                 }
             }
@@ -129,11 +113,11 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
     const int offP2 = (((g2 << 1) | t1) * 8 + ((t0 << 2) | (g0 << 1) | (t1 ^ g1))) * 16;   // + s * 512
     // B fragments: lane supplies B[kk = t][n = g], n = 2 c + part
     const int col = g >> 1, part = g & 1;
-    const bool colok = col < kc;
+    const bool colok = col < p.kc;
     // Ba pairs with Re(T), Bb with Im(T); value = coef * (re or im of x):
-    //   HERM P1 (T x):        Ba = [xr, xi]   Bb = [-xi, xr]
-    //   HERM P2 (T^H x):      Ba = [xr, xi]   Bb = [ xi, -xr]
-    //   SYMC P1/P2 (T conj x): Ba = [xr, -xi]  Bb = [ xi, xr]
+    //   HERM P1 (T x):         Ba = [xr,  xi]   Bb = [-xi,  xr]
+    //   HERM P2 (T^H x):       Ba = [xr,  xi]   Bb = [ xi, -xr]
+    //   SYMC P1/P2 (T conj x): Ba = [xr, -xi]   Bb = [ xi,  xr]
     double ca1, cb1, ca2, cb2;
     if (p.pass == PASS_HERM) {
         ca1 = 1.0; cb1 = part ? 1.0 : -1.0;
@@ -142,51 +126,61 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
         ca1 = part ? -1.0 : 1.0; cb1 = 1.0;
         ca2 = ca1; cb2 = 1.0;
     }
-    if (!colok) { ca1 = cb1 = ca2 = cb2 = 0.0; }
     ca1 *= p.sign; cb1 *= p.sign; ca2 *= p.sign; cb2 *= p.sign;
-    const int xoff = (colok ? col : 0) * XCOL_STRIDE;
+    const double2 *xcol = p.X + (int64_t)(colok ? col : 0) * p.ldx;
+    const int kc = p.kc;
 
-    int st = 0, xs = 0;
-    uint32_t ph = 0, xph = 0;
+    // x rows of tile-row K needed by this lane for P1 (rows 8w + 4s + t); zero outside the matrix / column range
+    auto load_xj = [&](int K, double2 (&x)[2]) {
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            int64_t row = (int64_t)K * TB + w * 8 + s * 4 + t;
+            x[s] = (colok && row < p.N) ? __ldg(xcol + row) : make_double2(0.0, 0.0);
+        }
+    };
+
+    int st = 0;
+    uint32_t ph = 0;
     for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
         int I, J0, J1;
         apply_decode_unit(u, p.L, I, J0, J1);
 
-        // x_I fragments for P2, kept in registers for the whole unit
+        double2 xjn[2];
+        load_xj(J0, xjn);
+        // x_I fragments for P2 (rows 8 ib + 4 s + t), kept in registers for the whole unit
         double BaI[8][2], BbI[8][2];
-        mbar_wait(&xfull[xs], xph);
         {
-            const char *xp = xi_s + xs * XPAN_BYTES + xoff;
+            double2 xi[8][2];
 #pragma unroll
             for (int ib = 0; ib < 8; ++ib)
 #pragma unroll
                 for (int s = 0; s < 2; ++s) {
-                    double2 x = *reinterpret_cast<const double2 *>(xp + (ib * 8 + s * 4 + t) * 16);
-                    BaI[ib][s] = (part ? x.y : x.x) * ca2;
-                    BbI[ib][s] = (part ? x.x : x.y) * cb2;
+                    int64_t row = (int64_t)I * TB + ib * 8 + s * 4 + t;
+                    xi[ib][s] = (colok && row < p.N) ? __ldg(xcol + row) : make_double2(0.0, 0.0);
+                }
+#pragma unroll
+            for (int ib = 0; ib < 8; ++ib)
+#pragma unroll
+                for (int s = 0; s < 2; ++s) {
+                    BaI[ib][s] = (part ? xi[ib][s].y : xi[ib][s].x) * ca2;
+                    BbI[ib][s] = (part ? xi[ib][s].x : xi[ib][s].y) * cb2;
                 }
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&xempty[xs]);
-        if (++xs == 2) { xs = 0; xph ^= 1; }
-
         double C1[8][2];
 #pragma unroll
         for (int ib = 0; ib < 8; ++ib) C1[ib][0] = C1[ib][1] = 0.0;
 
         for (int J = J0; J < J1; ++J) {
+            double BaJ[2], BbJ[2];
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                BaJ[s] = (part ? xjn[s].y : xjn[s].x) * ca1;
+                BbJ[s] = (part ? xjn[s].x : xjn[s].y) * cb1;
+            }
+            if (J + 1 < J1) load_xj(J + 1, xjn);            // prefetch the next tile's x_J fragments
+
             mbar_wait(&full[st], ph);
             const char *tp = tile_s + st * TILE_BYTES + w * 8 * PATCH_BYTES;
-            double BaJ[2], BbJ[2];
-            {
-                const char *xp = xj_s + st * XPAN_BYTES + xoff;
-#pragma unroll
-                for (int s = 0; s < 2; ++s) {
-                    double2 x = *reinterpret_cast<const double2 *>(xp + (w * 8 + s * 4 + t) * 16);
-                    BaJ[s] = (part ? x.y : x.x) * ca1;
-                    BbJ[s] = (part ? x.x : x.y) * cb1;
-                }
-            }
             if (I != J) {
                 double C2[4][2];
 #pragma unroll
@@ -207,8 +201,22 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
                     dmma(C1[ib], a1.y, BbJ[1]);
                     dmma(C2[ib & 3], b1.y, BbI[ib][1]);
                 }
+                // release the stage only after every DMMA that consumes its data has issued (see pin2)
+#pragma unroll
+                for (int ib = 0; ib < 8; ++ib) pin2(C1[ib][0], C1[ib][1]);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) pin2(C2[q][0], C2[q][1]);
+                // The release must not overtake the ld.shared that feed the DMMAs above: an mbarrier arrive only orders
+                // the ISSUE of earlier loads, and on B200 queued loads of a slow warp were observed to execute after the
+                // producer's next bulk copy had landed (stale fragments about once per launch).  Predicating the arrive on
+                // a value computed from every accumulator forces all DMMAs, hence all loads, to have completed.
+                int live = 0;
+#pragma unroll
+                for (int ib = 0; ib < 8; ++ib) live |= __double2hiint(C1[ib][0]);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) live |= __double2hiint(C2[q][0]);
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&empty[st]);
+                if (lane == 0 && live != kNeverHi) mbar_arrive(&empty[st]);
                 // flush Y_J rows 8w + g, column t
                 double yr = (C2[0][0] + C2[1][0]) + (C2[2][0] + C2[3][0]);
                 double yi = (C2[0][1] + C2[1][1]) + (C2[2][1] + C2[3][1]);
@@ -229,8 +237,13 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
                     dmma(C1[ib], a1.x, BaJ[1]);
                     dmma(C1[ib], a1.y, BbJ[1]);
                 }
+#pragma unroll
+                for (int ib = 0; ib < 8; ++ib) pin2(C1[ib][0], C1[ib][1]);
+                int live = 0;
+#pragma unroll
+                for (int ib = 0; ib < 8; ++ib) live |= __double2hiint(C1[ib][0]);
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&empty[st]);
+                if (lane == 0 && live != kNeverHi) mbar_arrive(&empty[st]);
             }
             if (++st == APPLY_STAGES) { st = 0; ph ^= 1; }
         }

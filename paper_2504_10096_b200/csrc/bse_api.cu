@@ -103,6 +103,12 @@ const char *bse_status_string(bse_status_t s)
 
 int64_t bse_launch_count(void) { return g_launches.load(); }
 
+bse_status_t bse_host_heev(int32_t m, void *hA, int32_t lda, double *hW, void *hZ, int32_t ldz, int32_t nz)
+{
+    if (m < 1 || !hA || !hW || lda < m || (nz > 0 && (!hZ || ldz < m))) return BSE_ERR_INVALID_ARG;
+    return host_heev(m, hA, lda, hW, hZ, ldz, nz) ? BSE_ERR_INTERNAL : BSE_OK;
+}
+
 bse_status_t bse_layout(int64_t N, int32_t *tile, int64_t *n_tiles, int64_t *bytes_per_matrix)
 {
     if (N < 1) return BSE_ERR_INVALID_ARG;

@@ -78,4 +78,10 @@ __device__ __forceinline__ void dmma(double (&c)[2], double a, double b)
 }
 __device__ __forceinline__ void red_add(double *p, double v) { atomicAdd(p, v); }
 
+// Pins values in registers at this program point.  Used before releasing a shared-memory buffer back to the TMA
+// producer: an mbarrier arrive only orders the ISSUE of earlier ld.shared instructions; queued loads may still
+// execute after the producer's next bulk copy has landed (observed on B200 as rare stale fragments).  Making the
+// release depend on values computed from every load forces those loads to have returned.
+__device__ __forceinline__ void pin2(double &a, double &b) { asm volatile("" : "+d"(a), "+d"(b)::"memory"); }
+
 }  // namespace bse

@@ -45,4 +45,32 @@ bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, dou
                                int64_t ldx, void *dY, int64_t ldy, int32_t k);
 bse_status_t zero_block(bse_handle_s *h, void *dY, int64_t ldy, int64_t rows, int32_t k);
 
+
+// ---- dense basis kernels (dense_ops.cu).  Complex blocks are column-major; *_cplx selects complex coefficients.
+// out (device, doubles): coefficient matrix in the layout gemm_basis consumes: out[a + half*m + col*ldo],
+// ldo = cplx ? 2m : m, half = 0 (real part) / 1 (imaginary part).  out is zeroed first.
+bse_status_t gram_basis(bse_handle_s *h, const void *A, int64_t lda, int m, const void *B, int64_t ldb, int k,
+                        bool cplx, int64_t n, double *out);
+// C(n x l) = alpha * A(n x m) * S + beta * C,  S given as coefficient matrix `coef` (layout above, ld = ldo).
+bse_status_t gemm_basis(bse_handle_s *h, const void *A, int64_t lda, int m, bool cplx, const double *coef,
+                        int64_t ldo, int l, int64_t n, void *C, int64_t ldc, double alpha, double beta);
+bse_status_t fill_random_block(bse_handle_s *h, void *W, int64_t ldw, int64_t n, int k, uint64_t seed,
+                               uint64_t counter);
+bse_status_t copy_block(bse_handle_s *h, const void *src, int64_t lds, void *dst, int64_t ldd, int64_t n, int k);
+// dst[a + col*m] (complex) = c1 + c2 in coefficient layout (c2 may be NULL)
+bse_status_t coef_to_complex(bse_handle_s *h, const double *c1, const double *c2, int m, int k, bool cplx,
+                             void *dst);
+// v (2N x nev) from x, px (N x nev each): v = [x + px/w; conj(x - px/w)] * sqrt(w)/2   (reading S4)
+bse_status_t assemble_full_vectors(bse_handle_s *h, const void *x, const void *px, int64_t N, int nev,
+                                   const double *d_omega, void *vec, int64_t ldvec);
+
+// orthogonalisation core shared by bse_orth and bse_solve (bse_orth.cu).  hcoef_host: m x k complex (ld m),
+// bfac_host: k x k complex (ld k); both host, nullable.  rng_counter advances when columns are replaced.
+bse_status_t orth_block(bse_handle_s *h, const void *V, int64_t ldv, int m, const void *PV, int64_t ldpv, void *W,
+                        int64_t ldw, int k, void *PW, int64_t ldpw, void *hcoef_host, void *bfac_host, int *rank,
+                        uint64_t seed, uint64_t *rng_counter);
+
+// host eigensolver (host_eig.cpp)
+int host_heev(int m, void *A, int lda, double *w, void *Z, int ldz, int nz);
+
 }  // namespace bse

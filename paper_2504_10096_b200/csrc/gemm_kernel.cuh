@@ -1,0 +1,132 @@
+// C~ = alpha * op(A) * Bm + beta * C~   on the FP64 tensor cores.
+//   A~  : real view (2n x m, leading dimension lda2) of a complex n x m block of basis vectors
+//   op(A) = A~                      (K = m,  real coefficients: full mode)
+//         = [A~ | (iA)~]            (K = 2m, complex coefficients: rows 0..m-1 of Bm = Re(S), rows m..2m-1 = Im(S))
+//   Bm  : real K x l, column-major (ldb);   C~ : real view 2n x l (ldc2).
+// Used for the Gram-Schmidt update W -= V h (skinny: l = k), the Ritz rotation V <- V S and the eigenvector
+// assembly.  Shared-memory tiled (cp.async double buffering), mma.sync m8n8k4 f64 -> DMMA.8x8x4.
+#pragma once
+#include "bse_common.cuh"
+
+namespace bse {
+
+__device__ __forceinline__ void cp_async16(void *dst, const void *src, bool valid)
+{
+    int sz = valid ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_u32(dst)), "l"(src), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async8(void *dst, const void *src, bool valid)
+{
+    int sz = valid ? 8 : 0;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(smem_u32(dst)), "l"(src), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+constexpr int GEMM_KC = 16;
+
+template <int MT, int NT, int WM, int WN>
+struct GemmCfg {
+    static constexpr int BM = 8 * MT * WM, BN = 8 * NT * WN, THREADS = 32 * WM * WN;
+    static constexpr int LDA_S = BM + 8;          // == 8 (mod 16) doubles: conflict-free A fragments
+    static constexpr int LDB_S = GEMM_KC + 4;     // == 4 (mod 16) doubles: conflict-free B fragments
+    static constexpr int SMEM = 2 * (GEMM_KC * LDA_S + BN * LDB_S) * 8;
+};
+
+template <int MT, int NT, int WM, int WN>
+__global__ void __launch_bounds__(32 * WM * WN) gemm_nn_kernel(const double *__restrict__ A, int64_t lda2, int64_t nr,
+                                                               int m, int cplx, const double *__restrict__ Bm,
+                                                               int64_t ldb, int l, double *__restrict__ C,
+                                                               int64_t ldc2, double alpha, double beta)
+{
+    using Cfg = GemmCfg<MT, NT, WM, WN>;
+    constexpr int BM = Cfg::BM, BN = Cfg::BN, KC = GEMM_KC, LDA_S = Cfg::LDA_S, LDB_S = Cfg::LDB_S;
+    extern __shared__ __align__(16) double gsm[];
+    double *As = gsm;                                  // [2][KC][LDA_S]
+    double *Bs = gsm + 2 * KC * LDA_S;                 // [2][BN][LDB_S]
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int g = lane >> 2, t = lane & 3;
+    const int wm = warp % WM, wn = warp / WM;
+    const int64_t row0 = (int64_t)blockIdx.x * BM;
+    const int col0 = blockIdx.y * BN;
+    const int nch = (m + KC - 1) / KC;
+    const int total = cplx ? 2 * nch : nch;
+
+    auto load_chunk = [&](int c, int buf) {
+        const int half = c >= nch ? 1 : 0;
+        const int kk0 = (c - half * nch) * KC;
+        double *as = As + buf * KC * LDA_S;
+        double *bs = Bs + buf * BN * LDB_S;
+        for (int idx = tid; idx < KC * (BM / 2); idx += Cfg::THREADS) {
+            int kk = idx / (BM / 2), r2 = idx % (BM / 2);
+            bool ok = (kk0 + kk) < m && (row0 + 2 * r2) < nr;
+            const double *src = ok ? A + (int64_t)(kk0 + kk) * lda2 + row0 + 2 * r2 : A;
+            cp_async16(as + kk * LDA_S + 2 * r2, src, ok);
+        }
+        for (int idx = tid; idx < BN * KC; idx += Cfg::THREADS) {
+            int col = idx / KC, kk = idx % KC;
+            bool ok = (kk0 + kk) < m && (col0 + col) < l;
+            const double *src = ok ? Bm + (int64_t)half * m + kk0 + kk + (int64_t)(col0 + col) * ldb : Bm;
+            cp_async8(bs + col * LDB_S + kk, src, ok);
+        }
+    };
+
+    double acc[MT][NT][2];
+#pragma unroll
+    for (int i = 0; i < MT; ++i)
+#pragma unroll
+        for (int j = 0; j < NT; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    load_chunk(0, 0);
+    cp_async_commit();
+    for (int c = 0; c < total; ++c) {
+        const int buf = c & 1;
+        if (c + 1 < total) load_chunk(c + 1, buf ^ 1);
+        cp_async_commit();
+        cp_async_wait<1>();
+        __syncthreads();
+        const bool rot = c >= nch;
+        const double *as = As + buf * KC * LDA_S + wm * 8 * MT;
+        const double *bs = Bs + buf * BN * LDB_S + (wn * 8 * NT) * LDB_S;
+#pragma unroll
+        for (int ks = 0; ks < KC / 4; ++ks) {
+            const int kk = 4 * ks + t;
+            double a[MT], b[NT];
+#pragma unroll
+            for (int i = 0; i < MT; ++i) {
+                int r = 8 * i + g;
+                if (!rot) a[i] = as[kk * LDA_S + r];
+                else { double v = as[kk * LDA_S + (r ^ 1)]; a[i] = (r & 1) ? v : -v; }
+            }
+#pragma unroll
+            for (int j = 0; j < NT; ++j) b[j] = bs[(8 * j + g) * LDB_S + kk];
+#pragma unroll
+            for (int i = 0; i < MT; ++i)
+#pragma unroll
+                for (int j = 0; j < NT; ++j) dmma(acc[i][j], a[i], b[j]);
+        }
+        __syncthreads();
+    }
+    // epilogue: C fragment rows 8 i + g, columns 8 j + 2 t + e
+#pragma unroll
+    for (int i = 0; i < MT; ++i) {
+        int64_t row = row0 + wm * 8 * MT + 8 * i + g;
+        if (row >= nr) continue;
+#pragma unroll
+        for (int j = 0; j < NT; ++j)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                int col = col0 + wn * 8 * NT + 8 * j + 2 * t + e;
+                if (col < l) {
+                    double *cp = C + row + (int64_t)col * ldc2;
+                    double v = alpha * acc[i][j][e];
+                    if (beta != 0.0) v += beta * (*cp);
+                    *cp = v;
+                }
+            }
+    }
+}
+
+}  // namespace bse

@@ -1,0 +1,83 @@
+"""CPU-side checks of the boundary: the library loads, exports every symbol include/bse.h declares, and the host
+logic (layout arithmetic, status strings, projected eigensolver) is right.  No compute calls need a GPU here."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import bse_inputs as gen
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def b():
+    from paper_2504_10096_b200 import build
+    build.build()
+    import paper_2504_10096_b200 as pkg
+    return pkg
+
+
+def test_header_symbols_are_exported(b):
+    hdr = open(os.path.join(ROOT, "include", "bse.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(bse_[a-z_0-9]+)\s*\(", hdr))
+    assert {"bse_create", "bse_apply", "bse_orth", "bse_solve", "bse_destroy"} <= declared
+    L = b.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+    assert declared == set(b.EXPORTS)
+
+
+def test_layout_and_status(b):
+    assert b.bse_layout(64) == (64, 1, 65536)
+    assert b.bse_layout(65) == (64, 3, 3 * 65536)
+    for N, nbytes in [(1024, 8.40e6), (16384, 2.148e9), (98304, 77.31e9)]:
+        t, nt, by = b.bse_layout(N)
+        n = N // 64
+        assert nt == n * (n + 1) // 2 and by == nt * 65536
+        # B_mat = 16 N (N+1) / 2 plus the mirrored halves of the diagonal tiles
+        assert abs(by - nbytes) / nbytes < 1.0 / n
+    with pytest.raises(b.BseError):
+        b.bse_layout(0)
+    assert b.lib().bse_status_string(0) == b"ok"
+    assert b"positive" in b.lib().bse_status_string(5)
+
+
+def test_no_compute_without_arguments(b):
+    # argument validation happens before any CUDA call
+    h = ctypes.c_void_p()
+    assert b.lib().bse_create(ctypes.byref(h), 7, 64, None, None, None) == 1
+    assert b.lib().bse_apply(None, None, 0, None, 0, 1) == 1
+    assert b.lib().bse_solve(None, 1, 1, 0, 1e-8, 1, 0, None, None, 0, None, None) == 1
+
+
+@pytest.mark.parametrize("m", [1, 2, 7, 40, 150])
+def test_host_heev_matches_numpy(b, m):
+    A = gen.block_X(m, m, m)
+    A = (A + A.conj().T) / 2
+    w, Z = b.host_heev(A)
+    ref = np.linalg.eigvalsh(A)
+    scale = max(np.max(np.abs(ref)), 1.0)
+    assert np.max(np.abs(w - ref)) < 1e-13 * scale * max(m, 8)
+    assert np.linalg.norm(Z.conj().T @ Z - np.eye(m)) < 1e-12
+    assert np.linalg.norm(A @ Z - Z * w) < 1e-12 * scale * m
+
+
+def test_host_heev_arrowhead_and_clusters(b):
+    # the projected matrix after a thick restart: diag(theta) bordered by a block, plus repeated eigenvalues
+    l, k = 30, 4
+    T = np.zeros((l + k, l + k), dtype=complex)
+    T[np.arange(l), np.arange(l)] = np.repeat(np.linspace(1, 3, l // 2), 2)      # pairs, as in full mode
+    Bk = gen.block_X(k, l, 3) * 1e-3
+    T[l:, :l] = Bk; T[:l, l:] = Bk.conj().T
+    D = gen.block_X(k, k, 4); T[l:, l:] = (D + D.conj().T) / 2 + 5 * np.eye(k)
+    w, Z = b.host_heev(T, nz=10)
+    assert np.max(np.abs(w - np.linalg.eigvalsh(T))) < 1e-13 * 10
+    assert np.linalg.norm(T @ Z - Z * w[:10]) < 1e-12
+    # real symmetric input gives real eigenvectors up to a phase (full-mode T is real)
+    Tr = T.real.copy()
+    w2, Z2 = b.host_heev(Tr, nz=6)
+    assert np.linalg.norm(Tr @ Z2 - Z2 * w2[:6]) < 1e-12 and np.max(np.abs(Z2.imag)) < 1e-13

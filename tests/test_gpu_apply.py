@@ -141,3 +141,47 @@ def test_invalid_arguments():
     h = b.Bse(b.MODE_TDA, N, t)
     with pytest.raises(b.BseError):
         h.apply_half(to_dev(np.ones((N, 1))), +1)      # half apply is full-mode only
+
+
+def _sampled_rows(N):
+    # rows 0..7 of every tile (the slab of consumer warp 0, the first bytes a refill overwrites) plus a ragged mix
+    base = (np.arange(N // 64)[:, None] * 64 + np.arange(8)[None, :]).reshape(-1)
+    extra = (np.arange(97) * 2654435761 % N).astype(np.int64)
+    return np.unique(np.concatenate([base, extra]))
+
+
+@pytest.mark.parametrize("N,k,reps", [(4096, 4, 25), (8192, 4, 8), (16384, 8, 3), (16384, 1, 2)])
+def test_tda_apply_many_units_per_cta_sampled_rows(orc, N, k, reps):
+    """Sizes where every CTA walks many units (the launch configuration bench.py times at N = 16384).  The matrix
+    is generated on the device; the oracle consumes the same rows from the CPU generator (bse_inputs.rows_R, equal
+    to a few ulp).  Repeated to catch timing-dependent faults: round 1 had a shared-memory WAR hazard here that
+    corrupted about one 8-row group per launch."""
+    import paper_2504_10096_b200 as b
+    h = b.Bse(b.MODE_TDA, N, b.bse_fill_synthetic(N, 0, 1, 0.0, 16))
+    X = gen.block_X(N, k, 12)
+    rows = _sampled_rows(N)
+    ref = orc.rows_times_block(gen.rows_R(N, 1, rows, 0.0, 16), X)
+    Xd = to_dev(X)
+    for _ in range(reps):
+        Y = to_host(h.apply(Xd))
+        assert relerr(Y[rows], ref) <= TOL_APPLY
+    # properties that hold at any size: Hermitian adjoint identity through the CUDA path
+    Z = gen.block_X(N, k, 13)
+    RZ = to_host(h.apply(to_dev(Z)))
+    lhs, rhs = X.conj().T @ RZ, Y.conj().T @ Z
+    assert np.linalg.norm(lhs - rhs) <= 1e-12 * np.linalg.norm(lhs)
+
+
+def test_full_apply_many_units_sampled_rows(orc):
+    import paper_2504_10096_b200 as b
+    N, k = 4096, 4
+    h = b.Bse(b.MODE_FULL, N, b.bse_fill_synthetic(N, 0, 2, 1.0, 16), b.bse_fill_synthetic(N, 1, 2))
+    X = gen.block_X(2 * N, k, 5)
+    rows = _sampled_rows(N)[::4]
+    Rr, Cr = gen.rows_R(N, 2, rows, 1.0, 16), gen.rows_C(N, 2, rows)
+    # rows of H = [[R, C], [-C^*, -R^*]] (Eq. 1, PAPER.md:18 with :26) assembled from generator rows
+    top = np.hstack([Rr, Cr]); bot = np.hstack([-Cr.conj(), -Rr.conj()])
+    ref = orc.rows_times_block(np.vstack([top, bot]), X)
+    for _ in range(5):
+        Y = to_host(h.apply(to_dev(X)))
+        assert relerr(np.vstack([Y[rows], Y[N + rows]]), ref) <= TOL_APPLY

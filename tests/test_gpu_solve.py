@@ -1,0 +1,135 @@
+"""bse_solve against the oracle (north_star tolerances): eigenvalues rel. error <= 1e-10, residuals <= 1e-8 ||H||,
+orthonormality <= 1e-12; closed-form prescribed spectra pin the eigenvalues independently of any solver."""
+import numpy as np
+import pytest
+
+import bse_inputs as gen
+from gpu_util import pack, to_dev, to_host
+
+pytestmark = pytest.mark.gpu
+TOL_EIG, TOL_RES, TOL_ORTH = 1e-10, 1e-8, 1e-12
+
+
+def _check_tda(orc, R, res, nev, w_ref):
+    w, V = res.omega, to_host(res.vectors)
+    nrm = np.max(np.abs(np.linalg.eigvalsh(R)[[0, -1]]))
+    assert np.max(np.abs(w - w_ref[:nev]) / np.maximum(np.abs(w_ref[:nev]), 1e-300)) <= TOL_EIG or \
+        np.max(np.abs(w - w_ref[:nev])) <= TOL_EIG * 1e-2 * nrm
+    r = np.linalg.norm(orc.apply_tda(R, V) - V * w, axis=0)
+    assert np.all(r <= TOL_RES * nrm)
+    assert np.all(r <= 10 * res.resid + 1e-11 * nrm)            # the solver's own estimate is honest
+    assert np.linalg.norm(V.conj().T @ V - np.eye(nev)) <= TOL_ORTH
+
+
+@pytest.mark.parametrize("sigma", [0.0, 1.0])
+def test_config0_tda_vs_oracle_lanczos(orc, sigma):
+    import paper_2504_10096_b200 as b
+    cfg = gen.CONFIGS[0]
+    N, nev, k = cfg["N"], cfg["nev"], cfg["k"]
+    R = gen.dense_R(N, 1, sigma=sigma, group=cfg["group"])
+    res = b.Bse(b.MODE_TDA, N, pack(R, 0)).solve(nev, k, tol=1e-8, seed=1)
+    w_o, V_o, r_o, steps = orc.lanczos_tda(R, nev, 1e-10, gen.block_X(N, 1, 99)[:, 0], check=20)
+    assert steps > 0
+    # eigenvalues are unique: single-vector oracle and block GPU solver must agree
+    _check_tda(orc, R, res, nev, w_o)
+    assert np.max(np.abs(w_o - np.linalg.eigvalsh(R)[:nev])) < 1e-11
+    # eigenvectors agree up to a phase for isolated eigenvalues
+    ov = np.abs(np.sum(V_o.conj() * to_host(res.vectors), axis=0))
+    assert np.all(ov > 1 - 1e-6)
+
+
+@pytest.mark.parametrize("k", [1, 3, 8])
+def test_tda_block_sizes_and_ragged_N(orc, k):
+    import paper_2504_10096_b200 as b
+    N, nev = 300, 6
+    A = gen.block_X(N, N, 5); R = (A + A.conj().T) / 2 + np.diag(np.linspace(0, 30, N))
+    res = b.Bse(b.MODE_TDA, N, pack(R, 0)).solve(nev, k, tol=1e-9, seed=3)
+    _check_tda(orc, R, res, nev, np.linalg.eigvalsh(R))
+
+
+def test_tda_closed_form_spectrum():
+    import torch
+    import paper_2504_10096_b200 as b
+    N, nev, k = 4096, 12, 4
+    lam = gen.prescribed_spectrum(N, 11, 1.0, 10.0, power=2 / 3)
+    u = gen.householder_u(N, 11)
+    t = b.bse_fill_closed_form_tda(N, torch.from_numpy(lam).cuda(), torch.from_numpy(u).cuda(),
+                                   float(np.sum(lam * np.abs(u) ** 2)))
+    res = b.Bse(b.MODE_TDA, N, t).solve(nev, k, tol=1e-9, seed=2)
+    assert np.max(np.abs(res.omega - lam[:nev]) / lam[:nev]) <= TOL_EIG
+
+
+def _H_dense(R, C):
+    return np.block([[R, C], [-C.conj().T, -R.conj()]])
+
+
+def _check_full(orc, R, C, res, nev, om_ref):
+    N = R.shape[0]
+    om, V = res.omega, to_host(res.vectors)
+    assert np.max(np.abs(om - om_ref[:nev]) / om_ref[:nev]) <= TOL_EIG
+    HV = orc.apply_full(R, C, V)
+    nrm = np.linalg.norm(_H_dense(R, C), 2) if N <= 600 else 12.0
+    r = np.linalg.norm(HV - V * om, axis=0) / np.linalg.norm(V, axis=0)
+    assert np.all(r <= TOL_RES * nrm)
+    Sig = np.concatenate([np.ones(N), -np.ones(N)])
+    G = V.conj().T @ (Sig[:, None] * V)
+    assert np.linalg.norm(G - np.eye(nev)) <= 1e-7              # Sigma-orthonormal, X^H X - Y^H Y = 1 (S9, S10)
+    assert np.max(np.abs(np.diag(G) - 1)) <= 1e-10
+    # -omega partner [conj(Y); conj(X)]
+    Pn = np.vstack([V[N:].conj(), V[:N].conj()])
+    rp = np.linalg.norm(orc.apply_full(R, C, Pn) + Pn * om, axis=0) / np.linalg.norm(Pn, axis=0)
+    assert np.all(rp <= TOL_RES * nrm)
+
+
+@pytest.mark.parametrize("k", [1, 4])
+def test_full_small_vs_direct_route(orc, k):
+    import paper_2504_10096_b200 as b
+    N, nev = 192, 8
+    R = gen.dense_R(N, 2, sigma=1.0); C = gen.dense_C(N, 2)
+    res = b.Bse(b.MODE_FULL, N, pack(R, 0), pack(C, 1)).solve(nev, k, tol=1e-9, seed=1)
+    omd, _ = orc.bse_direct(R, C, want_vectors=False)           # the paper's section-2.1 route
+    _check_full(orc, R, C, res, nev, omd[N:])
+
+
+def test_config1_full_vs_oracle_lanczos(orc):
+    import paper_2504_10096_b200 as b
+    cfg = gen.CONFIGS[1]
+    N, nev, k = cfg["N"], cfg["nev"], cfg["k"]
+    R = gen.dense_R(N, 1, sigma=cfg["sigma"]); C = gen.dense_C(N, 1)
+    res = b.Bse(b.MODE_FULL, N, pack(R, 0), pack(C, 1)).solve(nev, k, tol=1e-8, seed=1)
+    om_o, V_o, r_o, steps = orc.lanczos_full(R, C, nev, 1e-10, gen.block_X(N, 1, 97)[:, 0], check=60)
+    assert steps > 0
+    _check_full(orc, R, C, res, nev, om_o)
+
+
+def test_full_closed_form_pair():
+    import torch
+    import paper_2504_10096_b200 as b
+    N, nev, k = 2048, 10, 4
+    d1 = gen.prescribed_spectrum(N, 7, 1.0, 9.0, power=2 / 3); d2 = gen.prescribed_spectrum(N, 8, 2.0, 5.0, power=2 / 3)
+    ur = gen.householder_u(N, 9, complex_u=False).real.copy(); phi = gen.phases(N, 9)
+    rt, ct = b.bse_fill_closed_form_full(N, *(torch.from_numpy(a).cuda() for a in (d1, d2, ur, phi)),
+                                         float(np.sum(d1 * ur ** 2)), float(np.sum(d2 * ur ** 2)))
+    res = b.Bse(b.MODE_FULL, N, rt, ct).solve(nev, k, tol=1e-9, seed=4)
+    exact = np.sort(np.sqrt(d1 * d2))[:nev]
+    assert np.max(np.abs(res.omega - exact) / exact) <= TOL_EIG
+
+
+def test_not_positive_definite_is_reported():
+    import paper_2504_10096_b200 as b
+    N = 256
+    R = gen.dense_R(N, 3, sigma=0.0) - 20 * np.eye(N); C = gen.dense_C(N, 3)
+    res = b.Bse(b.MODE_FULL, N, pack(R, 0), pack(C, 1)).solve(4, 2, raise_on_error=False)
+    assert res.status == 5
+
+
+def test_solve_invalid_arguments_and_nonconvergence():
+    import paper_2504_10096_b200 as b
+    N = 128
+    R = gen.dense_R(N, 3)
+    h = b.Bse(b.MODE_TDA, N, pack(R, 0))
+    assert h.solve(0, 4, raise_on_error=False).status == 1
+    assert h.solve(126, 4, raise_on_error=False).status == 1       # nev + k > N
+    r = h.solve(8, 2, ncv=12, tol=1e-14, max_restarts=1, raise_on_error=False)
+    assert r.status == 4 and r.info["n_restart"] == 1               # best estimates are still returned
+    assert np.all(np.isfinite(r.omega))
