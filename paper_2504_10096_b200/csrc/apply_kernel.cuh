@@ -34,8 +34,6 @@ constexpr int APPLY_THREADS = (APPLY_CONSUMERS + 1) * 32;
 constexpr int APPLY_SMEM = APPLY_STAGES * TILE_BYTES + 128;
 
 enum { PASS_HERM = 0, PASS_SYMC = 1 };
-// high word no IEEE operation produces (a NaN payload): 'live != kNeverHi' is always true but cannot be folded
-constexpr int kNeverHi = 0x7ff8dead;
 
 struct ApplyParams {
     const char *tiles;
@@ -50,6 +48,7 @@ struct ApplyParams {
     double sign;        // s
     int L;              // unit length in tiles
     int64_t n_units;
+    int zero;           // always 0; a runtime value the assembler cannot fold (see the stage release below)
 };
 
 __host__ __device__ __forceinline__ int64_t apply_num_units(int nt, int L)
@@ -208,15 +207,17 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
                 for (int q = 0; q < 4; ++q) pin2(C2[q][0], C2[q][1]);
                 // The release must not overtake the ld.shared that feed the DMMAs above: an mbarrier arrive only orders
                 // the ISSUE of earlier loads, and on B200 queued loads of a slow warp were observed to execute after the
-                // producer's next bulk copy had landed (stale fragments about once per launch).  Predicating the arrive on
-                // a value computed from every accumulator forces all DMMAs, hence all loads, to have completed.
+                // producer's next bulk copy had landed (stale fragments about once per launch).  The barrier address is
+                // therefore made to depend on every accumulator (live & p.zero == 0, but not foldable): all DMMAs,
+                // hence all loads, have completed before the arrive can issue.
                 int live = 0;
 #pragma unroll
                 for (int ib = 0; ib < 8; ++ib) live |= __double2hiint(C1[ib][0]);
 #pragma unroll
                 for (int q = 0; q < 4; ++q) live |= __double2hiint(C2[q][0]);
                 __syncwarp();
-                if (lane == 0 && live != kNeverHi) mbar_arrive(&empty[st]);
+                if (lane == 0)
+                    mbar_arrive(reinterpret_cast<uint64_t *>(reinterpret_cast<char *>(&empty[st]) + (live & p.zero)));
                 // flush Y_J rows 8w + g, column t
                 double yr = (C2[0][0] + C2[1][0]) + (C2[2][0] + C2[3][0]);
                 double yi = (C2[0][1] + C2[1][1]) + (C2[2][1] + C2[3][1]);
@@ -243,7 +244,8 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
 #pragma unroll
                 for (int ib = 0; ib < 8; ++ib) live |= __double2hiint(C1[ib][0]);
                 __syncwarp();
-                if (lane == 0 && live != kNeverHi) mbar_arrive(&empty[st]);
+                if (lane == 0)
+                    mbar_arrive(reinterpret_cast<uint64_t *>(reinterpret_cast<char *>(&empty[st]) + (live & p.zero)));
             }
             if (++st == APPLY_STAGES) { st = 0; ph ^= 1; }
         }

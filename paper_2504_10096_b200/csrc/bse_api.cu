@@ -70,6 +70,7 @@ bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, dou
     if (const char *e = getenv("BSE_APPLY_UNIT")) { int v = atoi(e); if (v >= 1 && v <= 4096) L = v; }
     p.L = (int)L;
     p.n_units = apply_num_units(h->nt, p.L);
+    p.zero = 0;
     int grid = (int)(p.n_units < h->num_sms ? p.n_units : h->num_sms);
     for (int32_t c0 = 0; c0 < k; c0 += 4) {
         p.kc = (k - c0) < 4 ? (k - c0) : 4;

@@ -70,6 +70,15 @@ bse_status_t orth_block(bse_handle_s *h, const void *V, int64_t ldv, int m, cons
                         int64_t ldw, int k, void *PW, int64_t ldpw, void *hcoef_host, void *bfac_host, int *rank,
                         uint64_t seed, uint64_t *rng_counter);
 
+// the two halves of orth_block, for callers that recompute P(W) between projection and normalisation
+bse_status_t project_block(bse_handle_s *h, const void *V, int64_t ldv, int m, const void *PV, int64_t ldpv, void *W,
+                           int64_t ldw, int k, void *PW, int64_t ldpw, bool cplx, void *hcoef_host);
+bse_status_t block_norm_scale(bse_handle_s *h, const void *W, int64_t ldw, const void *PW, int64_t ldpw, int k,
+                              bool cplx, double *scale2);
+bse_status_t normalize_block(bse_handle_s *h, const void *V, int64_t ldv, int m, const void *PV, int64_t ldpv, void *W,
+                             int64_t ldw, int k, void *PW, int64_t ldpw, bool cplx, double scale2, void *hcoef_host,
+                             void *bfac_host, int *rank_out, uint64_t seed, uint64_t *rng_counter);
+
 // host eigensolver (host_eig.cpp)
 int host_heev(int m, void *A, int lda, double *w, void *Z, int ldz, int nz);
 

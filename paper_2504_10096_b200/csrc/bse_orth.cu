@@ -131,41 +131,76 @@ static bse_status_t project_pass(bse_handle_s *h, const void *V, int64_t ldv, co
     const int ldo = cplx ? 2 * m : m;
     ST(gram_basis(h, cplx ? V : PV, cplx ? ldv : ldpv, m, W, ldw, kc, cplx, n, coef));
     ST(gemm_basis(h, V, ldv, m, cplx, coef, ldo, kc, n, W, ldw, -1.0, 1.0));
-    if (!cplx) ST(gemm_basis(h, PV, ldpv, m, false, coef, ldo, kc, n, PW, ldpw, -1.0, 1.0));
+    if (!cplx && PW) ST(gemm_basis(h, PV, ldpv, m, false, coef, ldo, kc, n, PW, ldpw, -1.0, 1.0));
     return BSE_OK;
 }
 
-bse_status_t orth_block(bse_handle_s *h, const void *V, int64_t ldv, int m, const void *PV, int64_t ldpv, void *W,
-                        int64_t ldw, int k, void *PW, int64_t ldpw, void *hcoef_host, void *bfac_host, int *rank_out,
-                        uint64_t seed, uint64_t *rng_counter)
+// Euclidean squared column norms of a block (max over columns), used as the scale of rank decisions when the
+// P-image of the block is not available yet.
+static bse_status_t euclid_max_norm2(bse_handle_s *h, const void *W, int64_t ldw, int k, OrthWs &w, double *out)
 {
-    const int64_t n = h->N;
-    const bool cplx = (PV == nullptr);
+    std::vector<zc> G;
+    ST(block_gram(h, W, ldw, nullptr, 0, k, true, w, G));
+    double m2 = 0.0;
+    for (int j = 0; j < k; ++j) m2 = std::max(m2, G[j + (size_t)j * k].real());
+    *out = m2;
+    return BSE_OK;
+}
+
+// Block CGS, two passes against V (a5 + a6, twice).  PW may be NULL in the real inner product: then only W is
+// updated and the caller recomputes P(W) afterwards (what bse_solve does: updating PW by linear combination lets
+// PW drift away from P(W) exponentially over the iteration).
+bse_status_t project_block(bse_handle_s *h, const void *V, int64_t ldv, int m, const void *PV, int64_t ldpv, void *W,
+                           int64_t ldw, int k, void *PW, int64_t ldpw, bool cplx, void *hcoef_host)
+{
+    if (m <= 0) return BSE_OK;
     OrthWs w;
     ST(orth_ws(h, m, k, w));
-    std::vector<zc> G, Hc((size_t)(m > 0 ? m : 1) * k, zc(0.0)), B((size_t)k * k, zc(0.0));
-    char *Wc = (char *)W, *PWc = (char *)PW;
+    std::vector<zc> Hc((size_t)m * k, zc(0.0));
+    ST(project_pass(h, V, ldv, PV, ldpv, m, W, ldw, PW, ldpw, k, cplx, w.c1));
+    ST(project_pass(h, V, ldv, PV, ldpv, m, W, ldw, PW, ldpw, k, cplx, w.c2));
+    size_t bytes = (size_t)(cplx ? 2 * m : m) * k * 8;
+    BSE_CUDA(cudaMemcpyAsync(w.hc1, w.c1, bytes, cudaMemcpyDeviceToHost, h->stream));
+    BSE_CUDA(cudaMemcpyAsync(w.hc2, w.c2, bytes, cudaMemcpyDeviceToHost, h->stream));
+    BSE_CUDA(cudaStreamSynchronize(h->stream));
+    coef_to_host(w.hc1, m, k, cplx, Hc.data(), false);      // h = h1 + h2
+    coef_to_host(w.hc2, m, k, cplx, Hc.data(), true);
+    if (hcoef_host) std::memcpy(hcoef_host, Hc.data(), sizeof(zc) * (size_t)m * k);
+    return BSE_OK;
+}
 
-    // norms of the incoming block in the active inner product (threshold for rank decisions)
+bse_status_t block_norm_scale(bse_handle_s *h, const void *W, int64_t ldw, const void *PW, int64_t ldpw, int k,
+                              bool cplx, double *scale2)
+{
+    OrthWs w;
+    ST(orth_ws(h, 0, k, w));
+    if (!cplx && !PW) return euclid_max_norm2(h, W, ldw, k, w, scale2);
+    std::vector<zc> G;
     ST(block_gram(h, W, ldw, PW, ldpw, k, cplx, w, G));
-    double scale2 = 0.0, gmax = 0.0;
-    for (int j = 0; j < k; ++j) scale2 = std::max(scale2, G[j + (size_t)j * k].real());
+    double s2 = 0.0, gmax = 0.0;
+    for (int j = 0; j < k; ++j) s2 = std::max(s2, G[j + (size_t)j * k].real());
     for (auto &v : G) gmax = std::max(gmax, std::abs(v));
     if (!cplx)
         for (int j = 0; j < k; ++j)
             if (G[j + (size_t)j * k].real() < -1e-10 * gmax) return BSE_ERR_NOT_POSITIVE_DEFINITE;
+    *scale2 = s2;
+    return BSE_OK;
+}
 
-    // ---- block CGS, two passes against V (a5 + a6, twice)
-    if (m > 0) {
-        ST(project_pass(h, V, ldv, PV, ldpv, m, W, ldw, PW, ldpw, k, cplx, w.c1));
-        ST(project_pass(h, V, ldv, PV, ldpv, m, W, ldw, PW, ldpw, k, cplx, w.c2));
-        size_t bytes = (size_t)(cplx ? 2 * m : m) * k * 8;
-        BSE_CUDA(cudaMemcpyAsync(w.hc1, w.c1, bytes, cudaMemcpyDeviceToHost, h->stream));
-        BSE_CUDA(cudaMemcpyAsync(w.hc2, w.c2, bytes, cudaMemcpyDeviceToHost, h->stream));
-        BSE_CUDA(cudaStreamSynchronize(h->stream));
-        coef_to_host(w.hc1, m, k, cplx, Hc.data(), false);      // h = h1 + h2
-        coef_to_host(w.hc2, m, k, cplx, Hc.data(), true);
-    }
+// Intra-block orthonormalisation (a7) of a block already projected against V.  scale2: squared norm scale of the
+// block BEFORE projection in the active inner product (rank decisions are relative to it); hcoef_host (m x k, may
+// be NULL) receives the corrections of the column-wise path.
+bse_status_t normalize_block(bse_handle_s *h, const void *V, int64_t ldv, int m, const void *PV, int64_t ldpv, void *W,
+                             int64_t ldw, int k, void *PW, int64_t ldpw, bool cplx, double scale2, void *hcoef_host,
+                             void *bfac_host, int *rank_out, uint64_t seed, uint64_t *rng_counter)
+{
+    const int64_t n = h->N;
+    OrthWs w;
+    ST(orth_ws(h, m, k, w));
+    std::vector<zc> G, Hc((size_t)(m > 0 ? m : 1) * k, zc(0.0)), B((size_t)k * k, zc(0.0));
+    if (hcoef_host && m > 0) std::memcpy(Hc.data(), hcoef_host, sizeof(zc) * (size_t)m * k);
+    char *Wc = (char *)W, *PWc = (char *)PW;
+    double gmax = scale2;
 
     // ---- intra-block orthonormalisation (a7): CholQR2 on the column-scaled Gram matrix; column-wise fallback
     bool slow = false;
@@ -289,6 +324,21 @@ bse_status_t orth_block(bse_handle_s *h, const void *V, int64_t ldv, int m, cons
     if (hcoef_host && m > 0) std::memcpy(hcoef_host, Hc.data(), sizeof(zc) * (size_t)m * k);
     if (bfac_host) std::memcpy(bfac_host, B.data(), sizeof(zc) * (size_t)k * k);
     if (rank_out) *rank_out = rank;
+    return BSE_OK;
+}
+
+bse_status_t orth_block(bse_handle_s *h, const void *V, int64_t ldv, int m, const void *PV, int64_t ldpv, void *W,
+                        int64_t ldw, int k, void *PW, int64_t ldpw, void *hcoef_host, void *bfac_host, int *rank_out,
+                        uint64_t seed, uint64_t *rng_counter)
+{
+    const bool cplx = (PV == nullptr);
+    double scale2 = 0.0;
+    ST(block_norm_scale(h, W, ldw, PW, ldpw, k, cplx, &scale2));
+    std::vector<zc> Hc((size_t)(m > 0 ? m : 1) * k, zc(0.0));
+    ST(project_block(h, V, ldv, m, PV, ldpv, W, ldw, k, PW, ldpw, cplx, Hc.data()));
+    ST(normalize_block(h, V, ldv, m, PV, ldpv, W, ldw, k, PW, ldpw, cplx, scale2, Hc.data(), bfac_host, rank_out, seed,
+                       rng_counter));
+    if (hcoef_host && m > 0) std::memcpy(hcoef_host, Hc.data(), sizeof(zc) * (size_t)m * k);
     return BSE_OK;
 }
 

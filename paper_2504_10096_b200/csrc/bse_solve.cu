@@ -9,6 +9,8 @@
 #include <cmath>
 #include <complex>
 #include <vector>
+#include <cstdio>
+#include <cstdlib>
 
 #include "bse_internal.h"
 
@@ -69,19 +71,37 @@ struct Solver {
         return gemm_basis(h, basis.p, ld, rows, cplx, (const double *)coef.p, ldo, l, n, out, ldo_c, 1.0, 0.0);
     }
 
+    // W = V[:, c0+k .. c0+2k) <- operator applied to the block at c0 (TDA: R x;  full: M(P x), reading S4)
     bse_status_t apply_block(int c0)
     {
-        // W = V[:, c0+k .. c0+2k) <- operator applied to the block at c0
         if (!full) {
             ST(zero_block(h, col(V, c0 + k), ld, n, k));
             ST(launch_apply_pass(h, h->R, 0, 1.0, col(V, c0), ld, col(V, c0 + k), ld, k));
         } else {
-            bse_status_t st;
-            if ((st = bse_apply_half(h, -1, col(PV, c0), ld, col(V, c0 + k), ld, k))) return st;      // W = M(p)
-            if ((st = bse_apply_half(h, +1, col(V, c0 + k), ld, col(PV, c0 + k), ld, k))) return st;  // PW = P(W)
+            bse_status_t st = bse_apply_half(h, -1, col(PV, c0), ld, col(V, c0 + k), ld, k);      // W = M(p)
+            if (st) return st;
         }
         info.n_apply += 1;
         return BSE_OK;
+    }
+
+    // Orthogonalise the new block at column m against the first m columns and orthonormalise it (a5-a7).
+    // Full mode follows the oracle's order: project W, THEN pw = P(w) (a fresh apply), then the P-norm.
+    bse_status_t orth_new_block(int m, void *Hc, void *B, int *rank)
+    {
+        if (!full)
+            return orth_block(h, V.p, ld, m, nullptr, ld, col(V, m), ld, k, nullptr, ld, Hc, B, rank, seed, &rng);
+        double e_in = 0.0, e_after = 0.0, g_after = 0.0;
+        ST(block_norm_scale(h, col(V, m), ld, nullptr, ld, k, false, &e_in));
+        ST(project_block(h, V.p, ld, m, PV.p, ld, col(V, m), ld, k, nullptr, ld, false, Hc));
+        bse_status_t st = bse_apply_half(h, +1, col(V, m), ld, col(PV, m), ld, k);                // PW = P(W)
+        if (st) return st;
+        ST(block_norm_scale(h, col(V, m), ld, nullptr, ld, k, false, &e_after));
+        ST(block_norm_scale(h, col(V, m), ld, col(PV, m), ld, k, false, &g_after));
+        // scale of the incoming block in the P-norm, estimated through the Euclidean norms
+        double scale2 = (e_after > 0.0) ? g_after * (e_in / e_after) : g_after;
+        return normalize_block(h, V.p, ld, m, PV.p, ld, col(V, m), ld, k, col(PV, m), ld, false, scale2, Hc, B, rank,
+                               seed, &rng);
     }
 };
 
@@ -110,6 +130,11 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
 
     const double t_start = now_s();
     Solver s;
+    struct InfoGuard {      // report progress on every exit path
+        bse_info_t *out; Solver *sv; double t0;
+        ~InfoGuard() { if (out) { sv->info.norm_est = sv->normest; sv->info.seconds_total = now_s() - t0; *out = sv->info; } }
+    } guard{info_out, &s, t_start};
+    const bool verbose = getenv("BSE_VERBOSE") != nullptr;
     s.h = h; s.n = n; s.full = full; s.nev = nev; s.k = k; s.ncv = ncv; s.tol = tol; s.ld = n; s.seed = seed;
     s.info.ncv = ncv;
     const size_t basis_bytes = (size_t)n * (ncv + k) * 16;
@@ -150,8 +175,11 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
         s.info.seconds_apply += t1 - t0;
         const int m = s.mp + k;
         int rank = 0;
-        ST(orth_block(h, s.V.p, s.ld, m, full ? s.PV.p : nullptr, s.ld, s.col(s.V, m), s.ld, k,
-                      full ? s.col(s.PV, m) : nullptr, s.ld, Hc.data(), B.data(), &rank, seed, &s.rng));
+        {
+            bse_status_t st_o = s.orth_new_block(m, Hc.data(), B.data(), &rank);
+            if (verbose && st_o) fprintf(stderr, "[bse_solve] orthogonalisation failed (%d) at m = %d\n", (int)st_o, m);
+            if (st_o) return st_o;
+        }
         s.info.seconds_orth += now_s() - t1;
         for (int c = 0; c < k; ++c)
             for (int a = 0; a < m; ++a) {
@@ -189,6 +217,7 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
         }
         resid.assign(nz, 0.0);
         double tmax = std::max(std::fabs(theta[0]), std::fabs(theta[mp - 1]));
+        if (verbose) fprintf(stderr, "[bse_solve] restart %d mp %d theta0 %.6e theta_max %.6e\n", restarts, mp, theta[0], theta[mp - 1]);
         if (full && !(theta[0] > 0.0)) return BSE_ERR_NOT_POSITIVE_DEFINITE;
         s.normest = std::max(s.normest, full ? std::sqrt(tmax) : tmax);
         for (int i = 0; i < nz; ++i) {
@@ -272,8 +301,5 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
         ST(assemble_full_vectors(h, s.rot.p, s.V.p, n, nev, (const double *)s.omega_d.p, dVec, ldvec));
     }
     BSE_CUDA(cudaStreamSynchronize(h->stream));
-    s.info.norm_est = s.normest;
-    s.info.seconds_total = now_s() - t_start;
-    if (info_out) *info_out = s.info;
     return result;
 }
