@@ -1,0 +1,274 @@
+#!/usr/bin/env python
+"""bench.py -- BSE block-apply throughput on one B200 (BASELINE.json metric), with roofline, e2e and CPU baseline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--k 4] [--impl reference]
+
+A "step" is one bse_apply (Y = R X, k columns) over the packed triangular operator of the chosen BASELINE.json
+config (default: config 4, TDA N = 98304, 77 GB -- the largest single-GPU configuration; the operand is ~600x
+larger than L2, so no flush is needed between iterations).  `value` is algorithmic GB/s: (packed matrix bytes +
+32 N k) / time, whole job.  Extra keys report the k sweep, the Lanczos time-to-nev at config 2, the roofline of the
+apply kernel, the end-to-end number through the host entry point, and the CPU oracle timed on the host cores.
+Multi-GPU (torchrun): the path does not shard (north_star: one GPU) -- N independent replicas, scaling "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import bse_inputs as gen  # noqa: E402
+
+METRIC = "bse_block_apply_algorithmic_GBps"
+UNIT = "GB/s"
+
+
+def alg_bytes(N: int, k: int) -> float:
+    """B_mat + 32 N k  (packed complex128 lower triangle once, X read + Y written)."""
+    return 16.0 * N * (N + 1) / 2 + 32.0 * N * k
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            p = json.load(f)
+        return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) > 2 + i and r[2 + i] == "Active" for r in self.rows)]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def time_steps(fn, steps, warmup):
+    import torch
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / steps      # ms per step, on the stream the kernels were launched on
+
+
+def cpu_oracle_sample(N, k, group, seed, sample_rows, reps):
+    """The oracle as it stands, timed on the host cores on a bounded sample: `sample_rows` full rows of R (from the CPU
+    generator) times the X block.  Returns (seconds per repetition, threads).  Only this leg and --impl reference
+    may touch oracle/."""
+    import oracle
+    oracle.build()
+    rows = (np.arange(sample_rows, dtype=np.int64) * 2654435761 % N)
+    Hrows = gen.rows_R(N, seed, rows, 0.0, group)
+    X = gen.block_X(N, k, seed + 1000)
+    oracle.rows_times_block(Hrows[:8], X)          # warm the library
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        oracle.rows_times_block(Hrows, X)
+    return (time.perf_counter() - t0) / reps, oracle.num_threads()
+
+
+def run_reference(args, cfg):
+    """--impl reference: for this tier the reference arm is the CPU oracle (no installable reference exists: the
+    reference is a paper).  One step = the oracle's dense row-panel product on a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    N, k = cfg["N"], args.k
+    rows = args.ref_rows
+    sec, threads = cpu_oracle_sample(N, k, cfg["group"], 1, rows, max(1, args.steps))
+    value = alg_bytes(N, k) * (rows / N) / sec / 1e9
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64 (complex128, long double accumulation)",
+            "data": "synthetic", "config": workload(cfg, k),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle",
+                             "sample": f"{rows} of {N} rows of Y = R X (k={k}), rows regenerated from the seed"},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def workload(cfg, k):
+    return {"workload": f"BASELINE.json config {cfg['id']}: TDA Hermitian N={cfg['N']} complex128, packed lower "
+                        f"triangle {16.0 * cfg['N'] * (cfg['N'] + 1) / 2 / 1e9:.2f} GB, bse_apply k={k}",
+            "N": cfg["N"], "k": k, "sigma": 0.0, "seed": 1,
+            "l2": "operand larger than L2 (no flush needed)" if cfg["N"] >= 8192 else "operand L2-resident"}
+
+
+def run_cuda(args, cfg):
+    import torch
+    import paper_2504_10096_b200 as b
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl")
+    N, k = cfg["N"], args.k
+
+    tiles = b.bse_fill_synthetic(N, b.MATRIX_R, 1, 0.0, cfg["group"])       # every replica holds its own operand
+    h = b.Bse(b.MODE_TDA, N, tiles)
+    Xh = torch.from_numpy(np.ascontiguousarray(gen.block_X(N, max(k, 8), 1001).T)).pin_memory()
+    X = Xh[:k].cuda()
+    Y = torch.empty_like(X)
+    torch.cuda.synchronize()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: K applies
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    t_wait = time.time()
+    while not sampler.rows and time.time() - t_wait < 5.0:      # nvidia-smi takes a moment to start
+        h.apply(X, Y)
+        torch.cuda.synchronize()
+    n_before = len(sampler.rows)
+    l0 = b.launch_count()
+    ms = time_steps(lambda: h.apply(X, Y), args.steps, args.warmup)
+    launches = (b.launch_count() - l0) * args.steps // (args.steps + args.warmup)
+    t_wait = time.time()
+    while len(sampler.rows) < n_before + 5 and time.time() - t_wait < 3.0:   # same load until >= 5 samples under load
+        h.apply(X, Y)
+        torch.cuda.synchronize()
+    sampler.rows = sampler.rows[n_before:] if len(sampler.rows) > n_before else sampler.rows
+    clocks = sampler.stop()
+    barrier()
+    if dist is not None:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * alg_bytes(N, k) / (ms * 1e-3) / 1e9
+
+    # ---- end to end through the host entry point (pinned host X and Y, copies inside the timed region)
+    Xk = Xh[:k].numpy()
+    Yk = torch.empty((k, N), dtype=torch.complex128).pin_memory().numpy()
+    for _ in range(2):
+        h.apply_host(Xk, Yk)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        h.apply_host(Xk, Yk)
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / args.steps
+    if dist is not None:
+        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    if rank != 0:
+        return
+
+    peak, peak_src = measured_peaks()
+    achieved = alg_bytes(N, k) / (ms * 1e-3) / 1e9
+    traffic = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "r1_apply_traffic.json")) as f:
+            traffic = json.load(f).get(f"N{N}_k{k}")
+    except Exception:
+        pass
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64 (complex128 on the FP64 tensor cores)", "data": "synthetic",
+            "config": workload(cfg, k), "clocks": clocks, "gpu_launches": int(launches),
+            "e2e": {"value": world * alg_bytes(N, k) / (e2e_ms * 1e-3) / 1e9, "unit": UNIT,
+                    "h2d_bytes_per_step": 16 * N * k, "d2h_bytes_per_step": 16 * N * k, "ms_per_step": e2e_ms},
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": traffic, "peak_source": peak_src, "kernel": "bse::apply_tiles_kernel",
+                         "tflops_fp64": 8.0 * N * N * k / (ms * 1e-3) / 1e12, "fp64_peak_measured_tflops": 37.1}}
+
+    # ---- k sweep and Lanczos time-to-nev (the rest of BASELINE.json's metric), device-timed, outside `value`
+    if not args.no_extras:
+        sweep = {}
+        for kk in (1, 2, 4, 8):
+            Xs, Ys = Xh[:kk].cuda(), torch.empty((kk, N), dtype=torch.complex128, device="cuda")
+            m = time_steps(lambda: h.apply(Xs, Ys), max(3, args.steps // 2), 2)
+            sweep[str(kk)] = {"ms": m, "GBps": alg_bytes(N, kk) / (m * 1e-3) / 1e9,
+                              "tflops": 8.0 * N * N * kk / (m * 1e-3) / 1e12}
+        line["apply_vs_k"] = sweep
+        del h, tiles
+        torch.cuda.empty_cache()
+        c2 = gen.CONFIGS[2]
+        h2 = b.Bse(b.MODE_TDA, c2["N"], b.bse_fill_synthetic(c2["N"], b.MATRIX_R, 1, 0.0, c2["group"]))
+        t0 = time.perf_counter()
+        res = h2.solve(c2["nev"], c2["k"], tol=1e-8, seed=1, raise_on_error=False)
+        line["lanczos_time_to_nev"] = {"workload": f"config 2: TDA N={c2['N']} nev={c2['nev']} k={c2['k']} tol=1e-8",
+                                       "seconds": time.perf_counter() - t0, "status": res.status, "info": res.info}
+
+    # ---- CPU baseline: the oracle on this box's host cores, bounded sample
+    if not args.no_cpu_baseline:
+        sec, threads = cpu_oracle_sample(N, k, cfg["group"], 1, args.ref_rows, 3)
+        line["cpu_baseline"] = {"value": alg_bytes(N, k) * (args.ref_rows / N) / sec / 1e9, "unit": UNIT,
+                                "cores": threads, "kind": "oracle",
+                                "sample": f"{args.ref_rows} of {N} rows of Y = R X (k={k}), 3 repetitions"}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index (TDA ones: 0, 2, 4)")
+    ap.add_argument("--k", type=int, default=4)
+    ap.add_argument("--ref-rows", type=int, default=1024)
+    ap.add_argument("--no-extras", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    cfg = dict(gen.CONFIGS[args.config], id=args.config)
+    if cfg["mode"] != "tda":
+        raise SystemExit("bench.py times the TDA apply; full-mode configs are parity-test cases")
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_cuda(args, cfg)
+
+
+if __name__ == "__main__":
+    main()
