@@ -77,6 +77,16 @@ class ClockSampler:
                 "reasons": reasons, "samples": len(sm)}
 
 
+def max_over_ranks(value: float, dist, device) -> float:
+    """Timing of a multi-rank run is the MAX over ranks (every rank is an independent replica)."""
+    if dist is None:
+        return value
+    import torch
+    t = torch.tensor([value], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def time_steps(fn, steps, warmup):
     import torch
     for _ in range(warmup):
@@ -179,10 +189,7 @@ def run_cuda(args, cfg):
     sampler.rows = sampler.rows[n_before:] if len(sampler.rows) > n_before else sampler.rows
     clocks = sampler.stop()
     barrier()
-    if dist is not None:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dist, "cuda")
     value = world * alg_bytes(N, k) / (ms * 1e-3) / 1e9
 
     # ---- end to end through the host entry point (pinned host X and Y, copies inside the timed region)
@@ -196,10 +203,7 @@ def run_cuda(args, cfg):
         h.apply_host(Xk, Yk)
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - t0) * 1e3 / args.steps
-    if dist is not None:
-        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms = max_over_ranks(e2e_ms, dist, "cuda")
     if rank != 0:
         return
 

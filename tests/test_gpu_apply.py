@@ -185,3 +185,25 @@ def test_full_apply_many_units_sampled_rows(orc):
     for _ in range(5):
         Y = to_host(h.apply(to_dev(X)))
         assert relerr(np.vstack([Y[rows], Y[N + rows]]), ref) <= TOL_APPLY
+
+
+def test_config4_full_size_sampled_rows(orc):
+    """BASELINE.json config 4 (N = 98304, 77 GB operand filled on the device): rows of Y sampled across the matrix,
+    against the oracle fed with the same rows from the CPU generator.  Needs ~80 GB of HBM."""
+    import torch
+    import paper_2504_10096_b200 as b
+    cfg = gen.CONFIGS[4]
+    N, k = cfg["N"], 4
+    if torch.cuda.mem_get_info()[0] < 90e9:
+        pytest.skip("needs 90 GB of free device memory")
+    h = b.Bse(b.MODE_TDA, N, b.bse_fill_synthetic(N, 0, 1, 0.0, cfg["group"]))
+    X = gen.block_X(N, k, 12)
+    rows = np.unique(np.concatenate([(np.arange(40) * 2654435761 % N), [0, 7, 63, 64, N - 65, N - 64, N - 1],
+                                     np.arange(8) + 64 * 777]).astype(np.int64))
+    ref = orc.rows_times_block(gen.rows_R(N, 1, rows, 0.0, cfg["group"]), X)
+    Y = to_host(h.apply(to_dev(X)))
+    assert relerr(Y[rows], ref) <= TOL_APPLY
+    Z = gen.block_X(N, k, 13)
+    RZ = to_host(h.apply(to_dev(Z)))
+    lhs, rhs = X.conj().T @ RZ, Y.conj().T @ Z
+    assert np.linalg.norm(lhs - rhs) <= 1e-12 * np.linalg.norm(lhs)
