@@ -184,27 +184,36 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
                 double C2[4][2];
 #pragma unroll
                 for (int q = 0; q < 4; ++q) C2[q][0] = C2[q][1] = 0.0;
+                // two patches at a time, four independent accumulator chains interleaved: dependent DMMAs are 4 apart
 #pragma unroll
-                for (int ib = 0; ib < 8; ++ib) {
-                    const char *pp = tp + ib * PATCH_BYTES;
+                for (int ib = 0; ib < 8; ib += 2) {
+                    const char *pp = tp + ib * PATCH_BYTES, *pq = pp + PATCH_BYTES;
                     double2 a0 = *reinterpret_cast<const double2 *>(pp + offP1);
-                    double2 a1 = *reinterpret_cast<const double2 *>(pp + offP1 + 256);
+                    double2 c0 = *reinterpret_cast<const double2 *>(pq + offP1);
                     double2 b0 = *reinterpret_cast<const double2 *>(pp + offP2);
+                    double2 d0 = *reinterpret_cast<const double2 *>(pq + offP2);
+                    double2 a1 = *reinterpret_cast<const double2 *>(pp + offP1 + 256);
+                    double2 c1 = *reinterpret_cast<const double2 *>(pq + offP1 + 256);
                     double2 b1 = *reinterpret_cast<const double2 *>(pp + offP2 + 512);
+                    double2 d1 = *reinterpret_cast<const double2 *>(pq + offP2 + 512);
+                    const int q = ib & 2;
                     dmma(C1[ib], a0.x, BaJ[0]);
-                    dmma(C2[ib & 3], b0.x, BaI[ib][0]);
+                    dmma(C1[ib + 1], c0.x, BaJ[0]);
+                    dmma(C2[q], b0.x, BaI[ib][0]);
+                    dmma(C2[q + 1], d0.x, BaI[ib + 1][0]);
                     dmma(C1[ib], a0.y, BbJ[0]);
-                    dmma(C2[ib & 3], b0.y, BbI[ib][0]);
+                    dmma(C1[ib + 1], c0.y, BbJ[0]);
+                    dmma(C2[q], b0.y, BbI[ib][0]);
+                    dmma(C2[q + 1], d0.y, BbI[ib + 1][0]);
                     dmma(C1[ib], a1.x, BaJ[1]);
-                    dmma(C2[ib & 3], b1.x, BaI[ib][1]);
+                    dmma(C1[ib + 1], c1.x, BaJ[1]);
+                    dmma(C2[q], b1.x, BaI[ib][1]);
+                    dmma(C2[q + 1], d1.x, BaI[ib + 1][1]);
                     dmma(C1[ib], a1.y, BbJ[1]);
-                    dmma(C2[ib & 3], b1.y, BbI[ib][1]);
+                    dmma(C1[ib + 1], c1.y, BbJ[1]);
+                    dmma(C2[q], b1.y, BbI[ib][1]);
+                    dmma(C2[q + 1], d1.y, BbI[ib + 1][1]);
                 }
-                // release the stage only after every DMMA that consumes its data has issued (see pin2)
-#pragma unroll
-                for (int ib = 0; ib < 8; ++ib) pin2(C1[ib][0], C1[ib][1]);
-#pragma unroll
-                for (int q = 0; q < 4; ++q) pin2(C2[q][0], C2[q][1]);
                 // The release must not overtake the ld.shared that feed the DMMAs above: an mbarrier arrive only orders
                 // the ISSUE of earlier loads, and on B200 queued loads of a slow warp were observed to execute after the
                 // producer's next bulk copy had landed (stale fragments about once per launch).  The barrier address is
@@ -229,17 +238,22 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
                 }
             } else {
 #pragma unroll
-                for (int ib = 0; ib < 8; ++ib) {
-                    const char *pp = tp + ib * PATCH_BYTES;
-                    double2 a0 = *reinterpret_cast<const double2 *>(pp + offP1);
-                    double2 a1 = *reinterpret_cast<const double2 *>(pp + offP1 + 256);
-                    dmma(C1[ib], a0.x, BaJ[0]);
-                    dmma(C1[ib], a0.y, BbJ[0]);
-                    dmma(C1[ib], a1.x, BaJ[1]);
-                    dmma(C1[ib], a1.y, BbJ[1]);
-                }
+                for (int ib = 0; ib < 8; ib += 4) {     // diagonal tile: P1 only, four chains interleaved
+                    double2 a0[4], a1[4];
 #pragma unroll
-                for (int ib = 0; ib < 8; ++ib) pin2(C1[ib][0], C1[ib][1]);
+                    for (int r = 0; r < 4; ++r) {
+                        a0[r] = *reinterpret_cast<const double2 *>(tp + (ib + r) * PATCH_BYTES + offP1);
+                        a1[r] = *reinterpret_cast<const double2 *>(tp + (ib + r) * PATCH_BYTES + offP1 + 256);
+                    }
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) dmma(C1[ib + r], a0[r].x, BaJ[0]);
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) dmma(C1[ib + r], a0[r].y, BbJ[0]);
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) dmma(C1[ib + r], a1[r].x, BaJ[1]);
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) dmma(C1[ib + r], a1[r].y, BbJ[1]);
+                }
                 int live = 0;
 #pragma unroll
                 for (int ib = 0; ib < 8; ++ib) live |= __double2hiint(C1[ib][0]);

@@ -72,16 +72,12 @@ __device__ __forceinline__ double2 lds128(uint32_t addr)
 // Fragments: lane = 4 g + t;  a = A[g][t];  b = B[t][g];  c[0..1] = C[g][2t .. 2t+1].
 __device__ __forceinline__ void dmma(double (&c)[2], double a, double b)
 {
-    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
-        : "+d"(c[0]), "+d"(c[1])
-        : "d"(a), "d"(b));
+    // volatile: keeps the hand-interleaved order of independent accumulator chains (ptxas otherwise schedules
+    // dependent DMMAs back to back, paying the 26-cycle latency instead of the 16-cycle issue interval)
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+                 : "+d"(c[0]), "+d"(c[1])
+                 : "d"(a), "d"(b));
 }
 __device__ __forceinline__ void red_add(double *p, double v) { atomicAdd(p, v); }
-
-// Pins values in registers at this program point.  Used before releasing a shared-memory buffer back to the TMA
-// producer: an mbarrier arrive only orders the ISSUE of earlier ld.shared instructions; queued loads may still
-// execute after the producer's next bulk copy has landed (observed on B200 as rare stale fragments).  Making the
-// release depend on values computed from every load forces those loads to have returned.
-__device__ __forceinline__ void pin2(double &a, double &b) { asm volatile("" : "+d"(a), "+d"(b)::"memory"); }
 
 }  // namespace bse
