@@ -207,3 +207,39 @@ def test_config4_full_size_sampled_rows(orc):
     RZ = to_host(h.apply(to_dev(Z)))
     lhs, rhs = X.conj().T @ RZ, Y.conj().T @ Z
     assert np.linalg.norm(lhs - rhs) <= 1e-12 * np.linalg.norm(lhs)
+
+
+@pytest.mark.parametrize("N", [1, 2, 63, 65, 127])
+def test_tiny_and_ragged_sizes(orc, N):
+    import paper_2504_10096_b200 as b
+    R = _herm(N, 40 + N)
+    for k in (1, 4, 7):
+        X = gen.block_X(N, k, 41)
+        Y = to_host(b.Bse(b.MODE_TDA, N, pack(R, 0)).apply(to_dev(X)))
+        assert relerr(Y, orc.apply_tda(R, X)) <= TOL_APPLY
+
+
+def test_leading_dimensions_and_side_stream(orc):
+    """ldx, ldy > N through the raw C ABI, on a non-default stream."""
+    import ctypes
+    import torch
+    import paper_2504_10096_b200 as b
+    N, k, ldx, ldy = 200, 3, 256, 231
+    R = _herm(N, 51)
+    X = gen.block_X(N, k, 52)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        tiles = pack(R, 0)
+        Xd = torch.full((k, ldx), 7.0 + 1j, dtype=torch.complex128, device="cuda")
+        Xd[:, :N] = to_dev(X)
+        Yd = torch.full((k, ldy), 3.0 - 2j, dtype=torch.complex128, device="cuda")
+        h = b.Bse(b.MODE_TDA, N, tiles)                       # captures the current (side) stream
+        st = b.lib().bse_apply(h._h, Xd.data_ptr(), ldx, Yd.data_ptr(), ldy, k)
+        assert st == 0
+    s.synchronize()
+    Y = to_host(Yd)
+    assert relerr(Y[:N], orc.apply_tda(R, X)) <= TOL_APPLY
+    assert np.all(Y[N:] == 3.0 - 2j)                          # padding rows of Y are not touched
+    assert b.lib().bse_apply(h._h, Xd.data_ptr(), N - 1, Yd.data_ptr(), ldy, k) == 1     # ld < N
+    assert b.lib().bse_apply(h._h, Xd.data_ptr(), ldx, Yd.data_ptr(), ldy, 0) == 1       # k < 1
+    assert b.lib().bse_apply(h._h, Xd.data_ptr(), ldx, Xd.data_ptr(), ldx, k) == 1       # aliasing

@@ -152,3 +152,55 @@ def test_solve_invalid_arguments_and_nonconvergence():
     r = h.solve(8, 2, ncv=12, tol=1e-14, max_restarts=1, raise_on_error=False)
     assert r.status == 4 and r.info["n_restart"] == 1               # best estimates are still returned
     assert np.all(np.isfinite(r.omega))
+
+
+def _closed_tda(N, seed):
+    import torch
+    import paper_2504_10096_b200 as b
+    lam = gen.prescribed_spectrum(N, seed, 1.0, 10.0, power=2 / 3)
+    u = gen.householder_u(N, seed)
+    t = b.bse_fill_closed_form_tda(N, torch.from_numpy(lam).cuda(), torch.from_numpy(u).cuda(),
+                                   float(np.sum(lam * np.abs(u) ** 2)))
+    return b.Bse(b.MODE_TDA, N, t), lam
+
+
+def test_config2_size_closed_form_nev100():
+    """Config 2's size and request (N = 16384, nev = 100, k = 4, tol 1e-8) on an instance whose spectrum is known
+    exactly (R = Q diag(lam) Q^H): the CPU oracle cannot diagonalise N = 16384 in test time, the closed form can."""
+    h, lam = _closed_tda(16384, 21)
+    res = h.solve(100, 4, tol=1e-8, seed=1)
+    assert np.max(np.abs(res.omega - lam[:100]) / lam[:100]) <= TOL_EIG
+    V = res.vectors
+    G = (V.conj() @ V.T).cpu().numpy()
+    assert np.linalg.norm(G - np.eye(100)) <= 1e-11
+    R = h.apply(V)                                     # residual through the CUDA apply (parity-tested separately)
+    import torch
+    r = (R - V * torch.from_numpy(res.omega).cuda()[:, None]).norm(dim=1).cpu().numpy()
+    assert np.all(r <= TOL_RES * 10.0)
+
+
+def test_config3_size_closed_form_pair():
+    """Config 3's size (full mode, N = 32768, operator 65536) on the closed-form pair with omega = sqrt(d1 d2)."""
+    import torch
+    import paper_2504_10096_b200 as b
+    N, nev, k = 32768, 16, 4
+    if torch.cuda.mem_get_info()[0] < 30e9:
+        pytest.skip("needs 30 GB of free device memory")
+    d1 = gen.prescribed_spectrum(N, 7, 1.0, 9.0, power=2 / 3); d2 = gen.prescribed_spectrum(N, 8, 2.0, 5.0, power=2 / 3)
+    ur = gen.householder_u(N, 9, complex_u=False).real.copy(); phi = gen.phases(N, 9)
+    rt, ct = b.bse_fill_closed_form_full(N, *(torch.from_numpy(a).cuda() for a in (d1, d2, ur, phi)),
+                                         float(np.sum(d1 * ur ** 2)), float(np.sum(d2 * ur ** 2)))
+    res = b.Bse(b.MODE_FULL, N, rt, ct).solve(nev, k, tol=1e-8, seed=4)
+    exact = np.sort(np.sqrt(d1 * d2))[:nev]
+    assert np.max(np.abs(res.omega - exact) / exact) <= TOL_EIG
+
+
+def test_config4_size_closed_form():
+    """Config 4's size (N = 98304, 77 GB operand) with a prescribed spectrum; a reduced request (nev = 24, k = 8)
+    keeps the test short -- the full nev = 500 run is a bench item."""
+    import torch
+    if torch.cuda.mem_get_info()[0] < 100e9:
+        pytest.skip("needs 100 GB of free device memory")
+    h, lam = _closed_tda(98304, 23)
+    res = h.solve(24, 8, tol=1e-8, seed=2)
+    assert np.max(np.abs(res.omega - lam[:24]) / lam[:24]) <= TOL_EIG
