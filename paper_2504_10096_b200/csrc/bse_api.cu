@@ -14,6 +14,7 @@ std::atomic<int64_t> g_launches{0};
 static bse_status_t grow(void **p, size_t *have, size_t want)
 {
     if (*have >= want) return BSE_OK;
+    if (*have && want < *have + *have / 2) want = *have + *have / 2;      // geometric growth: no realloc per step
     if (*p) cudaFree(*p);
     *p = nullptr;
     *have = 0;
@@ -26,6 +27,7 @@ bse_status_t ensure_ws2(bse_handle_s *h, size_t bytes) { return grow(&h->ws2, &h
 bse_status_t ensure_pin(bse_handle_s *h, size_t bytes)
 {
     if (h->hpin_bytes >= bytes) return BSE_OK;
+    if (h->hpin_bytes && bytes < 2 * h->hpin_bytes) bytes = 2 * h->hpin_bytes;
     if (h->hpin) cudaFreeHost(h->hpin);
     h->hpin = nullptr;
     h->hpin_bytes = 0;

@@ -70,6 +70,7 @@ bse_status_t orth_block(bse_handle_s *h, const void *V, int64_t ldv, int m, cons
                         int64_t ldw, int k, void *PW, int64_t ldpw, void *hcoef_host, void *bfac_host, int *rank,
                         uint64_t seed, uint64_t *rng_counter);
 
+bse_status_t orth_reserve(bse_handle_s *h, int m_max, int k);
 // the two halves of orth_block, for callers that recompute P(W) between projection and normalisation
 bse_status_t project_block(bse_handle_s *h, const void *V, int64_t ldv, int m, const void *PV, int64_t ldpv, void *W,
                            int64_t ldw, int k, void *PW, int64_t ldpw, bool cplx, void *hcoef_host);

@@ -150,6 +150,13 @@ static bse_status_t euclid_max_norm2(bse_handle_s *h, const void *W, int64_t ldw
 // Block CGS, two passes against V (a5 + a6, twice).  PW may be NULL in the real inner product: then only W is
 // updated and the caller recomputes P(W) afterwards (what bse_solve does: updating PW by linear combination lets
 // PW drift away from P(W) exponentially over the iteration).
+// Reserve the orthogonalisation workspace for a basis of up to m_max columns (avoids reallocation while it grows).
+bse_status_t orth_reserve(bse_handle_s *h, int m_max, int k)
+{
+    OrthWs w;
+    return orth_ws(h, m_max, k, w);
+}
+
 bse_status_t project_block(bse_handle_s *h, const void *V, int64_t ldv, int m, const void *PV, int64_t ldpv, void *W,
                            int64_t ldw, int k, void *PW, int64_t ldpw, bool cplx, void *hcoef_host)
 {

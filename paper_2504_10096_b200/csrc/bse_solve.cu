@@ -145,6 +145,7 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
     ST(s.omega_d.alloc((size_t)nev * 8));
     s.T.assign((size_t)ncv * ncv, zc(0.0));
     const int ldT = ncv;
+    ST(orth_reserve(h, ncv + k, k));
 
     // ---- start block: random, orthonormalised in the active inner product
     ST(fill_random_block(h, s.V.p, s.ld, n, k, seed, s.rng));
