@@ -88,6 +88,7 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
         if (lane == 0) {
             int st = 0;
             uint32_t ph = 0;
+            const uint64_t pol = l2_policy_evict_first();     // the tile stream is read exactly once
             for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
                 int I, J0, J1;
                 apply_decode_unit(u, p.L, I, J0, J1);
@@ -95,7 +96,7 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
                 for (int J = J0; J < J1; ++J, src += TILE_BYTES) {
                     mbar_wait(&empty[st], ph ^ 1);
                     mbar_expect_tx(&full[st], (uint32_t)TILE_BYTES);
-                    bulk_g2s(tile_s + st * TILE_BYTES, src, TILE_BYTES, &full[st]);
+                    bulk_g2s_hint(tile_s + st * TILE_BYTES, src, TILE_BYTES, &full[st], pol);
                     if (++st == APPLY_STAGES) { st = 0; ph ^= 1; }
                 }
             }
