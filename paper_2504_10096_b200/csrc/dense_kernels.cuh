@@ -15,8 +15,10 @@ namespace bse {
 // gram:  out[a + o(n)] += sum_r A~[r, a] * Bx[r, n],   a < m,  n < ncols,  o(n) = n ldo  or  half_off + (n-k) ldo
 //   Bx columns n < k      : B~[:, n]
 //   Bx columns k <= n < 2k: (-iB)~[:, n - k]            (only when ncols == 2k, the complex case)
-// One warp owns 8 columns of A (an M-tile) and streams a chunk of rows with 32-byte sector loads straight
-// into DMMA A-fragments; B fragments come through L1/L2.  Partial sums are reduced with red.global.add.f64.
+// One warp owns 8 columns of A (an M-tile) and streams a chunk of rows.  The contraction index of a DMMA k-step is
+// free to permute, so lane (g, t) loads the FOUR consecutive rows r + 4t .. r + 4t + 3 of its column (two LDG.128,
+// i.e. the four lanes of a column fetch one full 128-byte line) and k-step s uses row r + 4t + s on both operands.
+// B fragments come through L1/L2.  Partial sums are reduced with red.global.add.f64.
 // ------------------------------------------------------------------------------------------------------
 template <int NT>
 __global__ void __launch_bounds__(256) gram_kernel(const double *__restrict__ A, int64_t lda2, int m,
@@ -28,13 +30,12 @@ __global__ void __launch_bounds__(256) gram_kernel(const double *__restrict__ A,
     const int g = lane >> 2, t = lane & 3;
     const int c0 = blockIdx.x * 64 + warp * 8;
     if (c0 >= m) return;
-    const int64_t r_begin = (int64_t)blockIdx.y * rows_per_cta;
-    const int64_t r_end = min(nr, r_begin + rows_per_cta);
+    const int64_t r_begin = (int64_t)blockIdx.y * rows_per_cta;           // multiple of 16
+    const int64_t r_end = min(nr, r_begin + rows_per_cta);                // even (nr = 2n)
     const bool aok = (c0 + g) < m;
-    const double *ap = A + (int64_t)(aok ? c0 + g : 0) * lda2;
+    const double2 *ap = reinterpret_cast<const double2 *>(A + (int64_t)(aok ? c0 + g : 0) * lda2);
 
-    // per n-tile B column pointer / rotation flag for this lane (n = 8 q + g)
-    const double *bp[NT];
+    const double2 *bp[NT];
     bool bok[NT], brot[NT];
 #pragma unroll
     for (int q = 0; q < NT; ++q) {
@@ -42,34 +43,40 @@ __global__ void __launch_bounds__(256) gram_kernel(const double *__restrict__ A,
         bok[q] = n < ncols;
         brot[q] = n >= k;
         int col = bok[q] ? (brot[q] ? n - k : n) : 0;
-        bp[q] = B + (int64_t)col * ldb2;
+        bp[q] = reinterpret_cast<const double2 *>(B + (int64_t)col * ldb2);
     }
     double acc[NT][2];
 #pragma unroll
     for (int q = 0; q < NT; ++q) acc[q][0] = acc[q][1] = 0.0;
 
-    constexpr int U = 4;
-    for (int64_t r = r_begin; r < r_end; r += 4 * U) {
-        double a[U], b[NT][U];
+    constexpr int U = 2;                                   // 2 x 16 rows per iteration
+    const double2 zero = make_double2(0.0, 0.0);
+    for (int64_t r = r_begin; r < r_end; r += 16 * U) {
+        double2 a[U][2], b[NT][U][2];
 #pragma unroll
-        for (int s = 0; s < U; ++s) {
-            int64_t row = r + 4 * s + t;
-            bool rok = row < r_end;
-            a[s] = (aok && rok) ? ap[row] : 0.0;
+        for (int u = 0; u < U; ++u) {
+            const int64_t row = r + 16 * u + 4 * t;        // first of this lane's four rows (even)
 #pragma unroll
-            for (int q = 0; q < NT; ++q) {
-                double v = 0.0;
-                if (bok[q] && rok) {
-                    if (!brot[q]) v = bp[q][row];
-                    else { v = bp[q][row ^ 1]; if (row & 1) v = -v; }
+            for (int h = 0; h < 2; ++h) {
+                const bool rok = (row + 2 * h) < r_end;    // pairs never straddle r_end (both even)
+                a[u][h] = (aok && rok) ? __ldg(ap + ((row + 2 * h) >> 1)) : zero;
+#pragma unroll
+                for (int q = 0; q < NT; ++q) {
+                    double2 v = (bok[q] && rok) ? __ldg(bp[q] + ((row + 2 * h) >> 1)) : zero;
+                    if (brot[q]) v = make_double2(v.y, -v.x);          // (-i w)~ : rows (2j, 2j+1) -> (w_i, -w_r)
+                    b[q][u][h] = v;
                 }
-                b[q][s] = v;
             }
         }
 #pragma unroll
-        for (int s = 0; s < U; ++s)
+        for (int u = 0; u < U; ++u)
 #pragma unroll
-            for (int q = 0; q < NT; ++q) dmma(acc[q], a[s], b[q][s]);
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int q = 0; q < NT; ++q) {
+                    dmma(acc[q], a[u][h].x, b[q][u][h].x);
+                    dmma(acc[q], a[u][h].y, b[q][u][h].y);
+                }
     }
     // C fragment: rows (A column) c0 + g, columns n = 8 q + 2 t, + 1
     if (aok) {

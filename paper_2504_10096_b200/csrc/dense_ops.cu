@@ -19,16 +19,19 @@ bse_status_t gram_basis(bse_handle_s *h, const void *A, int64_t lda, int m, cons
     rows = ((rows + 63) / 64) * 64;
     if (rows < 256) rows = 256;
     const int gy = (int)((nr + rows - 1) / rows);
-    // up to 4 complex (8 real) columns per launch: ncols = 2*kc <= 8 (complex) or kc <= 8 (real)
-    const int step = cplx ? 4 : 8;
+    // up to 8 complex / 16 real columns per launch (two N-tiles); one N-tile when it is enough
+    const int step = cplx ? 8 : 16;
     for (int c0 = 0; c0 < k; c0 += step) {
         int kc = (k - c0) < step ? (k - c0) : step;
+        const int ncols = cplx ? 2 * kc : kc;
         const double *Bp = (const double *)B + 2 * (int64_t)c0 * ldb;
         double *op = out + (int64_t)c0 * ldo;
-        // the kernel writes column n of its local problem at a + n*m; map to the coefficient layout by launching
-        // the real and imaginary halves with an output stride of ldo: handled inside via (m_out = ldo, half offset)
-        gram_kernel<1><<<dim3(gx, gy), 256, 0, h->stream>>>((const double *)A, 2 * lda, m, Bp, 2 * ldb, kc,
-                                                           cplx ? 2 * kc : kc, nr, rows, op, ldo, cplx ? m : 0);
+        if (ncols <= 8)
+            gram_kernel<1><<<dim3(gx, gy), 256, 0, h->stream>>>((const double *)A, 2 * lda, m, Bp, 2 * ldb, kc, ncols,
+                                                               nr, rows, op, ldo, cplx ? m : 0);
+        else
+            gram_kernel<2><<<dim3(gx, gy), 256, 0, h->stream>>>((const double *)A, 2 * lda, m, Bp, 2 * ldb, kc, ncols,
+                                                               nr, rows, op, ldo, cplx ? m : 0);
         count_launch();
     }
     BSE_CUDA(cudaGetLastError());
