@@ -57,6 +57,9 @@ def _load():
         lib.orc_lanczos_full.argtypes = [_i64, _c128, _c128, ctypes.c_int, ctypes.c_double, ctypes.c_int,
                                          ctypes.c_int, _c128, _f64, _c128, _f64]
         lib.orc_lanczos_full.restype = ctypes.c_int
+        lib.orc_lanczos_quadrature.argtypes = [_i64, _c128, _c128, ctypes.c_int, _f64, _f64]
+        lib.orc_lanczos_quadrature.restype = ctypes.c_int
+        lib.orc_quadrature_resolvent.argtypes = [ctypes.c_int, _f64, _f64, ctypes.c_int, _f64, ctypes.c_double, _c128]
         _lib = lib
     return _lib
 
@@ -175,3 +178,21 @@ def lanczos_full(R, C, nev, tol, x0, maxit=None, check=10):
     if steps == -1000000:
         raise np.linalg.LinAlgError("Omega is not positive definite")
     return om, Vec, res, steps
+
+
+def lanczos_quadrature(R, d, steps):
+    """Lanczos coefficients (alpha[steps], beta[steps+1], beta[0] = |d|) of the quadrature of PAPER.md:65 (TDA)."""
+    R = _c(R)
+    N = R.shape[0]
+    alpha = np.zeros(steps); beta = np.zeros(steps + 1)
+    done = _load().orc_lanczos_quadrature(N, R, _c(d).reshape(N), steps, alpha, beta)
+    return alpha[:done], beta[:done + 1]
+
+
+def quadrature_resolvent(alpha, beta, omega, eta):
+    """d^H (omega + i eta - R)^{-1} d from the continued fraction of the Jacobi matrix."""
+    alpha = np.ascontiguousarray(alpha, dtype=np.float64); beta = np.ascontiguousarray(beta, dtype=np.float64)
+    omega = np.ascontiguousarray(omega, dtype=np.float64)
+    out = np.zeros(len(omega), dtype=np.complex128)
+    _load().orc_quadrature_resolvent(len(alpha), alpha, beta, len(omega), omega, float(eta), out)
+    return out

@@ -555,3 +555,50 @@ done:
     free(Xb); free(Pb); free(alpha); free(beta); free(wv); free(pw); free(T); free(S); free(th);
     return result;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * Lanczos with quadrature rules ("a Lanczos iteration with quadrature rules to obtain the
+ * optical absorption spectrum directly, without explicitly computing the eigenpairs"), TDA case.
+ * Textbook three-term recurrence on the Hermitian R started at d / |d| (no reorthogonalisation, no stored basis):
+ *   beta_0 = |d|;  w = R v_j - beta_j v_{j-1};  alpha_j = Re(v_j^H w);  w -= alpha_j v_j;
+ *   beta_{j+1} = |w|;  v_{j+1} = w / beta_{j+1}.
+ * alpha[0..steps), beta[0..steps]: beta[0] = |d|, beta[j] (j >= 1) couples steps j-1 and j.
+ * Returns the number of steps done (stops early when beta_{j+1} = 0).
+ * The Gauss quadrature it defines reproduces the moments d^H R^p d, p <= 2 steps - 1, and the resolvent
+ *   d^H (z - R)^{-1} d  ~=  beta_0^2 / (z - alpha_0 - beta_1^2 / (z - alpha_1 - beta_2^2 / ( ... ))).
+ * ------------------------------------------------------------------------------------------ */
+int orc_lanczos_quadrature(int64_t N, const zc *R, const zc *d, int steps, double *alpha, double *beta)
+{
+    zc *v = (zc *)malloc(sizeof(zc) * N), *vp = (zc *)calloc(N, sizeof(zc)), *w = (zc *)malloc(sizeof(zc) * N);
+    double b0 = nrm2(N, d);
+    beta[0] = b0;
+    for (int64_t i = 0; i < N; ++i) v[i] = d[i] / b0;
+    int done = 0;
+    for (int j = 0; j < steps; ++j) {
+        orc_apply_tda(N, 1, R, v, w);
+        for (int64_t i = 0; i < N; ++i) w[i] -= beta[j] * vp[i] * (j > 0 ? 1.0 : 0.0);
+        ld a = 0.0L;
+        for (int64_t i = 0; i < N; ++i) a += (ld)creal(v[i]) * (ld)creal(w[i]) + (ld)cimag(v[i]) * (ld)cimag(w[i]);
+        alpha[j] = (double)a;
+        for (int64_t i = 0; i < N; ++i) w[i] -= alpha[j] * v[i];
+        double b = nrm2(N, w);
+        beta[j + 1] = b;
+        done = j + 1;
+        if (b == 0.0) break;
+        for (int64_t i = 0; i < N; ++i) { vp[i] = v[i]; v[i] = w[i] / b; }
+    }
+    free(v); free(vp); free(w);
+    return done;
+}
+
+/* Continued fraction of the Jacobi matrix: out[i] = beta_0^2 * [ (z_i - T)^{-1} ]_{00},  z_i = omega_i + i eta. */
+void orc_quadrature_resolvent(int steps, const double *alpha, const double *beta, int n_omega, const double *omega,
+                              double eta, zc *out)
+{
+    for (int i = 0; i < n_omega; ++i) {
+        zc z = omega[i] + I * eta;
+        zc f = z - alpha[steps - 1];
+        for (int j = steps - 2; j >= 0; --j) f = z - alpha[j] - beta[j + 1] * beta[j + 1] / f;
+        out[i] = beta[0] * beta[0] / f;
+    }
+}
