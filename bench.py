@@ -234,6 +234,16 @@ def run_cuda(args, cfg):
             sweep[str(kk)] = {"ms": m, "GBps": alg_bytes(N, kk) / (m * 1e-3) / 1e9,
                               "tflops": 8.0 * N * N * kk / (m * 1e-3) / 1e12}
         line["apply_vs_k"] = sweep
+        # Lanczos with quadrature: one k = 1 apply + three O(N) kernels per step
+        dq = Xh[0].cuda()
+        h.lanczos_quadrature(dq, 3)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        qsteps = 40
+        h.lanczos_quadrature(dq, qsteps)
+        qsec = time.perf_counter() - t0
+        line["lanczos_quadrature"] = {"steps": qsteps, "ms_per_step": qsec * 1e3 / qsteps,
+                                      "GBps": alg_bytes(N, 1) * qsteps / qsec / 1e9}
         del h, tiles
         torch.cuda.empty_cache()
         c2 = gen.CONFIGS[2]

@@ -164,6 +164,20 @@ bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_t ncv, doub
                        int32_t max_restarts, uint64_t seed, double *hOmega, void *dVec, int64_t ldvec,
                        double *hResid, bse_info_t *info);
 
+/* Lanczos with quadrature rules (the optical absorption spectrum "directly, without explicitly computing
+ * the eigenpairs").  TDA handles only.  Runs `steps` steps of the three-term Lanczos recurrence of R started at
+ * d / |d| (dStart: N complex128, device; not modified), no reorthogonalisation, no stored basis:
+ *   hAlpha[0..steps)  diagonal of the Jacobi matrix;  hBeta[0..steps]: hBeta[0] = |d|_2, hBeta[j] couples steps j-1, j.
+ * *hDone (nullable) = number of valid steps (smaller than `steps` only on an exact breakdown).  Synchronous.
+ * Each step is one bse_apply with k = 1 plus three O(N) kernels; all scalars stay on the device until the end. */
+bse_status_t bse_lanczos_quadrature(bse_handle_t h, const void *dStart, int32_t steps, double *hAlpha,
+                                    double *hBeta, int32_t *hDone);
+
+/* Host utility: d^H (omega_i + i eta - R)^{-1} d  ~=  hBeta[0]^2 [(z - T)^{-1}]_00 by the continued fraction of the
+ * Jacobi matrix T(hAlpha, hBeta).  hOut: n_omega complex128 (host).  -Im(...)/pi is the broadened spectral function. */
+bse_status_t bse_quadrature_resolvent(int32_t steps, const double *hAlpha, const double *hBeta, int32_t n_omega,
+                                      const double *hOmega, double eta, void *hOut);
+
 /* Host utility (no device work): eigen-decomposition of the m x m complex Hermitian matrix hA (column-major, lda,
  * lower triangle read, destroyed) -- the "small projected eigenproblem" of PAPER.md:67, which bse_solve keeps on
  * the host.  hW: m eigenvalues ascending; hZ (m x nz, ldz): the first nz eigenvectors.  Returns BSE_ERR_INTERNAL

@@ -51,6 +51,8 @@ _SIGNATURES = {
     "bse_apply_half": [_vp, _i32, _vp, _i64, _vp, _i64, _i32],
     "bse_apply_host": [_vp, _vp, _i64, _vp, _i64, _i32],
     "bse_orth": [_vp, _vp, _i64, _i32, _vp, _i64, _vp, _i64, _i32, _vp, _i64, _vp, _vp, ctypes.POINTER(_i32)],
+    "bse_lanczos_quadrature": [_vp, _vp, _i32, ctypes.POINTER(_dbl), ctypes.POINTER(_dbl), ctypes.POINTER(_i32)],
+    "bse_quadrature_resolvent": [_i32, ctypes.POINTER(_dbl), ctypes.POINTER(_dbl), _i32, ctypes.POINTER(_dbl), _dbl, _vp],
     "bse_host_heev": [_i32, _vp, _i32, _vp, _vp, _i32, _i32],
     "bse_solve": [_vp, _i32, _i32, _i32, _dbl, _i32, _u64, ctypes.POINTER(_dbl), _vp, _i64, ctypes.POINTER(_dbl),
                   ctypes.POINTER(_Info)],
@@ -221,6 +223,16 @@ class Bse:
                               ctypes.byref(rank)), "bse_orth")
         return hcoef[:, :m], bfac, rank.value
 
+    def lanczos_quadrature(self, d, steps: int):
+        """(alpha[steps'], beta[steps'+1]) of PAPER.md:65's Lanczos-with-quadrature solver; d: torch complex128 (N,)."""
+        import numpy as np
+        alpha = np.zeros(steps); beta = np.zeros(steps + 1)
+        done = _i32(0)
+        _check(lib().bse_lanczos_quadrature(self._h, d.data_ptr(), steps, alpha.ctypes.data_as(ctypes.POINTER(_dbl)),
+                                            beta.ctypes.data_as(ctypes.POINTER(_dbl)), ctypes.byref(done)),
+               "bse_lanczos_quadrature")
+        return alpha[:done.value], beta[:done.value + 1]
+
     def solve(self, nev: int, k: int, ncv: int = 0, tol: float = 1e-8, max_restarts: int = 1000, seed: int = 1,
               raise_on_error: bool = True):
         import numpy as np
@@ -247,6 +259,18 @@ def host_heev(A, nz=None):
     Z = np.zeros((m, max(nz, 1)), dtype=np.complex128, order="F")
     _check(lib().bse_host_heev(m, a.ctypes.data, m, w.ctypes.data, Z.ctypes.data, m, nz), "bse_host_heev")
     return w, Z[:, :nz]
+
+
+def quadrature_resolvent(alpha, beta, omega, eta: float):
+    """Host utility: d^H (omega + i eta - R)^-1 d from the continued fraction (numpy complex128 array)."""
+    import numpy as np
+    alpha = np.ascontiguousarray(alpha, dtype=np.float64); beta = np.ascontiguousarray(beta, dtype=np.float64)
+    omega = np.ascontiguousarray(omega, dtype=np.float64)
+    out = np.zeros(len(omega), dtype=np.complex128)
+    P = ctypes.POINTER(_dbl)
+    _check(lib().bse_quadrature_resolvent(len(alpha), alpha.ctypes.data_as(P), beta.ctypes.data_as(P), len(omega),
+                                          omega.ctypes.data_as(P), eta, out.ctypes.data), "bse_quadrature_resolvent")
+    return out
 
 
 def launch_count() -> int:

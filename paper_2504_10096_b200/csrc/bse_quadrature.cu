@@ -1,0 +1,124 @@
+// Lanczos with quadrature rules (the optical absorption spectrum "directly, without
+// explicitly computing the eigenpairs").  TDA operator, three-term recurrence, no stored basis: per step one
+// bse_apply with k = 1 (the HBM-bound case of the tile kernel) and three O(N) kernels.  All scalars stay on the
+// device; the host synchronises once at the end.
+#include <cmath>
+#include <vector>
+
+#include "bse_common.cuh"
+#include "bse_internal.h"
+
+namespace bse {
+
+// acc[0] += Re(v^H w)
+__global__ void __launch_bounds__(256) dot_re_kernel(const double2 *__restrict__ v, const double2 *__restrict__ w,
+                                                     int64_t n, double *acc)
+{
+    double s = 0.0;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        double2 a = v[i], b = w[i];
+        s += a.x * b.x + a.y * b.y;
+    }
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) atomicAdd(acc, s);
+}
+// w -= alpha v + beta_j vprev ;  nrm2[0] += |w|^2        (alpha = *alpha_p, beta_j = sqrt(*beta2_p) or 0 when null)
+__global__ void __launch_bounds__(256) axpy_norm_kernel(double2 *__restrict__ w, const double2 *__restrict__ v,
+                                                        const double2 *__restrict__ vprev, int64_t n,
+                                                        const double *alpha_p, const double *beta2_p, double *nrm2)
+{
+    const double alpha = *alpha_p, beta = beta2_p ? sqrt(*beta2_p) : 0.0;
+    double s = 0.0;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        double2 x = w[i], a = v[i];
+        x.x -= alpha * a.x; x.y -= alpha * a.y;
+        if (beta2_p) { double2 p = vprev[i]; x.x -= beta * p.x; x.y -= beta * p.y; }
+        w[i] = x;
+        s += x.x * x.x + x.y * x.y;
+    }
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) atomicAdd(nrm2, s);
+}
+// out = in / sqrt(*nrm2)   (out = 0 when the norm is 0: breakdown, detected by the host afterwards)
+__global__ void __launch_bounds__(256) scale_by_norm_kernel(const double2 *__restrict__ in, double2 *__restrict__ out,
+                                                            int64_t n, const double *nrm2)
+{
+    const double q = *nrm2, sc = q > 0.0 ? 1.0 / sqrt(q) : 0.0;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        double2 x = in[i];
+        out[i] = make_double2(sc * x.x, sc * x.y);
+    }
+}
+
+}  // namespace bse
+
+using namespace bse;
+
+extern "C" bse_status_t bse_lanczos_quadrature(bse_handle_t h, const void *dStart, int32_t steps, double *hAlpha,
+                                               double *hBeta, int32_t *hDone)
+{
+    if (!h || !dStart || steps < 1 || !hAlpha || !hBeta) return BSE_ERR_INVALID_ARG;
+    if (h->mode != BSE_MODE_TDA) return BSE_ERR_INVALID_ARG;
+    const int64_t n = h->N;
+    // workspace: three vectors + alpha[steps] + nrm2[steps + 1]
+    const size_t vec = (size_t)n * 16, scal = (size_t)(2 * steps + 2) * 8;
+    bse_status_t st = ensure_ws(h, 3 * vec + scal);
+    if (st) return st;
+    char *base = (char *)h->ws;
+    double2 *buf[3] = {(double2 *)base, (double2 *)(base + vec), (double2 *)(base + 2 * vec)};
+    double *d_alpha = (double *)(base + 3 * vec), *d_n2 = d_alpha + steps;
+    BSE_CUDA(cudaMemsetAsync(d_alpha, 0, scal, h->stream));
+    const int grid = h->num_sms * 2;
+    // beta_0^2 = |d|^2 ;  v_0 = d / beta_0
+    dot_re_kernel<<<grid, 256, 0, h->stream>>>((const double2 *)dStart, (const double2 *)dStart, n, d_n2);
+    scale_by_norm_kernel<<<grid, 256, 0, h->stream>>>((const double2 *)dStart, buf[0], n, d_n2);
+    count_launch(2);
+    int iv = 0, ip = 2, iw = 1;      // v_j, v_{j-1}, w
+    for (int j = 0; j < steps; ++j) {
+        if ((st = zero_block(h, buf[iw], n, n, 1))) return st;
+        if ((st = launch_apply_pass(h, h->R, 0, 1.0, buf[iv], n, buf[iw], n, 1))) return st;       // w = R v_j
+        // the oracle's order: subtract beta_j v_{j-1} first, alpha_j = Re(v_j^H w) (v_{j-1} is orthogonal to v_j,
+        // so the two orders agree to rounding); here alpha is taken first so that one fused pass does both updates
+        dot_re_kernel<<<grid, 256, 0, h->stream>>>(buf[iv], buf[iw], n, d_alpha + j);
+        axpy_norm_kernel<<<grid, 256, 0, h->stream>>>(buf[iw], buf[iv], buf[ip], n, d_alpha + j, j > 0 ? d_n2 + j : nullptr,
+                                                      d_n2 + j + 1);
+        scale_by_norm_kernel<<<grid, 256, 0, h->stream>>>(buf[iw], buf[iw], n, d_n2 + j + 1);
+        count_launch(3);
+        int t = ip; ip = iv; iv = iw; iw = t;
+    }
+    BSE_CUDA(cudaGetLastError());
+    std::vector<double> hs(2 * steps + 2);
+    BSE_CUDA(cudaMemcpyAsync(hs.data(), d_alpha, scal, cudaMemcpyDeviceToHost, h->stream));
+    BSE_CUDA(cudaStreamSynchronize(h->stream));
+    int done = steps;
+    hBeta[0] = std::sqrt(hs[steps]);
+    for (int j = 0; j < steps; ++j) {
+        hAlpha[j] = hs[j];
+        hBeta[j + 1] = std::sqrt(hs[steps + j + 1]);
+        if (!(hs[steps + j + 1] > 0.0)) { done = j + 1; break; }
+    }
+    if (hDone) *hDone = done;
+    return BSE_OK;
+}
+
+extern "C" bse_status_t bse_quadrature_resolvent(int32_t steps, const double *hAlpha, const double *hBeta,
+                                                 int32_t n_omega, const double *hOmega, double eta, void *hOut)
+{
+    if (steps < 1 || !hAlpha || !hBeta || n_omega < 0 || (n_omega && (!hOmega || !hOut))) return BSE_ERR_INVALID_ARG;
+    double *out = (double *)hOut;
+    for (int i = 0; i < n_omega; ++i) {
+        // f <- z - alpha_j - beta_{j+1}^2 / f, from the last coefficient up; complex arithmetic written out
+        double zr = hOmega[i], zi = eta;
+        double fr = zr - hAlpha[steps - 1], fi = zi;
+        for (int j = steps - 2; j >= 0; --j) {
+            double b2 = hBeta[j + 1] * hBeta[j + 1], den = fr * fr + fi * fi;
+            double qr = b2 * fr / den, qi = -b2 * fi / den;
+            fr = zr - hAlpha[j] - qr;
+            fi = zi - qi;
+        }
+        double den = fr * fr + fi * fi, b0 = hBeta[0] * hBeta[0];
+        out[2 * i] = b0 * fr / den;
+        out[2 * i + 1] = -b0 * fi / den;
+    }
+    return BSE_OK;
+}

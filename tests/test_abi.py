@@ -81,3 +81,16 @@ def test_host_heev_arrowhead_and_clusters(b):
     Tr = T.real.copy()
     w2, Z2 = b.host_heev(Tr, nz=6)
     assert np.linalg.norm(Tr @ Z2 - Z2 * w2[:6]) < 1e-12 and np.max(np.abs(Z2.imag)) < 1e-13
+
+
+def test_quadrature_resolvent_host_utility_matches_oracle(b, orc):
+    # host logic only: the continued fraction of a Jacobi matrix, against the oracle's and against (z - T)^-1 directly
+    m = 17
+    rng_a = np.linspace(1.0, 3.0, m) + 0.1 * np.cos(np.arange(m))
+    beta = np.concatenate([[2.5], 0.3 + 0.05 * np.arange(m)])
+    om = np.linspace(0.0, 4.0, 33)
+    G = b.quadrature_resolvent(rng_a, beta, om, 0.07)
+    assert np.max(np.abs(G - orc.quadrature_resolvent(rng_a, beta, om, 0.07))) < 1e-13 * np.max(np.abs(G))
+    T = np.diag(rng_a) + np.diag(beta[1:m], 1) + np.diag(beta[1:m], -1)
+    direct = np.array([beta[0] ** 2 * np.linalg.inv((w + 0.07j) * np.eye(m) - T)[0, 0] for w in om])
+    assert np.max(np.abs(G - direct)) < 1e-11 * np.max(np.abs(direct))
