@@ -204,6 +204,10 @@ def run_cuda(args, cfg):
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - t0) * 1e3 / args.steps
     e2e_ms = max_over_ranks(e2e_ms, dist, "cuda")
+    if dist is not None:
+        barrier()
+        dist.destroy_process_group()
+        dist = None
     if rank != 0:
         return
 
