@@ -3,6 +3,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <atomic>
+#include <cstdio>
+#include <cstdlib>
 
 #include "../../include/bse.h"
 
@@ -30,10 +32,15 @@ namespace bse {
 extern std::atomic<int64_t> g_launches;
 inline void count_launch(int n = 1) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
-#define BSE_CUDA(call)                                   \
-    do {                                                 \
-        cudaError_t e__ = (call);                        \
-        if (e__ != cudaSuccess) return BSE_ERR_CUDA;     \
+// BSE_VERBOSE=1 prints the failing CUDA call (status codes alone cannot say which one it was)
+#define BSE_CUDA(call)                                                                                   \
+    do {                                                                                                 \
+        cudaError_t e__ = (call);                                                                        \
+        if (e__ != cudaSuccess) {                                                                        \
+            if (getenv("BSE_VERBOSE"))                                                                   \
+                fprintf(stderr, "[bse] %s:%d %s -> %s\n", __FILE__, __LINE__, #call, cudaGetErrorString(e__)); \
+            return BSE_ERR_CUDA;                                                                         \
+        }                                                                                                \
     } while (0)
 
 bse_status_t ensure_ws(bse_handle_s *h, size_t bytes);
