@@ -4,6 +4,7 @@
 #include <new>
 
 #include "apply_kernel.cuh"
+#include "apply_kernel_k1.cuh"
 #include "bse_internal.h"
 #include "tile_layout.cuh"
 
@@ -55,8 +56,11 @@ bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, dou
     static bool attr_set = false;
     if (!attr_set) {
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_k1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         attr_set = true;
     }
+    bool use_k1 = true;                                // BSE_APPLY_K1=0: tensor-core kernel for single columns too
+    if (const char *e = getenv("BSE_APPLY_K1")) use_k1 = atoi(e) != 0;
     ApplyParams p;
     p.tiles = tiles;
     p.N = h->N;
@@ -78,7 +82,10 @@ bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, dou
         p.kc = (k - c0) < 4 ? (k - c0) : 4;
         p.X = reinterpret_cast<const double2 *>(dX) + (int64_t)c0 * ldx;
         p.Y = reinterpret_cast<double *>(dY) + 2 * (int64_t)c0 * ldy;
-        apply_tiles_kernel<<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+        if (p.kc == 1 && use_k1)
+            apply_tiles_k1_kernel<<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);     // plain-FMA single-column variant
+        else
+            apply_tiles_kernel<<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
         count_launch();
     }
     BSE_CUDA(cudaGetLastError());
