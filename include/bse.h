@@ -135,7 +135,9 @@ bse_status_t bse_apply_host(bse_handle_t h, const void *hX, int64_t ldx, void *h
  *   dBV  : NULL -> Euclidean complex inner product <x, y> = x^H y (TDA);
  *          else the n x m block P(V) and the REAL inner product <x, y> = Re(x^H P(y)) with real
  *          coefficients (full mode, reading S4); then dBW (n x k, = P(W) on entry) is
- *          required and is updated consistently (dBW_out = P(W_out));
+ *          required and is updated by the same linear combination as W, so dBW_out = P(W_out) up
+ *          to kappa(W_in) * eps: for an ill-conditioned block re-apply P afterwards (bse_solve
+ *          does, reading R3);
  *   dW   : n x k block, overwritten with the orthonormalised block;
  *   dHcoef: m x k (ld = m) device output, complex128 (imaginary parts 0 in the real case), nullable;
  *   dBfac : k x k (ld = k) device output, upper triangular, positive real diagonal, nullable;

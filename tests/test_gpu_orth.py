@@ -111,3 +111,32 @@ def test_P_inner_product_orth(orc):
     assert np.linalg.norm((Q.conj().T @ PQ).real - np.eye(k)) <= TOL_ORTH
     assert np.linalg.norm(PQ - orc.apply_half(R, C, Q, +1)) / np.linalg.norm(PQ) <= 1e-12
     assert np.linalg.norm(W - X @ h.real - Q @ B.real) / np.linalg.norm(W) <= 1e-13
+
+
+def test_P_inner_product_rank_deficient_and_ill_conditioned(orc):
+    """Full-mode inner product, column-wise path: one column nearly dependent on another (kappa ~ 1e6), one exactly
+    dependent on the basis and a previous column.  Coefficients stay real and the factorisation holds to rounding;
+    PW is carried by linear combination (include/bse.h), so P-orthonormality and PW = P(W) hold to kappa * eps."""
+    import paper_2504_10096_b200 as b
+    N, m, k = 256, 6, 4
+    R = gen.dense_R(N, 4, sigma=1.0); C = gen.dense_C(N, 4)
+    h_ = b.Bse(b.MODE_FULL, N, pack(R, 0), pack(C, 1))
+    X = gen.block_X(N, m, 6)
+    PX = orc.apply_half(R, C, X, +1)
+    Li = np.linalg.inv(np.linalg.cholesky((X.conj().T @ PX).real)).T
+    X, PX = X @ Li, PX @ Li
+    W = gen.block_X(N, k, 7)
+    W[:, 2] = W[:, 0] + 1e-6 * W[:, 2]                 # ill-conditioned pair
+    W[:, 3] = 2.0 * W[:, 1] - 0.5 * X[:, 2]            # exactly dependent (real combination)
+    PW = orc.apply_half(R, C, W, +1)
+    Wd, PWd = to_dev(W), to_dev(PW)
+    hc, bf, rank = h_.orth(to_dev(X), Wd, to_dev(PX), PWd)
+    Q, PQ, h, B = to_host(Wd), to_host(PWd), to_host(hc), to_host(bf)
+    assert rank == 3 and B[3, 3] == 0
+    assert np.max(np.abs(h.imag)) == 0 and np.max(np.abs(B.imag)) == 0
+    PQ_true = orc.apply_half(R, C, Q, +1)
+    assert np.linalg.norm((PX.conj().T @ Q).real) <= 1e-11
+    assert np.linalg.norm(PQ - PQ_true) / np.linalg.norm(PQ) <= 1e-9                        # kappa * eps
+    assert np.linalg.norm((Q.conj().T @ PQ).real - np.eye(k)) <= 1e-9
+    assert np.linalg.norm((Q.conj().T @ PQ_true).real - np.eye(k)) <= 1e-9
+    assert np.linalg.norm(W - X @ h.real - Q @ B.real) / np.linalg.norm(W) <= 1e-12

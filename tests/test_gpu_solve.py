@@ -217,3 +217,15 @@ def test_config4_size_closed_form():
     h, lam = _closed_tda(98304, 23)
     res = h.solve(24, 8, tol=1e-8, seed=2)
     assert np.max(np.abs(res.omega - lam[:24]) / lam[:24]) <= TOL_EIG
+
+
+@pytest.mark.parametrize("seed", [2, 3])
+def test_config0_other_matrix_seeds(orc, seed):
+    """repeat config 0 with seeds 2 and 3 (new matrix, new start block)."""
+    import paper_2504_10096_b200 as b
+    cfg = gen.CONFIGS[0]
+    R = gen.dense_R(cfg["N"], seed, sigma=1.0, group=cfg["group"])
+    res = b.Bse(b.MODE_TDA, cfg["N"], pack(R, 0)).solve(cfg["nev"], cfg["k"], tol=1e-8, seed=seed)
+    _check_tda(orc, R, res, cfg["nev"], np.linalg.eigvalsh(R))
+    w_o, _, _, steps = orc.lanczos_tda(R, cfg["nev"], 1e-10, gen.block_X(cfg["N"], 1, 90 + seed)[:, 0], check=20)
+    assert steps > 0 and np.max(np.abs(res.omega - w_o) / np.abs(w_o)) <= TOL_EIG
