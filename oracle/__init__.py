@@ -57,6 +57,7 @@ def _load():
         lib.orc_lanczos_full.argtypes = [_i64, _c128, _c128, ctypes.c_int, ctypes.c_double, ctypes.c_int,
                                          ctypes.c_int, _c128, _f64, _c128, _f64]
         lib.orc_lanczos_full.restype = ctypes.c_int
+        lib.orc_round_c64.argtypes = [_i64, _c128, _c128]
         lib.orc_lanczos_quadrature.argtypes = [_i64, _c128, _c128, ctypes.c_int, _f64, _f64]
         lib.orc_lanczos_quadrature.restype = ctypes.c_int
         lib.orc_quadrature_resolvent.argtypes = [ctypes.c_int, _f64, _f64, ctypes.c_int, _f64, ctypes.c_double, _c128]
@@ -195,4 +196,13 @@ def quadrature_resolvent(alpha, beta, omega, eta):
     omega = np.ascontiguousarray(omega, dtype=np.float64)
     out = np.zeros(len(omega), dtype=np.complex128)
     _load().orc_quadrature_resolvent(len(alpha), alpha, beta, len(omega), omega, float(eta), out)
+    return out
+
+
+def round_c64(A):
+    """The complex64-stored operand: every real and imaginary part rounded to
+    the nearest IEEE binary32 value, ties to even; returned as complex128."""
+    A = _c(A)
+    out = np.empty_like(A)
+    _load().orc_round_c64(A.size, A.reshape(-1), out.reshape(-1))
     return out

@@ -602,3 +602,39 @@ void orc_quadrature_resolvent(int steps, const double *alpha, const double *beta
         out[i] = beta[0] * beta[0] / f;
     }
 }
+
+/* ------------------------------------------------------------------------------------------
+ * Single-precision operand.  PAPER.md:111 and the caption of Table 2
+ * (PAPER.md:115): the paper's BSE matrices are computed and stored in single precision.  The
+ * complex64-stored operator is, by definition, the matrix whose entries are the IEEE 754 binary32
+ * round-to-nearest-even images of the real and imaginary parts; everything downstream (apply,
+ * Lanczos) is the same FP64 arithmetic on that matrix.  The rounding is written out from the
+ * format's definition (24-bit significand, exponents 2^-126 .. 2^127, gradual underflow with
+ * quantum 2^-149) instead of a cast, so that it can be checked by eye:
+ *     x = m 2^e, 1/2 <= |m| < 1     ->  rint(m 2^24) 2^(e-24)      (normal range, e >= -125)
+ *                                   ->  rint(x 2^149) 2^-149       (below 2^-126)
+ *     |result| >= 2^128             ->  +-infinity
+ * rint() rounds to nearest, ties to even, in the default rounding mode.
+ * Pins (tests/test_oracle_c64.py): hand-computed ties and neighbours of 1, the error bound
+ * |fl(x) - x| <= 2^-24 |x|, idempotence, exact agreement with the hardware conversion (numpy
+ * astype) on random and special inputs, Weyl's bound for the eigenvalues of the rounded matrix.
+ * ------------------------------------------------------------------------------------------ */
+static double round_binary32(double x)
+{
+    if (x == 0.0 || isnan(x) || isinf(x)) return x;
+    int e;
+    double m = frexp(x, &e);                       /* x = m 2^e, 1/2 <= |m| < 1 */
+    double r;
+    if (e >= -125) r = ldexp(rint(ldexp(m, 24)), e - 24);
+    else r = ldexp(rint(ldexp(x, 149)), -149);
+    if (fabs(r) >= ldexp(1.0, 128)) r = copysign(INFINITY, x);
+    return r;
+}
+void orc_round_c64(int64_t n, const zc *in, zc *out)
+{
+    double *o = (double *)out;                     /* parts written separately: re + I*im would turn -0 into +0 */
+    for (int64_t i = 0; i < n; ++i) {
+        o[2 * i] = round_binary32(creal(in[i]));
+        o[2 * i + 1] = round_binary32(cimag(in[i]));
+    }
+}
