@@ -250,6 +250,19 @@ def run_cuda(args, cfg):
                                       "GBps": alg_bytes(N, 1) * qsteps / qsec / 1e9}
         del h, tiles
         torch.cuda.empty_cache()
+        # complex64-stored operand: same N, half the stored bytes, FP64 arithmetic.
+        # Bytes are the complex64 store's; from k = 3 on the bound is the FP64 pipe, not HBM (ridge at 8 N^2 k / 37.1 TF).
+        t64 = b.bse_fill_synthetic(N, b.MATRIX_R, 1, 0.0, cfg["group"], storage=b.STORE_C64)
+        h64 = b.Bse(b.MODE_TDA, N, t64, storage=b.STORE_C64)
+        sweep64 = {}
+        for kk in (1, 2, 4, 8):
+            Xs, Ys = Xh[:kk].cuda(), torch.empty((kk, N), dtype=torch.complex128, device="cuda")
+            m = time_steps(lambda: h64.apply(Xs, Ys), max(3, args.steps // 2), 2)
+            by = 8.0 * N * (N + 1) / 2 + 32.0 * N * kk
+            sweep64[str(kk)] = {"ms": m, "GBps": by / (m * 1e-3) / 1e9, "tflops": 8.0 * N * N * kk / (m * 1e-3) / 1e12}
+        line["apply_vs_k_c64_store"] = sweep64
+        del h64, t64
+        torch.cuda.empty_cache()
         c2 = gen.CONFIGS[2]
         h2 = b.Bse(b.MODE_TDA, c2["N"], b.bse_fill_synthetic(c2["N"], b.MATRIX_R, 1, 0.0, c2["group"]))
         t0 = time.perf_counter()

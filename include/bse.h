@@ -33,6 +33,14 @@
  * of 16 bytes -- the order in which the FP64 tensor-core fragments of the apply kernel read it
  * from shared memory without bank conflicts, both as T and as T^H.  The layout is opaque to
  * callers: fill it with bse_pack_from_dense / bse_fill_synthetic / bse_fill_closed_form_*.
+ *
+ * Storage type (`storage` argument): BSE_STORE_C128 keeps the entries as complex128 (the layout
+ * above).  BSE_STORE_C64 keeps each entry as two IEEE binary32 values (the paper's matrices are
+ * single precision, PAPER.md:111 and the caption of Table 2): every size above
+ * halves (32768-byte tiles, 512-byte patches, 8-byte slots, same order), entries are rounded to
+ * nearest-even when the store is written, and the operator every later call works with IS the
+ * rounded matrix: fragments are widened to FP64 on load and all arithmetic, vectors and results
+ * stay complex128.  Half the HBM bytes per apply, twice the N per GPU.
  */
 #ifndef BSE_B200_H
 #define BSE_B200_H
@@ -57,6 +65,7 @@ typedef enum {
 
 enum { BSE_MODE_TDA = 0, BSE_MODE_FULL = 1 };
 enum { BSE_MATRIX_R = 0, BSE_MATRIX_C = 1 };
+enum { BSE_STORE_C128 = 0, BSE_STORE_C64 = 1 };
 
 typedef struct {
     int32_t n_apply;        /* operator applications (block applies; a full-mode step counts 2 half applies) */
@@ -69,18 +78,22 @@ typedef struct {
 
 const char *bse_status_string(bse_status_t s);
 
-/* Tile geometry for an N x N matrix: *tile = 64, *n_tiles = nt (nt+1)/2, *bytes = n_tiles * 65536.
- * N < 1 -> BSE_ERR_INVALID_ARG.  Output pointers may be NULL. */
-bse_status_t bse_layout(int64_t N, int32_t *tile, int64_t *n_tiles, int64_t *bytes_per_matrix);
+/* Tile geometry for an N x N matrix: *tile = 64, *n_tiles = nt (nt+1)/2, *bytes = n_tiles * 65536
+ * (BSE_STORE_C128) or n_tiles * 32768 (BSE_STORE_C64).  N < 1 or an unknown storage ->
+ * BSE_ERR_INVALID_ARG (every call below with a `storage` argument rejects unknown values the same
+ * way).  Output pointers may be NULL. */
+bse_status_t bse_layout(int64_t N, int32_t storage, int32_t *tile, int64_t *n_tiles,
+                        int64_t *bytes_per_matrix);
 
 /* dTiles <- lower triangle of the dense column-major N x N matrix dDense (leading dimension ld);
  * which = BSE_MATRIX_R (Hermitian: mirror is the conjugate, diagonal imaginary part dropped) or
- * BSE_MATRIX_C (symmetric: mirror is a copy).  Only entries (i, j) with j <= i are read. */
+ * BSE_MATRIX_C (symmetric: mirror is a copy).  Only entries (i, j) with j <= i are read.  dDense is
+ * complex128 for both storage types. */
 bse_status_t bse_pack_from_dense(const void *dDense, int64_t ld, int64_t N, int32_t which,
-                                 void *dTiles, void *stream);
+                                 void *dTiles, int32_t storage, void *stream);
 
 /* dDense (column-major, ld) <- the full N x N matrix the tiles represent (both triangles). Test helper. */
-bse_status_t bse_unpack_to_dense(const void *dTiles, int64_t N, int32_t which,
+bse_status_t bse_unpack_to_dense(const void *dTiles, int32_t storage, int64_t N, int32_t which,
                                  void *dDense, int64_t ld, void *stream);
 
 /* The synthetic "BSE-shaped" generator of BASELINE.json, evaluated on the device
@@ -88,27 +101,28 @@ bse_status_t bse_unpack_to_dense(const void *dTiles, int64_t N, int32_t which,
  *   R = diag(d_eps + sigma) + K,  K_ij = 0.1 (g1 + i g2) / (1 + |i-j|/64), d_eps ~ U[1,10] sorted in
  *   groups of `group` indices;  C_ij = C_ji = 0.05 (g1 + i g2) / (1 + |i-j|/64).
  * N % group != 0 -> BSE_ERR_INVALID_ARG (which = R only). */
-bse_status_t bse_fill_synthetic(void *dTiles, int64_t N, int32_t which, uint64_t seed, double sigma,
-                                int32_t group, void *stream);
+bse_status_t bse_fill_synthetic(void *dTiles, int32_t storage, int64_t N, int32_t which, uint64_t seed,
+                                double sigma, int32_t group, void *stream);
 
 /* Closed-form instance with a prescribed spectrum: R = Q diag(lam) Q^H, Q = I - 2 u u^H,
  *   R_ij = lam_i d_ij - 2 u_i conj(u_j) (lam_i + lam_j - 2 s),  s = sum_l lam_l |u_l|^2.
  * dLam: N doubles (device), dU: N complex128 (device, unit 2-norm).  which=BSE_MATRIX_R only. */
-bse_status_t bse_fill_closed_form_tda(void *dTiles, int64_t N, const double *dLam, const void *dU,
-                                      double s, void *stream);
+bse_status_t bse_fill_closed_form_tda(void *dTiles, int32_t storage, int64_t N, const double *dLam,
+                                      const void *dU, double s, void *stream);
 
 /* Closed-form pair with omega_i = sqrt(d1_i d2_i): M+- = Q diag(d1|d2) Q^T (real Householder, dUr real
  * unit vector), R = U (M+ + M-)/2 U^H, C = U (M+ - M-)/2 U^T, U = diag(exp(i phi)).
  * All inputs are device arrays of N doubles; s1 = sum d1 u^2, s2 = sum d2 u^2. */
-bse_status_t bse_fill_closed_form_full(void *dRTiles, void *dCTiles, int64_t N, const double *dD1,
-                                       const double *dD2, const double *dUr, const double *dPhi,
-                                       double s1, double s2, void *stream);
+bse_status_t bse_fill_closed_form_full(void *dRTiles, void *dCTiles, int32_t storage, int64_t N,
+                                       const double *dD1, const double *dD2, const double *dUr,
+                                       const double *dPhi, double s1, double s2, void *stream);
 
 /* Creates a handle.  BORROWS dRTiles (and dCTiles in full mode): the caller keeps them alive and
  * unmodified until bse_destroy.  mode = BSE_MODE_TDA (dCTiles ignored, may be NULL) or BSE_MODE_FULL
- * (dCTiles required).  Does not verify Hermitian / symmetric / positive-definite structure.
- * Workspace O(N k) is allocated lazily by later calls with cudaMalloc. */
-bse_status_t bse_create(bse_handle_t *h, int32_t mode, int64_t N, const void *dRTiles,
+ * (dCTiles required); `storage` is the type both stores were written with.  Does not verify
+ * Hermitian / symmetric / positive-definite structure.  Workspace O(N k) is allocated lazily by
+ * later calls with cudaMalloc. */
+bse_status_t bse_create(bse_handle_t *h, int32_t mode, int32_t storage, int64_t N, const void *dRTiles,
                         const void *dCTiles, void *stream);
 bse_status_t bse_destroy(bse_handle_t h);
 

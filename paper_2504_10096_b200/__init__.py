@@ -15,6 +15,7 @@ _LIBPATH = os.path.join(_HERE, "libbse_b200.so")
 _lib = None
 
 MODE_TDA, MODE_FULL = 0, 1
+STORE_C128, STORE_C64 = 0, 1      # storage type of the tile store (include/bse.h)
 MATRIX_R, MATRIX_C = 0, 1
 TILE = 64
 TILE_BYTES = 65536
@@ -39,13 +40,13 @@ class _Info(ctypes.Structure):
 _vp, _i64, _i32, _u64, _dbl = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_uint64, ctypes.c_double
 
 _SIGNATURES = {
-    "bse_layout": [_i64, ctypes.POINTER(_i32), ctypes.POINTER(_i64), ctypes.POINTER(_i64)],
-    "bse_pack_from_dense": [_vp, _i64, _i64, _i32, _vp, _vp],
-    "bse_unpack_to_dense": [_vp, _i64, _i32, _vp, _i64, _vp],
-    "bse_fill_synthetic": [_vp, _i64, _i32, _u64, _dbl, _i32, _vp],
-    "bse_fill_closed_form_tda": [_vp, _i64, _vp, _vp, _dbl, _vp],
-    "bse_fill_closed_form_full": [_vp, _vp, _i64, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp],
-    "bse_create": [ctypes.POINTER(_vp), _i32, _i64, _vp, _vp, _vp],
+    "bse_layout": [_i64, _i32, ctypes.POINTER(_i32), ctypes.POINTER(_i64), ctypes.POINTER(_i64)],
+    "bse_pack_from_dense": [_vp, _i64, _i64, _i32, _vp, _i32, _vp],
+    "bse_unpack_to_dense": [_vp, _i32, _i64, _i32, _vp, _i64, _vp],
+    "bse_fill_synthetic": [_vp, _i32, _i64, _i32, _u64, _dbl, _i32, _vp],
+    "bse_fill_closed_form_tda": [_vp, _i32, _i64, _vp, _vp, _dbl, _vp],
+    "bse_fill_closed_form_full": [_vp, _vp, _i32, _i64, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp],
+    "bse_create": [ctypes.POINTER(_vp), _i32, _i32, _i64, _vp, _vp, _vp],
     "bse_destroy": [_vp],
     "bse_apply": [_vp, _vp, _i64, _vp, _i64, _i32],
     "bse_apply_half": [_vp, _i32, _vp, _i64, _vp, _i64, _i32],
@@ -90,16 +91,16 @@ def _stream_ptr():
     return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
 
 
-def bse_layout(N: int):
+def bse_layout(N: int, storage: int = STORE_C128):
     t, n, b = _i32(), _i64(), _i64()
-    _check(lib().bse_layout(N, ctypes.byref(t), ctypes.byref(n), ctypes.byref(b)), "bse_layout")
+    _check(lib().bse_layout(N, storage, ctypes.byref(t), ctypes.byref(n), ctypes.byref(b)), "bse_layout")
     return t.value, n.value, b.value
 
 
-def alloc_tiles(N: int):
+def alloc_tiles(N: int, storage: int = STORE_C128):
     """Uninitialised device buffer for one packed matrix (torch uint8 tensor)."""
     import torch
-    _, _, nbytes = bse_layout(N)
+    _, _, nbytes = bse_layout(N, storage)
     return torch.empty(nbytes, dtype=torch.uint8, device="cuda")
 
 
@@ -112,40 +113,42 @@ def _ld(t):
     return t.shape[-1]
 
 
-def bse_pack_from_dense(dense_cm, N: int, which: int, tiles=None):
+def bse_pack_from_dense(dense_cm, N: int, which: int, tiles=None, storage: int = STORE_C128):
     """dense_cm: torch complex128 CUDA tensor of shape (N, N) holding the matrix COLUMN-major
     (dense_cm[j, i] = A_ij), e.g. torch.from_numpy(A.T.copy()).cuda()."""
-    tiles = alloc_tiles(N) if tiles is None else tiles
-    _check(lib().bse_pack_from_dense(dense_cm.data_ptr(), N, N, which, tiles.data_ptr(), _stream_ptr()),
+    tiles = alloc_tiles(N, storage) if tiles is None else tiles
+    _check(lib().bse_pack_from_dense(dense_cm.data_ptr(), N, N, which, tiles.data_ptr(), storage, _stream_ptr()),
            "bse_pack_from_dense")
     return tiles
 
 
-def bse_unpack_to_dense(tiles, N: int, which: int):
+def bse_unpack_to_dense(tiles, N: int, which: int, storage: int = STORE_C128):
     import torch
     out = torch.zeros((N, N), dtype=torch.complex128, device="cuda")
-    _check(lib().bse_unpack_to_dense(tiles.data_ptr(), N, which, out.data_ptr(), N, _stream_ptr()),
+    _check(lib().bse_unpack_to_dense(tiles.data_ptr(), storage, N, which, out.data_ptr(), N, _stream_ptr()),
            "bse_unpack_to_dense")
     return out      # out[j, i] = A_ij
 
 
-def bse_fill_synthetic(N: int, which: int, seed: int, sigma: float = 0.0, group: int = 16, tiles=None):
-    tiles = alloc_tiles(N) if tiles is None else tiles
-    _check(lib().bse_fill_synthetic(tiles.data_ptr(), N, which, seed, sigma, group, _stream_ptr()),
+def bse_fill_synthetic(N: int, which: int, seed: int, sigma: float = 0.0, group: int = 16, tiles=None,
+                       storage: int = STORE_C128):
+    tiles = alloc_tiles(N, storage) if tiles is None else tiles
+    _check(lib().bse_fill_synthetic(tiles.data_ptr(), storage, N, which, seed, sigma, group, _stream_ptr()),
            "bse_fill_synthetic")
     return tiles
 
 
-def bse_fill_closed_form_tda(N: int, lam, u, s: float, tiles=None):
-    tiles = alloc_tiles(N) if tiles is None else tiles
-    _check(lib().bse_fill_closed_form_tda(tiles.data_ptr(), N, lam.data_ptr(), u.data_ptr(), s, _stream_ptr()),
+def bse_fill_closed_form_tda(N: int, lam, u, s: float, tiles=None, storage: int = STORE_C128):
+    tiles = alloc_tiles(N, storage) if tiles is None else tiles
+    _check(lib().bse_fill_closed_form_tda(tiles.data_ptr(), storage, N, lam.data_ptr(), u.data_ptr(), s,
+                                          _stream_ptr()),
            "bse_fill_closed_form_tda")
     return tiles
 
 
-def bse_fill_closed_form_full(N: int, d1, d2, ur, phi, s1: float, s2: float):
-    rt, ct = alloc_tiles(N), alloc_tiles(N)
-    _check(lib().bse_fill_closed_form_full(rt.data_ptr(), ct.data_ptr(), N, d1.data_ptr(), d2.data_ptr(),
+def bse_fill_closed_form_full(N: int, d1, d2, ur, phi, s1: float, s2: float, storage: int = STORE_C128):
+    rt, ct = alloc_tiles(N, storage), alloc_tiles(N, storage)
+    _check(lib().bse_fill_closed_form_full(rt.data_ptr(), ct.data_ptr(), storage, N, d1.data_ptr(), d2.data_ptr(),
                                            ur.data_ptr(), phi.data_ptr(), s1, s2, _stream_ptr()),
            "bse_fill_closed_form_full")
     return rt, ct
@@ -163,12 +166,12 @@ class SolveResult:
 class Bse:
     """Handle wrapper (bse_create / bse_destroy).  Keeps the borrowed tile buffers alive."""
 
-    def __init__(self, mode: int, N: int, r_tiles, c_tiles=None):
-        self.mode, self.N = mode, N
+    def __init__(self, mode: int, N: int, r_tiles, c_tiles=None, storage: int = STORE_C128):
+        self.mode, self.N, self.storage = mode, N, storage
         self._keep = (r_tiles, c_tiles)
         self.n_op = 2 * N if mode == MODE_FULL else N
         h = _vp()
-        _check(lib().bse_create(ctypes.byref(h), mode, N, r_tiles.data_ptr(),
+        _check(lib().bse_create(ctypes.byref(h), mode, storage, N, r_tiles.data_ptr(),
                                 c_tiles.data_ptr() if c_tiles is not None else None, _stream_ptr()), "bse_create")
         self._h = h
 

@@ -28,7 +28,7 @@
 
 namespace bse {
 
-constexpr int APPLY_STAGES = 3;
+constexpr int APPLY_STAGES = 3;                          // ring depth for 64 KB (complex128) tiles; 6 for 32 KB (complex64)
 constexpr int APPLY_CONSUMERS = 8;                       // consumer warps
 constexpr int APPLY_THREADS = (APPLY_CONSUMERS + 1) * 32;
 constexpr int APPLY_SMEM = APPLY_STAGES * TILE_BYTES + 128;
@@ -69,16 +69,22 @@ __device__ __forceinline__ void apply_decode_unit(int64_t u, int L, int &I, int 
     J1 = min(J0 + L, I + 1);
 }
 
+// ES = bytes per stored complex entry (bse_common.cuh): 16 -> LDS.128 fragments, 8 -> LDS.64 + conversion to FP64.
+template <int ES>
 __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const ApplyParams p)
 {
+    constexpr int TBY = TB * TB * ES;                    // tile bytes
+    constexpr int PBY = 64 * ES;                         // 8 x 8 patch bytes
+    constexpr int NST = APPLY_STAGES * 16 / ES;          // stages: the ring always fills the same 192 KB
+    constexpr int S1 = 16 * ES, S2 = 32 * ES;            // second k-step of the P1 / P2 fragment (16 / 32 slots on)
     extern __shared__ __align__(1024) char smem[];
     char *tile_s = smem;
-    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + APPLY_STAGES * TILE_BYTES);
-    uint64_t *full = bars, *empty = bars + APPLY_STAGES;
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + NST * TBY);
+    uint64_t *full = bars, *empty = bars + NST;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
-        for (int s = 0; s < APPLY_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], APPLY_CONSUMERS); }
+        for (int s = 0; s < NST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], APPLY_CONSUMERS); }
         fence_barrier_init();
     }
     __syncthreads();
@@ -92,12 +98,12 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
             for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
                 int I, J0, J1;
                 apply_decode_unit(u, p.L, I, J0, J1);
-                const char *src = p.tiles + tile_index(I, J0) * (int64_t)TILE_BYTES;
-                for (int J = J0; J < J1; ++J, src += TILE_BYTES) {
+                const char *src = p.tiles + tile_index(I, J0) * (int64_t)TBY;
+                for (int J = J0; J < J1; ++J, src += TBY) {
                     mbar_wait(&empty[st], ph ^ 1);
-                    mbar_expect_tx(&full[st], (uint32_t)TILE_BYTES);
-                    bulk_g2s_hint(tile_s + st * TILE_BYTES, src, TILE_BYTES, &full[st], pol);
-                    if (++st == APPLY_STAGES) { st = 0; ph ^= 1; }
+                    mbar_expect_tx(&full[st], (uint32_t)TBY);
+                    bulk_g2s_hint(tile_s + st * TBY, src, TBY, &full[st], pol);
+                    if (++st == NST) { st = 0; ph ^= 1; }
                 }
             }
         }
@@ -109,8 +115,8 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
     const int g = lane >> 2, t = lane & 3;
     const int g2 = (g >> 2) & 1, g1 = (g >> 1) & 1, g0 = g & 1, t1 = (t >> 1) & 1, t0 = t & 1;
     // fragment byte offsets inside a patch (see patch_slot): P1 reads (a = g, b = 4 s + t), P2 reads (a = 4 s + t, b = g)
-    const int offP1 = (((g2 << 2) | g1) * 8 + ((g0 << 2) | (t0 << 1) | (g1 ^ t1))) * 16;   // + s * 256
-    const int offP2 = (((g2 << 1) | t1) * 8 + ((t0 << 2) | (g0 << 1) | (t1 ^ g1))) * 16;   // + s * 512
+    const int offP1 = (((g2 << 2) | g1) * 8 + ((g0 << 2) | (t0 << 1) | (g1 ^ t1))) * ES;   // + s * S1
+    const int offP2 = (((g2 << 1) | t1) * 8 + ((t0 << 2) | (g0 << 1) | (t1 ^ g1))) * ES;   // + s * S2
     // B fragments: lane supplies B[kk = t][n = g], n = 2 c + part
     const int col = g >> 1, part = g & 1;
     const bool colok = col < p.kc;
@@ -180,7 +186,7 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
             if (J + 1 < J1) load_xj(J + 1, xjn);            // prefetch the next tile's x_J fragments
 
             mbar_wait(&full[st], ph);
-            const char *tp = tile_s + st * TILE_BYTES + w * 8 * PATCH_BYTES;
+            const char *tp = tile_s + st * TBY + w * 8 * PBY;
             if (I != J) {
                 double C2[4][2];
 #pragma unroll
@@ -188,15 +194,15 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
                 // two patches at a time, four independent accumulator chains interleaved: dependent DMMAs are 4 apart
 #pragma unroll
                 for (int ib = 0; ib < 8; ib += 2) {
-                    const char *pp = tp + ib * PATCH_BYTES, *pq = pp + PATCH_BYTES;
-                    double2 a0 = *reinterpret_cast<const double2 *>(pp + offP1);
-                    double2 c0 = *reinterpret_cast<const double2 *>(pq + offP1);
-                    double2 b0 = *reinterpret_cast<const double2 *>(pp + offP2);
-                    double2 d0 = *reinterpret_cast<const double2 *>(pq + offP2);
-                    double2 a1 = *reinterpret_cast<const double2 *>(pp + offP1 + 256);
-                    double2 c1 = *reinterpret_cast<const double2 *>(pq + offP1 + 256);
-                    double2 b1 = *reinterpret_cast<const double2 *>(pp + offP2 + 512);
-                    double2 d1 = *reinterpret_cast<const double2 *>(pq + offP2 + 512);
+                    const char *pp = tp + ib * PBY, *pq = pp + PBY;
+                    double2 a0 = load_frag<ES>(pp + offP1);
+                    double2 c0 = load_frag<ES>(pq + offP1);
+                    double2 b0 = load_frag<ES>(pp + offP2);
+                    double2 d0 = load_frag<ES>(pq + offP2);
+                    double2 a1 = load_frag<ES>(pp + offP1 + S1);
+                    double2 c1 = load_frag<ES>(pq + offP1 + S1);
+                    double2 b1 = load_frag<ES>(pp + offP2 + S2);
+                    double2 d1 = load_frag<ES>(pq + offP2 + S2);
                     const int q = ib & 2;
                     dmma(C1[ib], a0.x, BaJ[0]);
                     dmma(C1[ib + 1], c0.x, BaJ[0]);
@@ -243,8 +249,8 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
                     double2 a0[4], a1[4];
 #pragma unroll
                     for (int r = 0; r < 4; ++r) {
-                        a0[r] = *reinterpret_cast<const double2 *>(tp + (ib + r) * PATCH_BYTES + offP1);
-                        a1[r] = *reinterpret_cast<const double2 *>(tp + (ib + r) * PATCH_BYTES + offP1 + 256);
+                        a0[r] = load_frag<ES>(tp + (ib + r) * PBY + offP1);
+                        a1[r] = load_frag<ES>(tp + (ib + r) * PBY + offP1 + S1);
                     }
 #pragma unroll
                     for (int r = 0; r < 4; ++r) dmma(C1[ib + r], a0[r].x, BaJ[0]);
@@ -262,7 +268,7 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
                 if (lane == 0)
                     mbar_arrive(reinterpret_cast<uint64_t *>(reinterpret_cast<char *>(&empty[st]) + (live & p.zero)));
             }
-            if (++st == APPLY_STAGES) { st = 0; ph ^= 1; }
+            if (++st == NST) { st = 0; ph ^= 1; }
         }
         // flush this warp's partial Y_I (all 64 rows, column t)
         if (t < kc) {

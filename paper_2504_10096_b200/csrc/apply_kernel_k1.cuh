@@ -20,16 +20,18 @@ __device__ __forceinline__ void cfma(double2 &acc, const double2 a, const double
     acc.y = fma(a.x, x.y, acc.y); acc.y = fma(a.y, x.x, acc.y);
 }
 
+template <int ES>
 __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_k1_kernel(const ApplyParams p)
 {
+    constexpr int TBY = TB * TB * ES, PBY = 64 * ES, NST = APPLY_STAGES * 16 / ES, S1 = 16 * ES, S2 = 32 * ES;
     extern __shared__ __align__(1024) char smem[];
     char *tile_s = smem;
-    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + APPLY_STAGES * TILE_BYTES);
-    uint64_t *full = bars, *empty = bars + APPLY_STAGES;
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + NST * TBY);
+    uint64_t *full = bars, *empty = bars + NST;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
-        for (int s = 0; s < APPLY_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], APPLY_CONSUMERS); }
+        for (int s = 0; s < NST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], APPLY_CONSUMERS); }
         fence_barrier_init();
     }
     __syncthreads();
@@ -42,12 +44,12 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_k1_kernel(const 
             for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
                 int I, J0, J1;
                 apply_decode_unit(u, p.L, I, J0, J1);
-                const char *src = p.tiles + tile_index(I, J0) * (int64_t)TILE_BYTES;
-                for (int J = J0; J < J1; ++J, src += TILE_BYTES) {
+                const char *src = p.tiles + tile_index(I, J0) * (int64_t)TBY;
+                for (int J = J0; J < J1; ++J, src += TBY) {
                     mbar_wait(&empty[st], ph ^ 1);
-                    mbar_expect_tx(&full[st], (uint32_t)TILE_BYTES);
-                    bulk_g2s_hint(tile_s + st * TILE_BYTES, src, TILE_BYTES, &full[st], pol);
-                    if (++st == APPLY_STAGES) { st = 0; ph ^= 1; }
+                    mbar_expect_tx(&full[st], (uint32_t)TBY);
+                    bulk_g2s_hint(tile_s + st * TBY, src, TBY, &full[st], pol);
+                    if (++st == NST) { st = 0; ph ^= 1; }
                 }
             }
         }
@@ -57,8 +59,8 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_k1_kernel(const 
     const int w = warp;
     const int g = lane >> 2, t = lane & 3;
     const int g2 = (g >> 2) & 1, g1 = (g >> 1) & 1, g0 = g & 1, t1 = (t >> 1) & 1, t0 = t & 1;
-    const int offP1 = (((g2 << 2) | g1) * 8 + ((g0 << 2) | (t0 << 1) | (g1 ^ t1))) * 16;   // + s * 256
-    const int offP2 = (((g2 << 1) | t1) * 8 + ((t0 << 2) | (g0 << 1) | (t1 ^ g1))) * 16;   // + s * 512
+    const int offP1 = (((g2 << 2) | g1) * 8 + ((g0 << 2) | (t0 << 1) | (g1 ^ t1))) * ES;   // + s * S1
+    const int offP2 = (((g2 << 1) | t1) * 8 + ((t0 << 2) | (g0 << 1) | (t1 ^ g1))) * ES;   // + s * S2
     const bool herm = (p.pass == PASS_HERM);
     const double sgn = p.sign;
     const double2 zero2 = make_double2(0.0, 0.0);
@@ -101,17 +103,17 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_k1_kernel(const 
             if (J + 1 < J1) load_xj(J + 1, xjn);            // prefetch the next tile's x_J rows
 
             mbar_wait(&full[st], ph);
-            const char *tp = tile_s + st * TILE_BYTES + w * 8 * PATCH_BYTES;
+            const char *tp = tile_s + st * TBY + w * 8 * PBY;
             int live = 0;
             if (I != J) {
                 double2 acc2[2] = {zero2, zero2};
 #pragma unroll
                 for (int ib = 0; ib < 8; ++ib) {
-                    const char *pp = tp + ib * PATCH_BYTES;
-                    const double2 a0 = *reinterpret_cast<const double2 *>(pp + offP1);
-                    const double2 a1 = *reinterpret_cast<const double2 *>(pp + offP1 + 256);
-                    const double2 b0 = *reinterpret_cast<const double2 *>(pp + offP2);
-                    const double2 b1 = *reinterpret_cast<const double2 *>(pp + offP2 + 512);
+                    const char *pp = tp + ib * PBY;
+                    const double2 a0 = load_frag<ES>(pp + offP1);
+                    const double2 a1 = load_frag<ES>(pp + offP1 + S1);
+                    const double2 b0 = load_frag<ES>(pp + offP2);
+                    const double2 b1 = load_frag<ES>(pp + offP2 + S2);
                     cfma(acc1[ib], a0, xj0);
                     cfma(acc2[0], b0, xi[ib][0]);
                     cfma(acc1[ib], a1, xj1);
@@ -137,9 +139,9 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_k1_kernel(const 
             } else {
 #pragma unroll
                 for (int ib = 0; ib < 8; ++ib) {
-                    const char *pp = tp + ib * PATCH_BYTES;
-                    const double2 a0 = *reinterpret_cast<const double2 *>(pp + offP1);
-                    const double2 a1 = *reinterpret_cast<const double2 *>(pp + offP1 + 256);
+                    const char *pp = tp + ib * PBY;
+                    const double2 a0 = load_frag<ES>(pp + offP1);
+                    const double2 a1 = load_frag<ES>(pp + offP1 + S1);
                     cfma(acc1[ib], a0, xj0);
                     cfma(acc1[ib], a1, xj1);
                 }
@@ -149,7 +151,7 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_k1_kernel(const 
                 if (lane == 0)
                     mbar_arrive(reinterpret_cast<uint64_t *>(reinterpret_cast<char *>(&empty[st]) + (live & p.zero)));
             }
-            if (++st == APPLY_STAGES) { st = 0; ph ^= 1; }
+            if (++st == NST) { st = 0; ph ^= 1; }
         }
         // flush this warp's partial Y_I: sum over the four t-lanes, lane t == 0 adds rows 8 ib + g
 #pragma unroll

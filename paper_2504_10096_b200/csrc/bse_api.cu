@@ -55,8 +55,10 @@ bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, dou
 {
     static bool attr_set = false;
     if (!attr_set) {
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_k1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_k1_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_k1_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         attr_set = true;
     }
     bool use_k1 = true;                                // BSE_APPLY_K1=0: tensor-core kernel for single columns too
@@ -82,10 +84,14 @@ bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, dou
         p.kc = (k - c0) < 4 ? (k - c0) : 4;
         p.X = reinterpret_cast<const double2 *>(dX) + (int64_t)c0 * ldx;
         p.Y = reinterpret_cast<double *>(dY) + 2 * (int64_t)c0 * ldy;
-        if (p.kc == 1 && use_k1)
-            apply_tiles_k1_kernel<<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);     // plain-FMA single-column variant
-        else
-            apply_tiles_kernel<<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+        const bool k1 = p.kc == 1 && use_k1;                 // plain-FMA single-column variant
+        if (h->es == ES_C128) {
+            if (k1) apply_tiles_k1_kernel<16><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            else apply_tiles_kernel<16><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+        } else {
+            if (k1) apply_tiles_k1_kernel<8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            else apply_tiles_kernel<8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+        }
         count_launch();
     }
     BSE_CUDA(cudaGetLastError());
@@ -119,48 +125,55 @@ bse_status_t bse_host_heev(int32_t m, void *hA, int32_t lda, double *hW, void *h
     return host_heev(m, hA, lda, hW, hZ, ldz, nz) ? BSE_ERR_INTERNAL : BSE_OK;
 }
 
-bse_status_t bse_layout(int64_t N, int32_t *tile, int64_t *n_tiles, int64_t *bytes_per_matrix)
+static inline bool storage_ok(int32_t storage) { return storage == BSE_STORE_C128 || storage == BSE_STORE_C64; }
+static inline int storage_es(int32_t storage) { return storage == BSE_STORE_C64 ? ES_C64 : ES_C128; }
+
+bse_status_t bse_layout(int64_t N, int32_t storage, int32_t *tile, int64_t *n_tiles, int64_t *bytes_per_matrix)
 {
-    if (N < 1) return BSE_ERR_INVALID_ARG;
+    if (N < 1 || !storage_ok(storage)) return BSE_ERR_INVALID_ARG;
     int64_t nt = (N + TB - 1) / TB;
     if (tile) *tile = TB;
     if (n_tiles) *n_tiles = nt * (nt + 1) / 2;
-    if (bytes_per_matrix) *bytes_per_matrix = nt * (nt + 1) / 2 * (int64_t)TILE_BYTES;
+    if (bytes_per_matrix) *bytes_per_matrix = nt * (nt + 1) / 2 * tile_bytes_es(storage_es(storage));
     return BSE_OK;
 }
 
-bse_status_t bse_pack_from_dense(const void *dDense, int64_t ld, int64_t N, int32_t which, void *dTiles, void *stream)
+bse_status_t bse_pack_from_dense(const void *dDense, int64_t ld, int64_t N, int32_t which, void *dTiles,
+                                 int32_t storage, void *stream)
 {
-    if (!dDense || !dTiles || N < 1 || ld < N || (which != 0 && which != 1)) return BSE_ERR_INVALID_ARG;
+    if (!dDense || !dTiles || N < 1 || ld < N || (which != 0 && which != 1) || !storage_ok(storage))
+        return BSE_ERR_INVALID_ARG;
     int64_t n_tiles;
-    bse_layout(N, nullptr, &n_tiles, nullptr);
+    bse_layout(N, storage, nullptr, &n_tiles, nullptr);
     dim3 grid;
     tile_grid(n_tiles, grid);
     pack_from_dense_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((const double2 *)dDense, ld, N, which,
-                                                                   (char *)dTiles, n_tiles);
+                                                                   (char *)dTiles, storage_es(storage), n_tiles);
     count_launch();
     BSE_CUDA(cudaGetLastError());
     return BSE_OK;
 }
 
-bse_status_t bse_unpack_to_dense(const void *dTiles, int64_t N, int32_t which, void *dDense, int64_t ld, void *stream)
+bse_status_t bse_unpack_to_dense(const void *dTiles, int32_t storage, int64_t N, int32_t which, void *dDense,
+                                 int64_t ld, void *stream)
 {
-    if (!dDense || !dTiles || N < 1 || ld < N || (which != 0 && which != 1)) return BSE_ERR_INVALID_ARG;
+    if (!dDense || !dTiles || N < 1 || ld < N || (which != 0 && which != 1) || !storage_ok(storage))
+        return BSE_ERR_INVALID_ARG;
     int64_t n_tiles;
-    bse_layout(N, nullptr, &n_tiles, nullptr);
+    bse_layout(N, storage, nullptr, &n_tiles, nullptr);
     dim3 grid;
     tile_grid(n_tiles, grid);
-    unpack_to_dense_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((const char *)dTiles, N, which, (double2 *)dDense,
-                                                                   ld, n_tiles);
+    unpack_to_dense_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((const char *)dTiles, storage_es(storage), N, which,
+                                                                   (double2 *)dDense, ld, n_tiles);
     count_launch();
     BSE_CUDA(cudaGetLastError());
     return BSE_OK;
 }
 
-bse_status_t bse_fill_synthetic(void *dTiles, int64_t N, int32_t which, uint64_t seed, double sigma, int32_t group,
-                                void *stream)
+bse_status_t bse_fill_synthetic(void *dTiles, int32_t storage, int64_t N, int32_t which, uint64_t seed, double sigma,
+                                int32_t group, void *stream)
 {
-    if (!dTiles || N < 1 || (which != 0 && which != 1)) return BSE_ERR_INVALID_ARG;
+    if (!dTiles || N < 1 || (which != 0 && which != 1) || !storage_ok(storage)) return BSE_ERR_INVALID_ARG;
     cudaStream_t s = (cudaStream_t)stream;
     double *deps = nullptr;
     if (which == 0) {
@@ -172,10 +185,10 @@ bse_status_t bse_fill_synthetic(void *dTiles, int64_t N, int32_t which, uint64_t
         count_launch();
     }
     int64_t n_tiles;
-    bse_layout(N, nullptr, &n_tiles, nullptr);
+    bse_layout(N, storage, nullptr, &n_tiles, nullptr);
     dim3 grid;
     tile_grid(n_tiles, grid);
-    fill_synthetic_kernel<<<grid, 256, 0, s>>>((char *)dTiles, N, which, stream_key(seed, which == 0 ? 2 : 3), sigma,
+    fill_synthetic_kernel<<<grid, 256, 0, s>>>((char *)dTiles, storage_es(storage), N, which, stream_key(seed, which == 0 ? 2 : 3), sigma,
                                                deps, n_tiles);
     count_launch();
     if (deps) cudaFreeAsync(deps, s);
@@ -183,41 +196,47 @@ bse_status_t bse_fill_synthetic(void *dTiles, int64_t N, int32_t which, uint64_t
     return BSE_OK;
 }
 
-bse_status_t bse_fill_closed_form_tda(void *dTiles, int64_t N, const double *dLam, const void *dU, double s, void *stream)
+bse_status_t bse_fill_closed_form_tda(void *dTiles, int32_t storage, int64_t N, const double *dLam, const void *dU,
+                                      double s, void *stream)
 {
-    if (!dTiles || !dLam || !dU || N < 1) return BSE_ERR_INVALID_ARG;
+    if (!dTiles || !dLam || !dU || N < 1 || !storage_ok(storage)) return BSE_ERR_INVALID_ARG;
     int64_t n_tiles;
-    bse_layout(N, nullptr, &n_tiles, nullptr);
+    bse_layout(N, storage, nullptr, &n_tiles, nullptr);
     dim3 grid;
     tile_grid(n_tiles, grid);
-    fill_closed_tda_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((char *)dTiles, N, dLam, (const double2 *)dU, s,
+    fill_closed_tda_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((char *)dTiles, storage_es(storage), N, dLam, (const double2 *)dU, s,
                                                                    n_tiles);
     count_launch();
     BSE_CUDA(cudaGetLastError());
     return BSE_OK;
 }
 
-bse_status_t bse_fill_closed_form_full(void *dRTiles, void *dCTiles, int64_t N, const double *dD1, const double *dD2,
-                                       const double *dUr, const double *dPhi, double s1, double s2, void *stream)
+bse_status_t bse_fill_closed_form_full(void *dRTiles, void *dCTiles, int32_t storage, int64_t N, const double *dD1,
+                                       const double *dD2, const double *dUr, const double *dPhi, double s1, double s2,
+                                       void *stream)
 {
-    if (!dRTiles || !dCTiles || !dD1 || !dD2 || !dUr || !dPhi || N < 1) return BSE_ERR_INVALID_ARG;
+    if (!dRTiles || !dCTiles || !dD1 || !dD2 || !dUr || !dPhi || N < 1 || !storage_ok(storage))
+        return BSE_ERR_INVALID_ARG;
     int64_t n_tiles;
-    bse_layout(N, nullptr, &n_tiles, nullptr);
+    bse_layout(N, storage, nullptr, &n_tiles, nullptr);
     dim3 grid;
     tile_grid(n_tiles, grid);
-    fill_closed_full_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((char *)dRTiles, N, 0, dD1, dD2, dUr, dPhi, s1, s2,
+    fill_closed_full_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((char *)dRTiles, storage_es(storage), N, 0, dD1, dD2, dUr, dPhi, s1,
+                                                                    s2,
                                                                     n_tiles);
-    fill_closed_full_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((char *)dCTiles, N, 1, dD1, dD2, dUr, dPhi, s1, s2,
+    fill_closed_full_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>((char *)dCTiles, storage_es(storage), N, 1, dD1, dD2, dUr, dPhi, s1,
+                                                                    s2,
                                                                     n_tiles);
     count_launch(2);
     BSE_CUDA(cudaGetLastError());
     return BSE_OK;
 }
 
-bse_status_t bse_create(bse_handle_t *out, int32_t mode, int64_t N, const void *dRTiles, const void *dCTiles,
-                        void *stream)
+bse_status_t bse_create(bse_handle_t *out, int32_t mode, int32_t storage, int64_t N, const void *dRTiles,
+                        const void *dCTiles, void *stream)
 {
-    if (!out || !dRTiles || N < 1 || (mode != BSE_MODE_TDA && mode != BSE_MODE_FULL)) return BSE_ERR_INVALID_ARG;
+    if (!out || !dRTiles || N < 1 || (mode != BSE_MODE_TDA && mode != BSE_MODE_FULL) || !storage_ok(storage))
+        return BSE_ERR_INVALID_ARG;
     if (mode == BSE_MODE_FULL && !dCTiles) return BSE_ERR_INVALID_ARG;
     int dev = 0;
     BSE_CUDA(cudaGetDevice(&dev));
@@ -228,6 +247,7 @@ bse_status_t bse_create(bse_handle_t *out, int32_t mode, int64_t N, const void *
     h->mode = mode;
     h->N = N;
     h->nt = (int)((N + TB - 1) / TB);
+    h->es = storage_es(storage);
     h->R = (const char *)dRTiles;
     h->C = (mode == BSE_MODE_FULL) ? (const char *)dCTiles : nullptr;
     h->stream = (cudaStream_t)stream;

@@ -25,6 +25,15 @@ __host__ __device__ __forceinline__ int tile_offset(int il, int jl)
 }
 __host__ __device__ __forceinline__ int64_t tile_index(int64_t I, int64_t J) { return I * (I + 1) / 2 + J; }
 
+// Storage type of the tile store: ES = bytes per complex entry, 16 (complex128) or 8 (complex64: the paper's
+// matrices are single precision; converted to FP64 when a fragment is loaded, all arithmetic
+// stays FP64).  Same tile order, same patch order, same slot function: only the slot size changes, and with 8-byte
+// slots both fragment reads touch 16 distinct 8-byte bank pairs per half-warp (slot mod 16 is a bijection of the
+// four lane bits of a half-warp for both offP1 and offP2), i.e. LDS.64 without bank conflicts.
+constexpr int ES_C128 = 16, ES_C64 = 8;
+__host__ __device__ __forceinline__ int64_t tile_bytes_es(int es) { return (int64_t)TB * TB * es; }
+__host__ __device__ __forceinline__ int tile_offset_es(int il, int jl, int es) { return (tile_offset(il, jl) >> 4) * es; }
+
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 __device__ __forceinline__ void mbar_init(uint64_t *b, int count)
@@ -84,6 +93,16 @@ __device__ __forceinline__ double2 lds128(uint32_t addr)
     double2 v;
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
     return v;
+}
+// One fragment entry (re, im) as doubles from a tile in shared memory.
+template <int ES> __device__ __forceinline__ double2 load_frag(const char *p);
+template <> __device__ __forceinline__ double2 load_frag<16>(const char *p) { return *reinterpret_cast<const double2 *>(p); }
+// F2F.F64.F32 runs at 16 results/clk/SM (measured); re-biasing the exponent with integer ops instead was measured
+// slower in both kernels (9.3 vs 8.6 ms at k = 1, 12.2 vs 11.0 ms at k = 4, N = 98304), so the conversion stays.
+template <> __device__ __forceinline__ double2 load_frag<8>(const char *p)
+{
+    const float2 f = *reinterpret_cast<const float2 *>(p);
+    return make_double2((double)f.x, (double)f.y);
 }
 // FP64 tensor-core MMA, D(8x8) += A(8x4, row) * B(4x8, col).  SASS: DMMA.8x8x4.
 // Fragments: lane = 4 g + t;  a = A[g][t];  b = B[t][g];  c[0..1] = C[g][2t .. 2t+1].

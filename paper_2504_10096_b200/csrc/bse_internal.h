@@ -12,6 +12,7 @@ struct bse_handle_s {
     int32_t mode;
     int64_t N;
     int nt;
+    int es;              // bytes per stored complex entry: 16 (BSE_STORE_C128) or 8 (BSE_STORE_C64)
     const char *R;
     const char *C;
     cudaStream_t stream;

@@ -7,8 +7,9 @@ namespace bse {
 
 // One thread per stored complex entry: grid.x covers the 4096 entries of a tile, blockIdx.y/z the tiles.
 // Source entry functor f(gi, gj) is only evaluated for gj <= gi < N (the lower triangle).
+// es = 16: complex128 entries; es = 8: each component rounded to nearest-even float (cvt.rn.f32.f64).
 template <class F>
-__device__ __forceinline__ void store_tile_entry(char *tiles, int64_t N, int which, int64_t tile, int I, int J,
+__device__ __forceinline__ void store_tile_entry(char *tiles, int es, int64_t N, int which, int64_t tile, int I, int J,
                                                  int il, int jl, F f)
 {
     int64_t gi = (int64_t)I * TB + il, gj = (int64_t)J * TB + jl;
@@ -22,7 +23,9 @@ __device__ __forceinline__ void store_tile_entry(char *tiles, int64_t N, int whi
             if (which == 0) v.y = -v.y;
         }
     }
-    *reinterpret_cast<double2 *>(tiles + tile * (int64_t)TILE_BYTES + tile_offset(il, jl)) = v;
+    char *dst = tiles + tile * tile_bytes_es(es) + tile_offset_es(il, jl, es);
+    if (es == ES_C128) *reinterpret_cast<double2 *>(dst) = v;
+    else *reinterpret_cast<float2 *>(dst) = make_float2(__double2float_rn(v.x), __double2float_rn(v.y));
 }
 
 __device__ __forceinline__ void tile_from_linear(int64_t tile, int &I, int &J)
@@ -37,7 +40,7 @@ __device__ __forceinline__ void tile_from_linear(int64_t tile, int &I, int &J)
 
 __global__ void __launch_bounds__(256) pack_from_dense_kernel(const double2 *__restrict__ dense, int64_t ld,
                                                               int64_t N, int which, char *__restrict__ tiles,
-                                                              int64_t n_tiles)
+                                                              int es, int64_t n_tiles)
 {
     int64_t tile = blockIdx.y + (int64_t)blockIdx.z * gridDim.y;
     if (tile >= n_tiles) return;
@@ -45,11 +48,11 @@ __global__ void __launch_bounds__(256) pack_from_dense_kernel(const double2 *__r
     tile_from_linear(tile, I, J);
     int e = blockIdx.x * blockDim.x + threadIdx.x;   // 0..4095, il fastest (coalesced dense reads)
     int il = e & 63, jl = e >> 6;
-    store_tile_entry(tiles, N, which, tile, I, J, il, jl,
+    store_tile_entry(tiles, es, N, which, tile, I, J, il, jl,
                      [&](int64_t gi, int64_t gj) { return dense[gi + gj * ld]; });
 }
 
-__global__ void __launch_bounds__(256) unpack_to_dense_kernel(const char *__restrict__ tiles, int64_t N, int which,
+__global__ void __launch_bounds__(256) unpack_to_dense_kernel(const char *__restrict__ tiles, int es, int64_t N, int which,
                                                               double2 *__restrict__ dense, int64_t ld, int64_t n_tiles)
 {
     int64_t tile = blockIdx.y + (int64_t)blockIdx.z * gridDim.y;
@@ -60,7 +63,10 @@ __global__ void __launch_bounds__(256) unpack_to_dense_kernel(const char *__rest
     int il = e & 63, jl = e >> 6;
     int64_t gi = (int64_t)I * TB + il, gj = (int64_t)J * TB + jl;
     if (gi >= N || gj >= N) return;
-    double2 v = *reinterpret_cast<const double2 *>(tiles + tile * (int64_t)TILE_BYTES + tile_offset(il, jl));
+    const char *src = tiles + tile * tile_bytes_es(es) + tile_offset_es(il, jl, es);
+    double2 v;
+    if (es == ES_C128) v = *reinterpret_cast<const double2 *>(src);
+    else { float2 f = *reinterpret_cast<const float2 *>(src); v = make_double2((double)f.x, (double)f.y); }
     dense[gi + gj * ld] = v;
     if (I != J) {   // mirror image of an off-diagonal tile
         if (which == 0) v.y = -v.y;
@@ -89,7 +95,7 @@ __global__ void transition_energies_kernel(double *__restrict__ d, int64_t N, in
     for (int a = 0; a < group; ++a) d[base + a] = v[a];
 }
 
-__global__ void __launch_bounds__(256) fill_synthetic_kernel(char *__restrict__ tiles, int64_t N, int which,
+__global__ void __launch_bounds__(256) fill_synthetic_kernel(char *__restrict__ tiles, int es, int64_t N, int which,
                                                              uint64_t h0, double sigma,
                                                              const double *__restrict__ deps, int64_t n_tiles)
 {
@@ -99,7 +105,7 @@ __global__ void __launch_bounds__(256) fill_synthetic_kernel(char *__restrict__ 
     tile_from_linear(tile, I, J);
     int e = blockIdx.x * blockDim.x + threadIdx.x;
     int il = e & 63, jl = e >> 6;
-    store_tile_entry(tiles, N, which, tile, I, J, il, jl, [&](int64_t gi, int64_t gj) {
+    store_tile_entry(tiles, es, N, which, tile, I, J, il, jl, [&](int64_t gi, int64_t gj) {
         double2 g = normal_pair(h0, (uint64_t)gi, (uint64_t)gj);
         double dec = 1.0 + fabs((double)gi - (double)gj) / 64.0;
         if (which == 0) {
@@ -111,7 +117,7 @@ __global__ void __launch_bounds__(256) fill_synthetic_kernel(char *__restrict__ 
 }
 
 // R_ij = lam_i d_ij - 2 u_i conj(u_j) (lam_i + lam_j - 2 s)
-__global__ void __launch_bounds__(256) fill_closed_tda_kernel(char *__restrict__ tiles, int64_t N,
+__global__ void __launch_bounds__(256) fill_closed_tda_kernel(char *__restrict__ tiles, int es, int64_t N,
                                                               const double *__restrict__ lam,
                                                               const double2 *__restrict__ u, double s, int64_t n_tiles)
 {
@@ -121,7 +127,7 @@ __global__ void __launch_bounds__(256) fill_closed_tda_kernel(char *__restrict__
     tile_from_linear(tile, I, J);
     int e = blockIdx.x * blockDim.x + threadIdx.x;
     int il = e & 63, jl = e >> 6;
-    store_tile_entry(tiles, N, 0, tile, I, J, il, jl, [&](int64_t gi, int64_t gj) {
+    store_tile_entry(tiles, es, N, 0, tile, I, J, il, jl, [&](int64_t gi, int64_t gj) {
         double2 a = u[gi], b = u[gj];
         double pr = a.x * b.x + a.y * b.y, pi = a.y * b.x - a.x * b.y;   // u_i conj(u_j)
         double f = -2.0 * (lam[gi] + lam[gj] - 2.0 * s);
@@ -132,7 +138,7 @@ __global__ void __launch_bounds__(256) fill_closed_tda_kernel(char *__restrict__
 }
 
 // R = U (M+ + M-)/2 U^H, C = U (M+ - M-)/2 U^T, M+- real closed forms as above with real u.
-__global__ void __launch_bounds__(256) fill_closed_full_kernel(char *__restrict__ tiles, int64_t N, int which,
+__global__ void __launch_bounds__(256) fill_closed_full_kernel(char *__restrict__ tiles, int es, int64_t N, int which,
                                                                const double *__restrict__ d1,
                                                                const double *__restrict__ d2,
                                                                const double *__restrict__ ur,
@@ -145,7 +151,7 @@ __global__ void __launch_bounds__(256) fill_closed_full_kernel(char *__restrict_
     tile_from_linear(tile, I, J);
     int e = blockIdx.x * blockDim.x + threadIdx.x;
     int il = e & 63, jl = e >> 6;
-    store_tile_entry(tiles, N, which, tile, I, J, il, jl, [&](int64_t gi, int64_t gj) {
+    store_tile_entry(tiles, es, N, which, tile, I, J, il, jl, [&](int64_t gi, int64_t gj) {
         double uu = ur[gi] * ur[gj];
         double mp = -2.0 * uu * (d1[gi] + d1[gj] - 2.0 * s1);
         double mm = -2.0 * uu * (d2[gi] + d2[gj] - 2.0 * s2);

@@ -34,6 +34,9 @@ def test_header_symbols_are_exported(b):
 def test_layout_and_status(b):
     assert b.bse_layout(64) == (64, 1, 65536)
     assert b.bse_layout(65) == (64, 3, 3 * 65536)
+    assert b.bse_layout(65, b.STORE_C64) == (64, 3, 3 * 32768)      # complex64 store: half the bytes, same tiles
+    with pytest.raises(b.BseError):
+        b.bse_layout(64, 7)
     for N, nbytes in [(1024, 8.40e6), (16384, 2.148e9), (98304, 77.31e9)]:
         t, nt, by = b.bse_layout(N)
         n = N // 64
@@ -49,7 +52,8 @@ def test_layout_and_status(b):
 def test_no_compute_without_arguments(b):
     # argument validation happens before any CUDA call
     h = ctypes.c_void_p()
-    assert b.lib().bse_create(ctypes.byref(h), 7, 64, None, None, None) == 1
+    assert b.lib().bse_create(ctypes.byref(h), 7, 0, 64, None, None, None) == 1
+    assert b.lib().bse_create(ctypes.byref(h), 0, 9, 64, ctypes.c_void_p(16), None, None) == 1     # unknown storage
     assert b.lib().bse_apply(None, None, 0, None, 0, 1) == 1
     assert b.lib().bse_solve(None, 1, 1, 0, 1e-8, 1, 0, None, None, 0, None, None) == 1
 
