@@ -178,3 +178,28 @@ def test_solve_full_on_rounded_operator(orc):
     HV = orc.apply_full(R32, C32, V)
     normH = np.linalg.norm(np.block([[R32, C32], [-C32.conj(), -R32.conj()]]), 2)
     assert np.max(np.linalg.norm(HV - V * res.omega, axis=0)) <= TOL_RES * normH
+
+
+def test_full_mode_at_paper_largest_size_sampled_rows(orc):
+    """Full BSE at N = 98304 (operator dimension 196608; R and C: 77 GB in complex64, too large for one GPU in
+    complex128): the size class of the paper's largest system.  Rows of Y = H X sampled across both halves, against
+    the oracle fed with the rounded rows of the CPU generator; plus the structure of Eq. 1 through the CUDA path:
+    the lower half is minus the conjugate of the upper half applied to the swapped, conjugated input."""
+    import torch
+    import paper_2504_10096_b200 as b
+    N, k, S = 98304, 2, b.STORE_C64
+    if torch.cuda.mem_get_info()[0] < 95e9:
+        pytest.skip("needs 95 GB of free device memory")
+    h = b.Bse(b.MODE_FULL, N, b.bse_fill_synthetic(N, 0, 1, 1.0, 64, storage=S), b.bse_fill_synthetic(N, 1, 1, storage=S),
+              storage=S)
+    X = gen.block_X(2 * N, k, 12)
+    rows = np.unique(np.concatenate([(np.arange(24) * 2654435761 % N), [0, 63, 64, N - 64, N - 1],
+                                     np.arange(8) + 64 * 777]).astype(np.int64))
+    Rr, Cr = orc.round_c64(gen.rows_R(N, 1, rows, 1.0, 64)), orc.round_c64(gen.rows_C(N, 1, rows))
+    top = np.hstack([Rr, Cr]); bot = np.hstack([-Cr.conj(), -Rr.conj()])      # Eq. 1 (PAPER.md:18) with :26
+    ref = orc.rows_times_block(np.vstack([top, bot]), X)
+    Y = to_host(h.apply(to_dev(X)))
+    assert relerr(np.vstack([Y[rows], Y[N + rows]]), ref) <= TOL_APPLY
+    Xs = np.vstack([X[N:].conj(), X[:N].conj()])
+    Ys = to_host(h.apply(to_dev(Xs)))
+    assert relerr(Ys[N:], -Y[:N].conj()) <= TOL_APPLY and relerr(Ys[:N], -Y[N:].conj()) <= TOL_APPLY
