@@ -57,8 +57,8 @@ bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, dou
     if (!attr_set) {
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_k1_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_k1_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_k1_kernel<16, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_k1_kernel<8, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         attr_set = true;
     }
     bool use_k1 = true;                                // BSE_APPLY_K1=0: tensor-core kernel for single columns too
@@ -86,10 +86,10 @@ bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, dou
         p.Y = reinterpret_cast<double *>(dY) + 2 * (int64_t)c0 * ldy;
         const bool k1 = p.kc == 1 && use_k1;                 // plain-FMA single-column variant
         if (h->es == ES_C128) {
-            if (k1) apply_tiles_k1_kernel<16><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            if (k1) apply_tiles_k1_kernel<16, 8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
             else apply_tiles_kernel<16><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
         } else {
-            if (k1) apply_tiles_k1_kernel<8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            if (k1) apply_tiles_k1_kernel<8, 8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
             else apply_tiles_kernel<8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
         }
         count_launch();
