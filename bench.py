@@ -31,9 +31,12 @@ METRIC = "bse_block_apply_algorithmic_GBps"
 UNIT = "GB/s"
 
 
+ES = 16.0      # bytes per stored entry; --storage c64 sets 8 (complex64-stored operand)
+
+
 def alg_bytes(N: int, k: int) -> float:
-    """B_mat + 32 N k  (packed complex128 lower triangle once, X read + Y written)."""
-    return 16.0 * N * (N + 1) / 2 + 32.0 * N * k
+    """B_mat + 32 N k  (packed lower triangle once, X read + Y written; complex128 vectors)."""
+    return ES * N * (N + 1) / 2 + 32.0 * N * k
 
 
 def measured_peaks():
@@ -109,6 +112,8 @@ def cpu_oracle_sample(N, k, group, seed, sample_rows, reps):
     oracle.build()
     rows = (np.arange(sample_rows, dtype=np.int64) * 2654435761 % N)
     Hrows = gen.rows_R(N, seed, rows, 0.0, group)
+    if ES == 8.0:
+        Hrows = oracle.round_c64(Hrows)            # the complex64-stored operator is the rounded matrix
     X = gen.block_X(N, k, seed + 1000)
     oracle.rows_times_block(Hrows[:8], X)          # warm the library
     t0 = time.perf_counter()
@@ -138,9 +143,10 @@ def run_reference(args, cfg):
 
 
 def workload(cfg, k):
-    return {"workload": f"BASELINE.json config {cfg['id']}: TDA Hermitian N={cfg['N']} complex128, packed lower "
-                        f"triangle {16.0 * cfg['N'] * (cfg['N'] + 1) / 2 / 1e9:.2f} GB, bse_apply k={k}",
-            "N": cfg["N"], "k": k, "sigma": 0.0, "seed": 1,
+    store = "complex128" if ES == 16.0 else "complex64-stored (FP64 arithmetic, complex128 vectors)"
+    return {"workload": f"BASELINE.json config {cfg['id']}: TDA Hermitian N={cfg['N']} {store}, packed lower "
+                        f"triangle {ES * cfg['N'] * (cfg['N'] + 1) / 2 / 1e9:.2f} GB, bse_apply k={k}",
+            "N": cfg["N"], "k": k, "sigma": 0.0, "seed": 1, "storage": "c128" if ES == 16.0 else "c64",
             "l2": "operand larger than L2 (no flush needed)" if cfg["N"] >= 8192 else "operand L2-resident"}
 
 
@@ -158,8 +164,9 @@ def run_cuda(args, cfg):
         dist.init_process_group("nccl")
     N, k = cfg["N"], args.k
 
-    tiles = b.bse_fill_synthetic(N, b.MATRIX_R, 1, 0.0, cfg["group"])       # every replica holds its own operand
-    h = b.Bse(b.MODE_TDA, N, tiles)
+    storage = b.STORE_C128 if ES == 16.0 else b.STORE_C64
+    tiles = b.bse_fill_synthetic(N, b.MATRIX_R, 1, 0.0, cfg["group"], storage=storage)   # one operand per replica
+    h = b.Bse(b.MODE_TDA, N, tiles, storage=storage)
     Xh = torch.from_numpy(np.ascontiguousarray(gen.block_X(N, max(k, 8), 1001).T)).pin_memory()
     X = Xh[:k].cuda()
     Y = torch.empty_like(X)
@@ -216,21 +223,31 @@ def run_cuda(args, cfg):
     traffic = None
     try:
         with open(os.path.join(ROOT, "profiles", "r1_apply_traffic.json")) as f:
-            traffic = json.load(f).get(f"N{N}_k{k}")
+            traffic = json.load(f).get(f"N{N}_k{k}" + ("" if ES == 16.0 else "_c64"))
     except Exception:
         pass
+    # north_star: roofline = min(bytes / HBM peak, flops / FP64 peak).  The FP64 figure is this repo's own DMMA
+    # microbenchmark (profiles/r1_microbench.md): MEASURED_PEAKS.json has no FP64 entry.
+    tflops = 8.0 * N * N * k / (ms * 1e-3) / 1e12
+    fp64_peak = 37.1
+    if 8.0 * N * N * k / (fp64_peak * 1e12) > alg_bytes(N, k) / (peak * 1e9):
+        roof = {"bound": "tensor", "achieved": tflops, "peak": fp64_peak, "unit": "TFLOP/s", "frac": tflops / fp64_peak,
+                "traffic": traffic, "peak_source": "own DMMA.8x8x4 microbenchmark (profiles/r1_microbench.md), FP64"}
+    else:
+        roof = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": traffic, "peak_source": peak_src}
+    roof.update({"kernel": "bse::apply_tiles_k1_kernel" if k == 1 else "bse::apply_tiles_kernel",
+                 "tflops_fp64": tflops, "fp64_peak_measured_tflops": fp64_peak, "GBps": achieved})
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64 (complex128 on the FP64 tensor cores)", "data": "synthetic",
             "config": workload(cfg, k), "clocks": clocks, "gpu_launches": int(launches),
             "e2e": {"value": world * alg_bytes(N, k) / (e2e_ms * 1e-3) / 1e9, "unit": UNIT,
                     "h2d_bytes_per_step": 16 * N * k, "d2h_bytes_per_step": 16 * N * k, "ms_per_step": e2e_ms},
-            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": traffic, "peak_source": peak_src, "kernel": "bse::apply_tiles_kernel",
-                         "tflops_fp64": 8.0 * N * N * k / (ms * 1e-3) / 1e12, "fp64_peak_measured_tflops": 37.1}}
+            "roofline": roof}
 
     # ---- k sweep and Lanczos time-to-nev (the rest of BASELINE.json's metric), device-timed, outside `value`
-    if not args.no_extras:
+    if not args.no_extras and ES == 16.0:
         sweep = {}
         for kk in (1, 2, 4, 8):
             Xs, Ys = Xh[:kk].cuda(), torch.empty((kk, N), dtype=torch.complex128, device="cuda")
@@ -287,11 +304,15 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config index (TDA ones: 0, 2, 4)")
     ap.add_argument("--k", type=int, default=4)
+    ap.add_argument("--storage", default="c128", choices=["c128", "c64"],
+                    help="c64: complex64-stored operand (SURVEY.md 8(f1)); the extras run for the default only")
     ap.add_argument("--ref-rows", type=int, default=1024)
     ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
+    global ES
+    ES = 16.0 if args.storage == "c128" else 8.0
     cfg = dict(gen.CONFIGS[args.config], id=args.config)
     if cfg["mode"] != "tda":
         raise SystemExit("bench.py times the TDA apply; full-mode configs are parity-test cases")
