@@ -2,16 +2,133 @@
 // eigenproblem may stay on the host").  Complex Hermitian m x m -> all eigenvalues (ascending) and the first nz
 // eigenvectors.  Householder reduction to real symmetric tridiagonal form, implicit-shift QL on the tridiagonal
 // with the plane rotations accumulated in a real matrix, then Z = Q * Zr.  No LAPACK dependency.
+//
+// Layout choices (m ~ 1000 at config 4, called once per restart):
+//   * the Hermitian matrix-vector product of the reduction walks the stored lower triangle by COLUMNS only
+//     (axpy for the part below the diagonal, dot for its conjugate-transposed image), per-thread accumulators;
+//   * the rotation sweep of a QL iteration is a dependency chain along the column index but independent across
+//     rows: Zr is stored in panels of 8 rows, [panel][column][8], so the chain runs on 8-row SIMD vectors with the
+//     updated column carried in registers (one load and one store per rotation and panel);
+//   * the back-transformation applies each reflector to 8 eigenvector columns at a time.
 #include <algorithm>
 #include <cmath>
 #include <complex>
 #include <cstdint>
 #include <numeric>
 #include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
 
 namespace bse {
 
 typedef std::complex<double> zc;
+
+namespace {
+constexpr int RP = 8;       // rows per panel of the rotation accumulator
+constexpr int JB = 8;       // eigenvector columns per back-transformation task
+inline int max_threads()
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+// The four hot loops, in explicit real arithmetic on interleaved (re, im) doubles (std::complex multiplication does
+// not vectorise without -ffast-math) and compiled for SSE2 / AVX2+FMA / AVX-512 with run-time dispatch, so that the
+// in-tree .so runs on whatever host CPU the GPU box has.
+#if defined(__x86_64__) && defined(__GNUC__) && !defined(__clang__)
+#define BSE_CLONES __attribute__((target_clones("default", "arch=x86-64-v3", "arch=x86-64-v4")))
+#else
+#define BSE_CLONES
+#endif
+
+// Columns c = c0, c0 + cs, ... of the Hermitian A22 (lower triangle, column-major, ld in complex elements):
+//   xl[c..n) += A22[c..n, c] v[c],   xl[c] += sum_{r > c} conj(A22[r, c]) v[r]
+BSE_CLONES void herm_matvec_columns(int n, const double *A22, int64_t ld, const double *v, double *xl, int c0, int cs)
+{
+    for (int c = c0; c < n; c += cs) {
+        const double *col = A22 + 2 * ((int64_t)c * ld);
+        const double vcr = v[2 * c], vci = v[2 * c + 1];
+        double sr = 0.0, si = 0.0;
+        xl[2 * c] += col[2 * c] * vcr;                 // real diagonal
+        xl[2 * c + 1] += col[2 * c] * vci;
+#pragma omp simd reduction(+ : sr, si)
+        for (int r = c + 1; r < n; ++r) {
+            const double ar = col[2 * r], ai = col[2 * r + 1];
+            xl[2 * r] += ar * vcr - ai * vci;
+            xl[2 * r + 1] += ar * vci + ai * vcr;
+            sr += ar * v[2 * r] + ai * v[2 * r + 1];
+            si += ar * v[2 * r + 1] - ai * v[2 * r];
+        }
+        xl[2 * c] += sr;
+        xl[2 * c + 1] += si;
+    }
+}
+
+// A22[c.., c] -= v w_c^* + w v_c^*  for columns c0 <= c < c1
+BSE_CLONES void rank2_update_columns(int n, double *A22, int64_t ld, const double *v, const double *x, int c0, int c1)
+{
+    for (int c = c0; c < c1; ++c) {
+        double *col = A22 + 2 * ((int64_t)c * ld);
+        const double wr = x[2 * c], wi = -x[2 * c + 1], ur = v[2 * c], ui = -v[2 * c + 1];   // conj(w_c), conj(v_c)
+#pragma omp simd
+        for (int r = c; r < n; ++r) {
+            const double vr = v[2 * r], vi = v[2 * r + 1], xr = x[2 * r], xi = x[2 * r + 1];
+            col[2 * r] -= vr * wr - vi * wi + xr * ur - xi * ui;
+            col[2 * r + 1] -= vr * wi + vi * wr + xr * ui + xi * ur;
+        }
+    }
+}
+
+// One panel of RP rows: rotations q = mm-1 down to ilo on columns (q, q+1); zb[(column) * RP + row]
+BSE_CLONES void rotate_panel(double *zb, int mm, int ilo, const double *rc, const double *rs)
+{
+    double f[RP];
+#pragma omp simd
+    for (int rr = 0; rr < RP; ++rr) f[rr] = zb[(size_t)mm * RP + rr];
+    for (int q = mm - 1; q >= ilo; --q) {
+        const double cq = rc[q], sq = rs[q];
+        double *zq = zb + (size_t)q * RP;
+#pragma omp simd
+        for (int rr = 0; rr < RP; ++rr) {
+            const double g = zq[rr];
+            zq[RP + rr] = sq * g + cq * f[rr];
+            f[rr] = cq * g - sq * f[rr];
+        }
+    }
+#pragma omp simd
+    for (int rr = 0; rr < RP; ++rr) zb[(size_t)ilo * RP + rr] = f[rr];
+}
+
+// z_j <- (I - tau v v^H) z_j for nb <= JB columns; v = vi[lo .. m) (interleaved), zc[jj] interleaved columns
+BSE_CLONES void reflect_columns(int lo, int m, const double *vi, double taur, double taui, double *const *zcol, int nb)
+{
+    double sr[JB], si[JB];
+    for (int jj = 0; jj < nb; ++jj) {
+        const double *z = zcol[jj];
+        double ar = 0.0, ai = 0.0;
+#pragma omp simd reduction(+ : ar, ai)
+        for (int r = lo; r < m; ++r) {                       // conj(v_r) z_r
+            ar += vi[2 * r] * z[2 * r] + vi[2 * r + 1] * z[2 * r + 1];
+            ai += vi[2 * r] * z[2 * r + 1] - vi[2 * r + 1] * z[2 * r];
+        }
+        sr[jj] = taur * ar - taui * ai;
+        si[jj] = taur * ai + taui * ar;
+    }
+    for (int jj = 0; jj < nb; ++jj) {
+        double *z = zcol[jj];
+        const double pr = sr[jj], pi = si[jj];
+#pragma omp simd
+        for (int r = lo; r < m; ++r) {
+            z[2 * r] -= vi[2 * r] * pr - vi[2 * r + 1] * pi;
+            z[2 * r + 1] -= vi[2 * r] * pi + vi[2 * r + 1] * pr;
+        }
+    }
+}
+}  // namespace
 
 // A (column-major, lda, lower triangle referenced and destroyed).  Returns 0, or >0 if QL failed to converge.
 int host_heev(int m, void *A_, int lda, double *w, void *Z_, int ldz, int nz)
@@ -24,7 +141,8 @@ int host_heev(int m, void *A_, int lda, double *w, void *Z_, int ldz, int nz)
     auto a = [&](int i, int j) -> zc & { return A[i + (int64_t)j * lda]; };
 
     // ---- Householder tridiagonalisation, lower variant:  A = Q T Q^H,  Q = H_0 H_1 ... H_{m-2},  H_i = I - tau v v^H
-    std::vector<zc> x(m), v(m);
+    const int nth = max_threads();
+    std::vector<zc> x(m), v(m), xt((size_t)nth * m);
     for (int i = 0; i < m - 1; ++i) {
         const int n = m - i - 1;                  // length of the column below the diagonal
         zc alpha = a(i + 1, i);
@@ -43,12 +161,27 @@ int host_heev(int m, void *A_, int lda, double *w, void *Z_, int ldz, int nz)
         a(i + 1, i) = 1.0;                         // v = A(i+1:m, i) with v_0 = 1
         if (t != zc(0.0)) {
             for (int r = 0; r < n; ++r) v[r] = a(i + 1 + r, i);
-            // x = tau * A22 * v   (A22 Hermitian, lower triangle stored)
-#pragma omp parallel for schedule(static) if (n > 128)
+            // x = tau * A22 * v   (A22 Hermitian, lower triangle stored), column by column:
+            //   x[c..n) += A22[c..n, c] v[c]   and   x[c] += sum_{r > c} conj(A22[r, c]) v[r]
+            const bool par = n > 128 && nth > 1;
+            int nt_act = 1;                           // the team the runtime actually grants (may be < nth)
+#pragma omp parallel num_threads(nth) if (par)
+            {
+#ifdef _OPENMP
+                const int tid = omp_get_thread_num(), team = omp_get_num_threads();
+#else
+                const int tid = 0, team = 1;
+#endif
+                if (tid == 0) nt_act = team;
+                zc *xl = &xt[(size_t)tid * m];
+                for (int r = 0; r < n; ++r) xl[r] = zc(0.0);
+                // cyclic columns: column lengths shrink linearly, a cyclic split balances them
+                herm_matvec_columns(n, reinterpret_cast<const double *>(&a(i + 1, i + 1)), lda,
+                                    reinterpret_cast<const double *>(v.data()), reinterpret_cast<double *>(xl), tid, team);
+            }
             for (int r = 0; r < n; ++r) {
                 zc s(0.0);
-                for (int c = 0; c <= r; ++c) s += a(i + 1 + r, i + 1 + c) * v[c];
-                for (int c = r + 1; c < n; ++c) s += std::conj(a(i + 1 + c, i + 1 + r)) * v[c];
+                for (int q = 0; q < nt_act; ++q) s += xt[(size_t)q * m + r];
                 x[r] = t * s;
             }
             zc dot(0.0);
@@ -56,22 +189,23 @@ int host_heev(int m, void *A_, int lda, double *w, void *Z_, int ldz, int nz)
             zc al = -0.5 * t * dot;
             for (int r = 0; r < n; ++r) x[r] += al * v[r];                 // w
             // A22 -= v w^H + w v^H   (lower triangle)
-#pragma omp parallel for schedule(static) if (n > 128)
-            for (int c = 0; c < n; ++c) {
-                zc wc = std::conj(x[c]), vc = std::conj(v[c]);
-                for (int r = c; r < n; ++r) a(i + 1 + r, i + 1 + c) -= v[r] * wc + x[r] * vc;
-            }
+#pragma omp parallel for schedule(static, 1) if (par)
+            for (int c0 = 0; c0 < n; c0 += 4)
+                rank2_update_columns(n, reinterpret_cast<double *>(&a(i + 1, i + 1)), lda,
+                                     reinterpret_cast<const double *>(v.data()), reinterpret_cast<const double *>(x.data()),
+                                     c0, std::min(c0 + 4, n));
         }
         d[i] = a(i, i).real();
     }
     d[m - 1] = a(m - 1, m - 1).real();
 
-    // ---- implicit QL on (d, e) with rotations accumulated in the real row-major matrix Zr (m x m)
-    std::vector<double> Zr((size_t)m * m, 0.0);
-    for (int i = 0; i < m; ++i) Zr[(size_t)i * m + i] = 1.0;
+    // ---- implicit QL on (d, e) with the rotations accumulated in Zr (real m x m), stored in panels of RP rows:
+    //      Zb[(panel * m + column) * RP + row_in_panel]
+    const int npan = (m + RP - 1) / RP;
+    std::vector<double> Zb((size_t)npan * m * RP, 0.0);
+    for (int i = 0; i < m; ++i) Zb[((size_t)(i / RP) * m + i) * RP + i % RP] = 1.0;
     std::vector<double> rc(m), rs(m);
     int fail = 0;
-    // shift e so that e[i] couples i and i+1 (already the case), e[m-1] = 0
     for (int l = 0; l < m; ++l) {
         int iter = 0;
         while (true) {
@@ -102,15 +236,12 @@ int host_heev(int m, void *A_, int lda, double *w, void *Z_, int ldz, int nz)
                 rc[i] = c; rs[i] = s;
             }
             const int ilo = under ? i + 1 : l;
-            // apply the recorded rotations (i = mm-1 down to ilo) to columns (i, i+1) of Zr, all rows in parallel
-#pragma omp parallel for schedule(static) if (m > 128)
-            for (int row = 0; row < m; ++row) {
-                double *z = &Zr[(size_t)row * m];
-                for (int q = mm - 1; q >= ilo; --q) {
-                    double f = z[q + 1];
-                    z[q + 1] = rs[q] * z[q] + rc[q] * f;
-                    z[q] = rc[q] * z[q] - rs[q] * f;
-                }
+            // apply the recorded rotations (q = mm-1 down to ilo) to columns (q, q+1): z[q+1] = s z[q] + c f,
+            // z[q] = c z[q] - s f with f the old z[q+1]; the new z[q] is the next step's f and stays in registers
+            if (mm - 1 >= ilo) {
+                const int64_t work = (int64_t)(mm - ilo) * m;
+#pragma omp parallel for schedule(static) if (work > 32768)
+                for (int pn = 0; pn < npan; ++pn) rotate_panel(&Zb[(size_t)pn * m * RP], mm, ilo, rc.data(), rs.data());
             }
             if (under) continue;
             d[l] -= p;
@@ -126,18 +257,23 @@ int host_heev(int m, void *A_, int lda, double *w, void *Z_, int ldz, int nz)
     for (int i = 0; i < m; ++i) w[i] = d[ord[i]];
     if (nz <= 0 || !Z) return fail;
 
-    // ---- Z = Q * Zr[:, ord[0..nz)]:  start from the real eigenvectors and apply H_{m-2} ... H_0 from the left
-    for (int j = 0; j < nz; ++j)
-        for (int i = 0; i < m; ++i) Z[i + (int64_t)j * ldz] = Zr[(size_t)i * m + ord[j]];
-#pragma omp parallel for schedule(static) if (m > 64)
-    for (int j = 0; j < nz; ++j) {
-        zc *z = Z + (int64_t)j * ldz;
+    // ---- Z = Q * Zr[:, ord[0..nz)]:  start from the real eigenvectors and apply H_{m-2} ... H_0 from the left,
+    //      each reflector to JB columns at a time (the reflector is read once per block, not once per column)
+#pragma omp parallel for schedule(dynamic, 1) if (m > 64)
+    for (int j0 = 0; j0 < nz; j0 += JB) {
+        const int nb = std::min(JB, nz - j0);
+        zc *zcol[JB];
+        for (int jj = 0; jj < nb; ++jj) {
+            zcol[jj] = Z + (int64_t)(j0 + jj) * ldz;
+            const int src = ord[j0 + jj];
+            for (int i = 0; i < m; ++i) zcol[jj][i] = Zb[((size_t)(i / RP) * m + src) * RP + i % RP];
+        }
+        double *zd[JB];
+        for (int jj = 0; jj < nb; ++jj) zd[jj] = reinterpret_cast<double *>(zcol[jj]);
         for (int i = m - 2; i >= 0; --i) {
             if (tau[i] == zc(0.0)) continue;
-            zc s(0.0);
-            for (int r = i + 1; r < m; ++r) s += std::conj(a(r, i)) * z[r];   // v^H z  (v_0 = 1 stored)
-            s *= tau[i];
-            for (int r = i + 1; r < m; ++r) z[r] -= a(r, i) * s;
+            // v_r = A[r, i], r = i+1 .. m-1 (v_{i+1} = 1 stored)
+            reflect_columns(i + 1, m, reinterpret_cast<const double *>(&a(0, i)), tau[i].real(), tau[i].imag(), zd, nb);
         }
     }
     return fail;
