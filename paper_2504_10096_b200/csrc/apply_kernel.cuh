@@ -43,7 +43,7 @@ struct ApplyParams {
     int64_t ldy;
     int64_t N;
     int nt;             // tile rows
-    int kc;             // columns in this pass (1..4)
+    int kc;             // columns in this pass (1..4; 5..8 for the NPC = 2 kernel)
     int pass;           // PASS_HERM / PASS_SYMC
     double sign;        // s
     int L;              // unit length in tiles
@@ -70,7 +70,11 @@ __device__ __forceinline__ void apply_decode_unit(int64_t u, int L, int &I, int 
 }
 
 // ES = bytes per stored complex entry (bse_common.cuh): 16 -> LDS.128 fragments, 8 -> LDS.64 + conversion to FP64.
-template <int ES>
+// NPC = patch columns per consumer warp.  NPC = 1: up to 4 columns of X, warp w owns tile columns 8w .. 8w+7.
+// NPC = 2 (5 .. 8 columns of X in ONE pass over the operand): warp w owns tile columns 16 (w >> 1) .. +15 and the
+// column half nh = w & 1 (columns 4 nh .. 4 nh + 3 of X): the same accumulators and x_I fragments as NPC = 1, twice
+// the DMMAs per tile, each stored tile still read from HBM once.
+template <int ES, int NPC>
 __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const ApplyParams p)
 {
     constexpr int TBY = TB * TB * ES;                    // tile bytes
@@ -111,14 +115,16 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
     }
 
     // ------------------------------------ consumer warps ------------------------------------------
-    const int w = warp;
+    const int nh = (NPC == 2) ? (warp & 1) : 0;           // which half of the (up to) 8 columns
+    const int w0 = (NPC == 2) ? (warp >> 1) * 2 : warp;   // first patch column of this warp
     const int g = lane >> 2, t = lane & 3;
     const int g2 = (g >> 2) & 1, g1 = (g >> 1) & 1, g0 = g & 1, t1 = (t >> 1) & 1, t0 = t & 1;
     // fragment byte offsets inside a patch (see patch_slot): P1 reads (a = g, b = 4 s + t), P2 reads (a = 4 s + t, b = g)
     const int offP1 = (((g2 << 2) | g1) * 8 + ((g0 << 2) | (t0 << 1) | (g1 ^ t1))) * ES;   // + s * S1
     const int offP2 = (((g2 << 1) | t1) * 8 + ((t0 << 2) | (g0 << 1) | (t1 ^ g1))) * ES;   // + s * S2
     // B fragments: lane supplies B[kk = t][n = g], n = 2 c + part
-    const int col = g >> 1, part = g & 1;
+    const int col = (g >> 1) + 4 * nh, part = g & 1;
+    const int tc = t + 4 * nh;                            // column of X / Y this lane's accumulator entries belong to
     const bool colok = col < p.kc;
     // Ba pairs with Re(T), Bb with Im(T); value = coef * (re or im of x):
     //   HERM P1 (T x):         Ba = [xr,  xi]   Bb = [-xi,  xr]
@@ -136,13 +142,15 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
     const double2 *xcol = p.X + (int64_t)(colok ? col : 0) * p.ldx;
     const int kc = p.kc;
 
-    // x rows of tile-row K needed by this lane for P1 (rows 8w + 4s + t); zero outside the matrix / column range
-    auto load_xj = [&](int K, double2 (&x)[2]) {
+    // x rows of tile-row K needed by this lane for P1 (rows 8 (w0 + pc) + 4s + t); zero outside the matrix / columns
+    auto load_xj = [&](int K, double2 (&x)[NPC][2]) {
 #pragma unroll
-        for (int s = 0; s < 2; ++s) {
-            int64_t row = (int64_t)K * TB + w * 8 + s * 4 + t;
-            x[s] = (colok && row < p.N) ? __ldg(xcol + row) : make_double2(0.0, 0.0);
-        }
+        for (int pc = 0; pc < NPC; ++pc)
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                int64_t row = (int64_t)K * TB + (w0 + pc) * 8 + s * 4 + t;
+                x[pc][s] = (colok && row < p.N) ? __ldg(xcol + row) : make_double2(0.0, 0.0);
+            }
     };
 
     int st = 0;
@@ -151,7 +159,7 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
         int I, J0, J1;
         apply_decode_unit(u, p.L, I, J0, J1);
 
-        double2 xjn[2];
+        double2 xjn[NPC][2];
         load_xj(J0, xjn);
         // x_I fragments for P2 (rows 8 ib + 4 s + t), kept in registers for the whole unit
         double BaI[8][2], BbI[8][2];
@@ -177,106 +185,109 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
         for (int ib = 0; ib < 8; ++ib) C1[ib][0] = C1[ib][1] = 0.0;
 
         for (int J = J0; J < J1; ++J) {
-            double BaJ[2], BbJ[2];
+            double BaJ[NPC][2], BbJ[NPC][2];
 #pragma unroll
-            for (int s = 0; s < 2; ++s) {
-                BaJ[s] = (part ? xjn[s].y : xjn[s].x) * ca1;
-                BbJ[s] = (part ? xjn[s].x : xjn[s].y) * cb1;
-            }
+            for (int pc = 0; pc < NPC; ++pc)
+#pragma unroll
+                for (int s = 0; s < 2; ++s) {
+                    BaJ[pc][s] = (part ? xjn[pc][s].y : xjn[pc][s].x) * ca1;
+                    BbJ[pc][s] = (part ? xjn[pc][s].x : xjn[pc][s].y) * cb1;
+                }
             if (J + 1 < J1) load_xj(J + 1, xjn);            // prefetch the next tile's x_J fragments
 
             mbar_wait(&full[st], ph);
-            const char *tp = tile_s + st * TBY + w * 8 * PBY;
-            if (I != J) {
-                double C2[4][2];
+            int live = 0;
+            double yr[NPC], yi[NPC];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) C2[q][0] = C2[q][1] = 0.0;
-                // two patches at a time, four independent accumulator chains interleaved: dependent DMMAs are 4 apart
+            for (int pc = 0; pc < NPC; ++pc) {
+                const char *tp = tile_s + st * TBY + (w0 + pc) * 8 * PBY;
+                if (I != J) {
+                    double C2[4][2];
 #pragma unroll
-                for (int ib = 0; ib < 8; ib += 2) {
-                    const char *pp = tp + ib * PBY, *pq = pp + PBY;
-                    double2 a0 = load_frag<ES>(pp + offP1);
-                    double2 c0 = load_frag<ES>(pq + offP1);
-                    double2 b0 = load_frag<ES>(pp + offP2);
-                    double2 d0 = load_frag<ES>(pq + offP2);
-                    double2 a1 = load_frag<ES>(pp + offP1 + S1);
-                    double2 c1 = load_frag<ES>(pq + offP1 + S1);
-                    double2 b1 = load_frag<ES>(pp + offP2 + S2);
-                    double2 d1 = load_frag<ES>(pq + offP2 + S2);
-                    const int q = ib & 2;
-                    dmma(C1[ib], a0.x, BaJ[0]);
-                    dmma(C1[ib + 1], c0.x, BaJ[0]);
-                    dmma(C2[q], b0.x, BaI[ib][0]);
-                    dmma(C2[q + 1], d0.x, BaI[ib + 1][0]);
-                    dmma(C1[ib], a0.y, BbJ[0]);
-                    dmma(C1[ib + 1], c0.y, BbJ[0]);
-                    dmma(C2[q], b0.y, BbI[ib][0]);
-                    dmma(C2[q + 1], d0.y, BbI[ib + 1][0]);
-                    dmma(C1[ib], a1.x, BaJ[1]);
-                    dmma(C1[ib + 1], c1.x, BaJ[1]);
-                    dmma(C2[q], b1.x, BaI[ib][1]);
-                    dmma(C2[q + 1], d1.x, BaI[ib + 1][1]);
-                    dmma(C1[ib], a1.y, BbJ[1]);
-                    dmma(C1[ib + 1], c1.y, BbJ[1]);
-                    dmma(C2[q], b1.y, BbI[ib][1]);
-                    dmma(C2[q + 1], d1.y, BbI[ib + 1][1]);
-                }
-                // The release must not overtake the ld.shared that feed the DMMAs above: an mbarrier arrive only orders
-                // the ISSUE of earlier loads, and on B200 queued loads of a slow warp were observed to execute after the
-                // producer's next bulk copy had landed (stale fragments about once per launch).  The barrier address is
-                // therefore made to depend on every accumulator (live & p.zero == 0, but not foldable): all DMMAs,
-                // hence all loads, have completed before the arrive can issue.
-                int live = 0;
+                    for (int q = 0; q < 4; ++q) C2[q][0] = C2[q][1] = 0.0;
+                    // two patches at a time, four independent accumulator chains interleaved: dependent DMMAs are 4 apart
 #pragma unroll
-                for (int ib = 0; ib < 8; ++ib) live |= __double2hiint(C1[ib][0]);
-#pragma unroll
-                for (int q = 0; q < 4; ++q) live |= __double2hiint(C2[q][0]);
-                __syncwarp();
-                if (lane == 0)
-                    mbar_arrive(reinterpret_cast<uint64_t *>(reinterpret_cast<char *>(&empty[st]) + (live & p.zero)));
-                // flush Y_J rows 8w + g, column t
-                double yr = (C2[0][0] + C2[1][0]) + (C2[2][0] + C2[3][0]);
-                double yi = (C2[0][1] + C2[1][1]) + (C2[2][1] + C2[3][1]);
-                int64_t row = (int64_t)J * TB + w * 8 + g;
-                if (t < kc && row < p.N) {
-                    double *y = p.Y + 2 * (row + (int64_t)t * p.ldy);
-                    red_add(y, yr);
-                    red_add(y + 1, yi);
-                }
-            } else {
-#pragma unroll
-                for (int ib = 0; ib < 8; ib += 4) {     // diagonal tile: P1 only, four chains interleaved
-                    double2 a0[4], a1[4];
-#pragma unroll
-                    for (int r = 0; r < 4; ++r) {
-                        a0[r] = load_frag<ES>(tp + (ib + r) * PBY + offP1);
-                        a1[r] = load_frag<ES>(tp + (ib + r) * PBY + offP1 + S1);
+                    for (int ib = 0; ib < 8; ib += 2) {
+                        const char *pp = tp + ib * PBY, *pq = pp + PBY;
+                        double2 a0 = load_frag<ES>(pp + offP1);
+                        double2 c0 = load_frag<ES>(pq + offP1);
+                        double2 b0 = load_frag<ES>(pp + offP2);
+                        double2 d0 = load_frag<ES>(pq + offP2);
+                        double2 a1 = load_frag<ES>(pp + offP1 + S1);
+                        double2 c1 = load_frag<ES>(pq + offP1 + S1);
+                        double2 b1 = load_frag<ES>(pp + offP2 + S2);
+                        double2 d1 = load_frag<ES>(pq + offP2 + S2);
+                        const int q = ib & 2;
+                        dmma(C1[ib], a0.x, BaJ[pc][0]);
+                        dmma(C1[ib + 1], c0.x, BaJ[pc][0]);
+                        dmma(C2[q], b0.x, BaI[ib][0]);
+                        dmma(C2[q + 1], d0.x, BaI[ib + 1][0]);
+                        dmma(C1[ib], a0.y, BbJ[pc][0]);
+                        dmma(C1[ib + 1], c0.y, BbJ[pc][0]);
+                        dmma(C2[q], b0.y, BbI[ib][0]);
+                        dmma(C2[q + 1], d0.y, BbI[ib + 1][0]);
+                        dmma(C1[ib], a1.x, BaJ[pc][1]);
+                        dmma(C1[ib + 1], c1.x, BaJ[pc][1]);
+                        dmma(C2[q], b1.x, BaI[ib][1]);
+                        dmma(C2[q + 1], d1.x, BaI[ib + 1][1]);
+                        dmma(C1[ib], a1.y, BbJ[pc][1]);
+                        dmma(C1[ib + 1], c1.y, BbJ[pc][1]);
+                        dmma(C2[q], b1.y, BbI[ib][1]);
+                        dmma(C2[q + 1], d1.y, BbI[ib + 1][1]);
                     }
+                    yr[pc] = (C2[0][0] + C2[1][0]) + (C2[2][0] + C2[3][0]);
+                    yi[pc] = (C2[0][1] + C2[1][1]) + (C2[2][1] + C2[3][1]);
+                    live |= __double2hiint(yr[pc]) | __double2hiint(yi[pc]);
+                } else {
 #pragma unroll
-                    for (int r = 0; r < 4; ++r) dmma(C1[ib + r], a0[r].x, BaJ[0]);
+                    for (int ib = 0; ib < 8; ib += 4) {     // diagonal tile: P1 only, four chains interleaved
+                        double2 a0[4], a1[4];
 #pragma unroll
-                    for (int r = 0; r < 4; ++r) dmma(C1[ib + r], a0[r].y, BbJ[0]);
+                        for (int r = 0; r < 4; ++r) {
+                            a0[r] = load_frag<ES>(tp + (ib + r) * PBY + offP1);
+                            a1[r] = load_frag<ES>(tp + (ib + r) * PBY + offP1 + S1);
+                        }
 #pragma unroll
-                    for (int r = 0; r < 4; ++r) dmma(C1[ib + r], a1[r].x, BaJ[1]);
+                        for (int r = 0; r < 4; ++r) dmma(C1[ib + r], a0[r].x, BaJ[pc][0]);
 #pragma unroll
-                    for (int r = 0; r < 4; ++r) dmma(C1[ib + r], a1[r].y, BbJ[1]);
+                        for (int r = 0; r < 4; ++r) dmma(C1[ib + r], a0[r].y, BbJ[pc][0]);
+#pragma unroll
+                        for (int r = 0; r < 4; ++r) dmma(C1[ib + r], a1[r].x, BaJ[pc][1]);
+#pragma unroll
+                        for (int r = 0; r < 4; ++r) dmma(C1[ib + r], a1[r].y, BbJ[pc][1]);
+                    }
                 }
-                int live = 0;
+            }
+            // The release must not overtake the ld.shared that feed the DMMAs above: an mbarrier arrive only orders
+            // the ISSUE of earlier loads, and on B200 queued loads of a slow warp were observed to execute after the
+            // producer's next bulk copy had landed (stale fragments about once per launch).  The barrier address is
+            // therefore made to depend on every accumulator (live & p.zero == 0, but not foldable): all DMMAs,
+            // hence all loads, have completed before the arrive can issue.  (yr, yi are sums of every C2 word.)
 #pragma unroll
-                for (int ib = 0; ib < 8; ++ib) live |= __double2hiint(C1[ib][0]);
-                __syncwarp();
-                if (lane == 0)
-                    mbar_arrive(reinterpret_cast<uint64_t *>(reinterpret_cast<char *>(&empty[st]) + (live & p.zero)));
+            for (int ib = 0; ib < 8; ++ib) live |= __double2hiint(C1[ib][0]);
+            __syncwarp();
+            if (lane == 0)
+                mbar_arrive(reinterpret_cast<uint64_t *>(reinterpret_cast<char *>(&empty[st]) + (live & p.zero)));
+            if (I != J) {                                   // flush Y_J rows 8 (w0 + pc) + g, column tc
+#pragma unroll
+                for (int pc = 0; pc < NPC; ++pc) {
+                    int64_t row = (int64_t)J * TB + (w0 + pc) * 8 + g;
+                    if (tc < kc && row < p.N) {
+                        double *y = p.Y + 2 * (row + (int64_t)tc * p.ldy);
+                        red_add(y, yr[pc]);
+                        red_add(y + 1, yi[pc]);
+                    }
+                }
             }
             if (++st == NST) { st = 0; ph ^= 1; }
         }
-        // flush this warp's partial Y_I (all 64 rows, column t)
-        if (t < kc) {
+        // flush this warp's partial Y_I (all 64 rows, column tc)
+        if (tc < kc) {
 #pragma unroll
             for (int ib = 0; ib < 8; ++ib) {
                 int64_t row = (int64_t)I * TB + ib * 8 + g;
                 if (row < p.N) {
-                    double *y = p.Y + 2 * (row + (int64_t)t * p.ldy);
+                    double *y = p.Y + 2 * (row + (int64_t)tc * p.ldy);
                     red_add(y, C1[ib][0]);
                     red_add(y + 1, C1[ib][1]);
                 }

@@ -53,13 +53,18 @@ bse_status_t zero_block(bse_handle_s *h, void *dY, int64_t ldy, int64_t rows, in
 bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, double sign, const void *dX,
                                int64_t ldx, void *dY, int64_t ldy, int32_t k)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+    // cudaFuncSetAttribute is per device: remember which devices of this process have been set up
+    static std::atomic<uint64_t> attr_devices{0};
+    int dev = 0;
+    BSE_CUDA(cudaGetDevice(&dev));
+    if (dev >= 64 || !(attr_devices.load(std::memory_order_acquire) & (1ull << dev))) {
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<16, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<16, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<8, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_k1_kernel<16, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_k1_kernel<8, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        attr_set = true;
+        if (dev < 64) attr_devices.fetch_or(1ull << dev, std::memory_order_release);
     }
     bool use_k1 = true;                                // BSE_APPLY_K1=0: tensor-core kernel for single columns too
     if (const char *e = getenv("BSE_APPLY_K1")) use_k1 = atoi(e) != 0;
@@ -80,19 +85,26 @@ bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, dou
     p.n_units = apply_num_units(h->nt, p.L);
     p.zero = 0;
     int grid = (int)(p.n_units < h->num_sms ? p.n_units : h->num_sms);
-    for (int32_t c0 = 0; c0 < k; c0 += 4) {
-        p.kc = (k - c0) < 4 ? (k - c0) : 4;
+    bool use_wide = true;                              // BSE_APPLY_WIDE=0: 4-column passes only
+    if (const char *e = getenv("BSE_APPLY_WIDE")) use_wide = atoi(e) != 0;
+    for (int32_t c0 = 0; c0 < k;) {
+        const int32_t left = k - c0;
+        const bool wide = use_wide && left > 4;        // 5 .. 8 columns in one pass over the operand
+        p.kc = wide ? (left < 8 ? left : 8) : (left < 4 ? left : 4);
         p.X = reinterpret_cast<const double2 *>(dX) + (int64_t)c0 * ldx;
         p.Y = reinterpret_cast<double *>(dY) + 2 * (int64_t)c0 * ldy;
         const bool k1 = p.kc == 1 && use_k1;                 // plain-FMA single-column variant
         if (h->es == ES_C128) {
             if (k1) apply_tiles_k1_kernel<16, 8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-            else apply_tiles_kernel<16><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            else if (wide) apply_tiles_kernel<16, 2><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            else apply_tiles_kernel<16, 1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
         } else {
             if (k1) apply_tiles_k1_kernel<8, 8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-            else apply_tiles_kernel<8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            else if (wide) apply_tiles_kernel<8, 2><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            else apply_tiles_kernel<8, 1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
         }
         count_launch();
+        c0 += p.kc;
     }
     BSE_CUDA(cudaGetLastError());
     return BSE_OK;

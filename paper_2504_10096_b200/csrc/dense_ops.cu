@@ -44,11 +44,13 @@ static bse_status_t launch_gemm(bse_handle_s *h, const double *A, int64_t lda2, 
                                 double beta)
 {
     using Cfg = GemmCfg<MT, NT, WM, WN>;
-    static bool attr = false;
-    if (!attr) {
+    static std::atomic<uint64_t> attr_devices{0};         // per device (cudaFuncSetAttribute is)
+    int dev = 0;
+    BSE_CUDA(cudaGetDevice(&dev));
+    if (dev >= 64 || !(attr_devices.load(std::memory_order_acquire) & (1ull << dev))) {
         BSE_CUDA(cudaFuncSetAttribute(gemm_nn_kernel<MT, NT, WM, WN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       Cfg::SMEM));
-        attr = true;
+        if (dev < 64) attr_devices.fetch_or(1ull << dev, std::memory_order_release);
     }
     dim3 grid((unsigned)((nr + Cfg::BM - 1) / Cfg::BM), (unsigned)((l + Cfg::BN - 1) / Cfg::BN));
     gemm_nn_kernel<MT, NT, WM, WN><<<grid, Cfg::THREADS, Cfg::SMEM, h->stream>>>(A, lda2, nr, m, cplx, Bm, ldb, l, C,

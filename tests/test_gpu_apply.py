@@ -243,3 +243,26 @@ def test_leading_dimensions_and_side_stream(orc):
     assert b.lib().bse_apply(h._h, Xd.data_ptr(), N - 1, Yd.data_ptr(), ldy, k) == 1     # ld < N
     assert b.lib().bse_apply(h._h, Xd.data_ptr(), ldx, Yd.data_ptr(), ldy, 0) == 1       # k < 1
     assert b.lib().bse_apply(h._h, Xd.data_ptr(), ldx, Xd.data_ptr(), ldx, k) == 1       # aliasing
+
+
+@pytest.mark.parametrize("k", [5, 7, 8, 11, 16])
+def test_wide_and_narrow_column_passes_agree_with_oracle(orc, k, monkeypatch):
+    """k > 4: the default takes 5..8 columns per pass over the operand (apply_tiles_kernel<ES, 2>), BSE_APPLY_WIDE=0
+    takes 4 at a time.  Both against the oracle, on a size with several units per CTA and a ragged last tile."""
+    import paper_2504_10096_b200 as b
+    N = 2000
+    R = gen.dense_R(N, 31, sigma=0.5)
+    X = gen.block_X(N, k, 32)
+    ref = orc.apply_tda(R, X)
+    h = b.Bse(b.MODE_TDA, N, pack(R, 0))
+    for wide in ("1", "0"):
+        monkeypatch.setenv("BSE_APPLY_WIDE", wide)
+        n0 = b.launch_count()
+        Y = to_host(h.apply(to_dev(X)))
+        launches = b.launch_count() - n0
+        assert relerr(Y, ref) <= TOL_APPLY
+        left, passes = k, 0
+        while left > 0:                        # the launcher's greedy rule (bse_api.cu, launch_apply_pass)
+            left -= (min(left, 8) if (wide == "1" and left > 4) else min(left, 4))
+            passes += 1
+        assert launches == passes
