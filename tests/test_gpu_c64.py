@@ -203,3 +203,19 @@ def test_full_mode_at_paper_largest_size_sampled_rows(orc):
     Xs = np.vstack([X[N:].conj(), X[:N].conj()])
     Ys = to_host(h.apply(to_dev(Xs)))
     assert relerr(Ys[N:], -Y[:N].conj()) <= TOL_APPLY and relerr(Ys[:N], -Y[N:].conj()) <= TOL_APPLY
+
+
+def test_lanczos_quadrature_on_rounded_operator(orc):
+    """bse_lanczos_quadrature over the complex64 store: the k = 1 kernel with widened fragments."""
+    import torch
+    import paper_2504_10096_b200 as b
+    N, steps = 320, 60
+    R = gen.dense_R(N, 3, sigma=0.0)
+    R32 = orc.round_c64(R)
+    d = gen.block_X(N, 1, 8)[:, 0]
+    h = b.Bse(b.MODE_TDA, N, _pack64(R, 0), storage=b.STORE_C64)
+    alpha, beta = h.lanczos_quadrature(torch.from_numpy(np.ascontiguousarray(d)).cuda(), steps)
+    ao, bo = orc.lanczos_quadrature(R32, d, steps)
+    assert np.max(np.abs(alpha - ao)) <= 1e-11 * 11 and np.max(np.abs(beta - bo)) <= 1e-11 * 11
+    a_unrounded, _ = orc.lanczos_quadrature(R, d, steps)
+    assert np.max(np.abs(alpha - a_unrounded)) > 1e-9            # it is the rounded operator that was applied
