@@ -222,8 +222,11 @@ def run_cuda(args, cfg):
     achieved = alg_bytes(N, k) / (ms * 1e-3) / 1e9
     traffic = None
     try:
-        with open(os.path.join(ROOT, "profiles", "r1_apply_traffic.json")) as f:
-            traffic = json.load(f).get(f"N{N}_k{k}" + ("" if ES == 16.0 else "_c64"))
+        import csv
+        with open(os.path.join(ROOT, "profiles", "r1_apply_traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == f"N{N}_k{k}" + ("" if ES == 16.0 else "_c64"):
+                    traffic = float(row["dram_bytes_per_launch"])
     except Exception:
         pass
     # north_star: roofline = min(bytes / HBM peak, flops / FP64 peak).  The FP64 figure is this repo's own DMMA
