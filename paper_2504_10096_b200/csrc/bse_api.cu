@@ -5,6 +5,7 @@
 
 #include "apply_kernel.cuh"
 #include "apply_kernel_k1.cuh"
+#include "apply_kernel_3m.cuh"
 #include "bse_internal.h"
 #include "tile_layout.cuh"
 
@@ -62,6 +63,8 @@ bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, dou
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<16, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<8, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_3m_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_3m_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_k1_kernel<16, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_k1_kernel<8, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         if (dev < 64) attr_devices.fetch_or(1ull << dev, std::memory_order_release);
@@ -87,6 +90,8 @@ bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, dou
     int grid = (int)(p.n_units < h->num_sms ? p.n_units : h->num_sms);
     bool use_wide = true;                              // BSE_APPLY_WIDE=0: 4-column passes only
     if (const char *e = getenv("BSE_APPLY_WIDE")) use_wide = atoi(e) != 0;
+    bool use_3m = true;                                // BSE_APPLY_3M=0: four-product form for 5 .. 8 columns
+    if (const char *e = getenv("BSE_APPLY_3M")) use_3m = atoi(e) != 0;
     for (int32_t c0 = 0; c0 < k;) {
         const int32_t left = k - c0;
         const bool wide = use_wide && left > 4;        // 5 .. 8 columns in one pass over the operand
@@ -96,10 +101,12 @@ bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, dou
         const bool k1 = p.kc == 1 && use_k1;                 // plain-FMA single-column variant
         if (h->es == ES_C128) {
             if (k1) apply_tiles_k1_kernel<16, 8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            else if (wide && use_3m) apply_tiles_3m_kernel<16><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
             else if (wide) apply_tiles_kernel<16, 2><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
             else apply_tiles_kernel<16, 1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
         } else {
             if (k1) apply_tiles_k1_kernel<8, 8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            else if (wide && use_3m) apply_tiles_3m_kernel<8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
             else if (wide) apply_tiles_kernel<8, 2><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
             else apply_tiles_kernel<8, 1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
         }

@@ -247,16 +247,18 @@ def test_leading_dimensions_and_side_stream(orc):
 
 @pytest.mark.parametrize("k", [5, 7, 8, 11, 16])
 def test_wide_and_narrow_column_passes_agree_with_oracle(orc, k, monkeypatch):
-    """k > 4: the default takes 5..8 columns per pass over the operand (apply_tiles_kernel<ES, 2>), BSE_APPLY_WIDE=0
-    takes 4 at a time.  Both against the oracle, on a size with several units per CTA and a ragged last tile."""
+    """k > 4: the default takes 5..8 columns per pass over the operand with three real products per complex product
+    (apply_tiles_3m_kernel); BSE_APPLY_3M=0 takes the four-product form (apply_tiles_kernel<ES, 2>), BSE_APPLY_WIDE=0
+    takes 4 columns at a time.  All against the oracle, on a size with several units per CTA and a ragged last tile."""
     import paper_2504_10096_b200 as b
     N = 2000
     R = gen.dense_R(N, 31, sigma=0.5)
     X = gen.block_X(N, k, 32)
     ref = orc.apply_tda(R, X)
     h = b.Bse(b.MODE_TDA, N, pack(R, 0))
-    for wide in ("1", "0"):
+    for wide, m3 in (("1", "1"), ("1", "0"), ("0", "1")):
         monkeypatch.setenv("BSE_APPLY_WIDE", wide)
+        monkeypatch.setenv("BSE_APPLY_3M", m3)
         n0 = b.launch_count()
         Y = to_host(h.apply(to_dev(X)))
         launches = b.launch_count() - n0
@@ -266,3 +268,34 @@ def test_wide_and_narrow_column_passes_agree_with_oracle(orc, k, monkeypatch):
             left -= (min(left, 8) if (wide == "1" and left > 4) else min(left, 4))
             passes += 1
         assert launches == passes
+
+
+@pytest.mark.parametrize("kind", ["real_x", "imag_x", "real_T", "imag_T", "one_column_dominant"])
+def test_three_product_form_special_operands(orc, kind):
+    """The 5..8-column kernel forms re/im from Q1 = Tr xr, Q2 = Ti xi, Q3 = (Tr + Ti)(xr +- xi): operands for which one
+    of the three products vanishes or dominates must still meet the normwise tolerance (a wrong sign in one row of the
+    combination table shows up as an O(1) error here), for both passes (HERM through R, SYMC through C) and both
+    half-apply signs."""
+    import paper_2504_10096_b200 as b
+    N, k = 330, 8
+    R, C = _herm(N, 61), _sym(N, 62)
+    x = gen.block_X(N, k, 63)
+    if kind == "real_x":
+        x = x.real + 0j
+    elif kind == "imag_x":
+        x = 1j * x.imag
+    elif kind == "real_T":
+        R, C = R.real + 0j, C.real + 0j
+    elif kind == "imag_T":
+        R = 1j * np.tril(R.imag, -1); R = R + R.conj().T + np.diag(np.arange(1.0, N + 1))
+        C = 1j * C.imag
+    else:
+        x[:, 3] *= 1e8
+    h = b.Bse(b.MODE_FULL, N, pack(R, 0), pack(C, 1))
+    for sign in (+1, -1):
+        Y, ref = to_host(h.apply_half(to_dev(x), sign)), orc.apply_half(R, C, x, sign)
+        assert relerr(Y, ref) <= TOL_APPLY
+        for c in range(k):                     # column by column: a large column must not drown the others
+            assert relerr(Y[:, c], ref[:, c]) <= TOL_APPLY
+    ht = b.Bse(b.MODE_TDA, N, pack(R, 0))
+    assert relerr(to_host(ht.apply(to_dev(x))), orc.apply_tda(R, x)) <= TOL_APPLY
