@@ -60,6 +60,9 @@ def _load():
         lib.orc_round_c64.argtypes = [_i64, _c128, _c128]
         lib.orc_lanczos_quadrature.argtypes = [_i64, _c128, _c128, ctypes.c_int, _f64, _f64]
         lib.orc_lanczos_quadrature.restype = ctypes.c_int
+        lib.orc_lanczos_quadrature_full.argtypes = [_i64, _c128, _c128, _c128, ctypes.c_int, _f64, _f64]
+        lib.orc_lanczos_quadrature_full.restype = ctypes.c_int
+        lib.orc_quadrature_resolvent_at.argtypes = [ctypes.c_int, _f64, _f64, ctypes.c_int, _c128, _c128]
         lib.orc_quadrature_resolvent.argtypes = [ctypes.c_int, _f64, _f64, ctypes.c_int, _f64, ctypes.c_double, _c128]
         _lib = lib
     return _lib
@@ -197,6 +200,27 @@ def quadrature_resolvent(alpha, beta, omega, eta):
     out = np.zeros(len(omega), dtype=np.complex128)
     _load().orc_quadrature_resolvent(len(alpha), alpha, beta, len(omega), omega, float(eta), out)
     return out
+
+
+def lanczos_quadrature_full(R, C, d, steps):
+    """Full-mode Lanczos-with-quadrature coefficients (PAPER.md:65 on the operator of Eq. 1): the recurrence of G = M o P
+    in the inner product Re(a^H P(b)) started at d; beta[0] = sqrt(Re(d^H P(d)))."""
+    R, C = _c(R), _c(C)
+    N = R.shape[0]
+    alpha = np.zeros(steps); beta = np.zeros(steps + 1)
+    done = _load().orc_lanczos_quadrature_full(N, R, C, _c(d).reshape(N), steps, alpha, beta)
+    if done == -1000000:
+        raise np.linalg.LinAlgError("Omega is not positive definite")
+    return alpha[:done], beta[:done + 1]
+
+
+def quadrature_resolvent_full(alpha, beta, omega, eta):
+    """u^H Sigma (omega + i eta - H)^{-1} u, u = [d; conj d]:  2 beta_0^2 [(z^2 - T)^{-1}]_00."""
+    alpha = np.ascontiguousarray(alpha, dtype=np.float64); beta = np.ascontiguousarray(beta, dtype=np.float64)
+    s = np.ascontiguousarray((np.asarray(omega, dtype=np.float64) + 1j * float(eta)) ** 2, dtype=np.complex128)
+    out = np.zeros(len(s), dtype=np.complex128)
+    _load().orc_quadrature_resolvent_at(len(alpha), alpha, beta, len(s), s, out)
+    return 2.0 * out
 
 
 def round_c64(A):

@@ -604,6 +604,67 @@ void orc_quadrature_resolvent(int steps, const double *alpha, const double *beta
 }
 
 /* ------------------------------------------------------------------------------------------
+ * Lanczos with quadrature rules, full (pseudo-Hermitian) case (PAPER.md:65 with the operator of Eq. 1,
+ * PAPER.md:18, A = R^*, C = C^T).  Reading (R7), derived from Eq. (1) with the maps of reading S4,
+ *   P(x) = R x + C conj(x),  M(y) = R y - C conj(y),  H [x; conj x] = [P x; -conj P x],  H [y; -conj y] = [M y; conj M y]:
+ * for u = [d; conj d] and Sigma = diag(I, -I),
+ *   u^H Sigma (z - H)^{-1} u  =  2 <d, (z^2 - G)^{-1} d>_P,     G = M o P,   <a, b>_P = Re(a^H P(b)),
+ * because (z - H)^{-1} = (z + H)(z^2 - H^2)^{-1}, H^2 [x; conj x] = [G x; conj G x], Sigma H = Omega with
+ * [a; conj a]^H Omega [b; conj b] = 2 <a, b>_P, and the term with z alone is the quadratic form of an antisymmetric
+ * matrix (P(i x) = i M(x)), hence zero.  G is self-adjoint in <.,.>_P, so the three-term recurrence of
+ * orc_lanczos_full WITHOUT reorthogonalisation and without a stored basis gives a real Jacobi matrix:
+ *   beta_0 = sqrt(<d, d>_P);  x_1 = d / beta_0, p_1 = P(x_1);
+ *   w = M(p_j) - beta_j x_{j-1};  alpha_j = Re(p_j^H w);  w -= alpha_j x_j;  pw = P(w);
+ *   beta_{j+1} = sqrt(Re(w^H pw));  x_{j+1} = w / beta_{j+1},  p_{j+1} = pw / beta_{j+1},
+ * and  u^H Sigma (z - H)^{-1} u ~= 2 beta_0^2 [ (z^2 - T)^{-1} ]_00  (continued fraction in z^2).
+ * The other start vector of the structure, [y; -conj y], equals -i [iy; conj(iy)]: call with d = i y.
+ * Odd moments: u^H Sigma H^(2p+1) u = 2 beta_0^2 (T^p)_00 for p <= 2 steps - 1; even moments vanish.
+ * Returns the number of steps done; -1000000 if Re(w^H P w) < 0 is met (Omega not positive definite).
+ * ------------------------------------------------------------------------------------------ */
+int orc_lanczos_quadrature_full(int64_t N, const zc *R, const zc *C, const zc *d, int steps, double *alpha, double *beta)
+{
+    zc *x = (zc *)malloc(sizeof(zc) * N), *xp = (zc *)calloc(N, sizeof(zc)), *p = (zc *)malloc(sizeof(zc) * N);
+    zc *w = (zc *)malloc(sizeof(zc) * N), *pw = (zc *)malloc(sizeof(zc) * N);
+    int done = 0;
+    orc_apply_half(N, 1, +1, R, C, d, p);
+    ld s0 = 0.0L;
+    for (int64_t i = 0; i < N; ++i) s0 += (ld)creal(d[i]) * (ld)creal(p[i]) + (ld)cimag(d[i]) * (ld)cimag(p[i]);
+    if (!(s0 > 0.0L)) { done = -1000000; goto out; }
+    beta[0] = sqrt((double)s0);
+    for (int64_t i = 0; i < N; ++i) { x[i] = d[i] / beta[0]; p[i] = p[i] / beta[0]; }
+    for (int j = 0; j < steps; ++j) {
+        orc_apply_half(N, 1, -1, R, C, p, w);                                  /* w = M(p_j) */
+        if (j > 0) for (int64_t i = 0; i < N; ++i) w[i] -= beta[j] * xp[i];
+        ld a = 0.0L;
+        for (int64_t i = 0; i < N; ++i) a += (ld)creal(p[i]) * (ld)creal(w[i]) + (ld)cimag(p[i]) * (ld)cimag(w[i]);
+        alpha[j] = (double)a;
+        for (int64_t i = 0; i < N; ++i) w[i] -= alpha[j] * x[i];
+        orc_apply_half(N, 1, +1, R, C, w, pw);                                 /* pw = P(w) */
+        ld b2 = 0.0L;
+        for (int64_t i = 0; i < N; ++i) b2 += (ld)creal(w[i]) * (ld)creal(pw[i]) + (ld)cimag(w[i]) * (ld)cimag(pw[i]);
+        if (b2 < 0.0L) { done = -1000000; goto out; }
+        double b = sqrt((double)b2);
+        beta[j + 1] = b;
+        done = j + 1;
+        if (b == 0.0) break;
+        for (int64_t i = 0; i < N; ++i) { xp[i] = x[i]; x[i] = w[i] / b; p[i] = pw[i] / b; }
+    }
+out:
+    free(x); free(xp); free(p); free(w); free(pw);
+    return done;
+}
+
+/* Continued fraction at arbitrary complex arguments: out[i] = beta_0^2 * [ (s_i - T)^{-1} ]_{00}. */
+void orc_quadrature_resolvent_at(int steps, const double *alpha, const double *beta, int n, const zc *s, zc *out)
+{
+    for (int i = 0; i < n; ++i) {
+        zc f = s[i] - alpha[steps - 1];
+        for (int j = steps - 2; j >= 0; --j) f = s[i] - alpha[j] - beta[j + 1] * beta[j + 1] / f;
+        out[i] = beta[0] * beta[0] / f;
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
  * Single-precision operand.  PAPER.md:111 and the caption of Table 2
  * (PAPER.md:115): the paper's BSE matrices are computed and stored in single precision.  The
  * complex64-stored operator is, by definition, the matrix whose entries are the IEEE 754 binary32
