@@ -294,6 +294,24 @@ def run_cuda(args, cfg):
         res = h2.solve(c2["nev"], c2["k"], tol=1e-8, seed=1, raise_on_error=False)
         line["lanczos_time_to_nev"] = {"workload": f"config 2: TDA N={c2['N']} nev={c2['nev']} k={c2['k']} tol=1e-8",
                                        "seconds": time.perf_counter() - t0, "status": res.status, "info": res.info}
+        del h2
+        torch.cuda.empty_cache()
+        # full-mode Lanczos with quadrature (PAPER.md:65 on Eq. 1) at config 3's size: per step two half applies with
+        # k = 1, each streaming R and C once (4 tile passes of 8.59 GB)
+        c3 = gen.CONFIGS[3]
+        N3 = c3["N"]
+        h3 = b.Bse(b.MODE_FULL, N3, b.bse_fill_synthetic(N3, b.MATRIX_R, 1, 1.0, c3["group"]),
+                   b.bse_fill_synthetic(N3, b.MATRIX_C, 1, 0.0, c3["group"]))
+        d3 = Xh[0][:N3].contiguous().cuda()
+        h3.lanczos_quadrature(d3, 3)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        h3.lanczos_quadrature(d3, qsteps)
+        qsec = time.perf_counter() - t0
+        line["lanczos_quadrature_full"] = {"workload": f"config 3 operator: full N={N3}, sigma=1", "steps": qsteps,
+                                           "ms_per_step": qsec * 1e3 / qsteps,
+                                           "GBps": 4 * alg_bytes(N3, 1) * qsteps / qsec / 1e9}
+        del h3
 
     # ---- CPU baseline: the oracle on this box's host cores, bounded sample
     if not args.no_cpu_baseline:

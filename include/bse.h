@@ -181,11 +181,19 @@ bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_t ncv, doub
                        double *hResid, bse_info_t *info);
 
 /* Lanczos with quadrature rules (the optical absorption spectrum "directly, without explicitly computing
- * the eigenpairs").  TDA handles only.  Runs `steps` steps of the three-term Lanczos recurrence of R started at
- * d / |d| (dStart: N complex128, device; not modified), no reorthogonalisation, no stored basis:
- *   hAlpha[0..steps)  diagonal of the Jacobi matrix;  hBeta[0..steps]: hBeta[0] = |d|_2, hBeta[j] couples steps j-1, j.
- * *hDone (nullable) = number of valid steps (smaller than `steps` only on an exact breakdown).  Synchronous.
- * Each step is one bse_apply with k = 1 plus three O(N) kernels; all scalars stay on the device until the end. */
+ * the eigenpairs").  No reorthogonalisation, no stored basis; dStart: N complex128, device, not modified.  Synchronous;
+ * all scalars stay on the device until the end.
+ *   TDA handle:  `steps` steps of the three-term Lanczos recurrence of R started at d / |d|:
+ *     hAlpha[0..steps)  diagonal of the Jacobi matrix T;  hBeta[0..steps]: hBeta[0] = |d|_2, hBeta[j] couples steps
+ *     j-1, j.  Each step is one bse_apply with k = 1 plus three O(N) kernels.
+ *   FULL handle (operator of Eq. 1, with A = R^*, C = C^T): the recurrence of G = M o P,
+ *     P(x) = R x + C conj(x), M(y) = R y - C conj(y), in the inner product <a, b>_P = Re(a^H P(b)) (the structured
+ *     iteration of bse_solve with k = 1), started at d / sqrt(<d, d>_P): hBeta[0] = sqrt(Re(d^H P(d))).  For
+ *     u = [d; conj d], Sigma = diag(I, -I):  u^H Sigma (z - H)^{-1} u = 2 hBeta[0]^2 [(z^2 - T)^{-1}]_00
+ *     (bse_quadrature_resolvent_full).  The other start vector of the structure, [y; -conj y], is d = i y.  Each
+ *     step is two half applies with k = 1 (R and C streamed once each) plus five O(N) kernels.
+ *     BSE_ERR_NOT_POSITIVE_DEFINITE when Re(w^H P(w)) < 0 is met (PAPER.md:49's precondition fails).
+ * *hDone (nullable) = number of valid steps (smaller than `steps` only on an exact breakdown). */
 bse_status_t bse_lanczos_quadrature(bse_handle_t h, const void *dStart, int32_t steps, double *hAlpha,
                                     double *hBeta, int32_t *hDone);
 
@@ -193,6 +201,11 @@ bse_status_t bse_lanczos_quadrature(bse_handle_t h, const void *dStart, int32_t 
  * Jacobi matrix T(hAlpha, hBeta).  hOut: n_omega complex128 (host).  -Im(...)/pi is the broadened spectral function. */
 bse_status_t bse_quadrature_resolvent(int32_t steps, const double *hAlpha, const double *hBeta, int32_t n_omega,
                                       const double *hOmega, double eta, void *hOut);
+
+/* Host utility, full mode: u^H Sigma (omega_i + i eta - H)^{-1} u ~= 2 hBeta[0]^2 [(z^2 - T)^{-1}]_00, u = [d; conj d],
+ * from the coefficients a FULL handle's bse_lanczos_quadrature returned.  hOut: n_omega complex128 (host). */
+bse_status_t bse_quadrature_resolvent_full(int32_t steps, const double *hAlpha, const double *hBeta, int32_t n_omega,
+                                           const double *hOmega, double eta, void *hOut);
 
 /* Host utility (no device work): eigen-decomposition of the m x m complex Hermitian matrix hA (column-major, lda,
  * lower triangle read, destroyed) -- the "small projected eigenproblem" of PAPER.md:67, which bse_solve keeps on

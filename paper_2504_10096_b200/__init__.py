@@ -54,6 +54,7 @@ _SIGNATURES = {
     "bse_orth": [_vp, _vp, _i64, _i32, _vp, _i64, _vp, _i64, _i32, _vp, _i64, _vp, _vp, ctypes.POINTER(_i32)],
     "bse_lanczos_quadrature": [_vp, _vp, _i32, ctypes.POINTER(_dbl), ctypes.POINTER(_dbl), ctypes.POINTER(_i32)],
     "bse_quadrature_resolvent": [_i32, ctypes.POINTER(_dbl), ctypes.POINTER(_dbl), _i32, ctypes.POINTER(_dbl), _dbl, _vp],
+    "bse_quadrature_resolvent_full": [_i32, ctypes.POINTER(_dbl), ctypes.POINTER(_dbl), _i32, ctypes.POINTER(_dbl), _dbl, _vp],
     "bse_host_heev": [_i32, _vp, _i32, _vp, _vp, _i32, _i32],
     "bse_solve": [_vp, _i32, _i32, _i32, _dbl, _i32, _u64, ctypes.POINTER(_dbl), _vp, _i64, ctypes.POINTER(_dbl),
                   ctypes.POINTER(_Info)],
@@ -273,6 +274,19 @@ def quadrature_resolvent(alpha, beta, omega, eta: float):
     P = ctypes.POINTER(_dbl)
     _check(lib().bse_quadrature_resolvent(len(alpha), alpha.ctypes.data_as(P), beta.ctypes.data_as(P), len(omega),
                                           omega.ctypes.data_as(P), eta, out.ctypes.data), "bse_quadrature_resolvent")
+    return out
+
+
+def quadrature_resolvent_full(alpha, beta, omega, eta: float):
+    """Host utility, full mode: u^H Sigma (omega + i eta - H)^-1 u, u = [d; conj d] (numpy complex128 array)."""
+    import numpy as np
+    alpha = np.ascontiguousarray(alpha, dtype=np.float64); beta = np.ascontiguousarray(beta, dtype=np.float64)
+    omega = np.ascontiguousarray(omega, dtype=np.float64)
+    out = np.zeros(len(omega), dtype=np.complex128)
+    P = ctypes.POINTER(_dbl)
+    _check(lib().bse_quadrature_resolvent_full(len(alpha), alpha.ctypes.data_as(P), beta.ctypes.data_as(P), len(omega),
+                                               omega.ctypes.data_as(P), eta, out.ctypes.data),
+           "bse_quadrature_resolvent_full")
     return out
 
 

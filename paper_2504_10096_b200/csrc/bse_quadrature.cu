@@ -54,11 +54,71 @@ __global__ void __launch_bounds__(256) scale_by_norm_kernel(const double2 *__res
 
 using namespace bse;
 
+// Full (pseudo-Hermitian) case: the recurrence of G = M o P in the inner product Re(a^H P(b)) (reading R7 of DESIGN.md;
+// oracle: orc_lanczos_quadrature_full).  Per step two half applies with k = 1 (each streams R and C once) and five
+// O(N) kernels; five vectors, scalars on the device, one host synchronisation at the end.
+static bse_status_t lanczos_quadrature_full(bse_handle_s *h, const void *dStart, int32_t steps, double *hAlpha,
+                                            double *hBeta, int32_t *hDone)
+{
+    const int64_t n = h->N;
+    const size_t vec = (size_t)n * 16, scal = (size_t)(3 * steps + 3) * 8;
+    bse_status_t st = ensure_ws(h, 5 * vec + scal);
+    if (st) return st;
+    char *base = (char *)h->ws;
+    double2 *xb[3] = {(double2 *)base, (double2 *)(base + vec), (double2 *)(base + 2 * vec)};   // x_j, x_{j-1}, w
+    double2 *pb[2] = {(double2 *)(base + 3 * vec), (double2 *)(base + 4 * vec)};                // p_j, pw
+    double *d_alpha = (double *)(base + 5 * vec), *d_b2 = d_alpha + steps, *d_junk = d_b2 + steps + 1;
+    BSE_CUDA(cudaMemsetAsync(d_alpha, 0, scal, h->stream));
+    const int grid = h->num_sms * 2;
+    auto half = [&](int sign, const double2 *x, double2 *y) -> bse_status_t {
+        bse_status_t s2 = zero_block(h, y, n, n, 1);
+        if (s2) return s2;
+        if ((s2 = launch_apply_pass(h, h->R, 0, 1.0, x, n, y, n, 1))) return s2;
+        return launch_apply_pass(h, h->C, 1, (double)sign, x, n, y, n, 1);
+    };
+    // beta_0^2 = Re(d^H P(d));  x_1 = d / beta_0,  p_1 = P(d) / beta_0
+    if ((st = half(+1, (const double2 *)dStart, pb[1]))) return st;
+    dot_re_kernel<<<grid, 256, 0, h->stream>>>((const double2 *)dStart, pb[1], n, d_b2);
+    scale_by_norm_kernel<<<grid, 256, 0, h->stream>>>((const double2 *)dStart, xb[0], n, d_b2);
+    scale_by_norm_kernel<<<grid, 256, 0, h->stream>>>(pb[1], pb[0], n, d_b2);
+    count_launch(3);
+    int ix = 0, ip = 2, iw = 1;
+    for (int j = 0; j < steps; ++j) {
+        if ((st = half(-1, pb[0], xb[iw]))) return st;                                      // w = M(p_j)
+        dot_re_kernel<<<grid, 256, 0, h->stream>>>(pb[0], xb[iw], n, d_alpha + j);         // alpha_j = Re(p_j^H w)
+        axpy_norm_kernel<<<grid, 256, 0, h->stream>>>(xb[iw], xb[ix], xb[ip], n, d_alpha + j, j > 0 ? d_b2 + j : nullptr,
+                                                      d_junk + j);                          // w -= alpha x_j + beta x_{j-1}
+        count_launch(2);
+        if ((st = half(+1, xb[iw], pb[1]))) return st;                                      // pw = P(w)
+        dot_re_kernel<<<grid, 256, 0, h->stream>>>(xb[iw], pb[1], n, d_b2 + j + 1);        // beta_{j+1}^2 = Re(w^H pw)
+        scale_by_norm_kernel<<<grid, 256, 0, h->stream>>>(xb[iw], xb[iw], n, d_b2 + j + 1);
+        scale_by_norm_kernel<<<grid, 256, 0, h->stream>>>(pb[1], pb[0], n, d_b2 + j + 1);
+        count_launch(3);
+        int t = ip; ip = ix; ix = iw; iw = t;
+    }
+    BSE_CUDA(cudaGetLastError());
+    std::vector<double> hs(2 * steps + 1);
+    BSE_CUDA(cudaMemcpyAsync(hs.data(), d_alpha, (size_t)(2 * steps + 1) * 8, cudaMemcpyDeviceToHost, h->stream));
+    BSE_CUDA(cudaStreamSynchronize(h->stream));
+    if (!(hs[steps] > 0.0)) return BSE_ERR_NOT_POSITIVE_DEFINITE;                          // <d, d>_P <= 0
+    int done = steps;
+    hBeta[0] = std::sqrt(hs[steps]);
+    for (int j = 0; j < steps; ++j) {
+        const double b2 = hs[steps + j + 1];
+        if (b2 < 0.0) return BSE_ERR_NOT_POSITIVE_DEFINITE;
+        hAlpha[j] = hs[j];
+        hBeta[j + 1] = std::sqrt(b2);
+        if (!(b2 > 0.0)) { done = j + 1; break; }
+    }
+    if (hDone) *hDone = done;
+    return BSE_OK;
+}
+
 extern "C" bse_status_t bse_lanczos_quadrature(bse_handle_t h, const void *dStart, int32_t steps, double *hAlpha,
                                                double *hBeta, int32_t *hDone)
 {
     if (!h || !dStart || steps < 1 || !hAlpha || !hBeta) return BSE_ERR_INVALID_ARG;
-    if (h->mode != BSE_MODE_TDA) return BSE_ERR_INVALID_ARG;
+    if (h->mode == BSE_MODE_FULL) return lanczos_quadrature_full(h, dStart, steps, hAlpha, hBeta, hDone);
     const int64_t n = h->N;
     // workspace: three vectors + alpha[steps] + nrm2[steps + 1]
     const size_t vec = (size_t)n * 16, scal = (size_t)(2 * steps + 2) * 8;
@@ -101,14 +161,14 @@ extern "C" bse_status_t bse_lanczos_quadrature(bse_handle_t h, const void *dStar
     return BSE_OK;
 }
 
-extern "C" bse_status_t bse_quadrature_resolvent(int32_t steps, const double *hAlpha, const double *hBeta,
-                                                 int32_t n_omega, const double *hOmega, double eta, void *hOut)
+// out = scale * beta_0^2 [(s - T)^{-1}]_00 with s = z (TDA) or s = z^2 (full mode), z = omega + i eta
+static void continued_fraction(int32_t steps, const double *hAlpha, const double *hBeta, int32_t n_omega,
+                               const double *hOmega, double eta, bool squared, double scale, double *out)
 {
-    if (steps < 1 || !hAlpha || !hBeta || n_omega < 0 || (n_omega && (!hOmega || !hOut))) return BSE_ERR_INVALID_ARG;
-    double *out = (double *)hOut;
     for (int i = 0; i < n_omega; ++i) {
-        // f <- z - alpha_j - beta_{j+1}^2 / f, from the last coefficient up; complex arithmetic written out
+        // f <- s - alpha_j - beta_{j+1}^2 / f, from the last coefficient up; complex arithmetic written out
         double zr = hOmega[i], zi = eta;
+        if (squared) { const double a = zr, b = zi; zr = a * a - b * b; zi = 2.0 * a * b; }
         double fr = zr - hAlpha[steps - 1], fi = zi;
         for (int j = steps - 2; j >= 0; --j) {
             double b2 = hBeta[j + 1] * hBeta[j + 1], den = fr * fr + fi * fi;
@@ -116,9 +176,24 @@ extern "C" bse_status_t bse_quadrature_resolvent(int32_t steps, const double *hA
             fr = zr - hAlpha[j] - qr;
             fi = zi - qi;
         }
-        double den = fr * fr + fi * fi, b0 = hBeta[0] * hBeta[0];
+        double den = fr * fr + fi * fi, b0 = scale * hBeta[0] * hBeta[0];
         out[2 * i] = b0 * fr / den;
         out[2 * i + 1] = -b0 * fi / den;
     }
+}
+
+extern "C" bse_status_t bse_quadrature_resolvent(int32_t steps, const double *hAlpha, const double *hBeta,
+                                                 int32_t n_omega, const double *hOmega, double eta, void *hOut)
+{
+    if (steps < 1 || !hAlpha || !hBeta || n_omega < 0 || (n_omega && (!hOmega || !hOut))) return BSE_ERR_INVALID_ARG;
+    continued_fraction(steps, hAlpha, hBeta, n_omega, hOmega, eta, false, 1.0, (double *)hOut);
+    return BSE_OK;
+}
+
+extern "C" bse_status_t bse_quadrature_resolvent_full(int32_t steps, const double *hAlpha, const double *hBeta,
+                                                      int32_t n_omega, const double *hOmega, double eta, void *hOut)
+{
+    if (steps < 1 || !hAlpha || !hBeta || n_omega < 0 || (n_omega && (!hOmega || !hOut))) return BSE_ERR_INVALID_ARG;
+    continued_fraction(steps, hAlpha, hBeta, n_omega, hOmega, eta, true, 2.0, (double *)hOut);
     return BSE_OK;
 }

@@ -75,9 +75,72 @@ def test_quadrature_invalid_arguments():
     import paper_2504_10096_b200 as b
     N = 64
     R = gen.dense_R(N, 3, sigma=1.0)
-    hf = b.Bse(b.MODE_FULL, N, pack(R, 0), pack(gen.dense_C(N, 3), 1))
     d = _dev_vec(gen.block_X(N, 1, 1)[:, 0])
-    with pytest.raises(b.BseError):
-        hf.lanczos_quadrature(d, 4)                       # TDA handles only
     h = b.Bse(b.MODE_TDA, N, pack(R, 0))
     assert b.lib().bse_lanczos_quadrature(h._h, d.data_ptr(), 0, None, None, None) == 1
+    # full mode: an indefinite Omega (R = -I, C = 0: <d, d>_P < 0) is reported, not iterated on
+    Z = np.zeros((N, N), dtype=complex)
+    hn = b.Bse(b.MODE_FULL, N, pack(-np.eye(N, dtype=complex), 0), pack(Z, 1))
+    with pytest.raises(b.BseError) as e:
+        hn.lanczos_quadrature(d, 4)
+    assert e.value.status == b.lib().bse_lanczos_quadrature(hn._h, d.data_ptr(), 4, (ctypes.c_double * 4)(),
+                                                            (ctypes.c_double * 5)(), None) != 0
+
+
+def test_full_mode_coefficients_and_resolvent_match_oracle(orc):
+    """Full (pseudo-Hermitian) quadrature (include/bse.h; oracle: lanczos_quadrature_full): coefficients against the
+    oracle while the two recurrences are the same to rounding, the converged resolvent against the exact
+    u^H Sigma (z - H)^-1 u from a dense solve of the block operator of Eq. (1)."""
+    import paper_2504_10096_b200 as b
+    N, steps = 192, 260
+    R, C = gen.dense_R(N, 5, sigma=1.0), gen.dense_C(N, 5)
+    d = gen.block_X(N, 1, 6)[:, 0]
+    h = b.Bse(b.MODE_FULL, N, pack(R, 0), pack(C, 1))
+    alpha, beta = h.lanczos_quadrature(_dev_vec(d), steps)
+    ao, bo = orc.lanczos_quadrature_full(R, C, d, steps)
+    assert len(alpha) == steps
+    sc = np.max(np.abs(ao))                                # ~ |H|^2
+    assert np.max(np.abs(alpha[:15] - ao[:15])) <= 1e-10 * sc and np.max(np.abs(beta[:16] - bo[:16])) <= 1e-10 * sc
+    assert abs(beta[0] ** 2 - np.vdot(d, R @ d + C @ d.conj()).real) <= 1e-13 * beta[0] ** 2
+    om = np.linspace(0.0, 12.0, 121); eta = 0.15
+    G40 = b.quadrature_resolvent_full(alpha[:40], beta[:41], om, eta)
+    Go40 = orc.quadrature_resolvent_full(ao[:40], bo[:41], om, eta)
+    assert np.max(np.abs(G40 - Go40)) <= 1e-9 * np.max(np.abs(Go40))
+    H = np.block([[R, C], [-C.conj(), -R.conj()]])
+    u = np.concatenate([d, d.conj()]); sig = np.concatenate([np.ones(N), -np.ones(N)])
+    exact = np.array([np.vdot(u, sig * np.linalg.solve((w + 1j * eta) * np.eye(2 * N) - H, u)) for w in om])
+    G = b.quadrature_resolvent_full(alpha, beta, om, eta)
+    Go = orc.quadrature_resolvent_full(ao, bo, om, eta)
+    err_o = np.max(np.abs(Go - exact)) / np.max(np.abs(exact))
+    assert np.max(np.abs(G - exact)) <= max(10 * err_o, 1e-6) * np.max(np.abs(exact))
+    assert err_o <= 1e-4                                    # the oracle itself has converged at this step count
+
+
+def test_full_mode_moments_at_a_many_tile_size(orc):
+    """N = 4096, device-generated R and C (every CTA walks several units; the k = 1 kernel in both passes): odd moments
+    u^H Sigma H^(2p+1) u = 2 beta_0^2 (T^p)_00 for p <= 2 steps - 1, with H^n u from the CUDA full apply (parity-tested in
+    test_gpu_apply.py), and the even moments vanish."""
+    import torch
+    import paper_2504_10096_b200 as b
+    N, steps = 4096, 6
+    h = b.Bse(b.MODE_FULL, N, b.bse_fill_synthetic(N, 0, 1, 1.0, 16), b.bse_fill_synthetic(N, 1, 1, 0.0, 16))
+    d = gen.block_X(N, 1, 9)[:, 0]
+    alpha, beta = h.lanczos_quadrature(_dev_vec(d), steps)
+    T = np.diag(alpha) + np.diag(beta[1:steps], 1) + np.diag(beta[1:steps], -1)
+    u = _dev_vec(np.concatenate([d, d.conj()])).reshape(1, 2 * N)
+    sig = torch.cat([torch.ones(N), -torch.ones(N)]).to(torch.complex128).cuda()
+    vs = [u]
+    for _ in range(2 * steps):
+        vs.append(h.apply(vs[-1]))
+    Tp = np.eye(steps)
+    uu = float(torch.vdot(u.flatten(), u.flatten()).real)
+    for p in range(2 * steps):
+        n = 2 * p + 1                       # Sigma H is Hermitian, so u^H Sigma H^n u = (H^a u)^H Sigma (H^c u), a + c = n
+        a, c = vs[n // 2], vs[n - n // 2]
+        exact = complex(torch.vdot(a.flatten(), sig * c.flatten()))
+        assert abs(exact.imag) <= 1e-9 * abs(exact.real)
+        assert abs(2 * beta[0] ** 2 * Tp[0, 0] - exact.real) <= 1e-8 * abs(exact.real), p
+        even = complex(torch.vdot(vs[p].flatten(), sig * vs[p].flatten()))      # u^H Sigma H^(2p) u
+        assert abs(even) <= 1e-9 * float(torch.vdot(vs[p].flatten(), vs[p].flatten()).real)
+        Tp = Tp @ T
+    assert uu > 0
