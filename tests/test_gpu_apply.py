@@ -189,24 +189,48 @@ def test_full_apply_many_units_sampled_rows(orc):
 
 def test_config4_full_size_sampled_rows(orc):
     """BASELINE.json config 4 (N = 98304, 77 GB operand filled on the device): rows of Y sampled across the matrix,
-    against the oracle fed with the same rows from the CPU generator.  Needs ~80 GB of HBM."""
+    against the oracle fed with the same rows from the CPU generator, for every kernel bench.py times at this size
+    (k = 1: plain-FMA kernel, k = 4: four-product DMMA kernel, k = 8: three-product DMMA kernel).  Needs ~80 GB of HBM."""
     import torch
     import paper_2504_10096_b200 as b
     cfg = gen.CONFIGS[4]
-    N, k = cfg["N"], 4
+    N = cfg["N"]
     if torch.cuda.mem_get_info()[0] < 90e9:
         pytest.skip("needs 90 GB of free device memory")
     h = b.Bse(b.MODE_TDA, N, b.bse_fill_synthetic(N, 0, 1, 0.0, cfg["group"]))
-    X = gen.block_X(N, k, 12)
+    X = gen.block_X(N, 8, 12)
     rows = np.unique(np.concatenate([(np.arange(40) * 2654435761 % N), [0, 7, 63, 64, N - 65, N - 64, N - 1],
                                      np.arange(8) + 64 * 777]).astype(np.int64))
     ref = orc.rows_times_block(gen.rows_R(N, 1, rows, 0.0, cfg["group"]), X)
-    Y = to_host(h.apply(to_dev(X)))
-    assert relerr(Y[rows], ref) <= TOL_APPLY
-    Z = gen.block_X(N, k, 13)
-    RZ = to_host(h.apply(to_dev(Z)))
-    lhs, rhs = X.conj().T @ RZ, Y.conj().T @ Z
-    assert np.linalg.norm(lhs - rhs) <= 1e-12 * np.linalg.norm(lhs)
+    for k in (4, 8, 1):
+        Y = to_host(h.apply(to_dev(X[:, :k])))
+        assert relerr(Y[rows], ref[:, :k]) <= TOL_APPLY, k
+        Z = gen.block_X(N, k, 13)
+        RZ = to_host(h.apply(to_dev(Z)))
+        lhs, rhs = X[:, :k].conj().T @ RZ, Y.conj().T @ Z
+        assert np.linalg.norm(lhs - rhs) <= 1e-12 * np.linalg.norm(lhs), k
+
+
+def test_config3_full_size_half_apply_sampled_rows(orc):
+    """BASELINE.json config 3 (full mode, N = 32768, R and C 8.6 GB each, filled on the device): sampled rows of
+    P(X) = R X + C conj(X) and M(X) = R X - C conj(X) -- the two products bse_solve issues per block step -- for the
+    four-product (k = 4) and three-product (k = 8) kernels, against the oracle on rows from the CPU generator."""
+    import torch
+    import paper_2504_10096_b200 as b
+    cfg = gen.CONFIGS[3]
+    N = cfg["N"]
+    if torch.cuda.mem_get_info()[0] < 30e9:
+        pytest.skip("needs 30 GB of free device memory")
+    h = b.Bse(b.MODE_FULL, N, b.bse_fill_synthetic(N, 0, 1, cfg["sigma"], cfg["group"]),
+              b.bse_fill_synthetic(N, 1, 1, 0.0, cfg["group"]))
+    X = gen.block_X(N, 8, 14)
+    rows = np.unique(np.concatenate([(np.arange(24) * 2654435761 % N), [0, 63, 64, N - 64, N - 1]]).astype(np.int64))
+    RX = orc.rows_times_block(gen.rows_R(N, 1, rows, cfg["sigma"], cfg["group"]), X)
+    CX = orc.rows_times_block(gen.rows_C(N, 1, rows), X.conj())
+    for k in (4, 8):
+        for sign in (+1, -1):
+            Y = to_host(h.apply_half(to_dev(X[:, :k]), sign))
+            assert relerr(Y[rows], (RX + sign * CX)[:, :k]) <= TOL_APPLY, (k, sign)
 
 
 @pytest.mark.parametrize("N", [1, 2, 63, 65, 127])
