@@ -41,6 +41,11 @@
  * nearest-even when the store is written, and the operator every later call works with IS the
  * rounded matrix: fragments are widened to FP64 on load and all arithmetic, vectors and results
  * stay complex128.  Half the HBM bytes per apply, twice the N per GPU.
+ * BSE_STORE_REAL_FORM (full mode, bse_layout and bse_create only): the two complex128 stores hold S = R + C and
+ * D = R - C -- the blocks Re(R+C), Im(R+C), Re(R-C), Im(R-C) of the real symmetric M_r of Eq. (3) --
+ * written by bse_to_real_form from stores of R and C.  The half applies then run in real arithmetic,
+ * P(x): re = Sr a - Di b, im = Si a + Dr b;  M(x): re = Dr a - Si b, im = Di a + Sr b  (x = a + i b),
+ * with half the flops of the complex form; every result is the same operator's to rounding.
  */
 #ifndef BSE_B200_H
 #define BSE_B200_H
@@ -65,7 +70,7 @@ typedef enum {
 
 enum { BSE_MODE_TDA = 0, BSE_MODE_FULL = 1 };
 enum { BSE_MATRIX_R = 0, BSE_MATRIX_C = 1 };
-enum { BSE_STORE_C128 = 0, BSE_STORE_C64 = 1 };
+enum { BSE_STORE_C128 = 0, BSE_STORE_C64 = 1, BSE_STORE_REAL_FORM = 2 };
 
 typedef struct {
     int32_t n_apply;        /* operator applications (block applies; a full-mode step counts 2 half applies) */
@@ -125,6 +130,11 @@ bse_status_t bse_fill_closed_form_full(void *dRTiles, void *dCTiles, int32_t sto
 bse_status_t bse_create(bse_handle_t *h, int32_t mode, int32_t storage, int64_t N, const void *dRTiles,
                         const void *dCTiles, void *stream);
 bse_status_t bse_destroy(bse_handle_t h);
+
+/* In place, on two BSE_STORE_C128 stores of the same N:  dRTiles <- S = R + C,  dCTiles <- D = R - C (every stored
+ * entry, mirrored halves and padding included).  Afterwards pass both to bse_create with BSE_STORE_REAL_FORM (mode
+ * FULL); they no longer represent R and C for any other call.  Asynchronous on `stream`. */
+bse_status_t bse_to_real_form(void *dRTiles, void *dCTiles, int64_t N, void *stream);
 
 /* Y = H X for a block of k >= 1 vectors.
  *   TDA : X, Y are N x k;   Y = R X.

@@ -1,0 +1,218 @@
+// Full-mode half apply in the REAL FORM of Eq. (3) ("8 N^2 k flops if evaluated in the
+// real form").  With S = R + C and D = R - C stored instead of R and C (bse_to_real_form), and x = a + i b,
+//     P(x) = R x + C conj(x):   re = Sr a - Di b,   im = Si a + Dr b        (the blocks of M_r in Eq. 3)
+//     M(x) = R x - C conj(x):   re = Dr a - Si b,   im = Di a + Sr b
+// and, for the transposed use of a stored tile (i in I, j in J, I > J), Re S_ji = Sr_ij, Im S_ji = -Di_ij,
+// Re D_ji = Dr_ij, Im D_ji = -Si_ij, so that
+//     P:  re_J += Sr^T a_I + Si^T b_I,   im_J += Dr^T b_I - Di^T a_I
+//     M:  re_J += Dr^T a_I + Di^T b_I,   im_J += Sr^T b_I - Si^T a_I.
+// One pass streams ONE store (tiles A = Ar + i Ai, read once, used twice) in one of two modes:
+//     MODE 0:  P1: re_I += Ar a_J,  im_I += Ai a_J;    P2: re_J += Ar^T a_I + Ai^T b_I
+//     MODE 1:  P1: re_I -= Ai b_J,  im_I += Ar b_J;    P2: im_J += Ar^T b_I - Ai^T a_I
+// P = MODE 0 over S + MODE 1 over D;  M = MODE 0 over D + MODE 1 over S.  Every product is REAL: the 8-wide N
+// dimension of a DMMA holds up to eight columns of X, 2 DMMAs per 8 x 8 x 4 block in each role (the three-product
+// complex kernel needs 3, the four-product one 4 for eight columns): half the flops of the complex form.
+// Same ring, producer, stage release and warp roles as apply_tiles_3m_kernel: warps 0..3 P1 (rows 32 rh .. +31 x
+// columns 32 ch .. +31, two accumulator sets kept for the unit), warps 4..7 P2 (columns 16 r .. +15, a_I and b_I
+// fragments in 64 registers, eight accumulator chains per tile), 64 DMMAs per tile per warp.
+#pragma once
+#include "apply_kernel.cuh"
+
+namespace bse {
+
+template <int MODE>
+__global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_real_kernel(const ApplyParams p)
+{
+    constexpr int ES = 16;
+    constexpr int TBY = TB * TB * ES;
+    constexpr int PBY = 64 * ES;
+    constexpr int NST = APPLY_STAGES * 16 / ES;
+    constexpr int S1 = 16 * ES, S2 = 32 * ES;
+    extern __shared__ __align__(1024) char smem[];
+    char *tile_s = smem;
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + NST * TBY);
+    uint64_t *full = bars, *empty = bars + NST;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NST; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], APPLY_CONSUMERS); }
+        fence_barrier_init();
+    }
+    __syncthreads();
+
+    if (warp == APPLY_CONSUMERS) {
+        if (lane == 0) {                                   // producer: identical to apply_tiles_kernel
+            int st = 0;
+            uint32_t ph = 0;
+            const uint64_t pol = l2_policy_evict_first();
+            for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
+                int I, J0, J1;
+                apply_decode_unit(u, p.L, I, J0, J1);
+                const char *src = p.tiles + tile_index(I, J0) * (int64_t)TBY;
+                for (int J = J0; J < J1; ++J, src += TBY) {
+                    mbar_wait(&empty[st], ph ^ 1);
+                    mbar_expect_tx(&full[st], (uint32_t)TBY);
+                    bulk_g2s_hint(tile_s + st * TBY, src, TBY, &full[st], pol);
+                    if (++st == NST) { st = 0; ph ^= 1; }
+                }
+            }
+        }
+        return;
+    }
+
+    const int g = lane >> 2, t = lane & 3;
+    const int g2 = (g >> 2) & 1, g1 = (g >> 1) & 1, g0 = g & 1, t1 = (t >> 1) & 1, t0 = t & 1;
+    const int offP1 = (((g2 << 2) | g1) * 8 + ((g0 << 2) | (t0 << 1) | (g1 ^ t1))) * ES;   // (a = g, b = 4 s + t)
+    const int offP2 = (((g2 << 1) | t1) * 8 + ((t0 << 2) | (g0 << 1) | (t1 ^ g1))) * ES;   // (a = 4 s + t, b = g)
+    // B fragments: lane supplies B[kk = t][n = g], n = column of X; accumulators c[e] = C[g][2 t + e]
+    const bool colok = g < p.kc;
+    const double2 *xcol = p.X + (int64_t)(colok ? g : 0) * p.ldx;
+    const int kc = p.kc;
+    int st = 0;
+    uint32_t ph = 0;
+
+    if (warp < 4) {
+        // ------------------------------ P1 warps ------------------------------
+        const int rh = warp & 1, ch = warp >> 1;
+        auto load_xj = [&](int K, double (&x)[4][2]) {     // a_J (MODE 0) or b_J (MODE 1), rows 8 (4 ch + pc) + 4 s + t
+#pragma unroll
+            for (int pc = 0; pc < 4; ++pc)
+#pragma unroll
+                for (int s = 0; s < 2; ++s) {
+                    int64_t row = (int64_t)K * TB + (4 * ch + pc) * 8 + s * 4 + t;
+                    x[pc][s] = (colok && row < p.N) ? __ldg(reinterpret_cast<const double *>(xcol + row) + MODE) : 0.0;
+                }
+        };
+        for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
+            int I, J0, J1;
+            apply_decode_unit(u, p.L, I, J0, J1);
+            double xjn[4][2];
+            load_xj(J0, xjn);
+            double U[4][2], W[4][2];                           // U = Ar x, W = Ai x
+#pragma unroll
+            for (int ib = 0; ib < 4; ++ib) U[ib][0] = U[ib][1] = W[ib][0] = W[ib][1] = 0.0;
+            for (int J = J0; J < J1; ++J) {
+                double xj[4][2];
+#pragma unroll
+                for (int pc = 0; pc < 4; ++pc) { xj[pc][0] = xjn[pc][0]; xj[pc][1] = xjn[pc][1]; }
+                if (J + 1 < J1) load_xj(J + 1, xjn);
+                mbar_wait(&full[st], ph);
+                const char *tp = tile_s + st * TBY + (4 * ch) * 8 * PBY + (4 * rh) * PBY;
+#pragma unroll
+                for (int pc = 0; pc < 4; ++pc)
+#pragma unroll
+                    for (int s = 0; s < 2; ++s) {
+                        double2 a[4];
+#pragma unroll
+                        for (int ib = 0; ib < 4; ++ib) a[ib] = load_frag<ES>(tp + (pc * 8 + ib) * PBY + offP1 + s * S1);
+#pragma unroll
+                        for (int ib = 0; ib < 4; ++ib) {
+                            dmma(U[ib], a[ib].x, xj[pc][s]);
+                            dmma(W[ib], a[ib].y, xj[pc][s]);
+                        }
+                    }
+                int live = 0;
+#pragma unroll
+                for (int ib = 0; ib < 4; ++ib) live |= __double2hiint(U[ib][0]) | __double2hiint(W[ib][0]);
+                __syncwarp();
+                if (lane == 0)
+                    mbar_arrive(reinterpret_cast<uint64_t *>(reinterpret_cast<char *>(&empty[st]) + (live & p.zero)));
+                if (++st == NST) { st = 0; ph ^= 1; }
+            }
+#pragma unroll
+            for (int ib = 0; ib < 4; ++ib) {
+                int64_t row = (int64_t)I * TB + (4 * rh + ib) * 8 + g;
+                if (row < p.N) {
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const int c = 2 * t + e;
+                        if (c < kc) {
+                            double *y = p.Y + 2 * (row + (int64_t)c * p.ldy);
+                            if (MODE == 0) { red_add(y, U[ib][e]); red_add(y + 1, W[ib][e]); }
+                            else { red_add(y, -W[ib][e]); red_add(y + 1, U[ib][e]); }
+                        }
+                    }
+                }
+            }
+        }
+        return;
+    }
+
+    // ------------------------------ P2 warps ------------------------------
+    const int r = warp - 4;
+    for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
+        int I, J0, J1;
+        apply_decode_unit(u, p.L, I, J0, J1);
+        // xA pairs with Ar^T, xB with Ai^T:  MODE 0: (a_I, b_I);  MODE 1: (b_I, -a_I)
+        double xA[8][2], xB[8][2];
+#pragma unroll
+        for (int ib = 0; ib < 8; ++ib)
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                int64_t row = (int64_t)I * TB + ib * 8 + s * 4 + t;
+                double2 x = (colok && row < p.N) ? __ldg(xcol + row) : make_double2(0.0, 0.0);
+                xA[ib][s] = MODE == 0 ? x.x : x.y;
+                xB[ib][s] = MODE == 0 ? x.y : -x.x;
+            }
+        for (int J = J0; J < J1; ++J) {
+            mbar_wait(&full[st], ph);
+            if (I != J) {
+                double ZA[2][2][2], ZB[2][2][2];             // [pc][ib parity][e]: eight independent chains
+#pragma unroll
+                for (int pc = 0; pc < 2; ++pc)
+#pragma unroll
+                    for (int q = 0; q < 2; ++q) ZA[pc][q][0] = ZA[pc][q][1] = ZB[pc][q][0] = ZB[pc][q][1] = 0.0;
+                const char *tp = tile_s + st * TBY + (2 * r) * 8 * PBY;
+#pragma unroll
+                for (int ib = 0; ib < 8; ib += 2) {
+                    double2 b[2][2][2];
+#pragma unroll
+                    for (int q = 0; q < 2; ++q)
+#pragma unroll
+                        for (int s = 0; s < 2; ++s)
+#pragma unroll
+                            for (int pc = 0; pc < 2; ++pc)
+                                b[q][s][pc] = load_frag<ES>(tp + (pc * 8 + ib + q) * PBY + offP2 + s * S2);
+#pragma unroll
+                    for (int s = 0; s < 2; ++s)
+#pragma unroll
+                        for (int q = 0; q < 2; ++q)
+#pragma unroll
+                            for (int pc = 0; pc < 2; ++pc) {
+                                dmma(ZA[pc][q], b[q][s][pc].x, xA[ib + q][s]);
+                                dmma(ZB[pc][q], b[q][s][pc].y, xB[ib + q][s]);
+                            }
+                }
+                double z[2][2];
+                int live = 0;
+#pragma unroll
+                for (int pc = 0; pc < 2; ++pc)
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        z[pc][e] = (ZA[pc][0][e] + ZA[pc][1][e]) + (ZB[pc][0][e] + ZB[pc][1][e]);
+                        live |= __double2hiint(z[pc][e]);
+                    }
+                __syncwarp();
+                if (lane == 0)
+                    mbar_arrive(reinterpret_cast<uint64_t *>(reinterpret_cast<char *>(&empty[st]) + (live & p.zero)));
+#pragma unroll
+                for (int pc = 0; pc < 2; ++pc) {
+                    int64_t row = (int64_t)J * TB + (2 * r + pc) * 8 + g;
+                    if (row < p.N) {
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) {
+                            const int c = 2 * t + e;
+                            if (c < kc) red_add(p.Y + 2 * (row + (int64_t)c * p.ldy) + MODE, z[pc][e]);
+                        }
+                    }
+                }
+            } else {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[st]);       // diagonal tile: stored in full, P1 only
+            }
+            if (++st == NST) { st = 0; ph ^= 1; }
+        }
+    }
+}
+
+}  // namespace bse

@@ -6,6 +6,7 @@
 #include "apply_kernel.cuh"
 #include "apply_kernel_k1.cuh"
 #include "apply_kernel_3m.cuh"
+#include "apply_kernel_real.cuh"
 #include "bse_internal.h"
 #include "tile_layout.cuh"
 
@@ -51,8 +52,7 @@ bse_status_t zero_block(bse_handle_s *h, void *dY, int64_t ldy, int64_t rows, in
     return BSE_OK;
 }
 
-bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, double sign, const void *dX,
-                               int64_t ldx, void *dY, int64_t ldy, int32_t k)
+static bse_status_t apply_kernel_attributes()
 {
     // cudaFuncSetAttribute is per device: remember which devices of this process have been set up
     static std::atomic<uint64_t> attr_devices{0};
@@ -63,22 +63,21 @@ bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, dou
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<16, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<8, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_3m_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_3m_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_k1_kernel<16, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_k1_kernel<8, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         if (dev < 64) attr_devices.fetch_or(1ull << dev, std::memory_order_release);
     }
-    bool use_k1 = true;                                // BSE_APPLY_K1=0: tensor-core kernel for single columns too
-    if (const char *e = getenv("BSE_APPLY_K1")) use_k1 = atoi(e) != 0;
-    ApplyParams p;
-    p.tiles = tiles;
+    return BSE_OK;
+}
+
+static void apply_unit_params(const bse_handle_s *h, ApplyParams &p, int &grid)
+{
     p.N = h->N;
     p.nt = h->nt;
-    p.pass = pass;
-    p.sign = sign;
-    p.ldx = ldx;
-    p.ldy = ldy;
     int64_t total_tiles = (int64_t)h->nt * (h->nt + 1) / 2;
     int64_t L = total_tiles / ((int64_t)h->num_sms * 12);
     if (L < 1) L = 1;
@@ -87,7 +86,49 @@ bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, dou
     p.L = (int)L;
     p.n_units = apply_num_units(h->nt, p.L);
     p.zero = 0;
-    int grid = (int)(p.n_units < h->num_sms ? p.n_units : h->num_sms);
+    grid = (int)(p.n_units < h->num_sms ? p.n_units : h->num_sms);
+}
+
+bse_status_t launch_real_pass(bse_handle_s *h, const char *tiles, int mode, const void *dX, int64_t ldx, void *dY,
+                              int64_t ldy, int32_t k)
+{
+    bse_status_t st = apply_kernel_attributes();
+    if (st) return st;
+    ApplyParams p;
+    int grid;
+    apply_unit_params(h, p, grid);
+    p.tiles = tiles;
+    p.pass = mode;
+    p.sign = 1.0;
+    p.ldx = ldx;
+    p.ldy = ldy;
+    for (int32_t c0 = 0; c0 < k; c0 += 8) {
+        p.kc = k - c0 < 8 ? k - c0 : 8;
+        p.X = reinterpret_cast<const double2 *>(dX) + (int64_t)c0 * ldx;
+        p.Y = reinterpret_cast<double *>(dY) + 2 * (int64_t)c0 * ldy;
+        if (mode == 0) apply_tiles_real_kernel<0><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+        else apply_tiles_real_kernel<1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+        count_launch();
+    }
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}
+
+bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, double sign, const void *dX,
+                               int64_t ldx, void *dY, int64_t ldy, int32_t k)
+{
+    bse_status_t st0 = apply_kernel_attributes();
+    if (st0) return st0;
+    bool use_k1 = true;                                // BSE_APPLY_K1=0: tensor-core kernel for single columns too
+    if (const char *e = getenv("BSE_APPLY_K1")) use_k1 = atoi(e) != 0;
+    ApplyParams p;
+    int grid;
+    apply_unit_params(h, p, grid);
+    p.tiles = tiles;
+    p.pass = pass;
+    p.sign = sign;
+    p.ldx = ldx;
+    p.ldy = ldy;
     bool use_wide = true;                              // BSE_APPLY_WIDE=0: 4-column passes only
     if (const char *e = getenv("BSE_APPLY_WIDE")) use_wide = atoi(e) != 0;
     bool use_3m = true;                                // BSE_APPLY_3M=0: four-product form for 5 .. 8 columns
@@ -149,7 +190,7 @@ static inline int storage_es(int32_t storage) { return storage == BSE_STORE_C64 
 
 bse_status_t bse_layout(int64_t N, int32_t storage, int32_t *tile, int64_t *n_tiles, int64_t *bytes_per_matrix)
 {
-    if (N < 1 || !storage_ok(storage)) return BSE_ERR_INVALID_ARG;
+    if (N < 1 || !(storage_ok(storage) || storage == BSE_STORE_REAL_FORM)) return BSE_ERR_INVALID_ARG;
     int64_t nt = (N + TB - 1) / TB;
     if (tile) *tile = TB;
     if (n_tiles) *n_tiles = nt * (nt + 1) / 2;
@@ -254,9 +295,11 @@ bse_status_t bse_fill_closed_form_full(void *dRTiles, void *dCTiles, int32_t sto
 bse_status_t bse_create(bse_handle_t *out, int32_t mode, int32_t storage, int64_t N, const void *dRTiles,
                         const void *dCTiles, void *stream)
 {
-    if (!out || !dRTiles || N < 1 || (mode != BSE_MODE_TDA && mode != BSE_MODE_FULL) || !storage_ok(storage))
+    const bool real_form = storage == BSE_STORE_REAL_FORM;
+    if (!out || !dRTiles || N < 1 || (mode != BSE_MODE_TDA && mode != BSE_MODE_FULL) || !(storage_ok(storage) || real_form))
         return BSE_ERR_INVALID_ARG;
     if (mode == BSE_MODE_FULL && !dCTiles) return BSE_ERR_INVALID_ARG;
+    if (real_form && mode != BSE_MODE_FULL) return BSE_ERR_INVALID_ARG;     // S = R + C, D = R - C need both matrices
     int dev = 0;
     BSE_CUDA(cudaGetDevice(&dev));
     int sms = 0;
@@ -267,11 +310,32 @@ bse_status_t bse_create(bse_handle_t *out, int32_t mode, int32_t storage, int64_
     h->N = N;
     h->nt = (int)((N + TB - 1) / TB);
     h->es = storage_es(storage);
+    h->real_form = real_form ? 1 : 0;
     h->R = (const char *)dRTiles;
     h->C = (mode == BSE_MODE_FULL) ? (const char *)dCTiles : nullptr;
     h->stream = (cudaStream_t)stream;
     h->num_sms = sms;
     *out = h;
+    return BSE_OK;
+}
+
+// (r, c) <- (r + c, r - c) on every stored double of the two tile stores
+__global__ void __launch_bounds__(256) to_real_form_kernel(double2 *__restrict__ r, double2 *__restrict__ c, int64_t n)
+{
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const double2 a = r[i], b = c[i];
+        r[i] = make_double2(a.x + b.x, a.y + b.y);
+        c[i] = make_double2(a.x - b.x, a.y - b.y);
+    }
+}
+
+bse_status_t bse_to_real_form(void *dRTiles, void *dCTiles, int64_t N, void *stream)
+{
+    if (!dRTiles || !dCTiles || N < 1) return BSE_ERR_INVALID_ARG;
+    const int64_t nt = (N + TB - 1) / TB, n = nt * (nt + 1) / 2 * TB * TB;
+    to_real_form_kernel<<<148 * 8, 256, 0, (cudaStream_t)stream>>>((double2 *)dRTiles, (double2 *)dCTiles, n);
+    count_launch();
+    BSE_CUDA(cudaGetLastError());
     return BSE_OK;
 }
 
@@ -291,6 +355,12 @@ bse_status_t bse_apply_half(bse_handle_t h, int32_t sign, const void *dX, int64_
     if (h->mode != BSE_MODE_FULL) return BSE_ERR_INVALID_ARG;
     bse_status_t st = zero_block(h, dY, ldy, h->N, k);
     if (st) return st;
+    if (h->real_form) {
+        // stores hold S = R + C (h->R) and D = R - C (h->C):  P = mode 0 over S + mode 1 over D,  M = mode 0 over D + mode 1 over S
+        const char *first = sign > 0 ? h->R : h->C, *second = sign > 0 ? h->C : h->R;
+        if ((st = launch_real_pass(h, first, 0, dX, ldx, dY, ldy, k))) return st;
+        return launch_real_pass(h, second, 1, dX, ldx, dY, ldy, k);
+    }
     st = launch_apply_pass(h, h->R, PASS_HERM, 1.0, dX, ldx, dY, ldy, k);
     if (st) return st;
     return launch_apply_pass(h, h->C, PASS_SYMC, (double)sign, dX, ldx, dY, ldy, k);

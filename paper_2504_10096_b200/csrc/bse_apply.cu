@@ -26,6 +26,31 @@ __global__ void neg_conj_inplace_kernel(double2 *__restrict__ y, int64_t ldy, in
     }
 }
 
+// u = (x1 + conj x2) / 2,  v = (x1 - conj x2) / 2
+__global__ void split_uv_kernel(const double2 *__restrict__ x1, const double2 *__restrict__ x2, int64_t ldx,
+                                double2 *__restrict__ u, double2 *__restrict__ v, int64_t n, int k)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    int c = blockIdx.y;
+    if (i < n && c < k) {
+        double2 a = x1[i + c * ldx], b = x2[i + c * ldx];
+        u[i + c * n] = make_double2(0.5 * (a.x + b.x), 0.5 * (a.y - b.y));
+        v[i + c * n] = make_double2(0.5 * (a.x - b.x), 0.5 * (a.y + b.y));
+    }
+}
+// y1 = pu + mv,  y2 = -conj(pu - mv)
+__global__ void combine_uv_kernel(const double2 *__restrict__ pu, const double2 *__restrict__ mv, double2 *__restrict__ y1,
+                                  double2 *__restrict__ y2, int64_t ldy, int64_t n, int k)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    int c = blockIdx.y;
+    if (i < n && c < k) {
+        double2 a = pu[i + c * n], b = mv[i + c * n];
+        y1[i + c * ldy] = make_double2(a.x + b.x, a.y + b.y);
+        y2[i + c * ldy] = make_double2(-(a.x - b.x), a.y - b.y);
+    }
+}
+
 }  // namespace bse
 
 using namespace bse;
@@ -44,10 +69,26 @@ bse_status_t bse_apply(bse_handle_t h, const void *dX, int64_t ldx, void *dY, in
     }
     // FULL:  Y1 = R X1 + C X2 ;  Y2 = -conj( R conj(X2) + C conj(X1) )     (Eq. 1 with A = R^*, C = C^T)
     if (ldx < 2 * N || ldy < 2 * N) return BSE_ERR_INVALID_ARG;
-    bse_status_t st = ensure_ws(h, (size_t)N * k * 16);
-    if (st) return st;
     const double2 *X1 = (const double2 *)dX, *X2 = X1 + N;
     double2 *Y1 = (double2 *)dY, *Y2 = Y1 + N;
+    if (h->real_form) {
+        // real-form store (S = R + C, D = R - C): with U = (X1 + conj X2)/2, V = (X1 - conj X2)/2,
+        //   Y1 = R X1 + C X2 = P(U) + M(V),   Y2 = -conj(R conj X2 + C conj X1) = -conj(P(U) - M(V))
+        bse_status_t st = ensure_ws(h, (size_t)4 * N * k * 16);
+        if (st) return st;
+        double2 *U = (double2 *)h->ws, *V = U + (size_t)N * k, *PU = V + (size_t)N * k, *MV = PU + (size_t)N * k;
+        dim3 grid((unsigned)((N + 255) / 256), (unsigned)k);
+        split_uv_kernel<<<grid, 256, 0, h->stream>>>(X1, X2, ldx, U, V, N, k);
+        count_launch();
+        if ((st = bse_apply_half(h, +1, U, N, PU, N, k))) return st;
+        if ((st = bse_apply_half(h, -1, V, N, MV, N, k))) return st;
+        combine_uv_kernel<<<grid, 256, 0, h->stream>>>(PU, MV, Y1, Y2, ldy, N, k);
+        count_launch();
+        BSE_CUDA(cudaGetLastError());
+        return BSE_OK;
+    }
+    bse_status_t st = ensure_ws(h, (size_t)N * k * 16);
+    if (st) return st;
     double2 *T1 = (double2 *)h->ws;   // conj(X2), N x k, ld N
     dim3 grid((unsigned)((N + 255) / 256), (unsigned)k);
     conj_copy_kernel<<<grid, 256, 0, h->stream>>>(X2, ldx, T1, N, N, k);

@@ -13,6 +13,7 @@ struct bse_handle_s {
     int64_t N;
     int nt;
     int es;              // bytes per stored complex entry: 16 (BSE_STORE_C128) or 8 (BSE_STORE_C64)
+    int real_form;       // BSE_STORE_REAL_FORM: R holds S = R + C, C holds D = R - C (full mode only, complex128)
     const char *R;
     const char *C;
     cudaStream_t stream;
@@ -51,6 +52,9 @@ bse_status_t ensure_pin(bse_handle_s *h, size_t bytes);
 // One pass over one matrix: Y += sign * (R X)  or  Y += sign * (C conj X), k columns (chunked by 4).
 bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, double sign, const void *dX,
                                int64_t ldx, void *dY, int64_t ldy, int32_t k);
+// One pass of the real-form half apply (apply_kernel_real.cuh): mode 0 / 1 over one store, k columns (chunked by 8).
+bse_status_t launch_real_pass(bse_handle_s *h, const char *tiles, int mode, const void *dX, int64_t ldx, void *dY,
+                              int64_t ldy, int32_t k);
 bse_status_t zero_block(bse_handle_s *h, void *dY, int64_t ldy, int64_t rows, int32_t k);
 
 

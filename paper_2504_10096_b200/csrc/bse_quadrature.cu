@@ -71,10 +71,7 @@ static bse_status_t lanczos_quadrature_full(bse_handle_s *h, const void *dStart,
     BSE_CUDA(cudaMemsetAsync(d_alpha, 0, scal, h->stream));
     const int grid = h->num_sms * 2;
     auto half = [&](int sign, const double2 *x, double2 *y) -> bse_status_t {
-        bse_status_t s2 = zero_block(h, y, n, n, 1);
-        if (s2) return s2;
-        if ((s2 = launch_apply_pass(h, h->R, 0, 1.0, x, n, y, n, 1))) return s2;
-        return launch_apply_pass(h, h->C, 1, (double)sign, x, n, y, n, 1);
+        return bse_apply_half(h, sign, x, n, y, n, 1);
     };
     // beta_0^2 = Re(d^H P(d));  x_1 = d / beta_0,  p_1 = P(d) / beta_0
     if ((st = half(+1, (const double2 *)dStart, pb[1]))) return st;
