@@ -300,8 +300,9 @@ def run_cuda(args, cfg):
         # k = 1, each streaming R and C once (4 tile passes of 8.59 GB)
         c3 = gen.CONFIGS[3]
         N3 = c3["N"]
-        h3 = b.Bse(b.MODE_FULL, N3, b.bse_fill_synthetic(N3, b.MATRIX_R, 1, 1.0, c3["group"]),
-                   b.bse_fill_synthetic(N3, b.MATRIX_C, 1, 0.0, c3["group"]))
+        r3 = b.bse_fill_synthetic(N3, b.MATRIX_R, 1, 1.0, c3["group"])
+        c3t = b.bse_fill_synthetic(N3, b.MATRIX_C, 1, 0.0, c3["group"])
+        h3 = b.Bse(b.MODE_FULL, N3, r3, c3t)
         d3 = Xh[0][:N3].contiguous().cuda()
         h3.lanczos_quadrature(d3, 3)
         torch.cuda.synchronize()
@@ -311,6 +312,28 @@ def run_cuda(args, cfg):
         line["lanczos_quadrature_full"] = {"workload": f"config 3 operator: full N={N3}, sigma=1", "steps": qsteps,
                                            "ms_per_step": qsec * 1e3 / qsteps,
                                            "GBps": 4 * alg_bytes(N3, 1) * qsteps / qsec / 1e9}
+
+        # full-mode half apply P(X) = R X + C conj(X) vs k: complex store (R and C passes) and the
+        # real-form store of Eq. (3) (S = R + C, D = R - C; apply_kernel_real.cuh).  Bytes: both stores once + X, Y.
+        def half_sweep(hh):
+            out = {}
+            for kk in (1, 4, 8):
+                Xs = Xh[:kk, :N3].contiguous().cuda()
+                Ys = torch.empty_like(Xs)
+                m = time_steps(lambda: hh.apply_half(Xs, 1, Ys), max(3, args.steps // 2), 2)
+                by = 2 * 16.0 * N3 * (N3 + 1) / 2 + 32.0 * N3 * kk
+                out[str(kk)] = {"ms": m, "GBps": by / (m * 1e-3) / 1e9}
+            return out
+        line["half_apply_vs_k_config3"] = half_sweep(h3)
+        del h3
+        b.bse_to_real_form(r3, c3t, N3)
+        h3 = b.Bse(b.MODE_FULL, N3, r3, c3t, storage=b.STORE_REAL_FORM)
+        line["half_apply_vs_k_config3_real_form"] = half_sweep(h3)
+        t0 = time.perf_counter()
+        res = h3.solve(c3["nev"], 8, tol=1e-8, seed=1, raise_on_error=False)
+        line["lanczos_time_to_nev_config3"] = {
+            "workload": f"config 3: full N={N3} nev={c3['nev']} k=8 tol=1e-8, real-form store", "seconds": time.perf_counter() - t0,
+            "status": res.status, "info": res.info}
         del h3
 
     # ---- CPU baseline: the oracle on this box's host cores, bounded sample
