@@ -46,6 +46,10 @@
  * written by bse_to_real_form from stores of R and C.  The half applies then run in real arithmetic,
  * P(x): re = Sr a - Di b, im = Si a + Dr b;  M(x): re = Dr a - Si b, im = Di a + Sr b  (x = a + i b),
  * with half the flops of the complex form; every result is the same operator's to rounding.
+ * BSE_STORE_REAL_FORM_C64: the same with binary32 planes, written by bse_to_real_form from BSE_STORE_C64 stores:
+ * S32 = fl32(R32 + C32), D32 = fl32(R32 - C32) (exact sum, one rounding to nearest-even).  The operator every later
+ * call works with is then R' = (S32 + D32)/2, C' = (S32 - D32)/2 (exact in FP64) -- within one binary32 ulp of the
+ * single-precision R32, C32, i.e. inside the precision of the data; arithmetic stays FP64.
  */
 #ifndef BSE_B200_H
 #define BSE_B200_H
@@ -70,7 +74,7 @@ typedef enum {
 
 enum { BSE_MODE_TDA = 0, BSE_MODE_FULL = 1 };
 enum { BSE_MATRIX_R = 0, BSE_MATRIX_C = 1 };
-enum { BSE_STORE_C128 = 0, BSE_STORE_C64 = 1, BSE_STORE_REAL_FORM = 2 };
+enum { BSE_STORE_C128 = 0, BSE_STORE_C64 = 1, BSE_STORE_REAL_FORM = 2, BSE_STORE_REAL_FORM_C64 = 3 };
 
 typedef struct {
     int32_t n_apply;        /* operator applications (block applies; a full-mode step counts 2 half applies) */
@@ -131,10 +135,11 @@ bse_status_t bse_create(bse_handle_t *h, int32_t mode, int32_t storage, int64_t 
                         const void *dCTiles, void *stream);
 bse_status_t bse_destroy(bse_handle_t h);
 
-/* In place, on two BSE_STORE_C128 stores of the same N:  dRTiles <- S = R + C,  dCTiles <- D = R - C (every stored
- * entry, mirrored halves and padding included).  Afterwards pass both to bse_create with BSE_STORE_REAL_FORM (mode
+/* In place, on two stores of the same N and `storage` (BSE_STORE_C128 or BSE_STORE_C64):  dRTiles <- S = R + C,
+ * dCTiles <- D = R - C (every stored entry, mirrored halves and padding included; binary32 planes are summed exactly
+ * and rounded once).  Afterwards pass both to bse_create with BSE_STORE_REAL_FORM / BSE_STORE_REAL_FORM_C64 (mode
  * FULL); they no longer represent R and C for any other call.  Asynchronous on `stream`. */
-bse_status_t bse_to_real_form(void *dRTiles, void *dCTiles, int64_t N, void *stream);
+bse_status_t bse_to_real_form(void *dRTiles, void *dCTiles, int32_t storage, int64_t N, void *stream);
 
 /* Y = H X for a block of k >= 1 vectors.
  *   TDA : X, Y are N x k;   Y = R X.

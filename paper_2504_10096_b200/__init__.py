@@ -15,7 +15,7 @@ _LIBPATH = os.path.join(_HERE, "libbse_b200.so")
 _lib = None
 
 MODE_TDA, MODE_FULL = 0, 1
-STORE_C128, STORE_C64, STORE_REAL_FORM = 0, 1, 2      # storage type of the tile store (include/bse.h)
+STORE_C128, STORE_C64, STORE_REAL_FORM, STORE_REAL_FORM_C64 = 0, 1, 2, 3      # storage type of the tile store (include/bse.h)
 MATRIX_R, MATRIX_C = 0, 1
 TILE = 64
 TILE_BYTES = 65536
@@ -48,7 +48,7 @@ _SIGNATURES = {
     "bse_fill_closed_form_full": [_vp, _vp, _i32, _i64, _vp, _vp, _vp, _vp, _dbl, _dbl, _vp],
     "bse_create": [ctypes.POINTER(_vp), _i32, _i32, _i64, _vp, _vp, _vp],
     "bse_destroy": [_vp],
-    "bse_to_real_form": [_vp, _vp, _i64, _vp],
+    "bse_to_real_form": [_vp, _vp, _i32, _i64, _vp],
     "bse_apply": [_vp, _vp, _i64, _vp, _i64, _i32],
     "bse_apply_half": [_vp, _i32, _vp, _i64, _vp, _i64, _i32],
     "bse_apply_host": [_vp, _vp, _i64, _vp, _i64, _i32],
@@ -165,9 +165,9 @@ class SolveResult:
     status: int
 
 
-def bse_to_real_form(r_tiles, c_tiles, N: int):
-    """In place: (R, C) complex128 stores -> (S = R + C, D = R - C); use with Bse(..., storage=STORE_REAL_FORM)."""
-    _check(lib().bse_to_real_form(r_tiles.data_ptr(), c_tiles.data_ptr(), N, _stream_ptr()), "bse_to_real_form")
+def bse_to_real_form(r_tiles, c_tiles, N: int, storage: int = STORE_C128):
+    """In place: (R, C) stores -> (S = R + C, D = R - C); use with Bse(..., storage=STORE_REAL_FORM[_C64])."""
+    _check(lib().bse_to_real_form(r_tiles.data_ptr(), c_tiles.data_ptr(), storage, N, _stream_ptr()), "bse_to_real_form")
     return r_tiles, c_tiles
 
 

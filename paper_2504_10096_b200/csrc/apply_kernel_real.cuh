@@ -20,10 +20,10 @@
 
 namespace bse {
 
-template <int MODE>
+// ES = 16: complex128 planes; ES = 8: binary32 planes widened to FP64 when a fragment is loaded (6-stage ring).
+template <int ES, int MODE>
 __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_real_kernel(const ApplyParams p)
 {
-    constexpr int ES = 16;
     constexpr int TBY = TB * TB * ES;
     constexpr int PBY = 64 * ES;
     constexpr int NST = APPLY_STAGES * 16 / ES;

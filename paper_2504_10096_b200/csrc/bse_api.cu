@@ -63,8 +63,10 @@ static bse_status_t apply_kernel_attributes()
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<16, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<8, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_kernel<16, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_kernel<16, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_kernel<8, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_kernel<8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_3m_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_3m_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_k1_kernel<16, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
@@ -106,8 +108,13 @@ bse_status_t launch_real_pass(bse_handle_s *h, const char *tiles, int mode, cons
         p.kc = k - c0 < 8 ? k - c0 : 8;
         p.X = reinterpret_cast<const double2 *>(dX) + (int64_t)c0 * ldx;
         p.Y = reinterpret_cast<double *>(dY) + 2 * (int64_t)c0 * ldy;
-        if (mode == 0) apply_tiles_real_kernel<0><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-        else apply_tiles_real_kernel<1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+        if (h->es == ES_C128) {
+            if (mode == 0) apply_tiles_real_kernel<16, 0><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            else apply_tiles_real_kernel<16, 1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+        } else {
+            if (mode == 0) apply_tiles_real_kernel<8, 0><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            else apply_tiles_real_kernel<8, 1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+        }
         count_launch();
     }
     BSE_CUDA(cudaGetLastError());
@@ -186,11 +193,15 @@ bse_status_t bse_host_heev(int32_t m, void *hA, int32_t lda, double *hW, void *h
 }
 
 static inline bool storage_ok(int32_t storage) { return storage == BSE_STORE_C128 || storage == BSE_STORE_C64; }
-static inline int storage_es(int32_t storage) { return storage == BSE_STORE_C64 ? ES_C64 : ES_C128; }
+static inline bool storage_real_form(int32_t storage) { return storage == BSE_STORE_REAL_FORM || storage == BSE_STORE_REAL_FORM_C64; }
+static inline int storage_es(int32_t storage)
+{
+    return (storage == BSE_STORE_C64 || storage == BSE_STORE_REAL_FORM_C64) ? ES_C64 : ES_C128;
+}
 
 bse_status_t bse_layout(int64_t N, int32_t storage, int32_t *tile, int64_t *n_tiles, int64_t *bytes_per_matrix)
 {
-    if (N < 1 || !(storage_ok(storage) || storage == BSE_STORE_REAL_FORM)) return BSE_ERR_INVALID_ARG;
+    if (N < 1 || !(storage_ok(storage) || storage_real_form(storage))) return BSE_ERR_INVALID_ARG;
     int64_t nt = (N + TB - 1) / TB;
     if (tile) *tile = TB;
     if (n_tiles) *n_tiles = nt * (nt + 1) / 2;
@@ -295,7 +306,7 @@ bse_status_t bse_fill_closed_form_full(void *dRTiles, void *dCTiles, int32_t sto
 bse_status_t bse_create(bse_handle_t *out, int32_t mode, int32_t storage, int64_t N, const void *dRTiles,
                         const void *dCTiles, void *stream)
 {
-    const bool real_form = storage == BSE_STORE_REAL_FORM;
+    const bool real_form = storage_real_form(storage);
     if (!out || !dRTiles || N < 1 || (mode != BSE_MODE_TDA && mode != BSE_MODE_FULL) || !(storage_ok(storage) || real_form))
         return BSE_ERR_INVALID_ARG;
     if (mode == BSE_MODE_FULL && !dCTiles) return BSE_ERR_INVALID_ARG;
@@ -329,11 +340,24 @@ __global__ void __launch_bounds__(256) to_real_form_kernel(double2 *__restrict__
     }
 }
 
-bse_status_t bse_to_real_form(void *dRTiles, void *dCTiles, int64_t N, void *stream)
+// the same on binary32 planes: the sum and difference are formed exactly in FP64 and rounded to nearest-even once
+__global__ void __launch_bounds__(256) to_real_form_c64_kernel(float2 *__restrict__ r, float2 *__restrict__ c, int64_t n)
 {
-    if (!dRTiles || !dCTiles || N < 1) return BSE_ERR_INVALID_ARG;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const float2 a = r[i], b = c[i];
+        r[i] = make_float2(__double2float_rn((double)a.x + (double)b.x), __double2float_rn((double)a.y + (double)b.y));
+        c[i] = make_float2(__double2float_rn((double)a.x - (double)b.x), __double2float_rn((double)a.y - (double)b.y));
+    }
+}
+
+bse_status_t bse_to_real_form(void *dRTiles, void *dCTiles, int32_t storage, int64_t N, void *stream)
+{
+    if (!dRTiles || !dCTiles || N < 1 || !storage_ok(storage)) return BSE_ERR_INVALID_ARG;
     const int64_t nt = (N + TB - 1) / TB, n = nt * (nt + 1) / 2 * TB * TB;
-    to_real_form_kernel<<<148 * 8, 256, 0, (cudaStream_t)stream>>>((double2 *)dRTiles, (double2 *)dCTiles, n);
+    if (storage == BSE_STORE_C64)
+        to_real_form_c64_kernel<<<148 * 8, 256, 0, (cudaStream_t)stream>>>((float2 *)dRTiles, (float2 *)dCTiles, n);
+    else
+        to_real_form_kernel<<<148 * 8, 256, 0, (cudaStream_t)stream>>>((double2 *)dRTiles, (double2 *)dCTiles, n);
     count_launch();
     BSE_CUDA(cudaGetLastError());
     return BSE_OK;

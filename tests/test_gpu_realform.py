@@ -125,3 +125,78 @@ def test_real_form_is_full_mode_only():
     with pytest.raises(b.BseError):
         b.Bse(b.MODE_TDA, N, pack(R, 0), storage=b.STORE_REAL_FORM)
     assert b.bse_layout(N, b.STORE_REAL_FORM) == b.bse_layout(N, b.STORE_C128)
+    assert b.bse_layout(N, b.STORE_REAL_FORM_C64) == b.bse_layout(N, b.STORE_C64)
+
+
+# ---- binary32 planes (BSE_STORE_REAL_FORM_C64): the operator is R' = (S32 + D32)/2, C' = (S32 - D32)/2 with
+# ---- S32 = fl32(fl32(R) + fl32(C)), D32 = fl32(fl32(R) - fl32(C))  (include/bse.h) -- built here from oracle.round_c64
+
+def _handle64(R, C):
+    import paper_2504_10096_b200 as b
+    N = R.shape[0]
+    rt = b.bse_pack_from_dense(to_dev(R), N, 0, storage=b.STORE_C64)
+    ct = b.bse_pack_from_dense(to_dev(C), N, 1, storage=b.STORE_C64)
+    b.bse_to_real_form(rt, ct, N, storage=b.STORE_C64)
+    return b.Bse(b.MODE_FULL, N, rt, ct, storage=b.STORE_REAL_FORM_C64)
+
+
+def _operator64(orc, R, C):
+    R32, C32 = orc.round_c64(R), orc.round_c64(C)
+    S32, D32 = orc.round_c64(R32 + C32), orc.round_c64(R32 - C32)      # the FP64 sum of two binary32 values is exact
+    return (S32 + D32) / 2, (S32 - D32) / 2, R32, C32
+
+
+@pytest.mark.parametrize("N", [64, 200, 448])
+@pytest.mark.parametrize("k", [1, 4, 8, 11])
+def test_c64_planes_half_apply_matches_oracle(orc, N, k):
+    R, C = _pair(N, 31)
+    Rp, Cp, R32, C32 = _operator64(orc, R, C)
+    h = _handle64(R, C)
+    x = gen.block_X(N, k, 24)
+    for sign in (+1, -1):
+        Y = to_host(h.apply_half(to_dev(x), sign))
+        assert relerr(Y, orc.apply_half(Rp, Cp, x, sign)) <= TOL_APPLY
+        e = relerr(Y, orc.apply_half(R32, C32, x, sign))
+        assert 1e-11 < e < 1e-6            # one binary32 ulp per entry away from the rounded (R, C), not equal to it
+    X = gen.block_X(2 * N, min(k, 5), 25)
+    assert relerr(to_host(h.apply(to_dev(X))), orc.apply_full(Rp, Cp, X)) <= TOL_APPLY
+
+
+def test_c64_planes_many_units_and_solve(orc):
+    from test_gpu_solve import _check_full
+    N, nev, k = 192, 8, 8
+    R = gen.dense_R(N, 2, sigma=1.0); C = gen.dense_C(N, 2)
+    Rp, Cp, _, _ = _operator64(orc, R, C)
+    res = _handle64(R, C).solve(nev, k, tol=1e-9, seed=1)
+    omd, _ = orc.bse_direct(Rp, Cp, want_vectors=False)
+    _check_full(orc, Rp, Cp, res, nev, omd[N:])
+    # many units per CTA: N = 4096, dense host matrices (134 MB each) packed through the binary32 store
+    N = 4096
+    R = gen.dense_R(N, 3, sigma=1.0); C = gen.dense_C(N, 3)
+    Rp, Cp, _, _ = _operator64(orc, R, C)
+    h = _handle64(R, C)
+    X = gen.block_X(N, 8, 5)
+    rows = np.unique(np.concatenate([np.arange(0, N, 397), [63, 64, N - 65, N - 1]]))
+    for sign in (+1, -1):
+        ref = orc.rows_times_block(Rp[rows], X) + sign * orc.rows_times_block(Cp[rows], X.conj())
+        for _ in range(4):
+            assert relerr(to_host(h.apply_half(to_dev(X), sign))[rows], ref) <= TOL_APPLY
+
+
+def test_config1_vs_oracle_golden_with_the_real_form_store(orc):
+    """BASELINE.json config 1 (full N = 2048, nev = 20, k = 4) through the real-form store: same stored oracle values,
+    residuals and Sigma-orthonormality as test_gpu_solve.test_config1_full_vs_oracle_golden."""
+    import os
+    from test_gpu_solve import _check_full, _golden
+    if not os.path.exists(os.path.join(os.path.dirname(__file__), "golden", "oracle_config1.txt")):
+        pytest.skip("tests/golden/oracle_config1.txt not generated yet")
+    cfg = gen.CONFIGS[1]
+    N, nev, k = cfg["N"], cfg["nev"], cfg["k"]
+    R = gen.dense_R(N, 1, sigma=cfg["sigma"]); C = gen.dense_C(N, 1)
+    res = _handle(R, C).solve(nev, k, tol=1e-8, seed=1)
+    gold = _golden("oracle_config1.txt")
+    distinct = [gold[0]]
+    for x in gold[1:]:
+        if x - distinct[-1] > 1e-7 * x:
+            distinct.append(x)
+    _check_full(orc, R, C, res, nev, np.array(distinct))
