@@ -273,6 +273,14 @@ def run_cuda(args, cfg):
         qsec = time.perf_counter() - t0
         line["lanczos_quadrature"] = {"steps": qsteps, "ms_per_step": qsec * 1e3 / qsteps,
                                       "GBps": alg_bytes(N, 1) * qsteps / qsec / 1e9}
+        # Lanczos time-to-nev on the timed operand itself (BASELINE.json config 4: nev = 500, block k = 8, tol 1e-8)
+        if cfg.get("id") == 4:
+            t0 = time.perf_counter()
+            res4 = h.solve(cfg["nev"], cfg["k"], tol=1e-8, seed=1, raise_on_error=False)
+            line["lanczos_time_to_nev_config4"] = {
+                "workload": f"config 4: TDA N={N} nev={cfg['nev']} k={cfg['k']} tol=1e-8", "seconds": time.perf_counter() - t0,
+                "status": res4.status, "info": res4.info}
+            del res4
         del h, tiles
         torch.cuda.empty_cache()
         # complex64-stored operand: same N, half the stored bytes, FP64 arithmetic.
@@ -290,6 +298,16 @@ def run_cuda(args, cfg):
         torch.cuda.empty_cache()
         c2 = gen.CONFIGS[2]
         h2 = b.Bse(b.MODE_TDA, c2["N"], b.bse_fill_synthetic(c2["N"], b.MATRIX_R, 1, 0.0, c2["group"]))
+        # BASELINE.json config 2's k sweep (k > 8 is processed in groups of 8 columns, one pass over the operand each)
+        sweep2 = {}
+        X2 = torch.randn(64, c2["N"], dtype=torch.complex128, device="cuda")
+        for kk in (1, 2, 4, 8, 16, 32, 64):
+            Xs, Ys = X2[:kk], torch.empty((kk, c2["N"]), dtype=torch.complex128, device="cuda")
+            m = time_steps(lambda: h2.apply(Xs, Ys), max(3, args.steps // 2), 2)
+            sweep2[str(kk)] = {"ms": m, "GBps": alg_bytes(c2["N"], kk) / (m * 1e-3) / 1e9,
+                               "tflops": 8.0 * c2["N"] ** 2 * kk / (m * 1e-3) / 1e12}
+        line["apply_vs_k_config2"] = sweep2
+        del X2
         t0 = time.perf_counter()
         res = h2.solve(c2["nev"], c2["k"], tol=1e-8, seed=1, raise_on_error=False)
         line["lanczos_time_to_nev"] = {"workload": f"config 2: TDA N={c2['N']} nev={c2['nev']} k={c2['k']} tol=1e-8",
