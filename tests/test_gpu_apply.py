@@ -214,15 +214,16 @@ def test_config4_full_size_sampled_rows(orc):
 def test_config3_full_size_half_apply_sampled_rows(orc):
     """BASELINE.json config 3 (full mode, N = 32768, R and C 8.6 GB each, filled on the device): sampled rows of
     P(X) = R X + C conj(X) and M(X) = R X - C conj(X) -- the two products bse_solve issues per block step -- for the
-    four-product (k = 4) and three-product (k = 8) kernels, against the oracle on rows from the CPU generator."""
+    four-product (k = 4) and three-product (k = 8) kernels and for the real-form kernel, against the oracle on rows from
+    the CPU generator."""
     import torch
     import paper_2504_10096_b200 as b
     cfg = gen.CONFIGS[3]
     N = cfg["N"]
     if torch.cuda.mem_get_info()[0] < 30e9:
         pytest.skip("needs 30 GB of free device memory")
-    h = b.Bse(b.MODE_FULL, N, b.bse_fill_synthetic(N, 0, 1, cfg["sigma"], cfg["group"]),
-              b.bse_fill_synthetic(N, 1, 1, 0.0, cfg["group"]))
+    rt, ct = b.bse_fill_synthetic(N, 0, 1, cfg["sigma"], cfg["group"]), b.bse_fill_synthetic(N, 1, 1, 0.0, cfg["group"])
+    h = b.Bse(b.MODE_FULL, N, rt, ct)
     X = gen.block_X(N, 8, 14)
     rows = np.unique(np.concatenate([(np.arange(24) * 2654435761 % N), [0, 63, 64, N - 64, N - 1]]).astype(np.int64))
     RX = orc.rows_times_block(gen.rows_R(N, 1, rows, cfg["sigma"], cfg["group"]), X)
@@ -231,6 +232,14 @@ def test_config3_full_size_half_apply_sampled_rows(orc):
         for sign in (+1, -1):
             Y = to_host(h.apply_half(to_dev(X[:, :k]), sign))
             assert relerr(Y[rows], (RX + sign * CX)[:, :k]) <= TOL_APPLY, (k, sign)
+    # the same stores rewritten as S = R + C, D = R - C (real form of Eq. 3): same operator
+    del h
+    b.bse_to_real_form(rt, ct, N)
+    hr = b.Bse(b.MODE_FULL, N, rt, ct, storage=b.STORE_REAL_FORM)
+    for k in (4, 8):
+        for sign in (+1, -1):
+            Y = to_host(hr.apply_half(to_dev(X[:, :k]), sign))
+            assert relerr(Y[rows], (RX + sign * CX)[:, :k]) <= TOL_APPLY, ("real form", k, sign)
 
 
 @pytest.mark.parametrize("N", [1, 2, 63, 65, 127])
