@@ -321,7 +321,8 @@ def run_cuda(args, cfg):
         r3 = b.bse_fill_synthetic(N3, b.MATRIX_R, 1, 1.0, c3["group"])
         c3t = b.bse_fill_synthetic(N3, b.MATRIX_C, 1, 0.0, c3["group"])
         h3 = b.Bse(b.MODE_FULL, N3, r3, c3t)
-        d3 = Xh[0][:N3].contiguous().cuda()
+        X3 = torch.randn(8, N3, dtype=torch.complex128, device="cuda")
+        d3 = X3[0].contiguous()
         h3.lanczos_quadrature(d3, 3)
         torch.cuda.synchronize()
         t0 = time.perf_counter()
@@ -336,7 +337,7 @@ def run_cuda(args, cfg):
         def half_sweep(hh):
             out = {}
             for kk in (1, 4, 8):
-                Xs = Xh[:kk, :N3].contiguous().cuda()
+                Xs = X3[:kk].contiguous()
                 Ys = torch.empty_like(Xs)
                 m = time_steps(lambda: hh.apply_half(Xs, 1, Ys), max(3, args.steps // 2), 2)
                 by = 2 * 16.0 * N3 * (N3 + 1) / 2 + 32.0 * N3 * kk
