@@ -135,11 +135,36 @@ bse_status_t bse_create(bse_handle_t *h, int32_t mode, int32_t storage, int64_t 
                         const void *dCTiles, void *stream);
 bse_status_t bse_destroy(bse_handle_t h);
 
-/* In place, on two stores of the same N and `storage` (BSE_STORE_C128 or BSE_STORE_C64):  dRTiles <- S = R + C,
+/* In place, on two stores (or two slices of stores, see bse_shard_layout) of n_tiles tiles each and the same
+ * `storage` (BSE_STORE_C128 or BSE_STORE_C64):  dRTiles <- S = R + C,
  * dCTiles <- D = R - C (every stored entry, mirrored halves and padding included; binary32 planes are summed exactly
  * and rounded once).  Afterwards pass both to bse_create with BSE_STORE_REAL_FORM / BSE_STORE_REAL_FORM_C64 (mode
  * FULL); they no longer represent R and C for any other call.  Asynchronous on `stream`. */
-bse_status_t bse_to_real_form(void *dRTiles, void *dCTiles, int32_t storage, int64_t N, void *stream);
+bse_status_t bse_to_real_form(void *dRTiles, void *dCTiles, int32_t storage, int64_t n_tiles, void *stream);
+
+/* ---- Sharding of the tile stream (the paper partitions matrices by rows). ----
+ * The packed store is ordered by tile row, so a range of tile rows [tile_row_begin, tile_row_end) is one contiguous
+ * slice of it.  bse_shard_layout splits the nt tile rows into n_shards ranges of (nearly) equal TILE COUNT
+ * (boundary r = the smallest I with I (I+1)/2 >= r * total / n_shards) and reports, for `shard`, the range, the number
+ * of its first tile in the whole store, its tile count and its size in bytes.  Output pointers may be NULL. */
+bse_status_t bse_shard_layout(int64_t N, int32_t storage, int32_t n_shards, int32_t shard, int32_t *tile_row_begin,
+                              int32_t *tile_row_end, int64_t *first_tile, int64_t *n_tiles, int64_t *bytes);
+
+/* bse_fill_synthetic for one slice: dTiles points at the slice (tile row tile_row_begin, column 0 first). */
+bse_status_t bse_fill_synthetic_shard(void *dTiles, int32_t storage, int64_t N, int32_t which, uint64_t seed,
+                                      double sigma, int32_t group, int32_t tile_row_begin, int32_t tile_row_end,
+                                      void *stream);
+
+/* A handle over ONE slice: dRSlice (and dCSlice) hold only the tiles of tile rows [tile_row_begin, tile_row_end).
+ * bse_apply and bse_apply_half on such a handle compute this slice's CONTRIBUTION to Y -- rows of the slice's tile rows
+ * from T X (P1) and rows of all tile columns J <= I from T^H X (P2) -- over the full length N: the sum over the
+ * shards of a partition is Y = H X.  X must be the whole block on every shard (16 N k bytes); the partial Y are
+ * summed by the caller (one all-reduce of 16 N k bytes per apply over NVLink when shards live on different GPUs:
+ * paper_2504_10096_b200.ShardedBse).  bse_solve, bse_orth and bse_lanczos_quadrature need the whole operator and
+ * return BSE_ERR_INVALID_ARG on a partial handle.  The general FULL-mode bse_apply is real-linear in the stores as
+ * well (its elementwise pre/post steps commute with the sum), for every storage type. */
+bse_status_t bse_create_shard(bse_handle_t *h, int32_t mode, int32_t storage, int64_t N, int32_t tile_row_begin,
+                              int32_t tile_row_end, const void *dRSlice, const void *dCSlice, void *stream);
 
 /* Y = H X for a block of k >= 1 vectors.
  *   TDA : X, Y are N x k;   Y = R X.

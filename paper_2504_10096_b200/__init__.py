@@ -49,6 +49,10 @@ _SIGNATURES = {
     "bse_create": [ctypes.POINTER(_vp), _i32, _i32, _i64, _vp, _vp, _vp],
     "bse_destroy": [_vp],
     "bse_to_real_form": [_vp, _vp, _i32, _i64, _vp],
+    "bse_shard_layout": [_i64, _i32, _i32, _i32, ctypes.POINTER(_i32), ctypes.POINTER(_i32), ctypes.POINTER(_i64),
+                         ctypes.POINTER(_i64), ctypes.POINTER(_i64)],
+    "bse_fill_synthetic_shard": [_vp, _i32, _i64, _i32, _u64, _dbl, _i32, _i32, _i32, _vp],
+    "bse_create_shard": [ctypes.POINTER(_vp), _i32, _i32, _i64, _i32, _i32, _vp, _vp, _vp],
     "bse_apply": [_vp, _vp, _i64, _vp, _i64, _i32],
     "bse_apply_half": [_vp, _i32, _vp, _i64, _vp, _i64, _i32],
     "bse_apply_host": [_vp, _vp, _i64, _vp, _i64, _i32],
@@ -165,22 +169,49 @@ class SolveResult:
     status: int
 
 
+def bse_shard_layout(N: int, n_shards: int, shard: int, storage: int = STORE_C128):
+    """(tile_row_begin, tile_row_end, first_tile, n_tiles, bytes) of one of n_shards slices of the packed store with
+    (nearly) equal tile counts.  Host-only: needs no device."""
+    rb, re, ft, nt, by = _i32(), _i32(), _i64(), _i64(), _i64()
+    _check(lib().bse_shard_layout(N, storage, n_shards, shard, ctypes.byref(rb), ctypes.byref(re), ctypes.byref(ft),
+                                  ctypes.byref(nt), ctypes.byref(by)), "bse_shard_layout")
+    return rb.value, re.value, ft.value, nt.value, by.value
+
+
+def bse_fill_synthetic_shard(N: int, which: int, seed: int, sigma: float, group: int, rows, storage: int = STORE_C128):
+    """The slice of bse_fill_synthetic's store holding tile rows rows = (begin, end) (torch uint8 tensor)."""
+    import torch
+    by = bse_layout(N, storage)[2] // bse_layout(N, storage)[1]
+    n_tiles = rows[1] * (rows[1] + 1) // 2 - rows[0] * (rows[0] + 1) // 2
+    tiles = torch.empty(max(n_tiles, 1) * by, dtype=torch.uint8, device="cuda")
+    _check(lib().bse_fill_synthetic_shard(tiles.data_ptr(), storage, N, which, seed, sigma, group, rows[0], rows[1],
+                                          _stream_ptr()), "bse_fill_synthetic_shard")
+    return tiles
+
+
 def bse_to_real_form(r_tiles, c_tiles, N: int, storage: int = STORE_C128):
     """In place: (R, C) stores -> (S = R + C, D = R - C); use with Bse(..., storage=STORE_REAL_FORM[_C64])."""
-    _check(lib().bse_to_real_form(r_tiles.data_ptr(), c_tiles.data_ptr(), storage, N, _stream_ptr()), "bse_to_real_form")
+    _check(lib().bse_to_real_form(r_tiles.data_ptr(), c_tiles.data_ptr(), storage, bse_layout(N, storage)[1], _stream_ptr()),
+           "bse_to_real_form")
     return r_tiles, c_tiles
 
 
 class Bse:
     """Handle wrapper (bse_create / bse_destroy).  Keeps the borrowed tile buffers alive."""
 
-    def __init__(self, mode: int, N: int, r_tiles, c_tiles=None, storage: int = STORE_C128):
-        self.mode, self.N, self.storage = mode, N, storage
+    def __init__(self, mode: int, N: int, r_tiles, c_tiles=None, storage: int = STORE_C128, rows=None):
+        """rows = (tile_row_begin, tile_row_end): r_tiles / c_tiles hold only that slice of the packed store
+        (bse_create_shard); apply / apply_half then return this slice's contribution to Y."""
+        self.mode, self.N, self.storage, self.rows = mode, N, storage, rows
         self._keep = (r_tiles, c_tiles)
         self.n_op = 2 * N if mode == MODE_FULL else N
         h = _vp()
-        _check(lib().bse_create(ctypes.byref(h), mode, storage, N, r_tiles.data_ptr(),
-                                c_tiles.data_ptr() if c_tiles is not None else None, _stream_ptr()), "bse_create")
+        cp = c_tiles.data_ptr() if c_tiles is not None else None
+        if rows is None:
+            _check(lib().bse_create(ctypes.byref(h), mode, storage, N, r_tiles.data_ptr(), cp, _stream_ptr()), "bse_create")
+        else:
+            _check(lib().bse_create_shard(ctypes.byref(h), mode, storage, N, rows[0], rows[1], r_tiles.data_ptr(), cp,
+                                          _stream_ptr()), "bse_create_shard")
         self._h = h
 
     def close(self):
@@ -258,6 +289,50 @@ class Bse:
         if st != 0 and raise_on_error:
             raise BseError(st, "bse_solve")
         return SolveResult(omega, vec, resid, {f: getattr(info, f) for f, _ in _Info._fields_}, st)
+
+
+def sum_partials(Y, group=None):
+    """Sum the shards' partial products in place over the process group (one all-reduce of 16 N k bytes; NCCL over
+    NVLink on GPUs).  A no-op without an initialised process group or with a single rank."""
+    import torch
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
+        dist.all_reduce(torch.view_as_real(Y), op=dist.ReduceOp.SUM, group=group)
+    return Y
+
+
+class ShardedBse:
+    """The operator's tile stream sharded over the ranks of a torch.distributed process group, one process per GPU
+    (the paper partitions the matrix by rows over MPI ranks).  Rank r holds the slice of
+    the packed store that bse_shard_layout assigns to it (contiguous tile rows, equal tile counts); X is replicated;
+    apply / apply_half run the local kernels on the slice and sum the partial Y with ONE all-reduce of 16 N k bytes.
+    Apply-level only: the solver calls need the whole operator on one GPU."""
+
+    def __init__(self, mode: int, N: int, r_slice, c_slice=None, rows=None, storage: int = STORE_C128, group=None):
+        self.local = Bse(mode, N, r_slice, c_slice, storage=storage, rows=rows)
+        self.group, self.N, self.mode = group, N, mode
+
+    @classmethod
+    def synthetic(cls, mode: int, N: int, seed: int, sigma: float, group_size: int, storage: int = STORE_C128, group=None,
+                  real_form: bool = False):
+        """Each rank generates its own slice of BASELINE.json's synthetic operator on its GPU (nothing crosses PCIe)."""
+        import torch.distributed as dist
+        on = dist.is_available() and dist.is_initialized()
+        world, rank = (dist.get_world_size(group), dist.get_rank(group)) if on else (1, 0)
+        rb, re, _, _, _ = bse_shard_layout(N, world, rank, storage)
+        r = bse_fill_synthetic_shard(N, MATRIX_R, seed, sigma, group_size, (rb, re), storage)
+        c = bse_fill_synthetic_shard(N, MATRIX_C, seed, 0.0, group_size, (rb, re), storage) if mode == MODE_FULL else None
+        if real_form:
+            _check(lib().bse_to_real_form(r.data_ptr(), c.data_ptr(), storage, re * (re + 1) // 2 - rb * (rb + 1) // 2,
+                                          _stream_ptr()), "bse_to_real_form")
+            storage = STORE_REAL_FORM if storage == STORE_C128 else STORE_REAL_FORM_C64
+        return cls(mode, N, r, c, (rb, re), storage, group)
+
+    def apply(self, X, Y=None):
+        return sum_partials(self.local.apply(X, Y), self.group)
+
+    def apply_half(self, X, sign: int, Y=None):
+        return sum_partials(self.local.apply_half(X, sign, Y), self.group)
 
 
 def host_heev(A, nz=None):

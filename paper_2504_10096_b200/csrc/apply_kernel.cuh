@@ -47,7 +47,8 @@ struct ApplyParams {
     int pass;           // PASS_HERM / PASS_SYMC
     double sign;        // s
     int L;              // unit length in tiles
-    int64_t n_units;
+    int64_t u_begin;    // first unit of this handle's tile rows (0 unless the handle is a shard)
+    int64_t n_units;    // one past the last unit
     int zero;           // always 0; a runtime value the assembler cannot fold (see the stage release below)
 };
 
@@ -55,6 +56,13 @@ __host__ __device__ __forceinline__ int64_t apply_num_units(int nt, int L)
 {
     int64_t bf = nt / L, r = nt % L;
     return (int64_t)L * bf * (bf + 1) / 2 + r * (bf + 1);
+}
+// first unit of tile row I (units are ordered by tile row, then by segment): the units of tile rows [I0, I1) are
+// the contiguous range [apply_first_unit(I0), apply_first_unit(I1))
+__host__ __device__ __forceinline__ int64_t apply_first_unit(int I, int L)
+{
+    int64_t b = I / L, r = I % L;
+    return (int64_t)L * b * (b + 1) / 2 + r * (b + 1);
 }
 // unit u -> (I, J0, J1): rows I in [bL, (b+1)L) have b+1 units each.
 __device__ __forceinline__ void apply_decode_unit(int64_t u, int L, int &I, int &J0, int &J1)
@@ -99,7 +107,7 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
             int st = 0;
             uint32_t ph = 0;
             const uint64_t pol = l2_policy_evict_first();     // the tile stream is read exactly once
-            for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
+            for (int64_t u = p.u_begin + blockIdx.x; u < p.n_units; u += gridDim.x) {
                 int I, J0, J1;
                 apply_decode_unit(u, p.L, I, J0, J1);
                 const char *src = p.tiles + tile_index(I, J0) * (int64_t)TBY;
@@ -155,7 +163,7 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_kernel(const App
 
     int st = 0;
     uint32_t ph = 0;
-    for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
+    for (int64_t u = p.u_begin + blockIdx.x; u < p.n_units; u += gridDim.x) {
         int I, J0, J1;
         apply_decode_unit(u, p.L, I, J0, J1);
 

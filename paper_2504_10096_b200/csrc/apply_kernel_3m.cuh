@@ -57,7 +57,7 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_3m_kernel(const 
             int st = 0;
             uint32_t ph = 0;
             const uint64_t pol = l2_policy_evict_first();
-            for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
+            for (int64_t u = p.u_begin + blockIdx.x; u < p.n_units; u += gridDim.x) {
                 int I, J0, J1;
                 apply_decode_unit(u, p.L, I, J0, J1);
                 const char *src = p.tiles + tile_index(I, J0) * (int64_t)TBY;
@@ -100,7 +100,7 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_3m_kernel(const 
                     x[pc][s] = (colok && row < p.N) ? __ldg(xcol + row) : make_double2(0.0, 0.0);
                 }
         };
-        for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
+        for (int64_t u = p.u_begin + blockIdx.x; u < p.n_units; u += gridDim.x) {
             int I, J0, J1;
             apply_decode_unit(u, p.L, I, J0, J1);
             double2 xjn[4][2];
@@ -167,7 +167,7 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_3m_kernel(const 
     const int r = warp - 4;                                   // tile columns 16 r .. 16 r + 15
     // xs = xi - xr in both passes; re = s (Q1 + Q2); im = s (c3 Q3 + c1 (Q1 - Q2)):  HERM c3 = 1, c1 = 1; SYMC c3 = -1, c1 = -1
     const double c31 = herm ? p.sign : -p.sign;
-    for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
+    for (int64_t u = p.u_begin + blockIdx.x; u < p.n_units; u += gridDim.x) {
         int I, J0, J1;
         apply_decode_unit(u, p.L, I, J0, J1);
         // x_I fragments (rows 8 ib + 4 s + t, column g), kept in registers for the whole unit

@@ -48,7 +48,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) apply_tiles_k1_kernel(const 
             int st = 0;
             uint32_t ph = 0;
             const uint64_t pol = l2_policy_evict_first();
-            for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
+            for (int64_t u = p.u_begin + blockIdx.x; u < p.n_units; u += gridDim.x) {
                 int I, J0, J1;
                 apply_decode_unit(u, p.L, I, J0, J1);
                 const char *src = p.tiles + tile_index(I, J0) * (int64_t)TBY;
@@ -87,7 +87,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) apply_tiles_k1_kernel(const 
 
     int st = 0;
     uint32_t ph = 0;
-    for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
+    for (int64_t u = p.u_begin + blockIdx.x; u < p.n_units; u += gridDim.x) {
         int I, J0, J1;
         apply_decode_unit(u, p.L, I, J0, J1);
 

@@ -45,7 +45,7 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_real_kernel(cons
             int st = 0;
             uint32_t ph = 0;
             const uint64_t pol = l2_policy_evict_first();
-            for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
+            for (int64_t u = p.u_begin + blockIdx.x; u < p.n_units; u += gridDim.x) {
                 int I, J0, J1;
                 apply_decode_unit(u, p.L, I, J0, J1);
                 const char *src = p.tiles + tile_index(I, J0) * (int64_t)TBY;
@@ -83,7 +83,7 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_real_kernel(cons
                     x[pc][s] = (colok && row < p.N) ? __ldg(reinterpret_cast<const double *>(xcol + row) + MODE) : 0.0;
                 }
         };
-        for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
+        for (int64_t u = p.u_begin + blockIdx.x; u < p.n_units; u += gridDim.x) {
             int I, J0, J1;
             apply_decode_unit(u, p.L, I, J0, J1);
             double xjn[4][2];
@@ -140,7 +140,7 @@ __global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_real_kernel(cons
 
     // ------------------------------ P2 warps ------------------------------
     const int r = warp - 4;
-    for (int64_t u = blockIdx.x; u < p.n_units; u += gridDim.x) {
+    for (int64_t u = p.u_begin + blockIdx.x; u < p.n_units; u += gridDim.x) {
         int I, J0, J1;
         apply_decode_unit(u, p.L, I, J0, J1);
         // xA pairs with Ar^T, xB with Ai^T:  MODE 0: (a_I, b_I);  MODE 1: (b_I, -a_I)

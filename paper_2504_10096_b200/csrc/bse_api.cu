@@ -1,4 +1,5 @@
 // C-ABI entry points: layout, pack / generators, handle, apply.  (orth: bse_orth.cu, solve: bse_solve.cu)
+#include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <new>
@@ -86,9 +87,11 @@ static void apply_unit_params(const bse_handle_s *h, ApplyParams &p, int &grid)
     if (L > 32) L = 32;
     if (const char *e = getenv("BSE_APPLY_UNIT")) { int v = atoi(e); if (v >= 1 && v <= 4096) L = v; }
     p.L = (int)L;
-    p.n_units = apply_num_units(h->nt, p.L);
+    p.u_begin = apply_first_unit(h->row_begin, p.L);
+    p.n_units = apply_first_unit(h->row_end, p.L);          // == apply_num_units(nt, L) for row_end == nt
     p.zero = 0;
-    grid = (int)(p.n_units < h->num_sms ? p.n_units : h->num_sms);
+    const int64_t count = p.n_units - p.u_begin;
+    grid = (int)(count < h->num_sms ? (count > 0 ? count : 1) : h->num_sms);
 }
 
 bse_status_t launch_real_pass(bse_handle_s *h, const char *tiles, int mode, const void *dX, int64_t ldx, void *dY,
@@ -99,7 +102,7 @@ bse_status_t launch_real_pass(bse_handle_s *h, const char *tiles, int mode, cons
     ApplyParams p;
     int grid;
     apply_unit_params(h, p, grid);
-    p.tiles = tiles;
+    p.tiles = tiles - tile_index(h->row_begin, 0) * tile_bytes_es(h->es);   // virtual base of the whole packed store
     p.pass = mode;
     p.sign = 1.0;
     p.ldx = ldx;
@@ -131,7 +134,7 @@ bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, dou
     ApplyParams p;
     int grid;
     apply_unit_params(h, p, grid);
-    p.tiles = tiles;
+    p.tiles = tiles - tile_index(h->row_begin, 0) * tile_bytes_es(h->es);   // virtual base of the whole packed store
     p.pass = pass;
     p.sign = sign;
     p.ldx = ldx;
@@ -244,7 +247,14 @@ bse_status_t bse_unpack_to_dense(const void *dTiles, int32_t storage, int64_t N,
 bse_status_t bse_fill_synthetic(void *dTiles, int32_t storage, int64_t N, int32_t which, uint64_t seed, double sigma,
                                 int32_t group, void *stream)
 {
+    return bse_fill_synthetic_shard(dTiles, storage, N, which, seed, sigma, group, 0, (int32_t)((N + TB - 1) / TB), stream);
+}
+
+bse_status_t bse_fill_synthetic_shard(void *dTiles, int32_t storage, int64_t N, int32_t which, uint64_t seed, double sigma,
+                                      int32_t group, int32_t tile_row_begin, int32_t tile_row_end, void *stream)
+{
     if (!dTiles || N < 1 || (which != 0 && which != 1) || !storage_ok(storage)) return BSE_ERR_INVALID_ARG;
+    if (tile_row_begin < 0 || tile_row_end < tile_row_begin || tile_row_end > (N + TB - 1) / TB) return BSE_ERR_INVALID_ARG;
     cudaStream_t s = (cudaStream_t)stream;
     double *deps = nullptr;
     if (which == 0) {
@@ -255,13 +265,15 @@ bse_status_t bse_fill_synthetic(void *dTiles, int32_t storage, int64_t N, int32_
                                                                                     stream_key(seed, 1));
         count_launch();
     }
-    int64_t n_tiles;
-    bse_layout(N, storage, nullptr, &n_tiles, nullptr);
-    dim3 grid;
-    tile_grid(n_tiles, grid);
-    fill_synthetic_kernel<<<grid, 256, 0, s>>>((char *)dTiles, storage_es(storage), N, which, stream_key(seed, which == 0 ? 2 : 3), sigma,
-                                               deps, n_tiles);
-    count_launch();
+    const int64_t tile0 = tile_index(tile_row_begin, 0), tile1 = tile_index(tile_row_end, 0);
+    if (tile1 > tile0) {
+        dim3 grid;
+        tile_grid(tile1 - tile0, grid);
+        // the kernel addresses tiles by their global number: pass the virtual base of the whole packed store
+        fill_synthetic_kernel<<<grid, 256, 0, s>>>((char *)dTiles - tile0 * tile_bytes_es(storage_es(storage)), storage_es(storage), N,
+                                                   which, stream_key(seed, which == 0 ? 2 : 3), sigma, deps, tile0, tile1);
+        count_launch();
+    }
     if (deps) cudaFreeAsync(deps, s);
     BSE_CUDA(cudaGetLastError());
     return BSE_OK;
@@ -322,6 +334,8 @@ bse_status_t bse_create(bse_handle_t *out, int32_t mode, int32_t storage, int64_
     h->nt = (int)((N + TB - 1) / TB);
     h->es = storage_es(storage);
     h->real_form = real_form ? 1 : 0;
+    h->row_begin = 0;
+    h->row_end = h->nt;
     h->R = (const char *)dRTiles;
     h->C = (mode == BSE_MODE_FULL) ? (const char *)dCTiles : nullptr;
     h->stream = (cudaStream_t)stream;
@@ -350,16 +364,55 @@ __global__ void __launch_bounds__(256) to_real_form_c64_kernel(float2 *__restric
     }
 }
 
-bse_status_t bse_to_real_form(void *dRTiles, void *dCTiles, int32_t storage, int64_t N, void *stream)
+bse_status_t bse_to_real_form(void *dRTiles, void *dCTiles, int32_t storage, int64_t n_tiles, void *stream)
 {
-    if (!dRTiles || !dCTiles || N < 1 || !storage_ok(storage)) return BSE_ERR_INVALID_ARG;
-    const int64_t nt = (N + TB - 1) / TB, n = nt * (nt + 1) / 2 * TB * TB;
+    if (!dRTiles || !dCTiles || n_tiles < 0 || !storage_ok(storage)) return BSE_ERR_INVALID_ARG;
+    if (n_tiles == 0) return BSE_OK;
+    const int64_t n = n_tiles * TB * TB;
     if (storage == BSE_STORE_C64)
         to_real_form_c64_kernel<<<148 * 8, 256, 0, (cudaStream_t)stream>>>((float2 *)dRTiles, (float2 *)dCTiles, n);
     else
         to_real_form_kernel<<<148 * 8, 256, 0, (cudaStream_t)stream>>>((double2 *)dRTiles, (double2 *)dCTiles, n);
     count_launch();
     BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}
+
+bse_status_t bse_shard_layout(int64_t N, int32_t storage, int32_t n_shards, int32_t shard, int32_t *tile_row_begin,
+                              int32_t *tile_row_end, int64_t *first_tile, int64_t *n_tiles, int64_t *bytes)
+{
+    if (N < 1 || !(storage_ok(storage) || storage_real_form(storage)) || n_shards < 1 || shard < 0 || shard >= n_shards)
+        return BSE_ERR_INVALID_ARG;
+    const int64_t nt = (N + TB - 1) / TB, total = nt * (nt + 1) / 2;
+    // boundary r: the smallest tile row I with I (I + 1) / 2 >= r * total / n_shards (equal tile counts to within one row)
+    auto bound = [&](int64_t r) -> int64_t {
+        if (r <= 0) return 0;
+        if (r >= n_shards) return nt;
+        const double target = (double)total * (double)r / (double)n_shards;
+        int64_t I = (int64_t)((std::sqrt(8.0 * target + 1.0) - 1.0) * 0.5);
+        while (I > 0 && (double)(I * (I + 1) / 2) >= target) --I;
+        while (I < nt && (double)(I * (I + 1) / 2) < target) ++I;
+        return I;
+    };
+    const int64_t b0 = bound(shard), b1 = bound(shard + 1);
+    if (tile_row_begin) *tile_row_begin = (int32_t)b0;
+    if (tile_row_end) *tile_row_end = (int32_t)b1;
+    if (first_tile) *first_tile = b0 * (b0 + 1) / 2;
+    if (n_tiles) *n_tiles = b1 * (b1 + 1) / 2 - b0 * (b0 + 1) / 2;
+    if (bytes) *bytes = (b1 * (b1 + 1) / 2 - b0 * (b0 + 1) / 2) * tile_bytes_es(storage_es(storage));
+    return BSE_OK;
+}
+
+bse_status_t bse_create_shard(bse_handle_t *out, int32_t mode, int32_t storage, int64_t N, int32_t tile_row_begin,
+                              int32_t tile_row_end, const void *dRSlice, const void *dCSlice, void *stream)
+{
+    if (N < 1) return BSE_ERR_INVALID_ARG;
+    const int64_t nt = (N + TB - 1) / TB;
+    if (tile_row_begin < 0 || tile_row_end < tile_row_begin || tile_row_end > nt) return BSE_ERR_INVALID_ARG;
+    bse_status_t st = bse_create(out, mode, storage, N, dRSlice, dCSlice, stream);
+    if (st) return st;
+    (*out)->row_begin = tile_row_begin;
+    (*out)->row_end = tile_row_end;
     return BSE_OK;
 }
 

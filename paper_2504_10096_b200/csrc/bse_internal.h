@@ -13,6 +13,7 @@ struct bse_handle_s {
     int64_t N;
     int nt;
     int es;              // bytes per stored complex entry: 16 (BSE_STORE_C128) or 8 (BSE_STORE_C64)
+    int row_begin, row_end;   // tile rows [row_begin, row_end) this handle's stores hold (0, nt unless created by bse_create_shard)
     int real_form;       // BSE_STORE_REAL_FORM: R holds S = R + C, C holds D = R - C (full mode only, complex128)
     const char *R;
     const char *C;
@@ -30,6 +31,9 @@ struct bse_handle_s {
 };
 
 namespace bse {
+
+// a handle created by bse_create_shard over part of the tile rows: apply / apply_half only
+inline bool is_partial(const bse_handle_s *h) { return h->row_begin != 0 || h->row_end != h->nt; }
 
 extern std::atomic<int64_t> g_launches;
 inline void count_launch(int n = 1) { g_launches.fetch_add(n, std::memory_order_relaxed); }

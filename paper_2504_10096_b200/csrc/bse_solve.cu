@@ -114,6 +114,7 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
                                   bse_info_t *info_out)
 {
     if (!h || nev < 1 || k < 1 || !hOmega || !dVec || !(tol > 0.0) || max_restarts < 0) return BSE_ERR_INVALID_ARG;
+    if (is_partial(h)) return BSE_ERR_INVALID_ARG;
     const int64_t n = h->N;
     const bool full = (h->mode == BSE_MODE_FULL);
     if ((int64_t)nev + k > n || ldvec < (full ? 2 * n : n)) return BSE_ERR_INVALID_ARG;

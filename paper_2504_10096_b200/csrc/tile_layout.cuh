@@ -97,10 +97,11 @@ __global__ void transition_energies_kernel(double *__restrict__ d, int64_t N, in
 
 __global__ void __launch_bounds__(256) fill_synthetic_kernel(char *__restrict__ tiles, int es, int64_t N, int which,
                                                              uint64_t h0, double sigma,
-                                                             const double *__restrict__ deps, int64_t n_tiles)
+                                                             const double *__restrict__ deps, int64_t tile0,
+                                                             int64_t tile1)
 {
-    int64_t tile = blockIdx.y + (int64_t)blockIdx.z * gridDim.y;
-    if (tile >= n_tiles) return;
+    int64_t tile = tile0 + blockIdx.y + (int64_t)blockIdx.z * gridDim.y;      // global tile number, [tile0, tile1)
+    if (tile >= tile1) return;
     int I, J;
     tile_from_linear(tile, I, J);
     int e = blockIdx.x * blockDim.x + threadIdx.x;

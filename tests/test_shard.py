@@ -1,0 +1,148 @@
+"""Sharding of the tile stream (include/bse.h): the partition helper (host only), the all-reduce plumbing
+on two gloo ranks (CPU), and -- on the GPU -- the sum of the shards' partial products against the oracle."""
+import os
+
+import numpy as np
+import pytest
+
+import bse_inputs as gen
+
+
+@pytest.mark.parametrize("N", [64, 1000, 16384, 98304])
+@pytest.mark.parametrize("G", [1, 2, 3, 8, 128])
+def test_shard_layout_partitions_the_store(N, G):
+    import paper_2504_10096_b200 as b
+    for storage in (b.STORE_C128, b.STORE_C64):
+        _, total, total_bytes = b.bse_layout(N, storage)
+        nt = (N + 63) // 64
+        prev_end, prev_tile, sizes = 0, 0, []
+        for r in range(G):
+            rb, re, ft, n, by = b.bse_shard_layout(N, G, r, storage)
+            assert rb == prev_end and ft == prev_tile == rb * (rb + 1) // 2           # contiguous, in order
+            assert n == re * (re + 1) // 2 - rb * (rb + 1) // 2 and by == n * (total_bytes // total)
+            prev_end, prev_tile = re, ft + n
+            sizes.append(n)
+        assert prev_end == nt and sum(sizes) == total                                # every tile exactly once
+        # balanced to within one tile row of the ideal share
+        assert max(sizes) - total / G <= nt + 1
+
+
+def _gloo_worker(rank, world, port, q):
+    import torch
+    import torch.distributed as dist
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import paper_2504_10096_b200 as b
+    Y = torch.full((3, 10), complex(rank + 1, -(rank + 1)), dtype=torch.complex128)
+    b.sum_partials(Y)
+    rows = b.bse_shard_layout(1000, world, rank)[:2]
+    q.put((rank, Y[0, 0].item(), rows))
+    dist.destroy_process_group()
+
+
+def test_sum_partials_on_two_gloo_ranks():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29500 + os.getpid() % 2000
+    ps = [ctx.Process(target=_gloo_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in ps: p.start()
+    out = sorted(q.get(timeout=120) for _ in ps)
+    for p in ps: p.join(60)
+    assert all(p.exitcode == 0 for p in ps)
+    assert out[0][1] == out[1][1] == complex(3, -3)                 # both ranks hold the sum
+    assert out[0][2][0] == 0 and out[0][2][1] == out[1][2][0] and out[1][2][1] == 16     # the two slices tile the rows
+
+
+# ------------------------------------------------- GPU: shards run one after another on one device -----------------
+
+def _slices(tiles, N, G, storage):
+    import paper_2504_10096_b200 as b
+    per_tile = b.bse_layout(N, storage)[2] // b.bse_layout(N, storage)[1]
+    out = []
+    for r in range(G):
+        rb, re, ft, n, by = b.bse_shard_layout(N, G, r, storage)
+        out.append(((rb, re), tiles[ft * per_tile: ft * per_tile + max(by, 1)]))
+    return out
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("G", [2, 3, 8])
+@pytest.mark.parametrize("k", [1, 4, 8])
+def test_tda_partial_products_sum_to_the_oracle(orc, G, k):
+    import torch
+    import paper_2504_10096_b200 as b
+    from gpu_util import pack, relerr, to_dev, to_host
+    N = 1000
+    R = gen.dense_R(1008, 41, sigma=0.5)[:N, :N]
+    X = gen.block_X(N, k, 42)
+    ref = orc.apply_tda(R, X)
+    for storage in (b.STORE_C128, b.STORE_C64):
+        tiles = b.bse_pack_from_dense(to_dev(R), N, 0, storage=storage)
+        Y = torch.zeros((k, N), dtype=torch.complex128, device="cuda")
+        for rows, sl in _slices(tiles, N, G, storage):
+            Y += b.Bse(b.MODE_TDA, N, sl, storage=storage, rows=rows).apply(to_dev(X))
+        want = ref if storage == b.STORE_C128 else orc.apply_tda(orc.round_c64(R), X)
+        assert relerr(to_host(Y), want) <= 1e-12
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("G", [2, 5])
+def test_full_mode_partial_products_complex_and_real_form(orc, G):
+    import torch
+    import paper_2504_10096_b200 as b
+    from gpu_util import pack, relerr, to_dev, to_host
+    N, k = 520, 8
+    R, C = gen.dense_R(528, 43, sigma=1.0)[:N, :N], gen.dense_C(N, 43)
+    x = gen.block_X(N, k, 44)
+    X2 = gen.block_X(2 * N, 3, 45)
+    for real in (False, True):
+        rt, ct = pack(R, 0), pack(C, 1)
+        storage = b.STORE_C128
+        if real:
+            b.bse_to_real_form(rt, ct, N)
+            storage = b.STORE_REAL_FORM
+        hs = [b.Bse(b.MODE_FULL, N, sr, sc, storage=storage, rows=rows)
+              for (rows, sr), (_, sc) in zip(_slices(rt, N, G, b.STORE_C128), _slices(ct, N, G, b.STORE_C128))]
+        for sign in (+1, -1):
+            Y = sum(h.apply_half(to_dev(x), sign) for h in hs)
+            assert relerr(to_host(Y), orc.apply_half(R, C, x, sign)) <= 1e-12
+        Y = sum(h.apply(to_dev(X2)) for h in hs)
+        assert relerr(to_host(Y), orc.apply_full(R, C, X2)) <= 1e-12
+        with pytest.raises(b.BseError):
+            hs[0].solve(4, 4)                                  # a partial handle is apply-level only
+
+
+@pytest.mark.gpu
+def test_generated_slices_equal_slices_of_the_generated_store():
+    import torch
+    import paper_2504_10096_b200 as b
+    N, G = 4096, 3
+    for which, sigma in ((0, 0.5), (1, 0.0)):
+        full = b.bse_fill_synthetic(N, which, 5, sigma, 16)
+        for r in range(G):
+            rb, re, ft, n, by = b.bse_shard_layout(N, G, r)
+            sl = b.bse_fill_synthetic_shard(N, which, 5, sigma, 16, (rb, re))
+            assert torch.equal(sl[:by], full[ft * 65536: ft * 65536 + by])
+
+
+@pytest.mark.gpu
+def test_sharded_bse_single_process_many_units(orc):
+    """ShardedBse without a process group is the one-rank case (its slice is the whole store); sampled rows at a size
+    where every CTA walks several units."""
+    import paper_2504_10096_b200 as b
+    from gpu_util import relerr, to_dev, to_host
+    N, k = 8192, 8
+    h = b.ShardedBse.synthetic(b.MODE_TDA, N, 1, 0.0, 16)
+    X = gen.block_X(N, k, 12)
+    rows = np.arange(0, N, 509)
+    ref = orc.rows_times_block(gen.rows_R(N, 1, rows, 0.0, 16), X)
+    assert relerr(to_host(h.apply(to_dev(X)))[rows], ref) <= 1e-12
+    # three slices generated separately, many units each, summed
+    import torch
+    Y = torch.zeros((k, N), dtype=torch.complex128, device="cuda")
+    for r in range(3):
+        rb, re = b.bse_shard_layout(N, 3, r)[:2]
+        sl = b.bse_fill_synthetic_shard(N, 0, 1, 0.0, 16, (rb, re))
+        Y += b.Bse(b.MODE_TDA, N, sl, rows=(rb, re)).apply(to_dev(X))
+    assert relerr(to_host(Y)[rows], ref) <= 1e-12
