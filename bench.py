@@ -165,8 +165,15 @@ def run_cuda(args, cfg):
     N, k = cfg["N"], args.k
 
     storage = b.STORE_C128 if ES == 16.0 else b.STORE_C64
-    tiles = b.bse_fill_synthetic(N, b.MATRIX_R, 1, 0.0, cfg["group"], storage=storage)   # one operand per replica
-    h = b.Bse(b.MODE_TDA, N, tiles, storage=storage)
+    shard = bool(args.shard)                                   # with one rank: the one-slice case of the same code path
+    if shard:
+        # ONE operand, its tile stream split over the ranks; each apply = local kernel + one all-reduce
+        h = b.ShardedBse.synthetic(b.MODE_TDA, N, 1, 0.0, cfg["group"], storage=storage)
+        tiles = None
+    else:
+        tiles = b.bse_fill_synthetic(N, b.MATRIX_R, 1, 0.0, cfg["group"], storage=storage)   # one operand per replica
+        h = b.Bse(b.MODE_TDA, N, tiles, storage=storage)
+    jobs = 1 if shard else world                                # independent operands in flight
     Xh = torch.from_numpy(np.ascontiguousarray(gen.block_X(N, max(k, 8), 1001).T)).pin_memory()
     X = Xh[:k].cuda()
     Y = torch.empty_like(X)
@@ -197,17 +204,28 @@ def run_cuda(args, cfg):
     clocks = sampler.stop()
     barrier()
     ms = max_over_ranks(ms, dist, "cuda")
-    value = world * alg_bytes(N, k) / (ms * 1e-3) / 1e9
+    value = jobs * alg_bytes(N, k) / (ms * 1e-3) / 1e9
 
     # ---- end to end through the host entry point (pinned host X and Y, copies inside the timed region)
     Xk = Xh[:k].numpy()
     Yk = torch.empty((k, N), dtype=torch.complex128).pin_memory().numpy()
+    if shard:
+        Xp, Yp = Xh[:k], torch.empty((k, N), dtype=torch.complex128).pin_memory()
+
+        def host_step():                                        # pinned host X -> device, sharded apply, Y -> pinned host
+            X.copy_(Xp, non_blocking=True)
+            h.apply(X, Y)
+            Yp.copy_(Y, non_blocking=True)
+            torch.cuda.synchronize()
+    else:
+        def host_step():
+            h.apply_host(Xk, Yk)
     for _ in range(2):
-        h.apply_host(Xk, Yk)
+        host_step()
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        h.apply_host(Xk, Yk)
+        host_step()
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - t0) * 1e3 / args.steps
     e2e_ms = max_over_ranks(e2e_ms, dist, "cuda")
@@ -220,6 +238,8 @@ def run_cuda(args, cfg):
 
     peak, peak_src = measured_peaks()
     achieved = alg_bytes(N, k) / (ms * 1e-3) / 1e9
+    if shard:                                                   # per GPU: 1 / world of the tiles, the whole X and Y
+        achieved = ((alg_bytes(N, k) - 32.0 * N * k) / world + 32.0 * N * k) / (ms * 1e-3) / 1e9
     traffic = None
     try:
         import csv
@@ -231,7 +251,7 @@ def run_cuda(args, cfg):
         pass
     # north_star: roofline = min(bytes / HBM peak, flops / FP64 peak).  The FP64 figure is this repo's own DMMA
     # microbenchmark (profiles/r1_microbench.md): MEASURED_PEAKS.json has no FP64 entry.
-    tflops = 8.0 * N * N * k / (ms * 1e-3) / 1e12
+    tflops = 8.0 * N * N * k / (ms * 1e-3) / 1e12 / (world if shard else 1)       # per GPU
     fp64_peak = 37.1
     if 8.0 * N * N * k / (fp64_peak * 1e12) > alg_bytes(N, k) / (peak * 1e9):
         roof = {"bound": "tensor", "achieved": tflops, "peak": fp64_peak, "unit": "TFLOP/s", "frac": tflops / fp64_peak,
@@ -247,15 +267,18 @@ def run_cuda(args, cfg):
                  "tflops_fp64": tflops, "tflops_fp64_executed": tflops * (0.75 if three_m else 1.0),
                  "fp64_peak_measured_tflops": fp64_peak, "GBps": achieved})
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "strong" if shard else "weak",
             "vs_baseline": None, "dtype": "f64 (complex128 on the FP64 tensor cores)", "data": "synthetic",
             "config": workload(cfg, k), "clocks": clocks, "gpu_launches": int(launches),
-            "e2e": {"value": world * alg_bytes(N, k) / (e2e_ms * 1e-3) / 1e9, "unit": UNIT,
+            "e2e": {"value": jobs * alg_bytes(N, k) / (e2e_ms * 1e-3) / 1e9, "unit": UNIT,
                     "h2d_bytes_per_step": 16 * N * k, "d2h_bytes_per_step": 16 * N * k, "ms_per_step": e2e_ms},
             "roofline": roof}
 
     # ---- k sweep and Lanczos time-to-nev (the rest of BASELINE.json's metric), device-timed, outside `value`
-    if not args.no_extras and ES == 16.0:
+    if shard:
+        line["config"]["parallelism"] = f"tile stream sharded over {world} GPUs (contiguous tile rows, equal tile counts), " \
+                                        "X replicated, one all-reduce of Y per apply"
+    if not args.no_extras and ES == 16.0 and not shard:
         sweep = {}
         for kk in (1, 2, 4, 8):
             Xs, Ys = Xh[:kk].cuda(), torch.empty((kk, N), dtype=torch.complex128, device="cuda")
@@ -374,6 +397,8 @@ def main():
     ap.add_argument("--k", type=int, default=4)
     ap.add_argument("--storage", default="c128", choices=["c128", "c64"],
                     help="c64: complex64-stored operand (SURVEY.md 8(f1)); the extras run for the default only")
+    ap.add_argument("--shard", action="store_true",
+                    help="N > 1 GPUs: shard ONE operand's tile stream over the ranks (strong scaling) instead of replicas")
     ap.add_argument("--ref-rows", type=int, default=1024)
     ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
