@@ -161,10 +161,29 @@ bse_status_t bse_fill_synthetic_shard(void *dTiles, int32_t storage, int64_t N, 
  * shards of a partition is Y = H X.  X must be the whole block on every shard (16 N k bytes); the partial Y are
  * summed by the caller (one all-reduce of 16 N k bytes per apply over NVLink when shards live on different GPUs:
  * paper_2504_10096_b200.ShardedBse).  bse_solve, bse_orth and bse_lanczos_quadrature need the whole operator and
- * return BSE_ERR_INVALID_ARG on a partial handle.  The general FULL-mode bse_apply is real-linear in the stores as
+ * return BSE_ERR_INVALID_ARG on a partial handle that has no communication hook (bse_set_comm).  The general FULL-mode bse_apply is real-linear in the stores as
  * well (its elementwise pre/post steps commute with the sum), for every storage type. */
 bse_status_t bse_create_shard(bse_handle_t *h, int32_t mode, int32_t storage, int64_t N, int32_t tile_row_begin,
                               int32_t tile_row_end, const void *dRSlice, const void *dCSlice, void *stream);
+
+/* Communication hook for partial handles (one process per GPU; the library itself links no communication library).
+ * fn(user, op, dBuf, n_doubles) must, on the handle's stream order, either
+ *   BSE_COMM_SUM  : replace dBuf[0 .. n_doubles) (device, FP64) by its sum over all ranks (an all-reduce), or
+ *   BSE_COMM_BCAST: replace it by rank 0's copy (a broadcast),
+ * and return 0 (anything else aborts the calling library function with BSE_ERR_INTERNAL).  With a hook installed
+ *   - bse_apply / bse_apply_half on a partial handle return the COMPLETE product (local contribution + one SUM of
+ *     16 N k bytes);
+ *   - bse_solve and bse_lanczos_quadrature run on partial handles: every rank executes the same host loop on
+ *     replicated vectors; each operator application is summed over the ranks, and every quantity the kernels
+ *     accumulate with floating-point atomics (projection coefficients, Gram matrices, recurrence scalars) as well as
+ *     the projected eigen-decomposition is broadcast from rank 0 before it is used, so that all ranks hold bitwise
+ *     identical bases and take identical decisions (same number of steps and restarts: no rank can fall out of the
+ *     collective sequence).  Vectors, orthogonalisation and restart are replicated (O(N ncv) per rank), the O(N^2)
+ *     tile stream is divided.
+ * fn = NULL removes the hook.  The hook is called from the thread that called the library function. */
+typedef int32_t (*bse_comm_fn)(void *user, int32_t op, void *dBuf, int64_t n_doubles);
+enum { BSE_COMM_SUM = 0, BSE_COMM_BCAST = 1 };
+bse_status_t bse_set_comm(bse_handle_t h, bse_comm_fn fn, void *user);
 
 /* Y = H X for a block of k >= 1 vectors.
  *   TDA : X, Y are N x k;   Y = R X.

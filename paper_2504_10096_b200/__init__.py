@@ -53,6 +53,7 @@ _SIGNATURES = {
                          ctypes.POINTER(_i64), ctypes.POINTER(_i64)],
     "bse_fill_synthetic_shard": [_vp, _i32, _i64, _i32, _u64, _dbl, _i32, _i32, _i32, _vp],
     "bse_create_shard": [ctypes.POINTER(_vp), _i32, _i32, _i64, _i32, _i32, _vp, _vp, _vp],
+    "bse_set_comm": [_vp, _vp, _vp],
     "bse_apply": [_vp, _vp, _i64, _vp, _i64, _i32],
     "bse_apply_half": [_vp, _i32, _vp, _i64, _vp, _i64, _i32],
     "bse_apply_host": [_vp, _vp, _i64, _vp, _i64, _i32],
@@ -311,6 +312,47 @@ class ShardedBse:
     def __init__(self, mode: int, N: int, r_slice, c_slice=None, rows=None, storage: int = STORE_C128, group=None):
         self.local = Bse(mode, N, r_slice, c_slice, storage=storage, rows=rows)
         self.group, self.N, self.mode = group, N, mode
+        self._cb = None
+        self.comm_calls = [0, 0]                                 # sums, broadcasts issued through the hook
+
+    def install_comm(self):
+        """Give the library the process group (bse_set_comm): its products become complete (local + one all-reduce) and
+        bse_solve / bse_lanczos_quadrature run on the sharded operator with replicated vectors (include/bse.h)."""
+        import torch
+        import torch.distributed as dist
+        group = self.group
+        src = dist.get_global_rank(group, 0) if group is not None else 0
+        calls = self.comm_calls
+
+        class _Dev:                                              # zero-copy view of the library's device buffer
+            def __init__(self, ptr, n):
+                self.__cuda_array_interface__ = {"shape": (n,), "typestr": "<f8", "data": (ptr, False), "version": 2}
+
+        def hook(user, op, ptr, n):
+            try:
+                t = torch.as_tensor(_Dev(ptr, n), device="cuda")
+                if op == 0:
+                    dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
+                else:
+                    dist.broadcast(t, src=src, group=group)
+                calls[op] += 1
+                return 0
+            except Exception as e:                               # never let an exception cross the C frame
+                import sys
+                print(f"[ShardedBse] communication hook failed: {e!r}", file=sys.stderr)
+                return 1
+
+        self._cb = ctypes.CFUNCTYPE(_i32, _vp, _i32, _vp, _i64)(hook)
+        _check(lib().bse_set_comm(self.local._h, ctypes.cast(self._cb, _vp), None), "bse_set_comm")
+        return self
+
+    def solve(self, *args, **kw):
+        assert self._cb is not None, "install_comm() first"
+        return self.local.solve(*args, **kw)
+
+    def lanczos_quadrature(self, d, steps: int):
+        assert self._cb is not None, "install_comm() first"
+        return self.local.lanczos_quadrature(d, steps)
 
     @classmethod
     def synthetic(cls, mode: int, N: int, seed: int, sigma: float, group_size: int, storage: int = STORE_C128, group=None,
@@ -329,10 +371,12 @@ class ShardedBse:
         return cls(mode, N, r, c, (rb, re), storage, group)
 
     def apply(self, X, Y=None):
-        return sum_partials(self.local.apply(X, Y), self.group)
+        Y = self.local.apply(X, Y)
+        return Y if self._cb is not None else sum_partials(Y, self.group)      # with the hook the library has summed
 
     def apply_half(self, X, sign: int, Y=None):
-        return sum_partials(self.local.apply_half(X, sign, Y), self.group)
+        Y = self.local.apply_half(X, sign, Y)
+        return Y if self._cb is not None else sum_partials(Y, self.group)
 
 
 def host_heev(A, nz=None):

@@ -94,6 +94,38 @@ static void apply_unit_params(const bse_handle_s *h, ApplyParams &p, int &grid)
     grid = (int)(count < h->num_sms ? (count > 0 ? count : 1) : h->num_sms);
 }
 
+bse_status_t comm_sum_block(bse_handle_s *h, void *dY, int64_t ld, int64_t rows, int k)
+{
+    if (!h->comm) return BSE_OK;
+    if (ld == rows) return h->comm(h->comm_user, BSE_COMM_SUM, dY, 2 * rows * k) ? BSE_ERR_INTERNAL : BSE_OK;
+    for (int c = 0; c < k; ++c)
+        if (h->comm(h->comm_user, BSE_COMM_SUM, (char *)dY + (size_t)c * ld * 16, 2 * rows)) return BSE_ERR_INTERNAL;
+    return BSE_OK;
+}
+bse_status_t comm_bcast_dev(bse_handle_s *h, void *dBuf, int64_t n_doubles)
+{
+    if (!h->comm || n_doubles <= 0) return BSE_OK;
+    return h->comm(h->comm_user, BSE_COMM_BCAST, dBuf, n_doubles) ? BSE_ERR_INTERNAL : BSE_OK;
+}
+bse_status_t comm_bcast_host(bse_handle_s *h, void *hBuf, size_t bytes)
+{
+    if (!h->comm || bytes == 0) return BSE_OK;
+    const size_t padded = (bytes + 7) / 8 * 8;
+    if (h->comm_buf_bytes < padded) {
+        if (h->comm_buf) cudaFree(h->comm_buf);
+        h->comm_buf = nullptr;
+        h->comm_buf_bytes = 0;
+        if (cudaMalloc(&h->comm_buf, padded) != cudaSuccess) { cudaGetLastError(); return BSE_ERR_ALLOC; }
+        h->comm_buf_bytes = padded;
+    }
+    BSE_CUDA(cudaMemsetAsync((char *)h->comm_buf + (padded - 8), 0, 8, h->stream));
+    BSE_CUDA(cudaMemcpyAsync(h->comm_buf, hBuf, bytes, cudaMemcpyHostToDevice, h->stream));
+    if (h->comm(h->comm_user, BSE_COMM_BCAST, h->comm_buf, (int64_t)(padded / 8))) return BSE_ERR_INTERNAL;
+    BSE_CUDA(cudaMemcpyAsync(hBuf, h->comm_buf, bytes, cudaMemcpyDeviceToHost, h->stream));
+    BSE_CUDA(cudaStreamSynchronize(h->stream));
+    return BSE_OK;
+}
+
 bse_status_t launch_real_pass(bse_handle_s *h, const char *tiles, int mode, const void *dX, int64_t ldx, void *dY,
                               int64_t ldy, int32_t k)
 {
@@ -336,6 +368,10 @@ bse_status_t bse_create(bse_handle_t *out, int32_t mode, int32_t storage, int64_
     h->real_form = real_form ? 1 : 0;
     h->row_begin = 0;
     h->row_end = h->nt;
+    h->comm = nullptr;
+    h->comm_user = nullptr;
+    h->comm_buf = nullptr;
+    h->comm_buf_bytes = 0;
     h->R = (const char *)dRTiles;
     h->C = (mode == BSE_MODE_FULL) ? (const char *)dCTiles : nullptr;
     h->stream = (cudaStream_t)stream;
@@ -416,12 +452,21 @@ bse_status_t bse_create_shard(bse_handle_t *out, int32_t mode, int32_t storage, 
     return BSE_OK;
 }
 
+bse_status_t bse_set_comm(bse_handle_t h, bse_comm_fn fn, void *user)
+{
+    if (!h) return BSE_ERR_INVALID_ARG;
+    h->comm = fn;
+    h->comm_user = fn ? user : nullptr;
+    return BSE_OK;
+}
+
 bse_status_t bse_destroy(bse_handle_t h)
 {
     if (!h) return BSE_ERR_INVALID_ARG;
     if (h->ws) cudaFree(h->ws);
     if (h->ws2) cudaFree(h->ws2);
     if (h->hpin) cudaFreeHost(h->hpin);
+    if (h->comm_buf) cudaFree(h->comm_buf);
     delete h;
     return BSE_OK;
 }
@@ -436,11 +481,13 @@ bse_status_t bse_apply_half(bse_handle_t h, int32_t sign, const void *dX, int64_
         // stores hold S = R + C (h->R) and D = R - C (h->C):  P = mode 0 over S + mode 1 over D,  M = mode 0 over D + mode 1 over S
         const char *first = sign > 0 ? h->R : h->C, *second = sign > 0 ? h->C : h->R;
         if ((st = launch_real_pass(h, first, 0, dX, ldx, dY, ldy, k))) return st;
-        return launch_real_pass(h, second, 1, dX, ldx, dY, ldy, k);
+        if ((st = launch_real_pass(h, second, 1, dX, ldx, dY, ldy, k))) return st;
+        return comm_sum_block(h, dY, ldy, h->N, k);
     }
     st = launch_apply_pass(h, h->R, PASS_HERM, 1.0, dX, ldx, dY, ldy, k);
     if (st) return st;
-    return launch_apply_pass(h, h->C, PASS_SYMC, (double)sign, dX, ldx, dY, ldy, k);
+    if ((st = launch_apply_pass(h, h->C, PASS_SYMC, (double)sign, dX, ldx, dY, ldy, k))) return st;
+    return comm_sum_block(h, dY, ldy, h->N, k);
 }
 
 }  // extern "C"

@@ -65,7 +65,8 @@ bse_status_t bse_apply(bse_handle_t h, const void *dX, int64_t ldx, void *dY, in
         if (ldx < N || ldy < N) return BSE_ERR_INVALID_ARG;
         bse_status_t st = zero_block(h, dY, ldy, N, k);
         if (st) return st;
-        return launch_apply_pass(h, h->R, 0 /*HERM*/, 1.0, dX, ldx, dY, ldy, k);
+        if ((st = launch_apply_pass(h, h->R, 0 /*HERM*/, 1.0, dX, ldx, dY, ldy, k))) return st;
+        return comm_sum_block(h, dY, ldy, N, k);
     }
     // FULL:  Y1 = R X1 + C X2 ;  Y2 = -conj( R conj(X2) + C conj(X1) )     (Eq. 1 with A = R^*, C = C^T)
     if (ldx < 2 * N || ldy < 2 * N) return BSE_ERR_INVALID_ARG;
@@ -102,7 +103,7 @@ bse_status_t bse_apply(bse_handle_t h, const void *dX, int64_t ldx, void *dY, in
     neg_conj_inplace_kernel<<<grid, 256, 0, h->stream>>>(Y2, ldy, N, k);             // Y2 = -conj(Z)
     count_launch();
     BSE_CUDA(cudaGetLastError());
-    return BSE_OK;
+    return comm_sum_block(h, dY, ldy, 2 * N, k);
 }
 
 bse_status_t bse_apply_host(bse_handle_t h, const void *hX, int64_t ldx, void *hY, int64_t ldy, int32_t k)

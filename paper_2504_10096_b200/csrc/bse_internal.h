@@ -14,6 +14,10 @@ struct bse_handle_s {
     int nt;
     int es;              // bytes per stored complex entry: 16 (BSE_STORE_C128) or 8 (BSE_STORE_C64)
     int row_begin, row_end;   // tile rows [row_begin, row_end) this handle's stores hold (0, nt unless created by bse_create_shard)
+    bse_comm_fn comm;    // bse_set_comm: sum / broadcast over the ranks that hold the other slices (NULL: none)
+    void *comm_user;
+    void *comm_buf;      // device staging for host-side broadcasts
+    size_t comm_buf_bytes;
     int real_form;       // BSE_STORE_REAL_FORM: R holds S = R + C, C holds D = R - C (full mode only, complex128)
     const char *R;
     const char *C;
@@ -34,6 +38,12 @@ namespace bse {
 
 // a handle created by bse_create_shard over part of the tile rows: apply / apply_half only
 inline bool is_partial(const bse_handle_s *h) { return h->row_begin != 0 || h->row_end != h->nt; }
+// partial handle that cannot complete its products: the solver-level calls refuse it
+inline bool is_incomplete(const bse_handle_s *h) { return is_partial(h) && !h->comm; }
+// communication through the hook (no-ops without one).  ld, rows in complex elements.
+bse_status_t comm_sum_block(bse_handle_s *h, void *dY, int64_t ld, int64_t rows, int k);
+bse_status_t comm_bcast_dev(bse_handle_s *h, void *dBuf, int64_t n_doubles);
+bse_status_t comm_bcast_host(bse_handle_s *h, void *hBuf, size_t bytes);
 
 extern std::atomic<int64_t> g_launches;
 inline void count_launch(int n = 1) { g_launches.fetch_add(n, std::memory_order_relaxed); }

@@ -357,7 +357,7 @@ extern "C" bse_status_t bse_orth(bse_handle_t h, const void *dV, int64_t ldv, in
                                  void *dW, int64_t ldw, int32_t k, void *dBW, int64_t ldbw, void *dHcoef, void *dBfac,
                                  int32_t *hRank)
 {
-    if (!h || !dW || k < 1 || m < 0 || ldw < h->N || is_partial(h)) return BSE_ERR_INVALID_ARG;
+    if (!h || !dW || k < 1 || m < 0 || ldw < h->N || is_incomplete(h)) return BSE_ERR_INVALID_ARG;
     if (m > 0 && (!dV || ldv < h->N)) return BSE_ERR_INVALID_ARG;
     if (dBV || dBW) {
         if (h->mode != BSE_MODE_FULL || !dBW || ldbw < h->N || (m > 0 && (!dBV || ldbv < h->N))) return BSE_ERR_INVALID_ARG;

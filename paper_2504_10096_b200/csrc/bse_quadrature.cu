@@ -76,6 +76,7 @@ static bse_status_t lanczos_quadrature_full(bse_handle_s *h, const void *dStart,
     // beta_0^2 = Re(d^H P(d));  x_1 = d / beta_0,  p_1 = P(d) / beta_0
     if ((st = half(+1, (const double2 *)dStart, pb[1]))) return st;
     dot_re_kernel<<<grid, 256, 0, h->stream>>>((const double2 *)dStart, pb[1], n, d_b2);
+    if ((st = comm_bcast_dev(h, d_b2, 1))) return st;
     scale_by_norm_kernel<<<grid, 256, 0, h->stream>>>((const double2 *)dStart, xb[0], n, d_b2);
     scale_by_norm_kernel<<<grid, 256, 0, h->stream>>>(pb[1], pb[0], n, d_b2);
     count_launch(3);
@@ -83,11 +84,13 @@ static bse_status_t lanczos_quadrature_full(bse_handle_s *h, const void *dStart,
     for (int j = 0; j < steps; ++j) {
         if ((st = half(-1, pb[0], xb[iw]))) return st;                                      // w = M(p_j)
         dot_re_kernel<<<grid, 256, 0, h->stream>>>(pb[0], xb[iw], n, d_alpha + j);         // alpha_j = Re(p_j^H w)
+        if ((st = comm_bcast_dev(h, d_alpha + j, 1))) return st;
         axpy_norm_kernel<<<grid, 256, 0, h->stream>>>(xb[iw], xb[ix], xb[ip], n, d_alpha + j, j > 0 ? d_b2 + j : nullptr,
                                                       d_junk + j);                          // w -= alpha x_j + beta x_{j-1}
         count_launch(2);
         if ((st = half(+1, xb[iw], pb[1]))) return st;                                      // pw = P(w)
         dot_re_kernel<<<grid, 256, 0, h->stream>>>(xb[iw], pb[1], n, d_b2 + j + 1);        // beta_{j+1}^2 = Re(w^H pw)
+        if ((st = comm_bcast_dev(h, d_b2 + j + 1, 1))) return st;
         scale_by_norm_kernel<<<grid, 256, 0, h->stream>>>(xb[iw], xb[iw], n, d_b2 + j + 1);
         scale_by_norm_kernel<<<grid, 256, 0, h->stream>>>(pb[1], pb[0], n, d_b2 + j + 1);
         count_launch(3);
@@ -114,7 +117,7 @@ static bse_status_t lanczos_quadrature_full(bse_handle_s *h, const void *dStart,
 extern "C" bse_status_t bse_lanczos_quadrature(bse_handle_t h, const void *dStart, int32_t steps, double *hAlpha,
                                                double *hBeta, int32_t *hDone)
 {
-    if (!h || !dStart || steps < 1 || !hAlpha || !hBeta || is_partial(h)) return BSE_ERR_INVALID_ARG;
+    if (!h || !dStart || steps < 1 || !hAlpha || !hBeta || is_incomplete(h)) return BSE_ERR_INVALID_ARG;
     if (h->mode == BSE_MODE_FULL) return lanczos_quadrature_full(h, dStart, steps, hAlpha, hBeta, hDone);
     const int64_t n = h->N;
     // workspace: three vectors + alpha[steps] + nrm2[steps + 1]
@@ -128,17 +131,21 @@ extern "C" bse_status_t bse_lanczos_quadrature(bse_handle_t h, const void *dStar
     const int grid = h->num_sms * 2;
     // beta_0^2 = |d|^2 ;  v_0 = d / beta_0
     dot_re_kernel<<<grid, 256, 0, h->stream>>>((const double2 *)dStart, (const double2 *)dStart, n, d_n2);
+    if ((st = comm_bcast_dev(h, d_n2, 1))) return st;
     scale_by_norm_kernel<<<grid, 256, 0, h->stream>>>((const double2 *)dStart, buf[0], n, d_n2);
     count_launch(2);
     int iv = 0, ip = 2, iw = 1;      // v_j, v_{j-1}, w
     for (int j = 0; j < steps; ++j) {
         if ((st = zero_block(h, buf[iw], n, n, 1))) return st;
         if ((st = launch_apply_pass(h, h->R, 0, 1.0, buf[iv], n, buf[iw], n, 1))) return st;       // w = R v_j
+        if ((st = comm_sum_block(h, buf[iw], n, n, 1))) return st;
         // the oracle's order: subtract beta_j v_{j-1} first, alpha_j = Re(v_j^H w) (v_{j-1} is orthogonal to v_j,
         // so the two orders agree to rounding); here alpha is taken first so that one fused pass does both updates
         dot_re_kernel<<<grid, 256, 0, h->stream>>>(buf[iv], buf[iw], n, d_alpha + j);
+        if ((st = comm_bcast_dev(h, d_alpha + j, 1))) return st;
         axpy_norm_kernel<<<grid, 256, 0, h->stream>>>(buf[iw], buf[iv], buf[ip], n, d_alpha + j, j > 0 ? d_n2 + j : nullptr,
                                                       d_n2 + j + 1);
+        if ((st = comm_bcast_dev(h, d_n2 + j + 1, 1))) return st;
         scale_by_norm_kernel<<<grid, 256, 0, h->stream>>>(buf[iw], buf[iw], n, d_n2 + j + 1);
         count_launch(3);
         int t = ip; ip = iv; iv = iw; iw = t;

@@ -77,6 +77,7 @@ struct Solver {
         if (!full) {
             ST(zero_block(h, col(V, c0 + k), ld, n, k));
             ST(launch_apply_pass(h, h->R, 0, 1.0, col(V, c0), ld, col(V, c0 + k), ld, k));
+            ST(comm_sum_block(h, col(V, c0 + k), ld, n, k));
         } else {
             bse_status_t st = bse_apply_half(h, -1, col(PV, c0), ld, col(V, c0 + k), ld, k);      // W = M(p)
             if (st) return st;
@@ -114,7 +115,7 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
                                   bse_info_t *info_out)
 {
     if (!h || nev < 1 || k < 1 || !hOmega || !dVec || !(tol > 0.0) || max_restarts < 0) return BSE_ERR_INVALID_ARG;
-    if (is_partial(h)) return BSE_ERR_INVALID_ARG;
+    if (is_incomplete(h)) return BSE_ERR_INVALID_ARG;
     const int64_t n = h->N;
     const bool full = (h->mode == BSE_MODE_FULL);
     if ((int64_t)nev + k > n || ldvec < (full ? 2 * n : n)) return BSE_ERR_INVALID_ARG;
@@ -205,6 +206,9 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
         nz = std::min(mp, (mp + nwant) / 2 + 1);
         S.assign((size_t)mp * nz, zc(0.0));
         if (host_heev(mp, A.data(), mp, theta.data(), S.data(), mp, nz)) return BSE_ERR_INTERNAL;
+        // sharded operator: rank 0's decomposition is everyone's (the host eigensolver's threaded sums may differ in the last bit)
+        ST(comm_bcast_host(h, theta.data(), sizeof(double) * mp));
+        ST(comm_bcast_host(h, S.data(), sizeof(zc) * (size_t)mp * nz));
         // residual estimates (a10):  r_i = || X_next B s_last,i ||  (Euclidean)
         std::vector<double> E((size_t)k * k, 0.0);   // Re(X_next^H X_next); identity in the TDA case
         if (full) {

@@ -35,7 +35,8 @@ bse_status_t gram_basis(bse_handle_s *h, const void *A, int64_t lda, int m, cons
         count_launch();
     }
     BSE_CUDA(cudaGetLastError());
-    return BSE_OK;
+    // the partial sums were combined with floating-point atomics: on a sharded operator rank 0's result is everyone's
+    return comm_bcast_dev(h, out, (int64_t)ldo * k);
 }
 
 template <int MT, int NT, int WM, int WN>

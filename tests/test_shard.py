@@ -146,3 +146,123 @@ def test_sharded_bse_single_process_many_units(orc):
         sl = b.bse_fill_synthetic_shard(N, 0, 1, 0.0, 16, (rb, re))
         Y += b.Bse(b.MODE_TDA, N, sl, rows=(rb, re)).apply(to_dev(X))
     assert relerr(to_host(Y)[rows], ref) <= 1e-12
+
+
+# ------------------------------------------------- GPU: the solver on a sharded operator, two host processes ----------
+# Both ranks use cuda:0 and exchange through gloo (host-staged): their kernels are ordinary finite launches that never
+# wait on one another -- only the HOSTS meet in collectives -- so sharing the device is safe; it is slow, not a hazard.
+
+def _solver_worker(rank, world, port, q):
+    try:
+        import torch
+        import torch.distributed as dist
+        os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        torch.cuda.set_device(0)
+        dist.init_process_group("gloo", rank=rank, world_size=world)
+        import paper_2504_10096_b200 as b
+        from gpu_util import pack, to_dev, to_host
+        out = {}
+        # TDA: apply, solve, quadrature on rank-local slices of the same packed store
+        N, k, nev = 320, 4, 6
+        R = gen.dense_R(N, 1, sigma=1.0)
+        C = gen.dense_C(N, 1)
+        X = gen.block_X(N, 8, 7)
+
+        def sliced(tiles, storage=b.STORE_C128):
+            rb, re, ft, n, by = b.bse_shard_layout(N, world, rank, storage)
+            per = b.bse_layout(N, storage)[2] // b.bse_layout(N, storage)[1]
+            return (rb, re), tiles[ft * per: ft * per + by]
+        rows, sl = sliced(pack(R, 0))
+        h = b.ShardedBse(b.MODE_TDA, N, sl, None, rows).install_comm()
+        out["tda_apply"] = to_host(h.apply(to_dev(X)))
+        res = h.solve(nev, k, tol=1e-9, seed=1)
+        out["tda_omega"], out["tda_vec"], out["tda_info"] = res.omega, to_host(res.vectors), res.info
+        a, bb = h.lanczos_quadrature(to_dev(X[:, 0]).reshape(-1), 10)
+        out["tda_quad"] = (a, bb)
+        out["tda_calls"] = list(h.comm_calls)
+        # full mode, real-form slices
+        rt, ct = pack(R, 0), pack(C, 1)
+        b.bse_to_real_form(rt, ct, N)
+        (rows, sr), (_, sc) = sliced(rt), sliced(ct)
+        hf = b.ShardedBse(b.MODE_FULL, N, sr, sc, rows, storage=b.STORE_REAL_FORM).install_comm()
+        out["full_half"] = to_host(hf.apply_half(to_dev(X), -1))
+        resf = hf.solve(4, k, tol=1e-9, seed=1)
+        out["full_omega"], out["full_vec"] = resf.omega, to_host(resf.vectors)
+        af, bf = hf.lanczos_quadrature(to_dev(X[:, 1]).reshape(-1), 8)
+        out["full_quad"] = (af, bf)
+        dist.barrier()
+        dist.destroy_process_group()
+        q.put((rank, out))
+    except Exception as e:                                      # report instead of hanging the parent
+        import traceback
+        q.put((rank, {"error": traceback.format_exc()}))
+
+
+@pytest.mark.gpu
+def test_solver_on_a_sharded_operator_two_ranks(orc):
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29700 + os.getpid() % 2000
+    ps = [ctx.Process(target=_solver_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in ps: p.start()
+    got = dict(q.get(timeout=600) for _ in ps)
+    for p in ps: p.join(120)
+    for r in (0, 1):
+        assert "error" not in got[r], got[r].get("error")
+    N, nev = 320, 6
+    R, C = gen.dense_R(N, 1, sigma=1.0), gen.dense_C(N, 1)
+    X = gen.block_X(N, 8, 7)
+    rel = lambda a, b_: np.linalg.norm(a - b_) / np.linalg.norm(b_)
+    for r in (0, 1):
+        o = got[r]
+        assert rel(o["tda_apply"], orc.apply_tda(R, X)) <= 1e-12
+        wj, _ = orc.jacobi_herm(R)
+        assert np.max(np.abs(o["tda_omega"] - wj[:nev]) / np.abs(wj[:nev])) <= 1e-10
+        V = o["tda_vec"]
+        assert np.linalg.norm(V.conj().T @ V - np.eye(nev)) <= 1e-12
+        assert np.max(np.linalg.norm(orc.apply_tda(R, V) - V * o["tda_omega"], axis=0)) <= 1e-8 * 12
+        ao, bo = orc.lanczos_quadrature(R, X[:, 0], 10)
+        assert np.max(np.abs(o["tda_quad"][0] - ao)) <= 1e-10 * 12 and np.max(np.abs(o["tda_quad"][1] - bo)) <= 1e-10 * 30
+        assert rel(o["full_half"], orc.apply_half(R, C, X, -1)) <= 1e-12
+        omd, _ = orc.bse_direct(R, C, want_vectors=False)
+        assert np.max(np.abs(o["full_omega"] - omd[N:N + 4]) / omd[N:N + 4]) <= 1e-10
+        Vf = o["full_vec"]
+        rr = np.linalg.norm(orc.apply_full(R, C, Vf) - Vf * o["full_omega"], axis=0) / np.linalg.norm(Vf, axis=0)
+        assert np.all(rr <= 1e-8 * 12)
+        af, bf = orc.lanczos_quadrature_full(R, C, X[:, 1], 8)
+        assert np.max(np.abs(o["full_quad"][0] - af)) <= 1e-10 * np.max(np.abs(af))
+        assert o["tda_calls"][0] > 0 and o["tda_calls"][1] > 0
+    # lock step: both ranks took the same path and hold bitwise identical results
+    assert got[0]["tda_info"]["n_apply"] == got[1]["tda_info"]["n_apply"]
+    assert got[0]["tda_info"]["n_restart"] == got[1]["tda_info"]["n_restart"]
+    assert np.array_equal(got[0]["tda_omega"], got[1]["tda_omega"]) and np.array_equal(got[0]["tda_vec"], got[1]["tda_vec"])
+    assert np.array_equal(got[0]["full_omega"], got[1]["full_omega"]) and np.array_equal(got[0]["full_vec"], got[1]["full_vec"])
+
+
+@pytest.mark.gpu
+def test_comm_hook_single_rank_counts_and_leaves_results_unchanged(orc):
+    """One rank, no process group needed for the arithmetic: the hook is called after every product and every
+    atomically accumulated quantity, and a one-rank sum / broadcast changes nothing."""
+    import ctypes
+    import paper_2504_10096_b200 as b
+    from gpu_util import pack, to_dev, to_host
+    N, k, nev = 320, 4, 6
+    R = gen.dense_R(N, 1, sigma=1.0)
+    h = b.Bse(b.MODE_TDA, N, pack(R, 0))
+    ref = h.solve(nev, k, tol=1e-9, seed=1)
+    calls = [0, 0]
+    cb = ctypes.CFUNCTYPE(ctypes.c_int32, ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p, ctypes.c_int64)(
+        lambda user, op, ptr, n: (calls.__setitem__(op, calls[op] + 1), 0)[1])
+    assert b.lib().bse_set_comm(h._h, ctypes.cast(cb, ctypes.c_void_p), None) == 0
+    res = h.solve(nev, k, tol=1e-9, seed=1)
+    assert np.max(np.abs(res.omega - ref.omega)) <= 1e-12 and res.info["n_apply"] == ref.info["n_apply"]
+    assert calls[0] == res.info["n_apply"] and calls[1] >= 2 * res.info["n_apply"]
+    # a failing hook aborts the call with an error status instead of continuing on partial data
+    bad = ctypes.CFUNCTYPE(ctypes.c_int32, ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p, ctypes.c_int64)(
+        lambda user, op, ptr, n: 1)
+    b.lib().bse_set_comm(h._h, ctypes.cast(bad, ctypes.c_void_p), None)
+    with pytest.raises(b.BseError):
+        h.apply(to_dev(gen.block_X(N, 2, 3)))
+    b.lib().bse_set_comm(h._h, None, None)
+    assert np.max(np.abs(h.solve(nev, k, tol=1e-9, seed=1).omega - ref.omega)) <= 1e-12
