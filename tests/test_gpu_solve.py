@@ -206,6 +206,10 @@ def test_config3_size_closed_form_pair():
     res = b.Bse(b.MODE_FULL, N, rt, ct).solve(nev, k, tol=1e-8, seed=4)
     exact = np.sort(np.sqrt(d1 * d2))[:nev]
     assert np.max(np.abs(res.omega - exact) / exact) <= TOL_EIG
+    # the same stores in the real form of Eq. (3) (S = R + C, D = R - C), block k = 8
+    b.bse_to_real_form(rt, ct, N)
+    res = b.Bse(b.MODE_FULL, N, rt, ct, storage=b.STORE_REAL_FORM).solve(nev, 8, tol=1e-8, seed=4)
+    assert np.max(np.abs(res.omega - exact) / exact) <= TOL_EIG
 
 
 def test_config4_size_closed_form():
