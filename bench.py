@@ -387,6 +387,41 @@ def run_cuda(args, cfg):
     print(json.dumps(line))
 
 
+def run_solve(spec):
+    """`--solve CFG:K[:NCV[:STORE]]` -- time-to-nev of one bse_solve alone (the second half of BASELINE.json's metric), on
+    the device-generated synthetic operator of BASELINE.json config CFG (2, 3 or 4), block size K, basis size NCV (0 =
+    default), STORE in {c128, c64, real, real64} (real*: the real-form store of DESIGN.md 5.5, full mode only).  Prints
+    one JSON line; profiles/r1_solve.md's rows are runs of this command."""
+    import torch
+    import paper_2504_10096_b200 as b
+    parts = spec.split(":")
+    cid, k = int(parts[0]), int(parts[1])
+    ncv = int(parts[2]) if len(parts) > 2 and parts[2] else 0
+    store = parts[3] if len(parts) > 3 else "c128"
+    cfg = gen.CONFIGS[cid]
+    N, full = cfg["N"], cfg["mode"] == "full"
+    base = b.STORE_C64 if store in ("c64", "real64") else b.STORE_C128
+    torch.cuda.set_device(0)
+    rt = b.bse_fill_synthetic(N, b.MATRIX_R, 1, cfg["sigma"], cfg["group"], storage=base)
+    ct = b.bse_fill_synthetic(N, b.MATRIX_C, 1, 0.0, cfg["group"], storage=base) if full else None
+    storage = base
+    if store.startswith("real"):
+        if not full:
+            raise SystemExit("the real-form store is a full-mode format")
+        b.bse_to_real_form(rt, ct, N, storage=base)
+        storage = b.STORE_REAL_FORM if base == b.STORE_C128 else b.STORE_REAL_FORM_C64
+    h = b.Bse(b.MODE_FULL if full else b.MODE_TDA, N, rt, ct, storage=storage)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    res = h.solve(cfg["nev"], k, ncv=ncv, tol=1e-8, seed=1, raise_on_error=False)
+    torch.cuda.synchronize()
+    sec = time.perf_counter() - t0
+    print(json.dumps({"solve": {"workload": f"config {cid}: {cfg['mode']} N={N} nev={cfg['nev']} k={k} tol=1e-8 sigma={cfg['sigma']}",
+                                "store": store, "seconds": sec, "status": res.status, "info": res.info,
+                                "omega_first": float(res.omega[0]), "omega_last": float(res.omega[-1]),
+                                "max_residual_estimate": float(res.resid.max())}}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -402,7 +437,12 @@ def main():
     ap.add_argument("--ref-rows", type=int, default=1024)
     ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--solve", default=None, metavar="CFG:K[:NCV[:STORE]]",
+                    help="time one bse_solve alone (see run_solve) instead of the apply benchmark")
     args = ap.parse_args()
+    if args.solve:
+        run_solve(args.solve)
+        return
     args.warmup = max(args.warmup, 3)
     global ES
     ES = 16.0 if args.storage == "c128" else 8.0
