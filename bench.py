@@ -389,16 +389,23 @@ def run_cuda(args, cfg):
 
 def run_solve(spec):
     """`--solve CFG:K[:NCV[:STORE]]` -- time-to-nev of one bse_solve alone (the second half of BASELINE.json's metric), on
-    the device-generated synthetic operator of BASELINE.json config CFG (2, 3 or 4), block size K, basis size NCV (0 =
+    the device-generated synthetic operator of BASELINE.json config CFG (2, 3 or 4; or MODE@N@NEV), block size K, basis size NCV (0 =
     default), STORE in {c128, c64, real, real64} (real*: the real-form store of DESIGN.md 5.5, full mode only).  Prints
     one JSON line; profiles/r1_solve.md's rows are runs of this command."""
     import torch
     import paper_2504_10096_b200 as b
     parts = spec.split(":")
-    cid, k = int(parts[0]), int(parts[1])
+    k = int(parts[1])
     ncv = int(parts[2]) if len(parts) > 2 and parts[2] else 0
     store = parts[3] if len(parts) > 3 else "c128"
-    cfg = gen.CONFIGS[cid]
+    if "@" in parts[0]:
+        # MODE@N@NEV: the same generator at another size, e.g. the paper's N = 10368 / 36288 / 103680 with nev = 100
+        # (PAPER.md:115-122, 180); sigma = 1 in full mode (DESIGN.md section 3), group 16
+        mode, n_, nev_ = parts[0].split("@")
+        cid, cfg = parts[0], dict(mode=mode, N=int(n_), group=16, nev=int(nev_), sigma=1.0 if mode == "full" else 0.0)
+    else:
+        cid = int(parts[0])
+        cfg = gen.CONFIGS[cid]
     N, full = cfg["N"], cfg["mode"] == "full"
     base = b.STORE_C64 if store in ("c64", "real64") else b.STORE_C128
     torch.cuda.set_device(0)

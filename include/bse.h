@@ -188,8 +188,11 @@ bse_status_t bse_set_comm(bse_handle_t h, bse_comm_fn fn, void *user);
 /* Y = H X for a block of k >= 1 vectors.
  *   TDA : X, Y are N x k;   Y = R X.
  *   FULL: X, Y are 2N x k, rows [X1; X2];  Y1 = R X1 + C X2,  Y2 = -(C^H X1 + R^* X2).
- * X and Y must not alias.  Asynchronous on the handle's stream.  Each stored tile of R (and C) is
- * read from HBM once per group of 4 columns (TDA) / 2 columns (FULL). */
+ * X and Y must not alias.  Asynchronous on the handle's stream.  TDA: each stored tile of R is read from HBM once
+ * per group of up to 8 columns (one column: plain-FMA kernel; 2..4: four real products per complex product on the
+ * FP64 tensor cores; 5..8: three).  FULL: four such passes per group (R and C, twice), or two half applies on a
+ * real-form store.  On a partial handle (bse_create_shard) the result is that slice's contribution, or the complete
+ * product when a communication hook is installed (bse_set_comm). */
 bse_status_t bse_apply(bse_handle_t h, const void *dX, int64_t ldx, void *dY, int64_t ldy, int32_t k);
 
 /* FULL mode only, N-row half vectors:  Y = R X + sign * C conj(X),  sign = +1 (P) or -1 (M).
