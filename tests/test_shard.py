@@ -266,3 +266,32 @@ def test_comm_hook_single_rank_counts_and_leaves_results_unchanged(orc):
         h.apply(to_dev(gen.block_X(N, 2, 3)))
     b.lib().bse_set_comm(h._h, None, None)
     assert np.max(np.abs(h.solve(nev, k, tol=1e-9, seed=1).omega - ref.omega)) <= 1e-12
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("L", [1, 2, 3, 5, 32])
+def test_unit_length_and_slices_every_kernel(orc, L, monkeypatch):
+    """The unit length L (tiles of one tile row a CTA accumulates before flushing Y_I) is chosen from the operand size;
+    BSE_APPLY_UNIT forces it here so that small matrices exercise multi-tile units, partial last units and slice
+    boundaries that are not multiples of L, for every apply kernel (k = 1 plain FMA, k = 4 four-product, k = 8
+    three-product, real form) and for 1 and 3 slices."""
+    import torch
+    import paper_2504_10096_b200 as b
+    from gpu_util import pack, relerr, to_dev, to_host
+    monkeypatch.setenv("BSE_APPLY_UNIT", str(L))
+    N = 1000
+    R, C = gen.dense_R(1008, 51, sigma=1.0)[:N, :N], gen.dense_C(N, 51)
+    rt, ct = pack(R, 0), pack(C, 1)
+    X = gen.block_X(N, 8, 52)
+    for G in (1, 3):
+        for k in (1, 4, 8):
+            Y = sum(b.Bse(b.MODE_TDA, N, sl, rows=rows).apply(to_dev(X[:, :k])) for rows, sl in _slices(rt, N, G, b.STORE_C128))
+            assert relerr(to_host(Y), orc.apply_tda(R, X[:, :k])) <= 1e-12, (G, k)
+    rs, cs = rt.clone(), ct.clone()
+    b.bse_to_real_form(rs, cs, N)
+    for G in (1, 3):
+        hs = [b.Bse(b.MODE_FULL, N, sr, sc, storage=b.STORE_REAL_FORM, rows=rows)
+              for (rows, sr), (_, sc) in zip(_slices(rs, N, G, b.STORE_C128), _slices(cs, N, G, b.STORE_C128))]
+        for sign in (+1, -1):
+            Y = sum(h.apply_half(to_dev(X), sign) for h in hs)
+            assert relerr(to_host(Y), orc.apply_half(R, C, X, sign)) <= 1e-12, (G, sign)
