@@ -275,6 +275,11 @@ bse_status_t bse_quadrature_resolvent_full(int32_t steps, const double *hAlpha, 
  * if the QL iteration fails. */
 bse_status_t bse_host_heev(int32_t m, void *hA, int32_t lda, double *hW, void *hZ, int32_t ldz, int32_t nz);
 
+/* The same for a REAL symmetric matrix (hA, hZ: doubles) -- the projected matrix of the full-mode iteration is real
+ * symmetric (real coefficients in the inner product Re(x^H P(y))): a quarter of the flops of the complex driver in the
+ * reduction and the back-transformation. */
+bse_status_t bse_host_syev(int32_t m, double *hA, int32_t lda, double *hW, double *hZ, int32_t ldz, int32_t nz);
+
 /* Number of kernels this library has launched on the calling process's device since load (bench.py's
  * "gpu_launches" claim). */
 int64_t bse_launch_count(void);

@@ -62,6 +62,7 @@ _SIGNATURES = {
     "bse_quadrature_resolvent": [_i32, ctypes.POINTER(_dbl), ctypes.POINTER(_dbl), _i32, ctypes.POINTER(_dbl), _dbl, _vp],
     "bse_quadrature_resolvent_full": [_i32, ctypes.POINTER(_dbl), ctypes.POINTER(_dbl), _i32, ctypes.POINTER(_dbl), _dbl, _vp],
     "bse_host_heev": [_i32, _vp, _i32, _vp, _vp, _i32, _i32],
+    "bse_host_syev": [_i32, _vp, _i32, _vp, _vp, _i32, _i32],
     "bse_solve": [_vp, _i32, _i32, _i32, _dbl, _i32, _u64, ctypes.POINTER(_dbl), _vp, _i64, ctypes.POINTER(_dbl),
                   ctypes.POINTER(_Info)],
 }
@@ -388,6 +389,18 @@ def host_heev(A, nz=None):
     w = np.zeros(m)
     Z = np.zeros((m, max(nz, 1)), dtype=np.complex128, order="F")
     _check(lib().bse_host_heev(m, a.ctypes.data, m, w.ctypes.data, Z.ctypes.data, m, nz), "bse_host_heev")
+    return w, Z[:, :nz]
+
+
+def host_syev(A, nz=None):
+    """Host utility: eigenvalues (ascending) and first nz eigenvectors of a REAL symmetric numpy matrix."""
+    import numpy as np
+    m = A.shape[0]
+    nz = m if nz is None else nz
+    a = np.asfortranarray(A, dtype=np.float64).copy(order="F")
+    w = np.zeros(m)
+    Z = np.zeros((m, max(nz, 1)), dtype=np.float64, order="F")
+    _check(lib().bse_host_syev(m, a.ctypes.data, m, w.ctypes.data, Z.ctypes.data, m, nz), "bse_host_syev")
     return w, Z[:, :nz]
 
 

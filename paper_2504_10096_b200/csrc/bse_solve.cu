@@ -200,12 +200,21 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
         // ---- Rayleigh-Ritz on the projected matrix (a8)
         double t2 = now_s();
         const int mp = s.mp;
-        A.assign((size_t)mp * mp, zc(0.0));
-        for (int j = 0; j < mp; ++j)
-            for (int i = 0; i < mp; ++i) A[i + (size_t)j * mp] = s.T[i + (size_t)j * ldT];
         nz = std::min(mp, (mp + nwant) / 2 + 1);
         S.assign((size_t)mp * nz, zc(0.0));
-        if (host_heev(mp, A.data(), mp, theta.data(), S.data(), mp, nz)) return BSE_ERR_INTERNAL;
+        if (full) {
+            // real coefficients (reading S4): T is real symmetric -> the real driver, a quarter of the reduction flops
+            std::vector<double> Ar((size_t)mp * mp), Sr((size_t)mp * nz);
+            for (int j = 0; j < mp; ++j)
+                for (int i = 0; i < mp; ++i) Ar[i + (size_t)j * mp] = s.T[i + (size_t)j * ldT].real();
+            if (host_syev(mp, Ar.data(), mp, theta.data(), Sr.data(), mp, nz)) return BSE_ERR_INTERNAL;
+            for (size_t q = 0; q < Sr.size(); ++q) S[q] = zc(Sr[q], 0.0);
+        } else {
+            A.assign((size_t)mp * mp, zc(0.0));
+            for (int j = 0; j < mp; ++j)
+                for (int i = 0; i < mp; ++i) A[i + (size_t)j * mp] = s.T[i + (size_t)j * ldT];
+            if (host_heev(mp, A.data(), mp, theta.data(), S.data(), mp, nz)) return BSE_ERR_INTERNAL;
+        }
         // sharded operator: rank 0's decomposition is everyone's (the host eigensolver's threaded sums may differ in the last bit)
         ST(comm_bcast_host(h, theta.data(), sizeof(double) * mp));
         ST(comm_bcast_host(h, S.data(), sizeof(zc) * (size_t)mp * nz));

@@ -130,6 +130,71 @@ BSE_CLONES void reflect_columns(int lo, int m, const double *vi, double taur, do
 }
 }  // namespace
 
+// Implicit QL on the real symmetric tridiagonal (d, e) with the rotations accumulated in Zr (real m x m) stored in
+// panels of RP rows, Zb[(panel * m + column) * RP + row_in_panel]; eigenvalues sorted ascending into w, ord = the
+// permutation.  Shared by the complex Hermitian and the real symmetric driver.  Returns 0, or >0 if QL failed.
+static int tridiag_ql(int m, std::vector<double> &d, std::vector<double> &e, std::vector<double> &Zb, std::vector<int> &ord,
+                      double *w)
+{
+    // ---- implicit QL on (d, e) with the rotations accumulated in Zr (real m x m), stored in panels of RP rows:
+    //      Zb[(panel * m + column) * RP + row_in_panel]
+    const int npan = (m + RP - 1) / RP;
+    Zb.assign((size_t)npan * m * RP, 0.0);
+    for (int i = 0; i < m; ++i) Zb[((size_t)(i / RP) * m + i) * RP + i % RP] = 1.0;
+    std::vector<double> rc(m), rs(m);
+    int fail = 0;
+    for (int l = 0; l < m; ++l) {
+        int iter = 0;
+        while (true) {
+            int mm = l;
+            for (; mm < m - 1; ++mm) {
+                double dd = std::fabs(d[mm]) + std::fabs(d[mm + 1]);
+                if (std::fabs(e[mm]) <= 2.3e-16 * dd) break;
+            }
+            if (mm == l) break;
+            if (++iter > 80) { fail = l + 1; break; }
+            double gg = (d[l + 1] - d[l]) / (2.0 * e[l]);
+            double r = std::hypot(gg, 1.0);
+            gg = d[mm] - d[l] + e[l] / (gg + std::copysign(r, gg));
+            double s = 1.0, c = 1.0, p = 0.0;
+            int i;
+            bool under = false;
+            for (i = mm - 1; i >= l; --i) {
+                double f = s * e[i], b = c * e[i];
+                r = std::hypot(f, gg);
+                e[i + 1] = r;
+                if (r == 0.0) { d[i + 1] -= p; e[mm] = 0.0; under = true; break; }
+                s = f / r; c = gg / r;
+                gg = d[i + 1] - p;
+                r = (d[i] - gg) * s + 2.0 * c * b;
+                p = s * r;
+                d[i + 1] = gg + p;
+                gg = c * r - b;
+                rc[i] = c; rs[i] = s;
+            }
+            const int ilo = under ? i + 1 : l;
+            // apply the recorded rotations (q = mm-1 down to ilo) to columns (q, q+1): z[q+1] = s z[q] + c f,
+            // z[q] = c z[q] - s f with f the old z[q+1]; the new z[q] is the next step's f and stays in registers
+            if (mm - 1 >= ilo) {
+                const int64_t work = (int64_t)(mm - ilo) * m;
+#pragma omp parallel for schedule(static) if (work > 32768)
+                for (int pn = 0; pn < npan; ++pn) rotate_panel(&Zb[(size_t)pn * m * RP], mm, ilo, rc.data(), rs.data());
+            }
+            if (under) continue;
+            d[l] -= p;
+            e[l] = gg;
+            e[mm] = 0.0;
+        }
+        if (fail) break;
+    }
+    // ---- sort ascending
+    ord.resize(m);
+    std::iota(ord.begin(), ord.end(), 0);
+    std::sort(ord.begin(), ord.end(), [&](int p, int q) { return d[p] < d[q]; });
+    for (int i = 0; i < m; ++i) w[i] = d[ord[i]];
+    return fail;
+}
+
 // A (column-major, lda, lower triangle referenced and destroyed).  Returns 0, or >0 if QL failed to converge.
 int host_heev(int m, void *A_, int lda, double *w, void *Z_, int ldz, int nz)
 {
@@ -199,62 +264,9 @@ int host_heev(int m, void *A_, int lda, double *w, void *Z_, int ldz, int nz)
     }
     d[m - 1] = a(m - 1, m - 1).real();
 
-    // ---- implicit QL on (d, e) with the rotations accumulated in Zr (real m x m), stored in panels of RP rows:
-    //      Zb[(panel * m + column) * RP + row_in_panel]
-    const int npan = (m + RP - 1) / RP;
-    std::vector<double> Zb((size_t)npan * m * RP, 0.0);
-    for (int i = 0; i < m; ++i) Zb[((size_t)(i / RP) * m + i) * RP + i % RP] = 1.0;
-    std::vector<double> rc(m), rs(m);
-    int fail = 0;
-    for (int l = 0; l < m; ++l) {
-        int iter = 0;
-        while (true) {
-            int mm = l;
-            for (; mm < m - 1; ++mm) {
-                double dd = std::fabs(d[mm]) + std::fabs(d[mm + 1]);
-                if (std::fabs(e[mm]) <= 2.3e-16 * dd) break;
-            }
-            if (mm == l) break;
-            if (++iter > 80) { fail = l + 1; break; }
-            double gg = (d[l + 1] - d[l]) / (2.0 * e[l]);
-            double r = std::hypot(gg, 1.0);
-            gg = d[mm] - d[l] + e[l] / (gg + std::copysign(r, gg));
-            double s = 1.0, c = 1.0, p = 0.0;
-            int i;
-            bool under = false;
-            for (i = mm - 1; i >= l; --i) {
-                double f = s * e[i], b = c * e[i];
-                r = std::hypot(f, gg);
-                e[i + 1] = r;
-                if (r == 0.0) { d[i + 1] -= p; e[mm] = 0.0; under = true; break; }
-                s = f / r; c = gg / r;
-                gg = d[i + 1] - p;
-                r = (d[i] - gg) * s + 2.0 * c * b;
-                p = s * r;
-                d[i + 1] = gg + p;
-                gg = c * r - b;
-                rc[i] = c; rs[i] = s;
-            }
-            const int ilo = under ? i + 1 : l;
-            // apply the recorded rotations (q = mm-1 down to ilo) to columns (q, q+1): z[q+1] = s z[q] + c f,
-            // z[q] = c z[q] - s f with f the old z[q+1]; the new z[q] is the next step's f and stays in registers
-            if (mm - 1 >= ilo) {
-                const int64_t work = (int64_t)(mm - ilo) * m;
-#pragma omp parallel for schedule(static) if (work > 32768)
-                for (int pn = 0; pn < npan; ++pn) rotate_panel(&Zb[(size_t)pn * m * RP], mm, ilo, rc.data(), rs.data());
-            }
-            if (under) continue;
-            d[l] -= p;
-            e[l] = gg;
-            e[mm] = 0.0;
-        }
-        if (fail) break;
-    }
-    // ---- sort ascending
-    std::vector<int> ord(m);
-    std::iota(ord.begin(), ord.end(), 0);
-    std::sort(ord.begin(), ord.end(), [&](int p, int q) { return d[p] < d[q]; });
-    for (int i = 0; i < m; ++i) w[i] = d[ord[i]];
+    std::vector<double> Zb;
+    std::vector<int> ord;
+    const int fail = tridiag_ql(m, d, e, Zb, ord, w);
     if (nz <= 0 || !Z) return fail;
 
     // ---- Z = Q * Zr[:, ord[0..nz)]:  start from the real eigenvectors and apply H_{m-2} ... H_0 from the left,
@@ -274,6 +286,129 @@ int host_heev(int m, void *A_, int lda, double *w, void *Z_, int ldz, int nz)
             if (tau[i] == zc(0.0)) continue;
             // v_r = A[r, i], r = i+1 .. m-1 (v_{i+1} = 1 stored)
             reflect_columns(i + 1, m, reinterpret_cast<const double *>(&a(0, i)), tau[i].real(), tau[i].imag(), zd, nb);
+        }
+    }
+    return fail;
+}
+
+
+// ------------------------------------------------------------------------------------------------------------------
+// Real symmetric variant (full mode: the projected matrix of the structure-preserving iteration is real symmetric,
+// SURVEY.md 8(a) a8): the same three stages in real arithmetic -- a quarter of the flops of the complex driver in the
+// reduction and the back-transformation, the same QL.
+// ------------------------------------------------------------------------------------------------------------------
+namespace {
+BSE_CLONES void sym_matvec_columns(int n, const double *A22, int64_t ld, const double *v, double *xl, int c0, int cs)
+{
+    for (int c = c0; c < n; c += cs) {
+        const double *col = A22 + (int64_t)c * ld;
+        const double vc = v[c];
+        double sr = 0.0;
+        xl[c] += col[c] * vc;
+#pragma omp simd reduction(+ : sr)
+        for (int r = c + 1; r < n; ++r) {
+            xl[r] += col[r] * vc;
+            sr += col[r] * v[r];
+        }
+        xl[c] += sr;
+    }
+}
+BSE_CLONES void rank2_update_columns_real(int n, double *A22, int64_t ld, const double *v, const double *x, int c0, int c1)
+{
+    for (int c = c0; c < c1; ++c) {
+        double *col = A22 + (int64_t)c * ld;
+        const double wc = x[c], vc = v[c];
+#pragma omp simd
+        for (int r = c; r < n; ++r) col[r] -= v[r] * wc + x[r] * vc;
+    }
+}
+BSE_CLONES void reflect_columns_real(int lo, int m, const double *vi, double tau, double *const *zcol, int nb)
+{
+    for (int jj = 0; jj < nb; ++jj) {
+        double *z = zcol[jj];
+        double a = 0.0;
+#pragma omp simd reduction(+ : a)
+        for (int r = lo; r < m; ++r) a += vi[r] * z[r];
+        const double p = tau * a;
+#pragma omp simd
+        for (int r = lo; r < m; ++r) z[r] -= vi[r] * p;
+    }
+}
+}  // namespace
+
+// A (real, column-major, lda, lower triangle referenced and destroyed); Z real m x nz.  Returns 0, or >0 if QL failed.
+int host_syev(int m, double *A, int lda, double *w, double *Z, int ldz, int nz)
+{
+    if (m <= 0) return 0;
+    if (nz > m) nz = m;
+    std::vector<double> d(m), e(m, 0.0), tau(m, 0.0);
+    auto a = [&](int i, int j) -> double & { return A[i + (int64_t)j * lda]; };
+    const int nth = max_threads();
+    std::vector<double> x(m), v(m), xt((size_t)nth * m);
+    for (int i = 0; i < m - 1; ++i) {
+        const int n = m - i - 1;
+        const double alpha = a(i + 1, i);
+        double xnorm2 = 0.0;
+        for (int r = i + 2; r < m; ++r) xnorm2 += a(r, i) * a(r, i);
+        double t = 0.0, beta = alpha;
+        if (xnorm2 != 0.0) {
+            beta = -std::copysign(std::sqrt(alpha * alpha + xnorm2), alpha);
+            t = (beta - alpha) / beta;
+            const double sc = 1.0 / (alpha - beta);
+            for (int r = i + 2; r < m; ++r) a(r, i) *= sc;
+        }
+        e[i] = beta;
+        tau[i] = t;
+        a(i + 1, i) = 1.0;
+        if (t != 0.0) {
+            for (int r = 0; r < n; ++r) v[r] = a(i + 1 + r, i);
+            const bool par = n > 256 && nth > 1;
+            int nt_act = 1;
+#pragma omp parallel num_threads(nth) if (par)
+            {
+#ifdef _OPENMP
+                const int tid = omp_get_thread_num(), team = omp_get_num_threads();
+#else
+                const int tid = 0, team = 1;
+#endif
+                if (tid == 0) nt_act = team;
+                double *xl = &xt[(size_t)tid * m];
+                for (int r = 0; r < n; ++r) xl[r] = 0.0;
+                sym_matvec_columns(n, &a(i + 1, i + 1), lda, v.data(), xl, tid, team);
+            }
+            double dot = 0.0;
+            for (int r = 0; r < n; ++r) {
+                double s = 0.0;
+                for (int q = 0; q < nt_act; ++q) s += xt[(size_t)q * m + r];
+                x[r] = t * s;
+                dot += x[r] * v[r];
+            }
+            const double al = -0.5 * t * dot;
+            for (int r = 0; r < n; ++r) x[r] += al * v[r];
+#pragma omp parallel for schedule(static, 1) if (par)
+            for (int c0 = 0; c0 < n; c0 += 8)
+                rank2_update_columns_real(n, &a(i + 1, i + 1), lda, v.data(), x.data(), c0, std::min(c0 + 8, n));
+        }
+        d[i] = a(i, i);
+    }
+    d[m - 1] = a(m - 1, m - 1);
+
+    std::vector<double> Zb;
+    std::vector<int> ord;
+    const int fail = tridiag_ql(m, d, e, Zb, ord, w);
+    if (nz <= 0 || !Z) return fail;
+#pragma omp parallel for schedule(dynamic, 1) if (m > 64)
+    for (int j0 = 0; j0 < nz; j0 += JB) {
+        const int nb = std::min(JB, nz - j0);
+        double *zcol[JB];
+        for (int jj = 0; jj < nb; ++jj) {
+            zcol[jj] = Z + (int64_t)(j0 + jj) * ldz;
+            const int src = ord[j0 + jj];
+            for (int i = 0; i < m; ++i) zcol[jj][i] = Zb[((size_t)(i / RP) * m + src) * RP + i % RP];
+        }
+        for (int i = m - 2; i >= 0; --i) {
+            if (tau[i] == 0.0) continue;
+            reflect_columns_real(i + 1, m, &a(0, i), tau[i], zcol, nb);
         }
     }
     return fail;

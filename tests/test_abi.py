@@ -87,6 +87,38 @@ def test_host_heev_arrowhead_and_clusters(b):
     assert np.linalg.norm(Tr @ Z2 - Z2 * w2[:6]) < 1e-12 and np.max(np.abs(Z2.imag)) < 1e-13
 
 
+@pytest.mark.parametrize("m", [1, 2, 7, 40, 150, 600])
+def test_host_syev_matches_numpy(b, m):
+    # the real symmetric driver used for the full-mode projected matrix (include/bse.h: bse_host_syev)
+    A = gen.block_X(m, m, m + 1).real
+    A = (A + A.T) / 2
+    nz = m if m < 600 else 200
+    w, Z = b.host_syev(A, nz=nz)
+    ref = np.linalg.eigvalsh(A)
+    scale = max(np.max(np.abs(ref)), 1.0)
+    assert np.max(np.abs(w - ref)) < 1e-13 * scale * max(m, 8)
+    assert np.linalg.norm(Z.T @ Z - np.eye(nz)) < 1e-12 * max(1, m / 50)
+    assert np.linalg.norm(A @ Z - Z * w[:nz]) < 1e-12 * scale * m
+    # the strictly upper triangle is never read
+    A2 = np.tril(A) + np.triu(np.full((m, m), 7.0), 1)
+    w2, _ = b.host_syev(A2, nz=0)
+    assert np.array_equal(w2, w)
+
+
+def test_host_syev_arrowhead_with_pairs_agrees_with_heev(b):
+    # full-mode projected matrix after a thick restart: paired Ritz values on the diagonal, a real border block
+    l, k = 40, 8
+    T = np.zeros((l + k, l + k))
+    T[np.arange(l), np.arange(l)] = np.repeat(np.linspace(0.3, 0.6, l // 2), 2)
+    Bk = gen.block_X(k, l, 5).real * 1e-4
+    T[l:, :l] = Bk; T[:l, l:] = Bk.T
+    D = gen.block_X(k, k, 6).real; T[l:, l:] = (D + D.T) / 2 + 4 * np.eye(k)
+    w, Z = b.host_syev(T, nz=l)
+    wh, _ = b.host_heev(T.astype(complex), nz=0)
+    assert np.max(np.abs(w - np.linalg.eigvalsh(T))) < 1e-13 * 10 and np.max(np.abs(w - wh)) < 1e-13 * 10
+    assert np.linalg.norm(T @ Z - Z * w[:l]) < 1e-12 and np.linalg.norm(Z.T @ Z - np.eye(l)) < 1e-12
+
+
 def test_quadrature_resolvent_host_utility_matches_oracle(b, orc):
     # host logic only: the continued fraction of a Jacobi matrix, against the oracle's and against (z - T)^-1 directly
     m = 17
