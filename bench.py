@@ -189,7 +189,12 @@ def run_cuda(args, cfg):
     sampler = ClockSampler(local)
     sampler.start()
     t_wait = time.time()
-    while not sampler.rows and time.time() - t_wait < 5.0:      # nvidia-smi takes a moment to start
+    if shard:
+        # every apply contains a collective: all ranks must issue the same number of them, so no rank-local stop rule
+        for _ in range(max(20, int(1.5e3 / max(1.0, alg_bytes(N, k) / world / 6.5e9)))):
+            h.apply(X, Y)
+        torch.cuda.synchronize()
+    while not shard and not sampler.rows and time.time() - t_wait < 5.0:      # nvidia-smi takes a moment to start
         h.apply(X, Y)
         torch.cuda.synchronize()
     n_before = len(sampler.rows)
@@ -197,7 +202,11 @@ def run_cuda(args, cfg):
     ms = time_steps(lambda: h.apply(X, Y), args.steps, args.warmup)
     launches = (b.launch_count() - l0) * args.steps // (args.steps + args.warmup)
     t_wait = time.time()
-    while len(sampler.rows) < n_before + 5 and time.time() - t_wait < 3.0:   # same load until >= 5 samples under load
+    if shard:
+        for _ in range(max(20, int(1.5e3 / max(1.0, alg_bytes(N, k) / world / 6.5e9)))):     # ~1.5 s of the same load
+            h.apply(X, Y)
+        torch.cuda.synchronize()
+    while not shard and len(sampler.rows) < n_before + 5 and time.time() - t_wait < 3.0:   # same load until >= 5 samples
         h.apply(X, Y)
         torch.cuda.synchronize()
     sampler.rows = sampler.rows[n_before:] if len(sampler.rows) > n_before else sampler.rows
@@ -263,7 +272,7 @@ def run_cuda(args, cfg):
     # pipe executes 6 N^2 k flops for the 8 N^2 k algorithmic ones of SURVEY.md 8(d) that `achieved` counts.
     three_m = 5 <= k <= 8
     roof.update({"kernel": "bse::apply_tiles_k1_kernel" if k == 1 else
-                 ("bse::apply_tiles_3m_kernel" if three_m else "bse::apply_tiles_kernel"),
+                 ("bse::apply_tiles_3m_kernel" if three_m else "bse::apply_tiles_rs_kernel"),
                  "tflops_fp64": tflops, "tflops_fp64_executed": tflops * (0.75 if three_m else 1.0),
                  "fp64_peak_measured_tflops": fp64_peak, "GBps": achieved})
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

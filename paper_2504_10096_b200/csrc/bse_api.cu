@@ -8,6 +8,7 @@
 #include "apply_kernel_k1.cuh"
 #include "apply_kernel_3m.cuh"
 #include "apply_kernel_real.cuh"
+#include "apply_kernel_rs.cuh"
 #include "bse_internal.h"
 #include "tile_layout.cuh"
 
@@ -64,6 +65,8 @@ static bse_status_t apply_kernel_attributes()
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<16, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<8, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_rs_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_rs_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_kernel<16, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_kernel<16, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_kernel<8, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
@@ -173,6 +176,8 @@ bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, dou
     p.ldy = ldy;
     bool use_wide = true;                              // BSE_APPLY_WIDE=0: 4-column passes only
     if (const char *e = getenv("BSE_APPLY_WIDE")) use_wide = atoi(e) != 0;
+    bool use_rs = true;                                // BSE_APPLY_RS=0: all-roles-per-warp form for 2 .. 4 columns (apply_kernel.cuh)
+    if (const char *e = getenv("BSE_APPLY_RS")) use_rs = atoi(e) != 0;
     bool use_3m = true;                                // BSE_APPLY_3M=0: four-product form for 5 .. 8 columns
     if (const char *e = getenv("BSE_APPLY_3M")) use_3m = atoi(e) != 0;
     for (int32_t c0 = 0; c0 < k;) {
@@ -186,11 +191,13 @@ bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, dou
             if (k1) apply_tiles_k1_kernel<16, 8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
             else if (wide && use_3m) apply_tiles_3m_kernel<16><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
             else if (wide) apply_tiles_kernel<16, 2><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            else if (use_rs) apply_tiles_rs_kernel<16><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
             else apply_tiles_kernel<16, 1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
         } else {
             if (k1) apply_tiles_k1_kernel<8, 8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
             else if (wide && use_3m) apply_tiles_3m_kernel<8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
             else if (wide) apply_tiles_kernel<8, 2><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            else if (use_rs) apply_tiles_rs_kernel<8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
             else apply_tiles_kernel<8, 1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
         }
         count_launch();

@@ -303,6 +303,27 @@ def test_wide_and_narrow_column_passes_agree_with_oracle(orc, k, monkeypatch):
         assert launches == passes
 
 
+@pytest.mark.parametrize("k", [2, 3, 4])
+def test_role_split_and_all_roles_kernels_agree_with_oracle(orc, k, monkeypatch):
+    """2..4 columns: the default is the role-split kernel (apply_kernel_rs.cuh); BSE_APPLY_RS=0 selects the
+    all-roles-per-warp kernel (apply_kernel.cuh).  Both against the oracle: TDA (HERM pass), full mode (HERM + SYMC passes,
+    both signs), complex128 and complex64 stores, a ragged size with several units per CTA."""
+    import paper_2504_10096_b200 as b
+    N = 2000
+    R, C = gen.dense_R(N, 31, sigma=1.0), gen.dense_C(N, 31)
+    X = gen.block_X(N, k, 33)
+    refs = {b.STORE_C128: (R, C), b.STORE_C64: (orc.round_c64(R), orc.round_c64(C))}
+    for storage, (Rs, Cs) in refs.items():
+        rt = b.bse_pack_from_dense(to_dev(R), N, 0, storage=storage)
+        ct = b.bse_pack_from_dense(to_dev(C), N, 1, storage=storage)
+        ht, hf = b.Bse(b.MODE_TDA, N, rt, storage=storage), b.Bse(b.MODE_FULL, N, rt, ct, storage=storage)
+        for rs in ("1", "0"):
+            monkeypatch.setenv("BSE_APPLY_RS", rs)
+            assert relerr(to_host(ht.apply(to_dev(X))), orc.apply_tda(Rs, X)) <= TOL_APPLY, (storage, rs)
+            for sign in (+1, -1):
+                assert relerr(to_host(hf.apply_half(to_dev(X), sign)), orc.apply_half(Rs, Cs, X, sign)) <= TOL_APPLY
+
+
 @pytest.mark.parametrize("kind", ["real_x", "imag_x", "real_T", "imag_T", "one_column_dominant"])
 def test_three_product_form_special_operands(orc, kind):
     """The 5..8-column kernel forms re/im from Q1 = Tr xr, Q2 = Ti xi, Q3 = (Tr + Ti)(xr +- xi): operands for which one
