@@ -353,3 +353,27 @@ def test_three_product_form_special_operands(orc, kind):
             assert relerr(Y[:, c], ref[:, c]) <= TOL_APPLY
     ht = b.Bse(b.MODE_TDA, N, pack(R, 0))
     assert relerr(to_host(ht.apply(to_dev(x))), orc.apply_tda(R, x)) <= TOL_APPLY
+
+
+@pytest.mark.parametrize("k", [4, 8])
+def test_repeated_launches_stay_within_rounding_of_each_other(k):
+    """Timing-dependent faults (the round-1 shared-memory WAR hazard corrupted about one 8-row group per launch) show up
+    as an entry that differs from the other launches by far more than the summation-order noise of the RED flushes:
+    200 launches of the role-split (k = 4) and three-product (k = 8) kernels and of the real-form kernel, many units per
+    CTA, every entry compared with the first launch."""
+    import torch
+    import paper_2504_10096_b200 as b
+    N = 8192
+    rt, ct = b.bse_fill_synthetic(N, 0, 1, 1.0, 16), b.bse_fill_synthetic(N, 1, 1, 0.0, 16)
+    X = torch.randn(k, N, dtype=torch.complex128, device="cuda", generator=torch.Generator("cuda").manual_seed(5))
+    ht = b.Bse(b.MODE_TDA, N, rt)
+    ref = ht.apply(X).clone()
+    scale = float(ref.abs().max())
+    worst = max(float((ht.apply(X) - ref).abs().max()) for _ in range(200))
+    assert worst <= 1e-13 * scale
+    del ht
+    b.bse_to_real_form(rt, ct, N)
+    hr = b.Bse(b.MODE_FULL, N, rt, ct, storage=b.STORE_REAL_FORM)
+    ref = hr.apply_half(X, -1).clone()
+    worst = max(float((hr.apply_half(X, -1) - ref).abs().max()) for _ in range(200))
+    assert worst <= 1e-13 * float(ref.abs().max())
