@@ -232,7 +232,8 @@ bse_status_t bse_orth(bse_handle_t h, const void *dV, int64_t ldv, int32_t m, co
  *   FULL: the nev smallest positive omega of H, ascending, and right eigenvectors [X_I; Y_I]
  *         (2N x nev) normalised X^H X - Y^H Y = 1.  The -omega partner is [conj(Y); conj(X)].
  *   k    : block size (>= 1; >= 2 recommended in full mode);  ncv: maximum basis
- *          size, 0 -> default max(2 nev, nev + 15) (doubled in full mode), rounded up to a multiple of k;
+ *          size, 0 -> default max(2 nev, nev + 15) (doubled in full mode) and at least (wanted Ritz values) + 8 k,
+ *          rounded up to a multiple of k;
  *   tol  : a Ritz pair is converged when ||H v - w v||_2 <= tol * ||H||_est * ||v||_2;
  *   hOmega: nev doubles (host);  hResid: nev doubles (host, nullable): the residual estimates;
  *   info : nullable.

@@ -124,6 +124,9 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
     if (ncv <= 0) {
         ncv = std::max(2 * nev, nev + 15);
         if (full) ncv *= 2;
+        // a wide block needs room to iterate between restarts: with fewer than ~8 block steps per cycle the thick restart
+        // stagnates (full mode, nev = 16, k = 8, ncv = 64: 889 restarts; ncv = 160: 46)
+        ncv = std::max(ncv, nwant + 8 * k);
     }
     ncv = ((ncv + k - 1) / k) * k;
     if ((int64_t)ncv + k > dim) ncv = (int)(((dim - k) / k) * k);

@@ -208,7 +208,9 @@ def test_config3_size_closed_form_pair():
     assert np.max(np.abs(res.omega - exact) / exact) <= TOL_EIG
     # the same stores in the real form of Eq. (3) (S = R + C, D = R - C), block k = 8
     b.bse_to_real_form(rt, ct, N)
-    res = b.Bse(b.MODE_FULL, N, rt, ct, storage=b.STORE_REAL_FORM).solve(nev, 8, tol=1e-8, seed=4)
+    # (ncv = 160: with the default basis of 64 columns a block of 8 leaves two to four block steps per restart cycle and the
+    # run needs close to the 1000 restarts allowed -- it then passes or fails with the summation order of the atomics)
+    res = b.Bse(b.MODE_FULL, N, rt, ct, storage=b.STORE_REAL_FORM).solve(nev, 8, ncv=160, tol=1e-8, seed=4)
     assert np.max(np.abs(res.omega - exact) / exact) <= TOL_EIG
 
 
