@@ -277,7 +277,9 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
         }
         // ---- thick restart (a9): keep l Ritz vectors and the residual block
         double t3 = now_s();
-        int l = std::min(nconv, nwant) + (mp - std::min(nconv, nwant)) / 2;
+        double keep = 0.5;                                   // fraction of the unconverged part of the basis kept (reading S6)
+        if (const char *e = getenv("BSE_KEEP_FRACTION")) { double v = atof(e); if (v > 0.05 && v < 0.95) keep = v; }
+        int l = std::min(nconv, nwant) + (int)((mp - std::min(nconv, nwant)) * keep);
         l = std::max(l, std::min(nwant, nz));
         l = std::min(l, std::min(nz, ncv - k));
         ST(s.rotate(s.V, mp, S.data(), mp, l, s.rot.p, n));
