@@ -438,6 +438,32 @@ def run_solve(spec):
                                 "max_residual_estimate": float(res.resid.max())}}))
 
 
+def run_slices(args, cfg):
+    """`--slices G` -- the G partial handles of a G-way partition of the timed operand, run ONE AFTER
+    ANOTHER on this GPU: per-slice apply time (what each of G GPUs would spend in its local kernel, before the all-reduce
+    of 16 N k bytes).  One JSON line; no multi-GPU claim."""
+    import torch
+    import paper_2504_10096_b200 as b
+    torch.cuda.set_device(0)
+    N, k = cfg["N"], args.k
+    storage = b.STORE_C128 if ES == 16.0 else b.STORE_C64
+    tiles = b.bse_fill_synthetic(N, b.MATRIX_R, 1, 0.0, cfg["group"], storage=storage)
+    per = b.bse_layout(N, storage)[2] // b.bse_layout(N, storage)[1]
+    X = torch.randn(k, N, dtype=torch.complex128, device="cuda")
+    Y = torch.empty_like(X)
+    out = {}
+    for G in sorted({1, args.slices}):
+        ms = []
+        for r in range(G):
+            rb, re, ft, n, by = b.bse_shard_layout(N, G, r, storage)
+            h = b.Bse(b.MODE_TDA, N, tiles[ft * per: ft * per + max(by, 1)], storage=storage, rows=(rb, re))
+            ms.append(time_steps(lambda: h.apply(X, Y), args.steps, args.warmup))
+        out[str(G)] = {"ms_per_slice": ms, "max_ms": max(ms), "sum_ms": sum(ms)}
+    whole = out["1"]["max_ms"]
+    print(json.dumps({"slices": {"workload": workload(cfg, k), "per_partition": out,
+                                 "balance": whole / (args.slices * out[str(args.slices)]["max_ms"])}}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -455,6 +481,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--solve", default=None, metavar="CFG:K[:NCV[:STORE]]",
                     help="time one bse_solve alone (see run_solve) instead of the apply benchmark")
+    ap.add_argument("--slices", type=int, default=0, metavar="G",
+                    help="time the G partial handles of a G-way partition one after another on this GPU (see run_slices)")
     args = ap.parse_args()
     if args.solve:
         run_solve(args.solve)
@@ -465,7 +493,9 @@ def main():
     cfg = dict(gen.CONFIGS[args.config], id=args.config)
     if cfg["mode"] != "tda":
         raise SystemExit("bench.py times the TDA apply; full-mode configs are parity-test cases")
-    if args.impl == "reference":
+    if args.slices > 0:
+        run_slices(args, cfg)
+    elif args.impl == "reference":
         run_reference(args, cfg)
     else:
         run_cuda(args, cfg)
