@@ -67,6 +67,10 @@ static bse_status_t apply_kernel_attributes()
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<8, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_rs_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_rs_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_k1_kernel<16, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_k1_kernel<16, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_k1_kernel<8, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_k1_kernel<8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_kernel<16, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_kernel<16, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
         BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_kernel<8, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
@@ -142,15 +146,22 @@ bse_status_t launch_real_pass(bse_handle_s *h, const char *tiles, int mode, cons
     p.sign = 1.0;
     p.ldx = ldx;
     p.ldy = ldy;
+    bool use_k1 = true;                                // BSE_APPLY_K1=0: tensor-core kernel for single columns too
+    if (const char *e = getenv("BSE_APPLY_K1")) use_k1 = atoi(e) != 0;
     for (int32_t c0 = 0; c0 < k; c0 += 8) {
         p.kc = k - c0 < 8 ? k - c0 : 8;
         p.X = reinterpret_cast<const double2 *>(dX) + (int64_t)c0 * ldx;
         p.Y = reinterpret_cast<double *>(dY) + 2 * (int64_t)c0 * ldy;
+        const bool k1 = p.kc == 1 && use_k1;                  // plain-FMA single-column variant
         if (h->es == ES_C128) {
-            if (mode == 0) apply_tiles_real_kernel<16, 0><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            if (k1 && mode == 0) apply_tiles_real_k1_kernel<16, 0><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            else if (k1) apply_tiles_real_k1_kernel<16, 1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            else if (mode == 0) apply_tiles_real_kernel<16, 0><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
             else apply_tiles_real_kernel<16, 1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
         } else {
-            if (mode == 0) apply_tiles_real_kernel<8, 0><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            if (k1 && mode == 0) apply_tiles_real_k1_kernel<8, 0><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            else if (k1) apply_tiles_real_k1_kernel<8, 1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
+            else if (mode == 0) apply_tiles_real_kernel<8, 0><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
             else apply_tiles_real_kernel<8, 1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
         }
         count_launch();
