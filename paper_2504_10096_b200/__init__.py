@@ -207,6 +207,8 @@ class Bse:
         self.mode, self.N, self.storage, self.rows = mode, N, storage, rows
         self._keep = (r_tiles, c_tiles)
         self.n_op = 2 * N if mode == MODE_FULL else N
+        import torch
+        self._stream = torch.cuda.current_stream()           # every call of this handle enqueues on this stream
         h = _vp()
         cp = c_tiles.data_ptr() if c_tiles is not None else None
         if rows is None:
@@ -329,13 +331,16 @@ class ShardedBse:
             def __init__(self, ptr, n):
                 self.__cuda_array_interface__ = {"shape": (n,), "typestr": "<f8", "data": (ptr, False), "version": 2}
 
+        stream = self.local._stream                          # the stream the library's kernels are ordered on
+
         def hook(user, op, ptr, n):
             try:
                 t = torch.as_tensor(_Dev(ptr, n), device="cuda")
-                if op == 0:
-                    dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
-                else:
-                    dist.broadcast(t, src=src, group=group)
+                with torch.cuda.stream(stream):                  # order the collective after the kernels that wrote the buffer
+                    if op == 0:
+                        dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
+                    else:
+                        dist.broadcast(t, src=src, group=group)
                 calls[op] += 1
                 return 0
             except Exception as e:                               # never let an exception cross the C frame
@@ -371,13 +376,18 @@ class ShardedBse:
             storage = STORE_REAL_FORM if storage == STORE_C128 else STORE_REAL_FORM_C64
         return cls(mode, N, r, c, (rb, re), storage, group)
 
+    def _sum(self, Y):
+        import torch
+        if self._cb is not None:                                 # with the hook the library has summed already
+            return Y
+        with torch.cuda.stream(self.local._stream):              # after the kernels that wrote Y
+            return sum_partials(Y, self.group)
+
     def apply(self, X, Y=None):
-        Y = self.local.apply(X, Y)
-        return Y if self._cb is not None else sum_partials(Y, self.group)      # with the hook the library has summed
+        return self._sum(self.local.apply(X, Y))
 
     def apply_half(self, X, sign: int, Y=None):
-        Y = self.local.apply_half(X, sign, Y)
-        return Y if self._cb is not None else sum_partials(Y, self.group)
+        return self._sum(self.local.apply_half(X, sign, Y))
 
 
 def host_heev(A, nz=None):
