@@ -19,6 +19,9 @@
  *   - all device work is enqueued on the `stream` given to bse_create (a cudaStream_t passed as
  *     void*; NULL = the legacy default stream).  bse_apply / bse_apply_half / bse_orth are
  *     asynchronous with respect to the host; bse_solve and the *_host calls are synchronous;
+ *   - bse_apply / bse_apply_half only enqueue a memset and kernel launches: after one warm-up call (one-time kernel
+ *     attribute setup) they can be captured in a CUDA graph on the handle's stream and replayed (launch-bound loops of
+ *     small products; tests/test_gpu_apply.py);
  *   - no call throws or exits; every call returns a bse_status_t;
  *   - there is no CPU fallback: without a CUDA device every compute call returns BSE_ERR_CUDA.
  *

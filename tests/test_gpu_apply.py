@@ -377,3 +377,34 @@ def test_repeated_launches_stay_within_rounding_of_each_other(k):
     ref = hr.apply_half(X, -1).clone()
     worst = max(float((hr.apply_half(X, -1) - ref).abs().max()) for _ in range(200))
     assert worst <= 1e-13 * float(ref.abs().max())
+
+
+def test_apply_is_capturable_in_a_cuda_graph(orc):
+    """bse_apply / bse_apply_half only enqueue work (a memset and kernel launches) on the handle's stream, so a
+    launch-bound loop of small products can be captured once and replayed: the graph is captured on the stream the
+    handle was created on, replayed with new contents of X, and must reproduce the oracle."""
+    import torch
+    import paper_2504_10096_b200 as b
+    N, k = 1024, 4
+    R, C = gen.dense_R(N, 1, sigma=1.0), gen.dense_C(N, 1)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        ht = b.Bse(b.MODE_TDA, N, pack(R, 0))
+        hf = b.Bse(b.MODE_FULL, N, pack(R, 0), pack(C, 1))
+        X = torch.zeros((k, N), dtype=torch.complex128, device="cuda")
+        Y = torch.empty_like(X); Z = torch.empty_like(X); W = torch.empty_like(X)
+        ht.apply(X, Y); hf.apply_half(X, -1, Z)             # warm-up outside the capture (one-time attribute setup)
+        s.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            ht.apply(X, Y)                                   # Y = R X
+            hf.apply_half(Y, -1, Z)                          # Z = M(Y)
+            ht.apply(Z, W)                                   # W = R Z
+    for seed in (3, 4):
+        x = gen.block_X(N, k, seed)
+        X.copy_(to_dev(x))
+        g.replay()
+        torch.cuda.synchronize()
+        y = orc.apply_tda(R, x); z = orc.apply_half(R, C, y, -1); w = orc.apply_tda(R, z)
+        assert relerr(to_host(Y), y) <= TOL_APPLY and relerr(to_host(Z), z) <= 3 * TOL_APPLY
+        assert relerr(to_host(W), w) <= 10 * TOL_APPLY       # three products deep: errors accumulate
