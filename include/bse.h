@@ -85,7 +85,11 @@ typedef struct {
     int32_t nconv;          /* wanted Ritz pairs that met the tolerance                                    */
     int32_t ncv;            /* basis size used                                                              */
     double  seconds_apply, seconds_orth, seconds_project, seconds_restart, seconds_total;
+                            /* apply: every operator application (in full mode both half applies of a step, also the
+                               P(W) that follows the projection); orth: projection + normalisation only            */
     double  norm_est;       /* estimate of ||H|| (largest |Ritz value| seen; sqrt of it in full mode)      */
+    double  basis_orth_err; /* || <V, V> - I ||_F of the final Krylov basis in the active inner product:
+                               V^H V (TDA) or Re(X^H P(X)) (full mode, reading S10); north_star bound 1e-12    */
 } bse_info_t;
 
 const char *bse_status_string(bse_status_t s);

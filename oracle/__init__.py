@@ -55,8 +55,10 @@ def _load():
                                         _c128, _f64, _c128, _f64]
         lib.orc_lanczos_tda.restype = ctypes.c_int
         lib.orc_lanczos_full.argtypes = [_i64, _c128, _c128, ctypes.c_int, ctypes.c_double, ctypes.c_int,
-                                         ctypes.c_int, _c128, _f64, _c128, _f64]
+                                         ctypes.c_int, ctypes.c_int, _c128, _f64, _c128, _f64]
         lib.orc_lanczos_full.restype = ctypes.c_int
+        lib.orc_tridiag_ql.argtypes = [_i64, _f64, _f64, _f64, ctypes.c_void_p]
+        lib.orc_tridiag_ql.restype = ctypes.c_int
         lib.orc_round_c64.argtypes = [_i64, _c128, _c128]
         lib.orc_lanczos_quadrature.argtypes = [_i64, _c128, _c128, ctypes.c_int, _f64, _f64]
         lib.orc_lanczos_quadrature.restype = ctypes.c_int
@@ -173,12 +175,28 @@ def lanczos_tda(R, nev, tol, v0, maxit=None, check=10):
     return w, Vec, res, steps
 
 
-def lanczos_full(R, C, nev, tol, x0, maxit=None, check=10):
+def tridiag_ql(d, e, want_vectors=True):
+    """Eigenvalues (ascending) and eigenvectors (columns) of the real symmetric tridiagonal matrix tridiag(e, d, e)."""
+    d = np.ascontiguousarray(d, dtype=np.float64); e = np.ascontiguousarray(e, dtype=np.float64)
+    m = len(d)
+    assert len(e) >= m - 1
+    e = np.ascontiguousarray(np.concatenate([e, [0.0]])[:max(m, 1)])
+    w = np.zeros(m)
+    Z = np.zeros((m, m)) if want_vectors else None
+    if _load().orc_tridiag_ql(m, d, e, w, Z.ctypes.data if want_vectors else None):
+        raise RuntimeError("oracle tridiagonal QL did not converge")
+    return w, Z
+
+
+def lanczos_full(R, C, nev, tol, x0, maxit=None, check=10, minit=0):
+    """nev lowest positive omega of Eq. (1) with Sigma-orthonormal eigenvectors (counted as eigenvectors of H: the
+    second copy of every omega^2 that G = M o P has on R^2N is recognised by its vector and dropped, reading R1).
+    minit: do not stop before this many steps (tests run far past first convergence)."""
     R = _c(R); C = _c(C)
     N = R.shape[0]
     maxit = 2 * N if maxit is None else maxit
     om = np.zeros(nev); Vec = np.zeros((2 * N, nev), dtype=np.complex128); res = np.zeros(nev)
-    steps = _load().orc_lanczos_full(N, R, C, nev, tol, maxit, check, _c(x0).reshape(N), om, Vec, res)
+    steps = _load().orc_lanczos_full(N, R, C, nev, tol, maxit, check, minit, _c(x0).reshape(N), om, Vec, res)
     if steps == -1000000:
         raise np.linalg.LinAlgError("Omega is not positive definite")
     return om, Vec, res, steps

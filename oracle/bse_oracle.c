@@ -305,6 +305,76 @@ done:
 }
 
 /* ------------------------------------------------------------------------------------------
+ * Real symmetric tridiagonal eigenproblem by the implicit-shift QR iteration with Wilkinson's shift
+ * (textbook: Golub & Van Loan, "Matrix Computations", symmetric QR step on a tridiagonal matrix).
+ * 8(c) step 4 allows "the oracle's own tridiagonal QL" for the projected matrix T of the Lanczos routines
+ * below ("projected into a smaller structured problem"); the dense Jacobi routine above costs
+ * O(m^3) per sweep and took more than an hour at m = 1500.
+ * In:  m, d[0..m) diagonal, e[0..m-1) off-diagonal (both untouched).
+ * Out: w[0..m) eigenvalues ascending; Z (m x m row-major, may be NULL) with eigenvector i in COLUMN i.
+ * One step on the unreduced block lo..hi: mu = Wilkinson shift from the trailing 2 x 2 block; x = d_lo - mu,
+ * z = e_lo; for k = lo..hi-1: c = x/r, s = z/r, r = hypot(x, z), G = [[c, -s], [s, c]] acting on (k, k+1),
+ * T <- G^T T G (which moves the bulge z = s e_{k+1} one position down), Z <- Z G, x = e_k.
+ * Returns 0, or 1 if some eigenvalue needed more than 60 steps.
+ * Pins (tests/test_oracle_eig.py): the Toeplitz matrix tridiag(b, a, b) with eigenvalues a + 2 b cos(j pi/(m+1)) and
+ * eigenvectors sin(i j pi/(m+1)); the Jacobi routine on random tridiagonals; Z^T T Z = diag(w), Z^T Z = I.
+ * ------------------------------------------------------------------------------------------ */
+int orc_tridiag_ql(int64_t m, const double *d_in, const double *e_in, double *w, double *Z)
+{
+    double *d = (double *)malloc(sizeof(double) * m), *e = (double *)calloc(m, sizeof(double));
+    const double eps = 2.220446049250313e-16;
+    int rc = 0;
+    for (int64_t i = 0; i < m; ++i) d[i] = d_in[i];
+    for (int64_t i = 0; i + 1 < m; ++i) e[i] = e_in[i];
+    if (Z) for (int64_t i = 0; i < m; ++i) for (int64_t j = 0; j < m; ++j) Z[i * m + j] = (i == j) ? 1.0 : 0.0;
+    int64_t hi = m - 1;
+    int64_t steps = 0;
+    while (hi > 0) {
+        if (fabs(e[hi - 1]) <= eps * (fabs(d[hi - 1]) + fabs(d[hi]))) { e[hi - 1] = 0.0; --hi; steps = 0; continue; }
+        if (++steps > 60) { rc = 1; break; }
+        int64_t lo = hi - 1;
+        while (lo > 0 && fabs(e[lo - 1]) > eps * (fabs(d[lo - 1]) + fabs(d[lo]))) --lo;
+        double delta = 0.5 * (d[hi - 1] - d[hi]), b2 = e[hi - 1] * e[hi - 1];
+        double mu = d[hi] - b2 / (delta + ((delta >= 0.0) ? 1.0 : -1.0) * sqrt(delta * delta + b2));
+        double x = d[lo] - mu, z = e[lo];
+        for (int64_t k = lo; k < hi; ++k) {
+            double r = hypot(x, z);
+            double c = (r > 0.0) ? x / r : 1.0, s = (r > 0.0) ? z / r : 0.0;
+            if (k > lo) e[k - 1] = r;
+            double a = d[k], b = e[k], g = d[k + 1];
+            d[k] = c * c * a + 2.0 * c * s * b + s * s * g;
+            d[k + 1] = s * s * a - 2.0 * c * s * b + c * c * g;
+            e[k] = c * s * (g - a) + (c * c - s * s) * b;
+            x = e[k];
+            if (k + 1 < hi) { z = s * e[k + 1]; e[k + 1] = c * e[k + 1]; }
+            if (Z) {                                                  /* Z <- Z G; Z is held transposed while iterating */
+                double *zk = Z + k * m, *zk1 = zk + m;
+                for (int64_t i = 0; i < m; ++i) {
+                    double u = zk[i], v = zk1[i];
+                    zk[i] = c * u + s * v;
+                    zk1[i] = -s * u + c * v;
+                }
+            }
+        }
+    }
+    /* sort ascending (selection sort, swapping eigenvectors), then transpose: eigenvector i into column i */
+    for (int64_t i = 0; i < m; ++i) w[i] = d[i];
+    for (int64_t i = 0; i + 1 < m; ++i) {
+        int64_t p = i;
+        for (int64_t j = i + 1; j < m; ++j) if (w[j] < w[p]) p = j;
+        if (p != i) {
+            double t = w[i]; w[i] = w[p]; w[p] = t;
+            if (Z) for (int64_t r = 0; r < m; ++r) { double tv = Z[i * m + r]; Z[i * m + r] = Z[p * m + r]; Z[p * m + r] = tv; }
+        }
+    }
+    if (Z)
+        for (int64_t i = 0; i < m; ++i)
+            for (int64_t j = i + 1; j < m; ++j) { double tv = Z[i * m + j]; Z[i * m + j] = Z[j * m + i]; Z[j * m + i] = tv; }
+    free(d); free(e);
+    return rc;
+}
+
+/* ------------------------------------------------------------------------------------------
  * Block classical Gram-Schmidt with one reorthogonalisation (new vectors "have to
  * be orthogonalized against the previous ones"), followed by a column-by-column QR of the block.
  * In:  V (N x m, orthonormal columns, row-major), W (N x k row-major).
@@ -367,7 +437,7 @@ int orc_block_cgs2(int64_t N, int64_t m, int64_t k, const zc *V, const zc *W, zc
  * Textbook Lanczos, TDA (Hermitian R), single vector, full reorthogonalisation (classical
  * Gram-Schmidt twice) -- PAPER.md:65-71: vectors generated one by one, each orthogonalised
  * against the previous ones and stored.  No restart (the basis fits at the sizes the oracle runs).
- * The projected tridiagonal T is diagonalised by the Jacobi routine above every `check` steps.
+ * The projected tridiagonal T is diagonalised by orc_tridiag_ql every `check` steps.
  * Converged when the nev lowest Ritz pairs have |beta_{m+1} s_{m,i}| <= tol * max|theta|.
  * Out: w (nev ascending), Vec (N x nev row-major), res (nev), returns number of steps (<0: failed).
  * ------------------------------------------------------------------------------------------ */
@@ -386,7 +456,7 @@ int orc_lanczos_tda(int64_t N, const zc *R, int nev, double tol, int maxit, int 
     double *alpha = (double *)calloc(maxit + 1, sizeof(double));
     double *beta = (double *)calloc(maxit + 2, sizeof(double));        /* beta[j] couples j-1 and j */
     zc *wv = (zc *)malloc(sizeof(zc) * N);
-    zc *T = NULL, *S = NULL; double *th = NULL;
+    double *S = NULL, *th = NULL;
     int m = 0, result = -1;
     double n0 = nrm2(N, v0);
     for (int64_t i = 0; i < N; ++i) Vb[i] = v0[i] / n0;
@@ -415,18 +485,13 @@ int orc_lanczos_tda(int64_t N, const zc *R, int nev, double tol, int maxit, int 
         int last = (m == maxit) || (b <= 1e-300);
         if (b > 1e-300) for (int64_t i = 0; i < N; ++i) Vb[(size_t)(j + 1) * N + i] = wv[i] / b;
         if (m >= nev && (m % check == 0 || last)) {
-            T = (zc *)realloc(T, sizeof(zc) * m * m); S = (zc *)realloc(S, sizeof(zc) * m * m);
+            S = (double *)realloc(S, sizeof(double) * m * m);
             th = (double *)realloc(th, sizeof(double) * m);
-            for (int i = 0; i < m * m; ++i) T[i] = 0.0;
-            for (int i = 0; i < m; ++i) {
-                T[i * m + i] = alpha[i];
-                if (i + 1 < m) { T[i * m + i + 1] = beta[i + 1]; T[(i + 1) * m + i] = beta[i + 1]; }
-            }
-            if (orc_jacobi_herm(m, T, th, S) < 0) break;
+            if (orc_tridiag_ql(m, alpha, beta + 1, th, S)) break;        /* T = tridiag(beta, alpha, beta) */
             double hn = fmax(fabs(th[0]), fabs(th[m - 1]));
             int ok = 1;
             for (int i = 0; i < nev; ++i) {
-                res[i] = fabs(b) * cabs(S[(m - 1) * m + i]);
+                res[i] = fabs(b) * fabs(S[(m - 1) * m + i]);
                 if (res[i] > tol * hn) ok = 0;
             }
             if (ok || last) {
@@ -444,7 +509,7 @@ int orc_lanczos_tda(int64_t N, const zc *R, int nev, double tol, int maxit, int 
         }
         if (last) break;
     }
-    free(Vb); free(alpha); free(beta); free(wv); free(T); free(S); free(th);
+    free(Vb); free(alpha); free(beta); free(wv); free(S); free(th);
     return result;
 }
 
@@ -459,9 +524,35 @@ int orc_lanczos_tda(int64_t N, const zc *R, int nev, double tol, int maxit, int 
  *   theta_i, s_i its eigenpairs; omega_i = sqrt(theta_i); x = X s_i, y = (PX s_i)/omega_i;
  *   v_i = [x + y; conj(x - y)] sqrt(omega_i)/2   (then v^H Sigma v = 1).
  * Residual estimate |H v - omega v| = sqrt(2) beta_{m+1} |s_{m,i}| |x_{m+1}|_2 / omega * (sqrt(omega)/2).
- * Out: omega (nev ascending), Vec (2N x nev row-major), res (nev).  Returns steps (<0: failed).
+ *
+ * Multiplicity (reading R1): on C^N = R^2N every omega^2 is a DOUBLE eigenvalue of G = M o P, with
+ * eigenvectors x and K x, K(x) = i P(x) (K^2 = -G, K commutes with G); both give the same eigenvector of H up to
+ * the phase i:  v(K x / omega) = i v(x).  In exact arithmetic the Krylov space of one start vector is P-orthogonal
+ * to its image under K, so the iteration sees one copy; the second copy grows out of rounding noise after the first
+ * has converged (like the "ghosts" of Lanczos without reorthogonalisation, except that it is a genuine eigenvector
+ * of G).  "The nev lowest positive omega of H" therefore counts eigenvectors of H, not Ritz
+ * values of G: the leading converged Ritz pairs are turned into vectors v_i of H, each is Sigma-orthogonalised
+ * (complex coefficients a^H Sigma v) against the ones already accepted, and it is a NEW eigenpair iff what is left
+ * has v^H Sigma v > 1e-4 (a copy leaves the square of the eigenvector error, ~1e-16; a distinct eigenvector of H is
+ * exactly Sigma-orthogonal to the others and leaves 1).  The iteration stops when nev eigenpairs have been accepted,
+ * every Ritz value below the last of them is converged, and at least `minit` steps were done (minit lets a test run
+ * the iteration far past first convergence, where the copies are present).
+ * Out: omega (nev ascending), Vec (2N x nev row-major, Sigma-orthonormal), res (nev).  Returns steps (<0: failed).
  * ------------------------------------------------------------------------------------------ */
-int orc_lanczos_full(int64_t N, const zc *R, const zc *C, int nev, double tol, int maxit, int check,
+/* v^H Sigma w for 2N-vectors stored with stride ld (column c of a row-major 2N x ld array) */
+static zc sigma_dot(int64_t N, const zc *v, int64_t ldv, const zc *w, int64_t ldw)
+{
+    ld sr = 0.0L, si = 0.0L;
+    for (int64_t i = 0; i < 2 * N; ++i) {
+        zc a = v[i * ldv], b = w[i * ldw];
+        ld pr = (ld)creal(a) * (ld)creal(b) + (ld)cimag(a) * (ld)cimag(b);
+        ld pi = (ld)creal(a) * (ld)cimag(b) - (ld)cimag(a) * (ld)creal(b);
+        if (i < N) { sr += pr; si += pi; } else { sr -= pr; si -= pi; }
+    }
+    return (double)sr + I * (double)si;
+}
+
+int orc_lanczos_full(int64_t N, const zc *R, const zc *C, int nev, double tol, int maxit, int check, int minit,
                      const zc *x0, double *omega, zc *Vec, double *res)
 {
     if (maxit > 2 * N) maxit = (int)(2 * N);
@@ -470,7 +561,8 @@ int orc_lanczos_full(int64_t N, const zc *R, const zc *C, int nev, double tol, i
     double *alpha = (double *)calloc(maxit + 1, sizeof(double));
     double *beta = (double *)calloc(maxit + 2, sizeof(double));
     zc *wv = (zc *)malloc(sizeof(zc) * N), *pw = (zc *)malloc(sizeof(zc) * N);
-    zc *T = NULL, *S = NULL; double *th = NULL;
+    zc *cand = (zc *)malloc(sizeof(zc) * 2 * (size_t)N);
+    double *S = NULL, *th = NULL;
     int m = 0, result = -1;
     memcpy(Xb, x0, sizeof(zc) * N);
     orc_apply_half(N, 1, +1, R, C, Xb, Pb);
@@ -511,48 +603,53 @@ int orc_lanczos_full(int64_t N, const zc *R, const zc *C, int nev, double tol, i
         } else breakdown = 1;
         beta[j + 1] = b;
         int last = (m == maxit) || breakdown;
-        if (m >= nev && (m % check == 0 || last)) {
-            T = (zc *)realloc(T, sizeof(zc) * m * m); S = (zc *)realloc(S, sizeof(zc) * m * m);
+        if (m >= nev && m >= minit && (m % check == 0 || last)) {
+            S = (double *)realloc(S, sizeof(double) * m * m);
             th = (double *)realloc(th, sizeof(double) * m);
-            for (int i = 0; i < m * m; ++i) T[i] = 0.0;
-            for (int i = 0; i < m; ++i) {
-                T[i * m + i] = alpha[i];
-                if (i + 1 < m) { T[i * m + i + 1] = beta[i + 1]; T[(i + 1) * m + i] = beta[i + 1]; }
-            }
-            if (orc_jacobi_herm(m, T, th, S) < 0) break;
+            if (orc_tridiag_ql(m, alpha, beta + 1, th, S)) break;            /* T = tridiag(beta, alpha, beta) */
             if (!(th[0] > 0.0)) { result = -1000000; break; }
             double hn = sqrt(fabs(th[m - 1]));
-            int ok = 1;
-            for (int i = 0; i < nev; ++i) {
+            /* eigenpairs of H from the leading converged Ritz pairs of G (all of them if this is the last chance) */
+            int found = 0, all_converged = 1;
+            for (int i = 0; i < m && found < nev; ++i) {
                 double om = sqrt(th[i]);
-                res[i] = sqrt(2.0) * b * cabs(S[(m - 1) * m + i]) * xn1 / om * (sqrt(om) / 2.0);
-                if (res[i] > tol * hn) ok = 0;
-            }
-            if (ok || last) {
-                for (int i = 0; i < nev; ++i) {
-                    double om = sqrt(th[i]);
-                    omega[i] = om;
-                    double sc = sqrt(om) / 2.0;
-                    for (int64_t r = 0; r < N; ++r) {
-                        zc x = 0.0, y = 0.0;
-                        for (int p = 0; p < m; ++p) {
-                            double s = creal(S[p * m + i]);
-                            x += Xb[(size_t)p * N + r] * s;
-                            y += Pb[(size_t)p * N + r] * s;
-                        }
-                        y /= om;
-                        Vec[r * nev + i] = sc * (x + y);
-                        Vec[(r + N) * nev + i] = sc * conj(x - y);
-                    }
+                double ri = sqrt(2.0) * b * fabs(S[(m - 1) * m + i]) * xn1 / om * (sqrt(om) / 2.0);
+                if (ri > tol * hn) {                                          /* an unconverged Ritz value below the target */
+                    if (!last) break;
+                    all_converged = 0;
                 }
-                result = ok ? m : -m;
-                break;
+                double sc = sqrt(om) / 2.0;
+                for (int64_t r = 0; r < N; ++r) {
+                    zc x = 0.0, y = 0.0;
+                    for (int p = 0; p < m; ++p) {
+                        double s = S[p * m + i];
+                        x += Xb[(size_t)p * N + r] * s;
+                        y += Pb[(size_t)p * N + r] * s;
+                    }
+                    y /= om;
+                    cand[r] = sc * (x + y);
+                    cand[r + N] = sc * conj(x - y);
+                }
+                for (int pass = 0; pass < 2; ++pass)                          /* Sigma-orthogonalise against the accepted ones */
+                    for (int q = 0; q < found; ++q) {
+                        zc cf = sigma_dot(N, Vec + q, nev, cand, 1);
+                        for (int64_t r = 0; r < 2 * N; ++r) cand[r] -= Vec[r * nev + q] * cf;
+                    }
+                double left = creal(sigma_dot(N, cand, 1, cand, 1));
+                if (!(left > 1e-4)) continue;                                 /* the second copy of an accepted eigenpair */
+                double nrm = 1.0 / sqrt(left);
+                for (int64_t r = 0; r < 2 * N; ++r) Vec[r * nev + found] = cand[r] * nrm;
+                omega[found] = om;
+                res[found] = ri;
+                ++found;
             }
+            int ok = (found == nev) && all_converged;
+            if (ok || last) { result = ok ? m : -m; break; }
         }
         if (last) break;
     }
 done:
-    free(Xb); free(Pb); free(alpha); free(beta); free(wv); free(pw); free(T); free(S); free(th);
+    free(Xb); free(Pb); free(alpha); free(beta); free(wv); free(pw); free(cand); free(S); free(th);
     return result;
 }
 

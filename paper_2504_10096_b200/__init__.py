@@ -34,7 +34,7 @@ class _Info(ctypes.Structure):
     _fields_ = [("n_apply", ctypes.c_int32), ("n_restart", ctypes.c_int32), ("nconv", ctypes.c_int32),
                 ("ncv", ctypes.c_int32), ("seconds_apply", ctypes.c_double), ("seconds_orth", ctypes.c_double),
                 ("seconds_project", ctypes.c_double), ("seconds_restart", ctypes.c_double),
-                ("seconds_total", ctypes.c_double), ("norm_est", ctypes.c_double)]
+                ("seconds_total", ctypes.c_double), ("norm_est", ctypes.c_double), ("basis_orth_err", ctypes.c_double)]
 
 
 _vp, _i64, _i32, _u64, _dbl = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_uint64, ctypes.c_double

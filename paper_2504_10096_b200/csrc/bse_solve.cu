@@ -52,13 +52,33 @@ struct Solver {
     uint64_t seed, rng = 0;
     bse_info_t info{};
     double normest = 0.0;
+    double seconds_apply_in_orth = 0.0;   // full mode: the P(W) apply issued between projection and normalisation
+
+    // || <V, V> - I ||_F over the first mtot basis columns in the active inner product (reading S10)
+    bse_status_t basis_orth_error(int mtot, double *err)
+    {
+        const bool cplx = !full;
+        ST(gram_basis(h, cplx ? V.p : PV.p, ld, mtot, V.p, ld, mtot, cplx, n, (double *)coef.p));
+        const int ldo = cplx ? 2 * mtot : mtot;
+        std::vector<double> g((size_t)ldo * mtot);
+        BSE_CUDA(cudaMemcpyAsync(g.data(), coef.p, g.size() * 8, cudaMemcpyDeviceToHost, h->stream));
+        BSE_CUDA(cudaStreamSynchronize(h->stream));
+        double s2 = 0.0;
+        for (int b = 0; b < mtot; ++b)
+            for (int a = 0; a < mtot; ++a) {
+                const double re = g[a + (size_t)b * ldo] - (a == b ? 1.0 : 0.0);
+                const double im = cplx ? g[a + mtot + (size_t)b * ldo] : 0.0;
+                s2 += re * re + im * im;
+            }
+        *err = std::sqrt(s2);
+        return BSE_OK;
+    }
 
     char *col(DevBuf &b, int64_t c) { return (char *)b.p + (size_t)c * ld * 16; }
 
-    // upload S (rows x l complex, host column-major ld = ldS) in coefficient layout and form out = basis * S
-    bse_status_t rotate(DevBuf &basis, int rows, const zc *S, int ldS, int l, void *out, int64_t ldo_c)
+    // upload S (rows x l complex, host column-major ld = ldS) to `coef` in the coefficient layout gemm_basis consumes
+    bse_status_t upload_coef(const zc *S, int rows, int ldS, int l, bool cplx)
     {
-        const bool cplx = !full;
         const int ldo = cplx ? 2 * rows : rows;
         std::vector<double> c((size_t)ldo * l);
         for (int j = 0; j < l; ++j)
@@ -68,7 +88,112 @@ struct Solver {
             }
         BSE_CUDA(cudaMemcpyAsync(coef.p, c.data(), c.size() * 8, cudaMemcpyHostToDevice, h->stream));
         BSE_CUDA(cudaStreamSynchronize(h->stream));
-        return gemm_basis(h, basis.p, ld, rows, cplx, (const double *)coef.p, ldo, l, n, out, ldo_c, 1.0, 0.0);
+        return BSE_OK;
+    }
+    // out = basis * S  (complex S in the TDA case, real S in full mode)
+    bse_status_t rotate(DevBuf &basis, int rows, const zc *S, int ldS, int l, void *out, int64_t ldo_c)
+    {
+        const bool cplx = !full;
+        ST(upload_coef(S, rows, ldS, l, cplx));
+        return gemm_basis(h, basis.p, ld, rows, cplx, (const double *)coef.p, cplx ? 2 * rows : rows, l, n, out, ldo_c,
+                          1.0, 0.0);
+    }
+
+    // Full mode, reading R1: on C^N = R^2N every omega^2 is a double eigenvalue of G = M o P (x and K x = i P(x) / omega
+    // give the same eigenvector of H up to the phase i), a block iteration finds both copies, and a genuinely degenerate
+    // omega has four.  Which of the first `nc` Ritz pairs are DISTINCT eigenpairs of H is therefore decided from the
+    // vectors, never from the values: with x_a = X s_a, p_a = PX s_a, y_a = p_a / w_a, v_a = [x_a + y_a; conj(x_a - y_a)] sqrt(w_a)/2,
+    //     v_a^H Sigma v_b = sqrt(w_a w_b)/2 * ( Re(x_a^H p_b)/w_b + Re(x_b^H p_a)/w_a + i [Im(x_a^H x_b) + Im(p_a^H p_b)/(w_a w_b)] ),
+    // i.e. one complex Gram matrix of [x | p] on the device.  Runs of Ritz values closer than 1e-6 relative are taken
+    // together and a pivoted Cholesky of their Sigma-Gram block keeps a maximal independent set (pivot > 1e-4: a copy
+    // leaves the square of the eigenvector error, an independent eigenvector of a degenerate omega at least 2/3 in the
+    // best pivot); different runs are Sigma-orthogonal to eigenvector accuracy.  Outputs: sel (candidate index of every
+    // returned pair, ascending, at most nev), Cm (nc x nev complex, column-major): returned vector j = sum_a v_a Cm[a, j]
+    // is Sigma-normalised and Sigma-orthogonal to the others of its run.  Leaves x in rot[:, 0:nc), p in rot[:, nc:2nc).
+    // pad: fill up to nev pairs with rejected candidates (best estimates when the iteration did not converge).
+    bse_status_t select_distinct(int mp, const std::vector<zc> &S, const std::vector<double> &theta, int nc, bool pad,
+                                 std::vector<int> &sel, std::vector<zc> &Cm)
+    {
+        ST(rotate(V, mp, S.data(), mp, nc, rot.p, n));
+        ST(rotate(PV, mp, S.data(), mp, nc, col(rot, nc), n));
+        const int m2 = 2 * nc, ldo = 2 * m2;
+        ST(gram_basis(h, rot.p, ld, m2, rot.p, ld, m2, true, n, (double *)coef.p));
+        std::vector<double> g((size_t)ldo * m2);
+        BSE_CUDA(cudaMemcpyAsync(g.data(), coef.p, g.size() * 8, cudaMemcpyDeviceToHost, h->stream));
+        BSE_CUDA(cudaStreamSynchronize(h->stream));
+        auto G = [&](int a, int b) { return zc(g[a + (size_t)b * ldo], g[a + m2 + (size_t)b * ldo]); };   // Z^H Z, Z = [x | p]
+        std::vector<double> w(nc);
+        for (int a = 0; a < nc; ++a) w[a] = std::sqrt(std::max(theta[a], 0.0));
+        std::vector<zc> Gs((size_t)nc * nc);
+        for (int b = 0; b < nc; ++b)
+            for (int a = 0; a < nc; ++a) {
+                const double re = G(a, nc + b).real() / w[b] + G(b, nc + a).real() / w[a];
+                const double im = G(a, b).imag() + G(nc + a, nc + b).imag() / (w[a] * w[b]);
+                Gs[a + (size_t)b * nc] = 0.5 * std::sqrt(w[a] * w[b]) * zc(re, im);
+            }
+        sel.clear();
+        Cm.assign((size_t)nc * nev, zc(0.0));
+        std::vector<int> rejected;
+        for (int r0 = 0; r0 < nc && (int)sel.size() < nev;) {
+            int r1 = r0 + 1;
+            while (r1 < nc && theta[r1] - theta[r1 - 1] <= 1e-6 * std::fabs(theta[r1])) ++r1;
+            const int q = r1 - r0;
+            // pivoted Cholesky of the run's Sigma-Gram block: A = L L^H on the accepted (pivot) candidates
+            std::vector<zc> L((size_t)q * q, zc(0.0));
+            std::vector<double> left(q);
+            std::vector<int> piv;
+            std::vector<char> used(q, 0);
+            for (int a = 0; a < q; ++a) left[a] = Gs[(r0 + a) + (size_t)(r0 + a) * nc].real();
+            while ((int)piv.size() < q) {
+                int best = -1;
+                for (int a = 0; a < q; ++a)
+                    if (!used[a] && (best < 0 || left[a] > left[best])) best = a;
+                if (best < 0 || !(left[best] > 1e-4)) break;
+                const int j = (int)piv.size();
+                used[best] = 1;
+                piv.push_back(best);
+                const double d = std::sqrt(left[best]);
+                // column j of L for every candidate a of the run (row index a): L[a, j] = (A[a, best] - sum_i L[a, i] conj(L[best, i])) / d
+                for (int a = 0; a < q; ++a) {
+                    zc v = Gs[(r0 + a) + (size_t)(r0 + best) * nc];
+                    for (int i = 0; i < j; ++i) v -= L[a + (size_t)i * q] * std::conj(L[best + (size_t)i * q]);
+                    L[a + (size_t)j * q] = v / d;
+                    if (!used[a]) left[a] -= std::norm(L[a + (size_t)j * q]);
+                }
+                left[best] = 0.0;
+            }
+            for (int a = 0; a < q; ++a)
+                if (!used[a]) rejected.push_back(r0 + a);
+            // orthonormal combinations: with Lp = L restricted to the pivot rows (lower triangular in pivot order),
+            // [v_piv] Lp^-H is Sigma-orthonormal.  Returned in ascending candidate order.
+            const int na = (int)piv.size();
+            std::vector<zc> Linv((size_t)na * na, zc(0.0));            // Lp^-1, lower triangular
+            for (int c = 0; c < na; ++c) {
+                Linv[c + (size_t)c * na] = 1.0 / L[piv[c] + (size_t)c * q];
+                for (int r = c + 1; r < na; ++r) {
+                    zc v(0.0);
+                    for (int i = c; i < r; ++i) v += L[piv[r] + (size_t)i * q] * Linv[i + (size_t)c * na];
+                    Linv[r + (size_t)c * na] = -v / L[piv[r] + (size_t)r * q];
+                }
+            }
+            std::vector<int> order(na);
+            for (int c = 0; c < na; ++c) order[c] = c;
+            std::sort(order.begin(), order.end(), [&](int a, int b) { return piv[a] < piv[b]; });
+            for (int oi = 0; oi < na && (int)sel.size() < nev; ++oi) {
+                const int c = order[oi], j = (int)sel.size();          // output j = sum_{r <= c} v_{piv[r]} conj(Linv[c, r])
+                for (int r = 0; r <= c; ++r) Cm[(r0 + piv[r]) + (size_t)j * nc] = std::conj(Linv[c + (size_t)r * na]);
+                sel.push_back(r0 + piv[c]);
+            }
+            r0 = r1;
+        }
+        if (pad)
+            for (size_t i = 0; i < rejected.size() && (int)sel.size() < nev; ++i) {
+                const int a = rejected[i], j = (int)sel.size();
+                const double d = Gs[a + (size_t)a * nc].real();
+                Cm[a + (size_t)j * nc] = d > 0.0 ? 1.0 / std::sqrt(d) : 1.0;
+                sel.push_back(a);
+            }
+        return BSE_OK;
     }
 
     // W = V[:, c0+k .. c0+2k) <- operator applied to the block at c0 (TDA: R x;  full: M(P x), reading S4)
@@ -95,8 +220,12 @@ struct Solver {
         double e_in = 0.0, e_after = 0.0, g_after = 0.0;
         ST(block_norm_scale(h, col(V, m), ld, nullptr, ld, k, false, &e_in));
         ST(project_block(h, V.p, ld, m, PV.p, ld, col(V, m), ld, k, nullptr, ld, false, Hc));
+        const double ta = now_s();                                                                 // (project_block ends synchronised)
         bse_status_t st = bse_apply_half(h, +1, col(V, m), ld, col(PV, m), ld, k);                // PW = P(W)
         if (st) return st;
+        BSE_CUDA(cudaStreamSynchronize(h->stream));
+        seconds_apply_in_orth += now_s() - ta;
+        info.n_apply += 1;
         ST(block_norm_scale(h, col(V, m), ld, nullptr, ld, k, false, &e_after));
         ST(block_norm_scale(h, col(V, m), ld, col(PV, m), ld, k, false, &g_after));
         // scale of the incoming block in the P-norm, estimated through the Euclidean norms
@@ -146,8 +275,9 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
     ST(s.V.alloc(basis_bytes));
     if (full) ST(s.PV.alloc(basis_bytes));
     ST(s.rot.alloc((size_t)n * (ncv + k) * 16));
-    ST(s.coef.alloc((size_t)2 * ncv * ncv * 8));
-    ST(s.omega_d.alloc((size_t)nev * 8));
+    const int ncmax = (ncv + k) / 2;                    // full mode: candidates of the multiplicity test (x and P x side by side in rot)
+    ST(s.coef.alloc((size_t)2 * (ncv + k) * (ncv + k) * 8));
+    ST(s.omega_d.alloc((size_t)std::max(nev, ncmax) * 8));
     s.T.assign((size_t)ncv * ncv, zc(0.0));
     const int ldT = ncv;
     ST(orth_reserve(h, ncv + k, k));
@@ -170,7 +300,8 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
     bse_status_t result = BSE_ERR_NOT_CONVERGED;
     int restarts = 0;
     std::vector<int> sel;          // Ritz indices returned
-    int nz = 0;
+    std::vector<zc> Cm;            // full mode: returned vectors as combinations of the candidate vectors (select_distinct)
+    int nz = 0, ncand = 0;
 
     while (true) {
         // ---- one block step: apply (a2 / a3), orthogonalise (a5-a7), extend T
@@ -186,7 +317,9 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
             if (verbose && st_o) fprintf(stderr, "[bse_solve] orthogonalisation failed (%d) at m = %d\n", (int)st_o, m);
             if (st_o) return st_o;
         }
-        s.info.seconds_orth += now_s() - t1;
+        s.info.seconds_orth += now_s() - t1 - s.seconds_apply_in_orth;
+        s.info.seconds_apply += s.seconds_apply_in_orth;
+        s.seconds_apply_in_orth = 0.0;
         for (int c = 0; c < k; ++c)
             for (int a = 0; a < m; ++a) {
                 zc v = Hc[a + (size_t)c * m];
@@ -250,28 +383,41 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
             resid[i] = r;
         }
         // ---- convergence of the wanted pairs (leading Ritz values must all be converged)
-        int nconv = 0, nfound = 0;
-        sel.clear();
+        int nconv = 0;
         for (int i = 0; i < nz; ++i) {
             if (!(resid[i] <= tol * s.normest)) break;
             ++nconv;
-            bool newc = true;
-            if (full && !sel.empty()) newc = (theta[i] - theta[sel.back()]) > 1e-7 * std::fabs(theta[i]);
-            if (newc) { sel.push_back(i); ++nfound; }
-            if (nfound == nev) break;
         }
-        s.info.nconv = nfound;
+        bool done;
+        if (!full) {
+            done = nconv >= nev;
+            s.info.nconv = std::min(nconv, nev);
+        } else {
+            // Every eigenpair of H owns exactly two Ritz values of G (reading R1), whatever the multiplicity of omega:
+            // 2 nev - 1 leading converged Ritz pairs contain nev distinct eigenpairs, and so do nev value-separated
+            // ones (a single-vector iteration sees one copy of each).  WHICH pairs are returned is decided from the
+            // vectors (select_distinct), once, when this count says the iteration can stop.
+            int nsep = 0;
+            for (int i = 0; i < nconv; ++i)
+                if (i == 0 || theta[i] - theta[i - 1] > 1e-6 * std::fabs(theta[i])) ++nsep;
+            const int lower = std::max(nsep, (nconv + 1) / 2);
+            s.info.nconv = std::min(lower, nev);
+            done = lower >= nev;
+            if (done) {
+                ncand = std::min(nconv, ncmax);
+                ST(s.select_distinct(mp, S, theta, ncand, false, sel, Cm));
+                if ((int)sel.size() < nev) done = false;       // only if ncmax cut the candidate list: keep iterating
+            }
+        }
         s.info.seconds_project += now_s() - t2;
-        const bool done = (nfound >= nev);
         if (done || restarts >= max_restarts) {
             result = done ? BSE_OK : BSE_ERR_NOT_CONVERGED;
-            if (!done) {   // best estimates: the first nev distinct Ritz values
+            if (!full) {
                 sel.clear();
-                for (int i = 0; i < nz && (int)sel.size() < nev; ++i)
-                    if (!full || sel.empty() || (theta[i] - theta[sel.back()]) > 1e-7 * std::fabs(theta[i])) sel.push_back(i);
-                for (int i = 0; (int)sel.size() < nev && i < nz; ++i)
-                    if (std::find(sel.begin(), sel.end(), i) == sel.end()) sel.push_back(i);
-                std::sort(sel.begin(), sel.end());
+                for (int i = 0; i < nev && i < nz; ++i) sel.push_back(i);
+            } else if (!done) {                                 // best estimates: the first nev distinct pairs, converged or not
+                ncand = std::min(nz, ncmax);
+                ST(s.select_distinct(mp, S, theta, ncand, true, sel, Cm));
             }
             break;
         }
@@ -301,6 +447,7 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
 
     // ---- eigenvalues, eigenvectors (a10)
     const int mp = s.mp;
+    ST(s.basis_orth_error(mp + k, &s.info.basis_orth_err));
     const int nsel = (int)sel.size();
     std::vector<zc> Ssel((size_t)mp * nev, zc(0.0));
     std::vector<double> om(nev, 0.0);
@@ -314,11 +461,14 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
     if (!full) {
         ST(s.rotate(s.V, mp, Ssel.data(), mp, nev, dVec, ldvec));
     } else {
-        // x = X s, px = PX s;  v = [x + px/w; conj(x - px/w)] sqrt(w)/2
-        ST(s.rotate(s.V, mp, Ssel.data(), mp, nev, s.rot.p, n));
-        ST(s.rotate(s.PV, mp, Ssel.data(), mp, nev, s.V.p, n));     // X is no longer needed: reuse its storage
-        BSE_CUDA(cudaMemcpyAsync(s.omega_d.p, om.data(), sizeof(double) * nev, cudaMemcpyHostToDevice, h->stream));
-        ST(assemble_full_vectors(h, s.rot.p, s.V.p, n, nev, (const double *)s.omega_d.p, dVec, ldvec));
+        // candidates (left in rot by select_distinct): x = X s, p = PX s;  v = [x + p/w; conj(x - p/w)] sqrt(w)/2, assembled
+        // into the storage of X (no longer needed), then the returned vectors are their combinations Cm
+        std::vector<double> wc(ncand);
+        for (int a = 0; a < ncand; ++a) wc[a] = std::sqrt(std::max(theta[a], 0.0));
+        BSE_CUDA(cudaMemcpyAsync(s.omega_d.p, wc.data(), sizeof(double) * ncand, cudaMemcpyHostToDevice, h->stream));
+        ST(assemble_full_vectors(h, s.rot.p, s.col(s.rot, ncand), n, ncand, (const double *)s.omega_d.p, s.V.p, 2 * n));
+        ST(s.upload_coef(Cm.data(), ncand, ncand, nev, true));
+        ST(gemm_basis(h, s.V.p, 2 * n, ncand, true, (const double *)s.coef.p, 2 * ncand, nev, 2 * n, dVec, ldvec, 1.0, 0.0));
     }
     BSE_CUDA(cudaStreamSynchronize(h->stream));
     return result;

@@ -8,17 +8,25 @@ from gpu_util import pack, to_dev, to_host
 
 pytestmark = pytest.mark.gpu
 TOL_EIG, TOL_RES, TOL_ORTH = 1e-10, 1e-8, 1e-12
+# Reading R8: the eigenvalue error of a Ritz pair is ~ residual^2 / gap.  At the literal sigma = 0
+# configs the wanted eigenvalues are ~1e-2 with gaps ~1e-2 and ||R|| ~ 11, so "1e-10 relative" asks for 1e-12 absolute
+# and residuals of 1e-8 ||R|| (eigenvalue error ~1e-12) leave no margin: configs 0 and 1, whose tolerance BASELINE.json
+# does not state, are solved with tol = 1e-10.  Configs 2 and 4 state tol 1e-8 and are certified through their residuals.
+TOL_SMALL = 1e-10
 
 
 def _check_tda(orc, R, res, nev, w_ref):
+    """north_star: eigenvalues to 1e-10 RELATIVE (no absolute escape: DESIGN.md section 2, reading R8 says which tol the
+    small-eigenvalue configs are solved with), residuals through the oracle apply, orthonormality of the vectors and of
+    the final Krylov basis."""
     w, V = res.omega, to_host(res.vectors)
     nrm = np.max(np.abs(np.linalg.eigvalsh(R)[[0, -1]]))
-    assert np.max(np.abs(w - w_ref[:nev]) / np.maximum(np.abs(w_ref[:nev]), 1e-300)) <= TOL_EIG or \
-        np.max(np.abs(w - w_ref[:nev])) <= TOL_EIG * 1e-2 * nrm
+    assert np.max(np.abs(w - w_ref[:nev]) / np.abs(w_ref[:nev])) <= TOL_EIG
     r = np.linalg.norm(orc.apply_tda(R, V) - V * w, axis=0)
     assert np.all(r <= TOL_RES * nrm)
     assert np.all(r <= 10 * res.resid + 1e-11 * nrm)            # the solver's own estimate is honest
     assert np.linalg.norm(V.conj().T @ V - np.eye(nev)) <= TOL_ORTH
+    assert res.info["basis_orth_err"] <= TOL_ORTH                # ||V^H V - I||_F of the whole final basis
 
 
 @pytest.mark.parametrize("sigma", [0.0, 1.0])
@@ -27,7 +35,7 @@ def test_config0_tda_vs_oracle_lanczos(orc, sigma):
     cfg = gen.CONFIGS[0]
     N, nev, k = cfg["N"], cfg["nev"], cfg["k"]
     R = gen.dense_R(N, 1, sigma=sigma, group=cfg["group"])
-    res = b.Bse(b.MODE_TDA, N, pack(R, 0)).solve(nev, k, tol=1e-8, seed=1)
+    res = b.Bse(b.MODE_TDA, N, pack(R, 0)).solve(nev, k, tol=TOL_SMALL, seed=1)
     w_o, V_o, r_o, steps = orc.lanczos_tda(R, nev, 1e-10, gen.block_X(N, 1, 99)[:, 0], check=20)
     assert steps > 0
     # eigenvalues are unique: single-vector oracle and block GPU solver must agree
@@ -66,15 +74,18 @@ def _H_dense(R, C):
 def _check_full(orc, R, C, res, nev, om_ref):
     N = R.shape[0]
     om, V = res.omega, to_host(res.vectors)
-    nref = min(nev, len(om_ref))
-    assert np.max(np.abs(om[:nref] - om_ref[:nref]) / om_ref[:nref]) <= TOL_EIG
+    assert len(om_ref) >= nev
+    assert np.max(np.abs(om - om_ref[:nev]) / om_ref[:nev]) <= TOL_EIG
     HV = orc.apply_full(R, C, V)
     nrm = np.linalg.norm(_H_dense(R, C), 2) if N <= 600 else 12.0
     r = np.linalg.norm(HV - V * om, axis=0) / np.linalg.norm(V, axis=0)
     assert np.all(r <= TOL_RES * nrm)
     Sig = np.concatenate([np.ones(N), -np.ones(N)])
     G = V.conj().T @ (Sig[:, None] * V)
-    assert np.linalg.norm(G - np.eye(nev)) <= 1e-7              # Sigma-orthonormal, X^H X - Y^H Y = 1 (S9, S10)
+    # Reading S10: the 1e-12 figure is for the basis, orthonormal in <x, z>_P = Re(x^H P(z)); eigenvectors of distinct
+    # omega are Sigma-orthogonal only to their own accuracy (residual / gap), their normalisation X^H X - Y^H Y = 1 is exact
+    assert res.info["basis_orth_err"] <= TOL_ORTH
+    assert np.linalg.norm(G - np.eye(nev)) <= 1e-7
     assert np.max(np.abs(np.diag(G) - 1)) <= 1e-10
     # -omega partner [conj(Y); conj(X)]
     Pn = np.vstack([V[N:].conj(), V[:N].conj()])
@@ -110,17 +121,12 @@ def test_config1_full_vs_oracle_golden(orc):
     cfg = gen.CONFIGS[1]
     N, nev, k = cfg["N"], cfg["nev"], cfg["k"]
     R = gen.dense_R(N, 1, sigma=cfg["sigma"]); C = gen.dense_C(N, 1)
-    res = b.Bse(b.MODE_FULL, N, pack(R, 0), pack(C, 1)).solve(nev, k, tol=1e-8, seed=1)
-    # Reading R1: every omega^2 is a DOUBLE eigenvalue of G = M o P on C^N ~ R^2N.  The single-vector
-    # oracle converged both copies (after 1500 steps its 20 lowest Ritz values are 10 pairs agreeing to 1e-13), so the
-    # stored list holds the 10 lowest distinct omega, each twice; the CUDA solver returns 20 distinct omega.
+    res = b.Bse(b.MODE_FULL, N, pack(R, 0), pack(C, 1)).solve(nev, k, tol=TOL_SMALL, seed=1)
+    # Reading R1: every omega^2 is a DOUBLE eigenvalue of G = M o P on C^N ~ R^2N; oracle and CUDA solver
+    # both count eigenvectors of H (the copy is recognised by its vector), so the stored list is 20 distinct omega.
     gold = _golden("oracle_config1.txt")
-    distinct = [gold[0]]
-    for x in gold[1:]:
-        if x - distinct[-1] > 1e-7 * x:
-            distinct.append(x)
-    assert len(distinct) == 10 and np.all(np.diff(res.omega) > 1e-7 * res.omega[1:])
-    _check_full(orc, R, C, res, nev, np.array(distinct))
+    assert len(gold) == nev and np.all(np.diff(gold) > 1e-6 * gold[1:])
+    _check_full(orc, R, C, res, nev, gold)
 
 
 def test_config0_matches_stored_oracle_values(orc):
@@ -128,10 +134,9 @@ def test_config0_matches_stored_oracle_values(orc):
     cfg = gen.CONFIGS[0]
     for sigma in (0.0, 1.0):
         R = gen.dense_R(cfg["N"], 1, sigma=sigma, group=cfg["group"])
-        res = b.Bse(b.MODE_TDA, cfg["N"], pack(R, 0)).solve(cfg["nev"], cfg["k"], tol=1e-8, seed=5)
+        res = b.Bse(b.MODE_TDA, cfg["N"], pack(R, 0)).solve(cfg["nev"], cfg["k"], tol=TOL_SMALL, seed=5)
         ref = _golden(f"oracle_config0_sigma{int(sigma)}.txt")
-        assert np.max(np.abs(res.omega - ref)) <= TOL_EIG * 1e-2 * 11.0 or \
-            np.max(np.abs(res.omega - ref) / np.abs(ref)) <= TOL_EIG
+        assert np.max(np.abs(res.omega - ref) / np.abs(ref)) <= TOL_EIG
 
 
 def test_full_closed_form_pair():
@@ -196,7 +201,7 @@ def test_config3_size_closed_form_pair():
     """Config 3's size (full mode, N = 32768, operator 65536) on the closed-form pair with omega = sqrt(d1 d2)."""
     import torch
     import paper_2504_10096_b200 as b
-    N, nev, k = 32768, 16, 4
+    N, nev, k = 32768, 100, 4
     if torch.cuda.mem_get_info()[0] < 30e9:
         pytest.skip("needs 30 GB of free device memory")
     d1 = gen.prescribed_spectrum(N, 7, 1.0, 9.0, power=2 / 3); d2 = gen.prescribed_spectrum(N, 8, 2.0, 5.0, power=2 / 3)
@@ -208,21 +213,21 @@ def test_config3_size_closed_form_pair():
     assert np.max(np.abs(res.omega - exact) / exact) <= TOL_EIG
     # the same stores in the real form of Eq. (3) (S = R + C, D = R - C), block k = 8
     b.bse_to_real_form(rt, ct, N)
-    # (ncv = 160: with the default basis of 64 columns a block of 8 leaves two to four block steps per restart cycle and the
-    # run needs close to the 1000 restarts allowed -- it then passes or fails with the summation order of the atomics)
-    res = b.Bse(b.MODE_FULL, N, rt, ct, storage=b.STORE_REAL_FORM).solve(nev, 8, ncv=160, tol=1e-8, seed=4)
+    res = b.Bse(b.MODE_FULL, N, rt, ct, storage=b.STORE_REAL_FORM).solve(nev, 8, tol=1e-8, seed=4)
     assert np.max(np.abs(res.omega - exact) / exact) <= TOL_EIG
+    assert res.info["basis_orth_err"] <= TOL_ORTH
 
 
 def test_config4_size_closed_form():
-    """Config 4's size (N = 98304, 77 GB operand) with a prescribed spectrum; a reduced request (nev = 24, k = 8)
-    keeps the test short -- the full nev = 500 run is a bench item."""
+    """Config 4's size and request (N = 98304, 77 GB operand, nev = 500, k = 8, tol 1e-8) with a prescribed spectrum:
+    the restart logic at a basis of 1000 columns with hundreds of locked pairs, against exactly known eigenvalues."""
     import torch
     if torch.cuda.mem_get_info()[0] < 100e9:
         pytest.skip("needs 100 GB of free device memory")
     h, lam = _closed_tda(98304, 23)
-    res = h.solve(24, 8, tol=1e-8, seed=2)
-    assert np.max(np.abs(res.omega - lam[:24]) / lam[:24]) <= TOL_EIG
+    res = h.solve(500, 8, tol=1e-8, seed=2)
+    assert np.max(np.abs(res.omega - lam[:500]) / lam[:500]) <= TOL_EIG
+    assert res.info["basis_orth_err"] <= TOL_ORTH
 
 
 @pytest.mark.parametrize("seed", [2, 3])
@@ -231,7 +236,7 @@ def test_config0_other_matrix_seeds(orc, seed):
     import paper_2504_10096_b200 as b
     cfg = gen.CONFIGS[0]
     R = gen.dense_R(cfg["N"], seed, sigma=1.0, group=cfg["group"])
-    res = b.Bse(b.MODE_TDA, cfg["N"], pack(R, 0)).solve(cfg["nev"], cfg["k"], tol=1e-8, seed=seed)
+    res = b.Bse(b.MODE_TDA, cfg["N"], pack(R, 0)).solve(cfg["nev"], cfg["k"], tol=TOL_SMALL, seed=seed)
     _check_tda(orc, R, res, cfg["nev"], np.linalg.eigvalsh(R))
     w_o, _, _, steps = orc.lanczos_tda(R, cfg["nev"], 1e-10, gen.block_X(cfg["N"], 1, 90 + seed)[:, 0], check=20)
     assert steps > 0 and np.max(np.abs(res.omega - w_o) / np.abs(w_o)) <= TOL_EIG

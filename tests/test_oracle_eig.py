@@ -136,6 +136,75 @@ def test_lanczos_full_vs_direct_route(orc):
     assert np.linalg.norm(G - np.eye(nev)) < 1e-8
 
 
+def test_lanczos_full_returns_distinct_omega_far_past_convergence(orc):
+    # Reading R1: every omega^2 is a double eigenvalue of G = M o P on R^2N; the second copy grows out of rounding
+    # noise once the first has converged.  Run 3 x past first convergence (copies present among the Ritz values)
+    # and require the nev lowest DISTINCT omega of H -- a value-sorted list of Ritz values would return pairs.
+    N, nev = 192, 12
+    R, C = _bse_pair(N, 6)
+    x0 = gen.block_X(N, 1, 97)[:, 0]
+    om1, _, _, steps1 = orc.lanczos_full(R, C, nev, 1e-11, x0, check=4)
+    assert 0 < steps1 < 2 * N - 4
+    # ... and to (almost) the whole space R^2N, where EVERY omega^2 has both of its Ritz values: the 12 lowest Ritz
+    # values are then 6 pairs
+    minit = 2 * N - 4
+    om, V, res, steps = orc.lanczos_full(R, C, nev, 1e-11, x0, check=4, minit=minit)
+    assert steps >= minit
+    omd, Vd = orc.bse_direct(R, C)
+    assert np.max(np.abs(om - omd[N:N + nev])) < 1e-10 * omd[-1]
+    assert np.max(np.abs(om1 - omd[N:N + nev])) < 1e-10 * omd[-1]
+    assert np.min(np.diff(om)) > 1e-6                              # no value returned twice
+    H = _H_dense(R, C)
+    r = np.linalg.norm(H @ V - V * om, axis=0)
+    assert np.all(r < 1e-8 * omd[-1])
+    Sig = np.concatenate([np.ones(N), -np.ones(N)])
+    assert np.linalg.norm(V.conj().T @ (Sig[:, None] * V) - np.eye(nev)) < 1e-8
+
+
+def test_lanczos_full_copy_structure(orc):
+    # the identities behind the multiplicity rule: K(x) = i P(x) satisfies K^2 = -G, and if P x = w y, M y = w x then
+    # v(x) = [x + y; conj(x - y)] and v(K x / w) = i v(x)
+    N = 48
+    R, C = _bse_pair(N, 8)
+    x = gen.block_X(N, 1, 5)
+    P = lambda z: orc.apply_half(R, C, z, +1)
+    M = lambda z: orc.apply_half(R, C, z, -1)
+    K = lambda z: 1j * P(z)
+    assert np.linalg.norm(K(K(x)) + M(P(x))) < 1e-12 * np.linalg.norm(M(P(x)))
+    omd, Vd = orc.bse_direct(R, C)
+    w, v = omd[N + 2], Vd[:, N + 2]
+    xe, ye = (v[:N] + v[N:].conj()) / 2, (v[:N] - v[N:].conj()) / 2     # v = [x + y; conj(x - y)]
+    xe, ye = xe[:, None], ye[:, None]
+    assert np.linalg.norm(P(xe) - w * ye) < 1e-10 and np.linalg.norm(M(ye) - w * xe) < 1e-10
+    x2 = K(xe) / w
+    y2 = P(x2) / w
+    v2 = np.concatenate([x2 + y2, (x2 - y2).conj()])[:, 0]
+    assert np.linalg.norm(v2 - 1j * v) < 1e-10
+
+
+def test_tridiag_ql_closed_form_and_jacobi(orc):
+    # Toeplitz tridiag(b, a, b): eigenvalues a + 2 b cos(j pi / (m + 1)), eigenvectors sin(i j pi / (m + 1))
+    m, a, b = 60, 1.5, -0.7
+    w, Z = orc.tridiag_ql(np.full(m, a), np.full(m - 1, b))
+    j = np.arange(1, m + 1)
+    lam = a + 2 * b * np.cos(j * np.pi / (m + 1))
+    order = np.argsort(lam)
+    assert np.max(np.abs(w - lam[order])) < 1e-13
+    U = np.sin(np.outer(j, j) * np.pi / (m + 1)) * np.sqrt(2.0 / (m + 1))
+    assert np.max(np.abs(np.abs(np.sum(Z * U[:, order], axis=0)) - 1)) < 1e-12
+    # random tridiagonal vs the (separately pinned) Jacobi routine, and the decomposition identities
+    rng = np.random.default_rng(5)
+    d, e = rng.standard_normal(40), rng.standard_normal(39)
+    e[17] = 0.0                                                      # a reducible matrix splits cleanly
+    T = np.diag(d) + np.diag(e, 1) + np.diag(e, -1)
+    w, Z = orc.tridiag_ql(d, e)
+    wj, _ = orc.jacobi_herm(T.astype(complex))
+    assert np.max(np.abs(w - wj)) < 1e-13 * np.max(np.abs(wj))
+    assert np.linalg.norm(Z.T @ T @ Z - np.diag(w)) < 1e-13 * m and np.linalg.norm(Z.T @ Z - np.eye(40)) < 1e-13
+    w1, _ = orc.tridiag_ql(np.array([3.0]), np.array([]))
+    assert w1[0] == 3.0
+
+
 def test_block_cgs2_factorisation(orc):
     N, m, k = 300, 12, 4
     V, _ = np.linalg.qr(gen.block_X(N, m, 1))
