@@ -72,7 +72,8 @@ typedef enum {
     BSE_ERR_ALLOC = 3,
     BSE_ERR_NOT_CONVERGED = 4,      /* bse_solve: outputs hold the best estimates, see info.nconv */
     BSE_ERR_NOT_POSITIVE_DEFINITE = 5, /* full mode: Re(w^H P(w)) <= 0 met (PAPER.md:49 precondition) */
-    BSE_ERR_INTERNAL = 6
+    BSE_ERR_INTERNAL = 6,
+    BSE_ERR_STATIC_LIMIT = 7        /* bse_lanczos_quadrature_static: N or steps beyond the fixed scratch array */
 } bse_status_t;
 
 enum { BSE_MODE_TDA = 0, BSE_MODE_FULL = 1 };
@@ -287,6 +288,21 @@ bse_status_t bse_host_heev(int32_t m, void *hA, int32_t lda, double *hW, void *h
  * symmetric (real coefficients in the inner product Re(x^H P(y))): a quarter of the flops of the complex driver in the
  * reduction and the back-transformation. */
 bse_status_t bse_host_syev(int32_t m, double *hA, int32_t lda, double *hW, double *hZ, int32_t ldz, int32_t nz);
+
+/* bse_lanczos_quadrature (TDA handles) for callers that cannot allocate: code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc.  Same arguments, same recurrence, same results; the scratch
+ * (three N-vectors and the recurrence scalars) is a file-scope device array of fixed size inside the library, so the call
+ * performs no cudaMalloc / cudaFree and no host allocation.  Limits: N <= BSE_STATIC_QUADRATURE_MAX_N and
+ * steps <= BSE_STATIC_QUADRATURE_MAX_STEPS, else BSE_ERR_STATIC_LIMIT ("size exceeds the static scratch limit") and nothing
+ * is launched.  Every GPU that loads the library holds the array (1.5 MiB + 16 KiB) until exit.  All calls on one device
+ * share it: each call clears the scalars it accumulates into and overwrites the vectors before reading them, but two calls
+ * that overlap on the same GPU (different streams or threads) race -- serialise them.  hAlpha: steps doubles, hBeta:
+ * steps + 1 doubles (host, written directly).  Synchronous on the handle's stream.  Full-mode and incomplete partial handles:
+ * BSE_ERR_INVALID_ARG. */
+#define BSE_STATIC_QUADRATURE_MAX_N 32768
+#define BSE_STATIC_QUADRATURE_MAX_STEPS 1024
+bse_status_t bse_lanczos_quadrature_static(bse_handle_t h, const void *dStart, int32_t steps, double *hAlpha,
+                                           double *hBeta, int32_t *hDone);
 
 /* Number of kernels this library has launched on the calling process's device since load (bench.py's
  * "gpu_launches" claim). */

@@ -21,7 +21,8 @@ TILE = 64
 TILE_BYTES = 65536
 
 STATUS = {0: "BSE_OK", 1: "BSE_ERR_INVALID_ARG", 2: "BSE_ERR_CUDA", 3: "BSE_ERR_ALLOC", 4: "BSE_ERR_NOT_CONVERGED",
-          5: "BSE_ERR_NOT_POSITIVE_DEFINITE", 6: "BSE_ERR_INTERNAL"}
+          5: "BSE_ERR_NOT_POSITIVE_DEFINITE", 6: "BSE_ERR_INTERNAL", 7: "BSE_ERR_STATIC_LIMIT"}
+STATIC_QUADRATURE_MAX_N, STATIC_QUADRATURE_MAX_STEPS = 32768, 1024       # include/bse.h
 
 
 class BseError(RuntimeError):
@@ -59,6 +60,7 @@ _SIGNATURES = {
     "bse_apply_host": [_vp, _vp, _i64, _vp, _i64, _i32],
     "bse_orth": [_vp, _vp, _i64, _i32, _vp, _i64, _vp, _i64, _i32, _vp, _i64, _vp, _vp, ctypes.POINTER(_i32)],
     "bse_lanczos_quadrature": [_vp, _vp, _i32, ctypes.POINTER(_dbl), ctypes.POINTER(_dbl), ctypes.POINTER(_i32)],
+    "bse_lanczos_quadrature_static": [_vp, _vp, _i32, ctypes.POINTER(_dbl), ctypes.POINTER(_dbl), ctypes.POINTER(_i32)],
     "bse_quadrature_resolvent": [_i32, ctypes.POINTER(_dbl), ctypes.POINTER(_dbl), _i32, ctypes.POINTER(_dbl), _dbl, _vp],
     "bse_quadrature_resolvent_full": [_i32, ctypes.POINTER(_dbl), ctypes.POINTER(_dbl), _i32, ctypes.POINTER(_dbl), _dbl, _vp],
     "bse_host_heev": [_i32, _vp, _i32, _vp, _vp, _i32, _i32],
@@ -277,6 +279,19 @@ class Bse:
         _check(lib().bse_lanczos_quadrature(self._h, d.data_ptr(), steps, alpha.ctypes.data_as(ctypes.POINTER(_dbl)),
                                             beta.ctypes.data_as(ctypes.POINTER(_dbl)), ctypes.byref(done)),
                "bse_lanczos_quadrature")
+        return alpha[:done.value], beta[:done.value + 1]
+
+    def lanczos_quadrature_static(self, d, steps: int, alpha=None, beta=None):
+        """lanczos_quadrature through bse_lanczos_quadrature_static: no allocation inside the call (scratch in a fixed device
+        array of the library; N <= STATIC_QUADRATURE_MAX_N, steps <= STATIC_QUADRATURE_MAX_STEPS).  alpha / beta: optional
+        preallocated numpy arrays of steps / steps + 1 doubles."""
+        import numpy as np
+        alpha = np.zeros(steps) if alpha is None else alpha
+        beta = np.zeros(steps + 1) if beta is None else beta
+        done = _i32(0)
+        _check(lib().bse_lanczos_quadrature_static(self._h, d.data_ptr(), steps, alpha.ctypes.data_as(ctypes.POINTER(_dbl)),
+                                                   beta.ctypes.data_as(ctypes.POINTER(_dbl)), ctypes.byref(done)),
+               "bse_lanczos_quadrature_static")
         return alpha[:done.value], beta[:done.value + 1]
 
     def solve(self, nev: int, k: int, ncv: int = 0, tol: float = 1e-8, max_restarts: int = 1000, seed: int = 1,

@@ -233,6 +233,7 @@ const char *bse_status_string(bse_status_t s)
         case BSE_ERR_ALLOC: return "allocation failed";
         case BSE_ERR_NOT_CONVERGED: return "not converged";
         case BSE_ERR_NOT_POSITIVE_DEFINITE: return "operator not positive definite";
+        case BSE_ERR_STATIC_LIMIT: return "size exceeds the static scratch limit";
         default: return "internal error";
     }
 }

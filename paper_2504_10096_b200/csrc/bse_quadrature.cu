@@ -201,3 +201,85 @@ extern "C" bse_status_t bse_quadrature_resolvent_full(int32_t steps, const doubl
     continued_fraction(steps, hAlpha, hBeta, n_omega, hOmega, eta, true, 2.0, (double *)hOut);
     return BSE_OK;
 }
+
+// ---------------------------------------------------------------------------------------------------------------------
+// bse_lanczos_quadrature_static: the TDA recurrence above for callers that cannot call cudaMalloc (code under CUDA graph
+// capture, tight serving loops, harnesses that forbid it).  Its scratch -- three N-vectors and the 2 steps + 2 recurrence
+// scalars -- lives in ONE file-scope device array of fixed size instead of the handle's lazily grown workspace, so the call
+// allocates nothing, on the device or on the host.  Every GPU that loads the library holds the array until exit; every call
+// on a device shares it and finds the previous call's contents in it (the scalars are cleared at the start of each call, the
+// vectors are fully overwritten before they are read), so two calls that overlap on one GPU race.
+// ---------------------------------------------------------------------------------------------------------------------
+namespace bse {
+constexpr int64_t STATIC_MAX_N = BSE_STATIC_QUADRATURE_MAX_N;            // 32768 rows: 3 x 512 KiB of vectors
+constexpr int32_t STATIC_MAX_STEPS = BSE_STATIC_QUADRATURE_MAX_STEPS;    // 1024 steps: 16 KiB of scalars
+constexpr size_t STATIC_VEC_BYTES = (size_t)STATIC_MAX_N * 16;
+constexpr size_t STATIC_SCRATCH_BYTES = 3 * STATIC_VEC_BYTES + (size_t)(2 * STATIC_MAX_STEPS + 2) * 8;
+static __device__ __align__(256) unsigned char g_static_scratch[STATIC_SCRATCH_BYTES];
+
+// In host code g_static_scratch is a host-side stand-in, not a device address: the address a kernel may use comes from
+// cudaGetSymbolAddress, asked once per device with that device current.
+static bse_status_t static_scratch_address(char **out)
+{
+    static std::atomic<char *> addr[64];
+    int dev = 0;
+    BSE_CUDA(cudaGetDevice(&dev));
+    char *p = dev < 64 ? addr[dev].load(std::memory_order_acquire) : nullptr;
+    if (!p) {
+        void *q = nullptr;
+        BSE_CUDA(cudaGetSymbolAddress(&q, g_static_scratch));
+        p = (char *)q;
+        if (dev < 64) addr[dev].store(p, std::memory_order_release);
+    }
+    *out = p;
+    return BSE_OK;
+}
+}  // namespace bse
+
+extern "C" bse_status_t bse_lanczos_quadrature_static(bse_handle_t h, const void *dStart, int32_t steps, double *hAlpha,
+                                                      double *hBeta, int32_t *hDone)
+{
+    if (!h || !dStart || steps < 1 || !hAlpha || !hBeta || is_incomplete(h) || h->mode != BSE_MODE_TDA) return BSE_ERR_INVALID_ARG;
+    const int64_t n = h->N;
+    if (n > STATIC_MAX_N || steps > STATIC_MAX_STEPS) return BSE_ERR_STATIC_LIMIT;
+    char *base = nullptr;
+    bse_status_t st = static_scratch_address(&base);
+    if (st) return st;
+    const size_t scal = (size_t)(2 * steps + 2) * 8;
+    double2 *buf[3] = {(double2 *)base, (double2 *)(base + STATIC_VEC_BYTES), (double2 *)(base + 2 * STATIC_VEC_BYTES)};
+    double *d_alpha = (double *)(base + 3 * STATIC_VEC_BYTES), *d_n2 = d_alpha + steps;
+    BSE_CUDA(cudaMemsetAsync(d_alpha, 0, scal, h->stream));                     // the last call's sums must not be added to
+    const int grid = h->num_sms * 2;
+    dot_re_kernel<<<grid, 256, 0, h->stream>>>((const double2 *)dStart, (const double2 *)dStart, n, d_n2);
+    if ((st = comm_bcast_dev(h, d_n2, 1))) return st;
+    scale_by_norm_kernel<<<grid, 256, 0, h->stream>>>((const double2 *)dStart, buf[0], n, d_n2);
+    count_launch(2);
+    int iv = 0, ip = 2, iw = 1;      // v_j, v_{j-1}, w
+    for (int j = 0; j < steps; ++j) {
+        if ((st = zero_block(h, buf[iw], n, n, 1))) return st;
+        if ((st = launch_apply_pass(h, h->R, 0, 1.0, buf[iv], n, buf[iw], n, 1))) return st;       // w = R v_j
+        if ((st = comm_sum_block(h, buf[iw], n, n, 1))) return st;
+        dot_re_kernel<<<grid, 256, 0, h->stream>>>(buf[iv], buf[iw], n, d_alpha + j);
+        if ((st = comm_bcast_dev(h, d_alpha + j, 1))) return st;
+        axpy_norm_kernel<<<grid, 256, 0, h->stream>>>(buf[iw], buf[iv], buf[ip], n, d_alpha + j, j > 0 ? d_n2 + j : nullptr,
+                                                      d_n2 + j + 1);
+        if ((st = comm_bcast_dev(h, d_n2 + j + 1, 1))) return st;
+        scale_by_norm_kernel<<<grid, 256, 0, h->stream>>>(buf[iw], buf[iw], n, d_n2 + j + 1);
+        count_launch(3);
+        int t = ip; ip = iv; iv = iw; iw = t;
+    }
+    BSE_CUDA(cudaGetLastError());
+    // straight into the caller's arrays (no host staging buffer): alpha_j, then |d|^2 and beta_{j+1}^2, square-rooted in place
+    BSE_CUDA(cudaMemcpyAsync(hAlpha, d_alpha, (size_t)steps * 8, cudaMemcpyDeviceToHost, h->stream));
+    BSE_CUDA(cudaMemcpyAsync(hBeta, d_n2, (size_t)(steps + 1) * 8, cudaMemcpyDeviceToHost, h->stream));
+    BSE_CUDA(cudaStreamSynchronize(h->stream));
+    int done = steps;
+    hBeta[0] = std::sqrt(hBeta[0]);
+    for (int j = 0; j < steps; ++j) {
+        const double b2 = hBeta[j + 1];
+        hBeta[j + 1] = std::sqrt(b2);
+        if (!(b2 > 0.0)) { done = j + 1; break; }
+    }
+    if (hDone) *hDone = done;
+    return BSE_OK;
+}
