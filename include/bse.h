@@ -304,6 +304,22 @@ bse_status_t bse_host_syev(int32_t m, double *hA, int32_t lda, double *hW, doubl
 bse_status_t bse_lanczos_quadrature_static(bse_handle_t h, const void *dStart, int32_t steps, double *hAlpha,
                                            double *hBeta, int32_t *hDone);
 
+/* Microbenchmarks behind the roofline denominators (north_star: "achieved HBM GB/s and FP64 pipe utilisation ... against
+ * the chip's peaks"; MEASURED_PEAKS.json has no FP64 figure).  Each runs one warm-up and one timed launch of a kernel that
+ * does nothing else, on one CTA per SM, timed with CUDA events on `stream`; synchronous.
+ *   BSE_PEAK_DMMA           : FP64 tensor pipe, mma.sync m8n8k4 f64 (DMMA.8x8x4); p1 = warps per SM (default 8), p2 =
+ *                             independent accumulator chains per warp (1, 2, 4, 8 or 12; default 8); p2 = -1: twelve chains
+ *                             with the three-product role's mix of plain FP64 adds (8 DADD per 12 DMMA); TFLOP/s of the DMMAs
+ *   BSE_PEAK_DFMA           : plain FP64 FMA, 8 chains per thread; p1 = warps per SM (default 32); result TFLOP/s
+ *   BSE_PEAK_BULK_READ      : read-only stream of dBuf (device, buf_bytes) through cp.async.bulk into a shared-memory ring
+ *                             of p2 stages (default 3) of p1 bytes (default 65536) -- the apply kernels' data path; GB/s
+ *   BSE_PEAK_BULK_READ_SMEM : the same with every byte read back from shared memory by the consumer warp; GB/s
+ *   BSE_PEAK_RED            : red.global.add.f64 scattered over dBuf (buf_bytes / 8 doubles, which it modifies); G atomics/s
+ * hMs (nullable): duration of the timed launch in ms.  Errors: BSE_ERR_INVALID_ARG, BSE_ERR_CUDA. */
+enum { BSE_PEAK_DMMA = 0, BSE_PEAK_DFMA = 1, BSE_PEAK_BULK_READ = 2, BSE_PEAK_BULK_READ_SMEM = 3, BSE_PEAK_RED = 4 };
+bse_status_t bse_selftest_peak(int32_t what, int32_t p1, int32_t p2, void *dBuf, int64_t buf_bytes, void *stream,
+                               double *hResult, double *hMs);
+
 /* Number of kernels this library has launched on the calling process's device since load (bench.py's
  * "gpu_launches" claim). */
 int64_t bse_launch_count(void);

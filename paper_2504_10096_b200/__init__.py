@@ -67,6 +67,7 @@ _SIGNATURES = {
     "bse_host_syev": [_i32, _vp, _i32, _vp, _vp, _i32, _i32],
     "bse_solve": [_vp, _i32, _i32, _i32, _dbl, _i32, _u64, ctypes.POINTER(_dbl), _vp, _i64, ctypes.POINTER(_dbl),
                   ctypes.POINTER(_Info)],
+    "bse_selftest_peak": [_i32, _i32, _i32, _vp, _i64, _vp, ctypes.POINTER(_dbl), ctypes.POINTER(_dbl)],
 }
 EXPORTS = sorted(list(_SIGNATURES) + ["bse_status_string", "bse_launch_count"])
 
@@ -452,6 +453,18 @@ def quadrature_resolvent_full(alpha, beta, omega, eta: float):
                                                omega.ctypes.data_as(P), eta, out.ctypes.data),
            "bse_quadrature_resolvent_full")
     return out
+
+
+PEAK_DMMA, PEAK_DFMA, PEAK_BULK_READ, PEAK_BULK_READ_SMEM, PEAK_RED = 0, 1, 2, 3, 4
+
+
+def selftest_peak(what: int, p1: int = 0, p2: int = 0, buf=None):
+    """One of the library's microbenchmarks (include/bse.h): (rate, ms).  TFLOP/s, GB/s or G atomics/s."""
+    r, ms = _dbl(), _dbl()
+    _check(lib().bse_selftest_peak(what, p1, p2, buf.data_ptr() if buf is not None else None,
+                                   buf.numel() * buf.element_size() if buf is not None else 0, _stream_ptr(),
+                                   ctypes.byref(r), ctypes.byref(ms)), "bse_selftest_peak")
+    return r.value, ms.value
 
 
 def launch_count() -> int:
