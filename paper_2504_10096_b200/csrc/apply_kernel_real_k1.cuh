@@ -1,34 +1,25 @@
-// Single-column variant of the tile kernels of apply_tiles.cuh (k = 1: the paper's own iteration generates its vectors "one by one",
-// PAPER.md:71, and the Lanczos-with-quadrature solver is a single-vector recurrence).
-//
-// With one column the 8-wide N dimension of a DMMA is 3/4 empty, so the tensor-core kernel pays the FP64 work (and
-// the power) of k = 4.  Here the same tile ring feeds plain complex FMAs, and -- with no MMA fragment layout to
-// honour -- every entry is loaded (and, for the complex64 store, widened) ONCE and used for both products.  Lane
-// (g, t) of consumer warp w reads, per 8 x 8 patch (ib, jb = w) and s = 0, 1, the entry
-//     a = T[r][c],  r = 8 ib + g,  c = 8 w + 4 s + t          (the conflict-free P1 fragment read)
-//     P1:  acc1[ib] += a * xj[s]            (xj = x_J[c] or conj(x_J[c]))          -> Y_I[r], summed over t and s
-//     P2:  acc2[s]  += a * conj(x_I[r])                                           -> Y_J[c], summed over ib and g
-// acc1 is summed over the four t-lanes once per unit, acc2 over the eight g-lanes once per tile (warp shuffles),
-// then added to Y with red.global.add.f64.  HERM: Y_J += conj(acc2) (= T^H x_I);  SYMC: Y_J += acc2 (= T^T conj(x_I)).
-// 128 DFMA and 16 shared-memory loads per tile per warp.
+// Single-column kernels of the real-form store (Eq. 3; roles and modes as RoleReal in apply_tiles.cuh).
 #pragma once
-#include "apply_common.cuh"
+#include "apply_kernel_k1.cuh"
 
 namespace bse {
 
-__device__ __forceinline__ void cfma(double2 &acc, const double2 a, const double2 x)
+// Single-column variant of apply_tiles_kernel<ES, RoleReal<MODE>> (plain FMAs, every entry loaded once and used for both products, as in
+// apply_kernel_k1.cuh): per stored entry (Ar, Ai) two FMAs for P1 and two for P2 -- half of the complex single-column
+// kernel -- so that the binary32-plane store, whose DMMA kernel is bound by the tensor pipe for every k, streams at the
+// HBM rate when k = 1 (the full-mode quadrature recurrence at the paper's precision).
+//   MODE 0:  (re_I, im_I) += (Ar, Ai) a_J;    re_J += Ar a_I + Ai b_I
+//   MODE 1:  (re_I, im_I) += (-Ai, Ar) b_J;   im_J += Ar b_I - Ai a_I
+template <int MODE> __device__ __forceinline__ void rfma1(double2 &acc, const double2 a, const double xs)
 {
-    acc.x = fma(a.x, x.x, acc.x); acc.x = fma(-a.y, x.y, acc.x);
-    acc.y = fma(a.x, x.y, acc.y); acc.y = fma(a.y, x.x, acc.y);
+    if (MODE == 0) { acc.x = fma(a.x, xs, acc.x); acc.y = fma(a.y, xs, acc.y); }
+    else { acc.x = fma(-a.y, xs, acc.x); acc.y = fma(a.x, xs, acc.y); }
 }
 
-// NW consumer warps (8 or 16) + the producer warp.  NW = 16 (warp w owns tile columns 4w .. 4w+3: half a patch
-// column, s = w & 1 of patch column jb = w >> 1; four consumer warps per scheduler, 96 registers) was measured
-// SLOWER than NW = 8 at N = 98304 (complex64 store 7.6 vs 7.0 ms, complex128 12.1 vs 11.1 ms): only NW = 8 is
-// instantiated.
-template <int ES, int NW>
-__global__ void __launch_bounds__((NW + 1) * 32, 1) apply_tiles_k1_kernel(const ApplyParams p)
+template <int ES, int MODE>
+__global__ void __launch_bounds__(APPLY_THREADS, 1) apply_tiles_real_k1_kernel(const ApplyParams p)
 {
+    constexpr int NW = 8;
     constexpr int TBY = TB * TB * ES, PBY = 64 * ES, NST = APPLY_STAGES * 16 / ES, S1 = 16 * ES;
     constexpr int NS = 16 / NW;                          // k-halves (s) of a patch column handled by one warp: 2 or 1
     extern __shared__ __align__(1024) char smem[];
@@ -69,8 +60,6 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) apply_tiles_k1_kernel(const 
     const int g = lane >> 2, t = lane & 3;
     const int g2 = (g >> 2) & 1, g1 = (g >> 1) & 1, g0 = g & 1, t1 = (t >> 1) & 1, t0 = t & 1;
     const int offP1 = (((g2 << 2) | g1) * 8 + ((g0 << 2) | (t0 << 1) | (g1 ^ t1))) * ES + s0 * S1;   // + s * S1
-    const bool herm = (p.pass == PASS_HERM);
-    const double sgn = p.sign;
     const double2 zero2 = make_double2(0.0, 0.0);
     const double2 *x = p.X;
 
@@ -83,7 +72,6 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) apply_tiles_k1_kernel(const 
             v[s] = row < p.N ? __ldg(x + row) : zero2;
         }
     };
-    const double sgn_im = herm ? sgn : -sgn;             // P1 operand: x_J (HERM) or conj(x_J) (SYMC), times the pass sign
 
     int st = 0;
     uint32_t ph = 0;
@@ -93,31 +81,31 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) apply_tiles_k1_kernel(const 
 
         double2 xjn[NS];
         load_xj(J0, xjn);
-        // conj(x_I[8 ib + g]) times the pass sign: the P2 operand, in registers for the whole unit
+        // P2 operands (u, v) pairing with (Ar, Ai): MODE 0 (a_I, b_I), MODE 1 (b_I, -a_I); in registers for the whole unit
         double2 xi[8];
 #pragma unroll
         for (int ib = 0; ib < 8; ++ib) {
             int64_t row = (int64_t)I * TB + ib * 8 + g;
             double2 a = row < p.N ? __ldg(x + row) : zero2;
-            xi[ib] = make_double2(sgn * a.x, -sgn * a.y);
+            xi[ib] = MODE == 0 ? a : make_double2(a.y, -a.x);
         }
         double2 acc1[8];
 #pragma unroll
         for (int ib = 0; ib < 8; ++ib) acc1[ib] = zero2;
 
         for (int J = J0; J < J1; ++J) {
-            double2 xj[NS];
+            double xj[NS];                                  // a_J (MODE 0) or b_J (MODE 1)
 #pragma unroll
-            for (int s = 0; s < NS; ++s) xj[s] = make_double2(sgn * xjn[s].x, sgn_im * xjn[s].y);
+            for (int s = 0; s < NS; ++s) xj[s] = MODE == 0 ? xjn[s].x : xjn[s].y;
             if (J + 1 < J1) load_xj(J + 1, xjn);            // prefetch the next tile's x_J rows
 
             mbar_wait(&full[st], ph);
             const char *tp = tile_s + st * TBY + jb * 8 * PBY + offP1;
             int live = 0;
             if (I != J) {
-                double2 acc2[NS];
+                double acc2[NS];
 #pragma unroll
-                for (int s = 0; s < NS; ++s) acc2[s] = zero2;
+                for (int s = 0; s < NS; ++s) acc2[s] = 0.0;
 #pragma unroll
                 for (int h = 0; h < 8; h += 4) {             // four patch rows at a time (register budget)
                     double2 a[4][NS];
@@ -129,33 +117,27 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) apply_tiles_k1_kernel(const 
                     for (int r = 0; r < 4; ++r)
 #pragma unroll
                         for (int s = 0; s < NS; ++s) {
-                            cfma(acc1[h + r], a[r][s], xj[s]);
-                            cfma(acc2[s], a[r][s], xi[h + r]);
+                            rfma1<MODE>(acc1[h + r], a[r][s], xj[s]);
+                            acc2[s] = fma(a[r][s].x, xi[h + r].x, acc2[s]);
+                            acc2[s] = fma(a[r][s].y, xi[h + r].y, acc2[s]);
                         }
                 }
                 // dependent release (see apply_common.cuh): values computed from every load of this stage
 #pragma unroll
                 for (int ib = 0; ib < 8; ++ib) live |= __double2hiint(acc1[ib].x);
 #pragma unroll
-                for (int s = 0; s < NS; ++s) live |= __double2hiint(acc2[s].x);
+                for (int s = 0; s < NS; ++s) live |= __double2hiint(acc2[s]);
                 __syncwarp();
                 if (lane == 0)
                     mbar_arrive(reinterpret_cast<uint64_t *>(reinterpret_cast<char *>(&empty[st]) + (live & p.zero)));
                 // sum over the eight g-lanes (lane bits 2..4), then lanes g == 0 add Y_J[c0 + 4s + t]
 #pragma unroll
                 for (int s = 0; s < NS; ++s) {
-                    double yr = acc2[s].x, yi = acc2[s].y;
+                    double yr = acc2[s];
 #pragma unroll
-                    for (int m = 4; m < 32; m <<= 1) {
-                        yr += __shfl_xor_sync(0xffffffffu, yr, m);
-                        yi += __shfl_xor_sync(0xffffffffu, yi, m);
-                    }
+                    for (int m = 4; m < 32; m <<= 1) yr += __shfl_xor_sync(0xffffffffu, yr, m);
                     const int64_t row = (int64_t)J * TB + c0 + s * 4 + t;
-                    if (g == 0 && row < p.N) {
-                        double *y = p.Y + 2 * row;
-                        red_add(y, yr);
-                        red_add(y + 1, herm ? -yi : yi);
-                    }
+                    if (g == 0 && row < p.N) red_add(p.Y + 2 * row + MODE, yr);      // re_J (MODE 0) / im_J (MODE 1)
                 }
             } else {
 #pragma unroll
@@ -168,7 +150,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) apply_tiles_k1_kernel(const 
 #pragma unroll
                     for (int r = 0; r < 4; ++r)
 #pragma unroll
-                        for (int s = 0; s < NS; ++s) cfma(acc1[h + r], a[r][s], xj[s]);
+                        for (int s = 0; s < NS; ++s) rfma1<MODE>(acc1[h + r], a[r][s], xj[s]);
                 }
 #pragma unroll
                 for (int ib = 0; ib < 8; ++ib) live |= __double2hiint(acc1[ib].x);
@@ -193,5 +175,6 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) apply_tiles_k1_kernel(const 
         }
     }
 }
+
 
 }  // namespace bse
