@@ -268,11 +268,11 @@ def run_cuda(args, cfg):
     else:
         roof = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": traffic, "peak_source": peak_src}
-    # 5 .. 8 columns: the kernel forms each complex product from three real ones (apply_kernel_3m.cuh), so the tensor
+    # 5 .. 8 columns: the kernel forms each complex product from three real ones (Role3M, apply_tiles.cuh), so the tensor
     # pipe executes 6 N^2 k flops for the 8 N^2 k algorithmic ones of SURVEY.md 8(d) that `achieved` counts.
     three_m = 5 <= k <= 8
     roof.update({"kernel": "bse::apply_tiles_k1_kernel" if k == 1 else
-                 ("bse::apply_tiles_3m_kernel" if three_m else "bse::apply_tiles_rs_kernel"),
+                 ("bse::apply_tiles_kernel<16, Role3M>" if three_m else "bse::apply_tiles_kernel<16, Role4M>"),
                  "tflops_fp64": tflops, "tflops_fp64_executed": tflops * (0.75 if three_m else 1.0),
                  "fp64_peak_measured_tflops": fp64_peak, "GBps": achieved})
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -365,7 +365,7 @@ def run_cuda(args, cfg):
                                            "GBps": 4 * alg_bytes(N3, 1) * qsteps / qsec / 1e9}
 
         # full-mode half apply P(X) = R X + C conj(X) vs k: complex store (R and C passes) and the
-        # real-form store of Eq. (3) (S = R + C, D = R - C; apply_kernel_real.cuh).  Bytes: both stores once + X, Y.
+        # real-form store of Eq. (3) (S = R + C, D = R - C; RoleReal in apply_tiles.cuh).  Bytes: both stores once + X, Y.
         def half_sweep(hh):
             out = {}
             for kk in (1, 4, 8):

@@ -4,11 +4,7 @@
 #include <cstdlib>
 #include <new>
 
-#include "apply_kernel.cuh"
-#include "apply_kernel_k1.cuh"
-#include "apply_kernel_3m.cuh"
-#include "apply_kernel_real.cuh"
-#include "apply_kernel_rs.cuh"
+#include "bse_common.cuh"
 #include "bse_internal.h"
 #include "tile_layout.cuh"
 
@@ -54,53 +50,6 @@ bse_status_t zero_block(bse_handle_s *h, void *dY, int64_t ldy, int64_t rows, in
     return BSE_OK;
 }
 
-static bse_status_t apply_kernel_attributes()
-{
-    // cudaFuncSetAttribute is per device: remember which devices of this process have been set up
-    static std::atomic<uint64_t> attr_devices{0};
-    int dev = 0;
-    BSE_CUDA(cudaGetDevice(&dev));
-    if (dev >= 64 || !(attr_devices.load(std::memory_order_acquire) & (1ull << dev))) {
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<16, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<16, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_kernel<8, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_rs_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_rs_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_k1_kernel<16, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_k1_kernel<16, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_k1_kernel<8, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_k1_kernel<8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_kernel<16, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_kernel<16, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_kernel<8, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_real_kernel<8, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_3m_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_3m_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_k1_kernel<16, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        BSE_CUDA(cudaFuncSetAttribute(apply_tiles_k1_kernel<8, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, APPLY_SMEM));
-        if (dev < 64) attr_devices.fetch_or(1ull << dev, std::memory_order_release);
-    }
-    return BSE_OK;
-}
-
-static void apply_unit_params(const bse_handle_s *h, ApplyParams &p, int &grid)
-{
-    p.N = h->N;
-    p.nt = h->nt;
-    int64_t total_tiles = (int64_t)h->nt * (h->nt + 1) / 2;
-    int64_t L = total_tiles / ((int64_t)h->num_sms * 12);
-    if (L < 1) L = 1;
-    if (L > 32) L = 32;
-    if (const char *e = getenv("BSE_APPLY_UNIT")) { int v = atoi(e); if (v >= 1 && v <= 4096) L = v; }
-    p.L = (int)L;
-    p.u_begin = apply_first_unit(h->row_begin, p.L);
-    p.n_units = apply_first_unit(h->row_end, p.L);          // == apply_num_units(nt, L) for row_end == nt
-    p.zero = 0;
-    const int64_t count = p.n_units - p.u_begin;
-    grid = (int)(count < h->num_sms ? (count > 0 ? count : 1) : h->num_sms);
-}
-
 bse_status_t comm_sum_block(bse_handle_s *h, void *dY, int64_t ld, int64_t rows, int k)
 {
     if (!h->comm) return BSE_OK;
@@ -130,91 +79,6 @@ bse_status_t comm_bcast_host(bse_handle_s *h, void *hBuf, size_t bytes)
     if (h->comm(h->comm_user, BSE_COMM_BCAST, h->comm_buf, (int64_t)(padded / 8))) return BSE_ERR_INTERNAL;
     BSE_CUDA(cudaMemcpyAsync(hBuf, h->comm_buf, bytes, cudaMemcpyDeviceToHost, h->stream));
     BSE_CUDA(cudaStreamSynchronize(h->stream));
-    return BSE_OK;
-}
-
-bse_status_t launch_real_pass(bse_handle_s *h, const char *tiles, int mode, const void *dX, int64_t ldx, void *dY,
-                              int64_t ldy, int32_t k)
-{
-    bse_status_t st = apply_kernel_attributes();
-    if (st) return st;
-    ApplyParams p;
-    int grid;
-    apply_unit_params(h, p, grid);
-    p.tiles = tiles - tile_index(h->row_begin, 0) * tile_bytes_es(h->es);   // virtual base of the whole packed store
-    p.pass = mode;
-    p.sign = 1.0;
-    p.ldx = ldx;
-    p.ldy = ldy;
-    bool use_k1 = true;                                // BSE_APPLY_K1=0: tensor-core kernel for single columns too
-    if (const char *e = getenv("BSE_APPLY_K1")) use_k1 = atoi(e) != 0;
-    for (int32_t c0 = 0; c0 < k; c0 += 8) {
-        p.kc = k - c0 < 8 ? k - c0 : 8;
-        p.X = reinterpret_cast<const double2 *>(dX) + (int64_t)c0 * ldx;
-        p.Y = reinterpret_cast<double *>(dY) + 2 * (int64_t)c0 * ldy;
-        const bool k1 = p.kc == 1 && use_k1;                  // plain-FMA single-column variant
-        if (h->es == ES_C128) {
-            if (k1 && mode == 0) apply_tiles_real_k1_kernel<16, 0><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-            else if (k1) apply_tiles_real_k1_kernel<16, 1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-            else if (mode == 0) apply_tiles_real_kernel<16, 0><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-            else apply_tiles_real_kernel<16, 1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-        } else {
-            if (k1 && mode == 0) apply_tiles_real_k1_kernel<8, 0><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-            else if (k1) apply_tiles_real_k1_kernel<8, 1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-            else if (mode == 0) apply_tiles_real_kernel<8, 0><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-            else apply_tiles_real_kernel<8, 1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-        }
-        count_launch();
-    }
-    BSE_CUDA(cudaGetLastError());
-    return BSE_OK;
-}
-
-bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, double sign, const void *dX,
-                               int64_t ldx, void *dY, int64_t ldy, int32_t k)
-{
-    bse_status_t st0 = apply_kernel_attributes();
-    if (st0) return st0;
-    bool use_k1 = true;                                // BSE_APPLY_K1=0: tensor-core kernel for single columns too
-    if (const char *e = getenv("BSE_APPLY_K1")) use_k1 = atoi(e) != 0;
-    ApplyParams p;
-    int grid;
-    apply_unit_params(h, p, grid);
-    p.tiles = tiles - tile_index(h->row_begin, 0) * tile_bytes_es(h->es);   // virtual base of the whole packed store
-    p.pass = pass;
-    p.sign = sign;
-    p.ldx = ldx;
-    p.ldy = ldy;
-    bool use_wide = true;                              // BSE_APPLY_WIDE=0: 4-column passes only
-    if (const char *e = getenv("BSE_APPLY_WIDE")) use_wide = atoi(e) != 0;
-    bool use_rs = true;                                // BSE_APPLY_RS=0: all-roles-per-warp form for 2 .. 4 columns (apply_kernel.cuh)
-    if (const char *e = getenv("BSE_APPLY_RS")) use_rs = atoi(e) != 0;
-    bool use_3m = true;                                // BSE_APPLY_3M=0: four-product form for 5 .. 8 columns
-    if (const char *e = getenv("BSE_APPLY_3M")) use_3m = atoi(e) != 0;
-    for (int32_t c0 = 0; c0 < k;) {
-        const int32_t left = k - c0;
-        const bool wide = use_wide && left > 4;        // 5 .. 8 columns in one pass over the operand
-        p.kc = wide ? (left < 8 ? left : 8) : (left < 4 ? left : 4);
-        p.X = reinterpret_cast<const double2 *>(dX) + (int64_t)c0 * ldx;
-        p.Y = reinterpret_cast<double *>(dY) + 2 * (int64_t)c0 * ldy;
-        const bool k1 = p.kc == 1 && use_k1;                 // plain-FMA single-column variant
-        if (h->es == ES_C128) {
-            if (k1) apply_tiles_k1_kernel<16, 8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-            else if (wide && use_3m) apply_tiles_3m_kernel<16><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-            else if (wide) apply_tiles_kernel<16, 2><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-            else if (use_rs) apply_tiles_rs_kernel<16><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-            else apply_tiles_kernel<16, 1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-        } else {
-            if (k1) apply_tiles_k1_kernel<8, 8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-            else if (wide && use_3m) apply_tiles_3m_kernel<8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-            else if (wide) apply_tiles_kernel<8, 2><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-            else if (use_rs) apply_tiles_rs_kernel<8><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-            else apply_tiles_kernel<8, 1><<<grid, APPLY_THREADS, APPLY_SMEM, h->stream>>>(p);
-        }
-        count_launch();
-        c0 += p.kc;
-    }
-    BSE_CUDA(cudaGetLastError());
     return BSE_OK;
 }
 
@@ -401,6 +265,8 @@ bse_status_t bse_create(bse_handle_t *out, int32_t mode, int32_t storage, int64_
     h->C = (mode == BSE_MODE_FULL) ? (const char *)dCTiles : nullptr;
     h->stream = (cudaStream_t)stream;
     h->num_sms = sms;
+    bse_status_t st = handle_finalize(h);
+    if (st) { bse_destroy(h); return st; }
     *out = h;
     return BSE_OK;
 }
@@ -474,7 +340,7 @@ bse_status_t bse_create_shard(bse_handle_t *out, int32_t mode, int32_t storage, 
     if (st) return st;
     (*out)->row_begin = tile_row_begin;
     (*out)->row_end = tile_row_end;
-    return BSE_OK;
+    return handle_finalize(*out);                            // the unit range of this slice
 }
 
 bse_status_t bse_set_comm(bse_handle_t h, bse_comm_fn fn, void *user)
@@ -490,29 +356,11 @@ bse_status_t bse_destroy(bse_handle_t h)
     if (!h) return BSE_ERR_INVALID_ARG;
     if (h->ws) cudaFree(h->ws);
     if (h->ws2) cudaFree(h->ws2);
+    if (h->ws_op) cudaFree(h->ws_op);
     if (h->hpin) cudaFreeHost(h->hpin);
     if (h->comm_buf) cudaFree(h->comm_buf);
     delete h;
     return BSE_OK;
-}
-
-bse_status_t bse_apply_half(bse_handle_t h, int32_t sign, const void *dX, int64_t ldx, void *dY, int64_t ldy, int32_t k)
-{
-    if (!h || !dX || !dY || k < 1 || ldx < h->N || ldy < h->N || (sign != 1 && sign != -1)) return BSE_ERR_INVALID_ARG;
-    if (h->mode != BSE_MODE_FULL) return BSE_ERR_INVALID_ARG;
-    bse_status_t st = zero_block(h, dY, ldy, h->N, k);
-    if (st) return st;
-    if (h->real_form) {
-        // stores hold S = R + C (h->R) and D = R - C (h->C):  P = mode 0 over S + mode 1 over D,  M = mode 0 over D + mode 1 over S
-        const char *first = sign > 0 ? h->R : h->C, *second = sign > 0 ? h->C : h->R;
-        if ((st = launch_real_pass(h, first, 0, dX, ldx, dY, ldy, k))) return st;
-        if ((st = launch_real_pass(h, second, 1, dX, ldx, dY, ldy, k))) return st;
-        return comm_sum_block(h, dY, ldy, h->N, k);
-    }
-    st = launch_apply_pass(h, h->R, PASS_HERM, 1.0, dX, ldx, dY, ldy, k);
-    if (st) return st;
-    if ((st = launch_apply_pass(h, h->C, PASS_SYMC, (double)sign, dX, ldx, dY, ldy, k))) return st;
-    return comm_sum_block(h, dY, ldy, h->N, k);
 }
 
 }  // extern "C"

@@ -23,6 +23,14 @@ struct bse_handle_s {
     const char *C;
     cudaStream_t stream;
     int num_sms;
+    // apply kernels: unit walk of this handle's tile rows and the operand workspace (images + Ypad, apply_prep.cuh),
+    // all fixed by handle_finalize at creation: the apply calls themselves never allocate and read no environment
+    int unit_L;
+    int64_t u_begin, n_units;
+    int grid;
+    int use_k1;          // single columns take the plain-FMA kernels (BSE_APPLY_K1=0 at creation: tensor-core kernels)
+    void *ws_op;
+    size_t ws_op_bytes;
     // lazily grown scratch (device)
     void *ws;
     size_t ws_bytes;
@@ -63,12 +71,13 @@ bse_status_t ensure_ws(bse_handle_s *h, size_t bytes);
 bse_status_t ensure_ws2(bse_handle_s *h, size_t bytes);
 bse_status_t ensure_pin(bse_handle_s *h, size_t bytes);
 
-// One pass over one matrix: Y += sign * (R X)  or  Y += sign * (C conj X), k columns (chunked by 4).
-bse_status_t launch_apply_pass(bse_handle_s *h, const char *tiles, int pass, double sign, const void *dX,
-                               int64_t ldx, void *dY, int64_t ldy, int32_t k);
-// One pass of the real-form half apply (apply_kernel_real.cuh): mode 0 / 1 over one store, k columns (chunked by 8).
-bse_status_t launch_real_pass(bse_handle_s *h, const char *tiles, int mode, const void *dX, int64_t ldx, void *dY,
-                              int64_t ldy, int32_t k);
+// unit walk parameters and operand workspace of a handle (bse_create / bse_create_shard)
+bse_status_t handle_finalize(bse_handle_s *h);
+// The products of this handle's tile rows WITHOUT the sum over the other slices (callers add comm_sum_block):
+//   apply_tda_local : Y = R X                       (N x k, TDA handles)
+//   apply_half_local: Y = R X + sign C conj(X)      (N x k, full-mode handles; complex or real-form stores)
+bse_status_t apply_tda_local(bse_handle_s *h, const void *dX, int64_t ldx, void *dY, int64_t ldy, int32_t k);
+bse_status_t apply_half_local(bse_handle_s *h, int sign, const void *dX, int64_t ldx, void *dY, int64_t ldy, int32_t k);
 bse_status_t zero_block(bse_handle_s *h, void *dY, int64_t ldy, int64_t rows, int32_t k);
 
 

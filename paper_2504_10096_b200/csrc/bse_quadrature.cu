@@ -136,8 +136,7 @@ extern "C" bse_status_t bse_lanczos_quadrature(bse_handle_t h, const void *dStar
     count_launch(2);
     int iv = 0, ip = 2, iw = 1;      // v_j, v_{j-1}, w
     for (int j = 0; j < steps; ++j) {
-        if ((st = zero_block(h, buf[iw], n, n, 1))) return st;
-        if ((st = launch_apply_pass(h, h->R, 0, 1.0, buf[iv], n, buf[iw], n, 1))) return st;       // w = R v_j
+        if ((st = apply_tda_local(h, buf[iv], n, buf[iw], n, 1))) return st;                      // w = R v_j
         if ((st = comm_sum_block(h, buf[iw], n, n, 1))) return st;
         // the oracle's order: subtract beta_j v_{j-1} first, alpha_j = Re(v_j^H w) (v_{j-1} is orthogonal to v_j,
         // so the two orders agree to rounding); here alpha is taken first so that one fused pass does both updates
@@ -256,8 +255,7 @@ extern "C" bse_status_t bse_lanczos_quadrature_static(bse_handle_t h, const void
     count_launch(2);
     int iv = 0, ip = 2, iw = 1;      // v_j, v_{j-1}, w
     for (int j = 0; j < steps; ++j) {
-        if ((st = zero_block(h, buf[iw], n, n, 1))) return st;
-        if ((st = launch_apply_pass(h, h->R, 0, 1.0, buf[iv], n, buf[iw], n, 1))) return st;       // w = R v_j
+        if ((st = apply_tda_local(h, buf[iv], n, buf[iw], n, 1))) return st;                      // w = R v_j
         if ((st = comm_sum_block(h, buf[iw], n, n, 1))) return st;
         dot_re_kernel<<<grid, 256, 0, h->stream>>>(buf[iv], buf[iw], n, d_alpha + j);
         if ((st = comm_bcast_dev(h, d_alpha + j, 1))) return st;

@@ -200,8 +200,7 @@ struct Solver {
     bse_status_t apply_block(int c0)
     {
         if (!full) {
-            ST(zero_block(h, col(V, c0 + k), ld, n, k));
-            ST(launch_apply_pass(h, h->R, 0, 1.0, col(V, c0), ld, col(V, c0 + k), ld, k));
+            ST(apply_tda_local(h, col(V, c0), ld, col(V, c0 + k), ld, k));
             ST(comm_sum_block(h, col(V, c0 + k), ld, n, k));
         } else {
             bse_status_t st = bse_apply_half(h, -1, col(PV, c0), ld, col(V, c0 + k), ld, k);      // W = M(p)

@@ -278,36 +278,34 @@ def test_leading_dimensions_and_side_stream(orc):
     assert b.lib().bse_apply(h._h, Xd.data_ptr(), ldx, Xd.data_ptr(), ldx, k) == 1       # aliasing
 
 
-@pytest.mark.parametrize("k", [5, 7, 8, 11, 16])
-def test_wide_and_narrow_column_passes_agree_with_oracle(orc, k, monkeypatch):
-    """k > 4: the default takes 5..8 columns per pass over the operand with three real products per complex product
-    (apply_tiles_3m_kernel); BSE_APPLY_3M=0 takes the four-product form (apply_tiles_kernel<ES, 2>), BSE_APPLY_WIDE=0
-    takes 4 columns at a time.  All against the oracle, on a size with several units per CTA and a ragged last tile."""
+@pytest.mark.parametrize("k", [5, 7, 8, 9, 11, 16])
+def test_column_groups_agree_with_oracle(orc, k):
+    """k > 4: 5..8 columns per pass over the operand with three real products per complex product (Role3M), the rest with
+    the four-product role (2..4 columns) or the single-column kernel.  Against the oracle, on a size with several units per
+    CTA and a ragged last tile; the launch count is pre-pass + tile pass + post-pass per group (one kernel for k = 1)."""
     import paper_2504_10096_b200 as b
     N = 2000
     R = gen.dense_R(N, 31, sigma=0.5)
     X = gen.block_X(N, k, 32)
     ref = orc.apply_tda(R, X)
     h = b.Bse(b.MODE_TDA, N, pack(R, 0))
-    for wide, m3 in (("1", "1"), ("1", "0"), ("0", "1")):
-        monkeypatch.setenv("BSE_APPLY_WIDE", wide)
-        monkeypatch.setenv("BSE_APPLY_3M", m3)
-        n0 = b.launch_count()
-        Y = to_host(h.apply(to_dev(X)))
-        launches = b.launch_count() - n0
-        assert relerr(Y, ref) <= TOL_APPLY
-        left, passes = k, 0
-        while left > 0:                        # the launcher's greedy rule (bse_api.cu, launch_apply_pass)
-            left -= (min(left, 8) if (wide == "1" and left > 4) else min(left, 4))
-            passes += 1
-        assert launches == passes
+    n0 = b.launch_count()
+    Y = to_host(h.apply(to_dev(X)))
+    launches = b.launch_count() - n0
+    assert relerr(Y, ref) <= TOL_APPLY
+    left, expect = k, 0
+    while left > 0:                            # the launcher's greedy rule (bse_apply.cu, group_width)
+        w = min(left, 8) if left > 4 else left
+        expect += 1 if w == 1 else 3
+        left -= w
+    assert launches == expect
 
 
-@pytest.mark.parametrize("k", [2, 3, 4])
-def test_role_split_and_all_roles_kernels_agree_with_oracle(orc, k, monkeypatch):
-    """2..4 columns: the default is the role-split kernel (apply_kernel_rs.cuh); BSE_APPLY_RS=0 selects the
-    all-roles-per-warp kernel (apply_kernel.cuh).  Both against the oracle: TDA (HERM pass), full mode (HERM + SYMC passes,
-    both signs), complex128 and complex64 stores, a ragged size with several units per CTA."""
+@pytest.mark.parametrize("k", [2, 3, 4, 6, 8])
+def test_tile_roles_every_store_agree_with_oracle(orc, k, monkeypatch):
+    """The tile kernels' roles (four-product 2..4 columns, three-product 5..8) against the oracle: TDA (HERM pass), full mode
+    (HERM + SYMC passes, both signs), complex128 and complex64 stores, a ragged size with several units per CTA; and single
+    columns through the tensor-core kernels (BSE_APPLY_K1=0 at handle creation)."""
     import paper_2504_10096_b200 as b
     N = 2000
     R, C = gen.dense_R(N, 31, sigma=1.0), gen.dense_C(N, 31)
@@ -317,11 +315,15 @@ def test_role_split_and_all_roles_kernels_agree_with_oracle(orc, k, monkeypatch)
         rt = b.bse_pack_from_dense(to_dev(R), N, 0, storage=storage)
         ct = b.bse_pack_from_dense(to_dev(C), N, 1, storage=storage)
         ht, hf = b.Bse(b.MODE_TDA, N, rt, storage=storage), b.Bse(b.MODE_FULL, N, rt, ct, storage=storage)
-        for rs in ("1", "0"):
-            monkeypatch.setenv("BSE_APPLY_RS", rs)
-            assert relerr(to_host(ht.apply(to_dev(X))), orc.apply_tda(Rs, X)) <= TOL_APPLY, (storage, rs)
-            for sign in (+1, -1):
-                assert relerr(to_host(hf.apply_half(to_dev(X), sign)), orc.apply_half(Rs, Cs, X, sign)) <= TOL_APPLY
+        assert relerr(to_host(ht.apply(to_dev(X))), orc.apply_tda(Rs, X)) <= TOL_APPLY, storage
+        for sign in (+1, -1):
+            assert relerr(to_host(hf.apply_half(to_dev(X), sign)), orc.apply_half(Rs, Cs, X, sign)) <= TOL_APPLY
+        if k == 2:
+            monkeypatch.setenv("BSE_APPLY_K1", "0")
+            h1, hf1 = b.Bse(b.MODE_TDA, N, rt, storage=storage), b.Bse(b.MODE_FULL, N, rt, ct, storage=storage)
+            monkeypatch.delenv("BSE_APPLY_K1")
+            assert relerr(to_host(h1.apply(to_dev(X[:, :1]))), orc.apply_tda(Rs, X[:, :1])) <= TOL_APPLY
+            assert relerr(to_host(hf1.apply_half(to_dev(X[:, :1]), -1)), orc.apply_half(Rs, Cs, X[:, :1], -1)) <= TOL_APPLY
 
 
 @pytest.mark.parametrize("kind", ["real_x", "imag_x", "real_T", "imag_T", "one_column_dominant"])

@@ -45,7 +45,7 @@ def test_general_apply_matches_oracle(orc, N, k):
 
 def test_unit_impulses_every_block_sign_and_conjugation(orc):
     """One non-zero entry of R or C at a time (diagonal tile, off-diagonal tile, tile border): a wrong sign or a swapped
-    plane in the mode tables of apply_kernel_real.cuh is an O(1) error here."""
+    plane in the mode tables of RoleReal in apply_tiles.cuh is an O(1) error here."""
     N = 130
     x = gen.block_X(N, 2, 5)
     for (i, j) in [(0, 0), (5, 3), (63, 0), (64, 63), (100, 7), (129, 64), (129, 129)]:
