@@ -249,29 +249,32 @@ def run_cuda(args, cfg):
     achieved = alg_bytes(N, k) / (ms * 1e-3) / 1e9
     if shard:                                                   # per GPU: 1 / world of the tiles, the whole X and Y
         achieved = ((alg_bytes(N, k) - 32.0 * N * k) / world + 32.0 * N * k) / (ms * 1e-3) / 1e9
-    traffic = None
+    traffic, traffic_src = None, None
     try:
         import csv
-        with open(os.path.join(ROOT, "profiles", "r1_apply_traffic.csv")) as f:
+        # QUOTED from the committed ncu capture of the same kernel and workload (profiles/r2_apply_traffic.csv names the
+        # capture); null when no capture of this workload exists -- it is not measured by the run that prints it
+        with open(os.path.join(ROOT, "profiles", "r2_apply_traffic.csv")) as f:
             for row in csv.DictReader(f):
                 if row["workload"] == f"N{N}_k{k}" + ("" if ES == 16.0 else "_c64"):
                     traffic = float(row["dram_bytes_per_launch"])
+                    traffic_src = row["source"]
     except Exception:
         pass
     # north_star: roofline = min(bytes / HBM peak, flops / FP64 peak).  The FP64 figure is this repo's own DMMA
-    # microbenchmark (profiles/r1_microbench.md): MEASURED_PEAKS.json has no FP64 entry.
+    # microbenchmark (bse_selftest_peak, `bench.py --peaks`): MEASURED_PEAKS.json has no FP64 entry.
     tflops = 8.0 * N * N * k / (ms * 1e-3) / 1e12 / (world if shard else 1)       # per GPU
-    fp64_peak = 37.1
+    fp64_peak = b.selftest_peak(b.PEAK_DMMA, 8, 8)[0]                              # measured now, by the library's own DMMA probe
     if 8.0 * N * N * k / (fp64_peak * 1e12) > alg_bytes(N, k) / (peak * 1e9):
         roof = {"bound": "tensor", "achieved": tflops, "peak": fp64_peak, "unit": "TFLOP/s", "frac": tflops / fp64_peak,
-                "traffic": traffic, "peak_source": "own DMMA.8x8x4 microbenchmark (profiles/r1_microbench.md), FP64"}
+                "traffic": traffic, "peak_source": "bse_selftest_peak(BSE_PEAK_DMMA) measured in this run (burst; `python bench.py --peaks` has the sustained one)"}
     else:
         roof = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": traffic, "peak_source": peak_src}
     # 5 .. 8 columns: the kernel forms each complex product from three real ones (Role3M, apply_tiles.cuh), so the tensor
     # pipe executes 6 N^2 k flops for the 8 N^2 k algorithmic ones of SURVEY.md 8(d) that `achieved` counts.
     three_m = 5 <= k <= 8
-    roof.update({"kernel": "bse::apply_tiles_k1_kernel" if k == 1 else
+    roof.update({"traffic_source": traffic_src, "kernel": "bse::apply_tiles_k1_kernel" if k == 1 else
                  ("bse::apply_tiles_kernel<16, Role3M>" if three_m else "bse::apply_tiles_kernel<16, Role4M>"),
                  "tflops_fp64": tflops, "tflops_fp64_executed": tflops * (0.75 if three_m else 1.0),
                  "fp64_peak_measured_tflops": fp64_peak, "GBps": achieved})
@@ -438,6 +441,93 @@ def run_solve(spec):
                                 "max_residual_estimate": float(res.resid.max())}}))
 
 
+def measure_peaks(b, sustained_s: float = 0.0):
+    """The library's own microbenchmarks (bse_selftest_peak): burst figures from one timed launch each; with
+    sustained_s > 0 also the rate of back-to-back launches over that many seconds (power cap reached)."""
+    import torch
+    out = {}
+
+    def sustained(what, p1, p2, buf=None):
+        t0, acc, n = time.perf_counter(), [], 0
+        while time.perf_counter() - t0 < sustained_s:
+            acc.append(b.selftest_peak(what, p1, p2, buf)[0]); n += 1
+        tail = acc[len(acc) // 2:]
+        return float(np.mean(tail)) if tail else None
+
+    out["dmma_tflops"] = b.selftest_peak(b.PEAK_DMMA, 8, 8)[0]
+    out["dmma_with_dadd_mix_tflops"] = b.selftest_peak(b.PEAK_DMMA, 8, -1)[0]
+    out["dfma_tflops"] = b.selftest_peak(b.PEAK_DFMA, 32, 0)[0]
+    buf = torch.empty(8 << 30, dtype=torch.uint8, device="cuda")
+    buf.zero_()
+    out["bulk_read_GBps"] = b.selftest_peak(b.PEAK_BULK_READ, 65536, 3, buf)[0]
+    out["bulk_read_smem_readback_GBps"] = b.selftest_peak(b.PEAK_BULK_READ_SMEM, 65536, 3, buf)[0]
+    small = torch.zeros(1536 * 1024, dtype=torch.float64, device="cuda")
+    out["red_f64_Gops"] = b.selftest_peak(b.PEAK_RED, 0, 0, small)[0]
+    if sustained_s > 0:
+        out["dmma_tflops_sustained"] = sustained(b.PEAK_DMMA, 32, 8)
+        out["dmma_with_dadd_mix_tflops_sustained"] = sustained(b.PEAK_DMMA, 32, -1)
+        out["bulk_read_GBps_sustained"] = sustained(b.PEAK_BULK_READ, 65536, 3, buf)
+        out["sustained_seconds_each"] = sustained_s
+    del buf, small
+    torch.cuda.empty_cache()
+    return out
+
+
+def run_peaks(args):
+    """`--peaks`: one JSON line with the roofline denominators measured by the library itself (profiles/r2_peaks.md)."""
+    import torch
+    import paper_2504_10096_b200 as b
+    torch.cuda.set_device(0)
+    sampler = ClockSampler(0)
+    sampler.start()
+    out = measure_peaks(b, sustained_s=2.0)
+    out["clocks"] = sampler.stop()
+    hbm, src = measured_peaks()
+    out["hbm_copy_GBps_driver"] = hbm
+    print(json.dumps({"peaks": out}))
+
+
+def run_dense(spec):
+    """`--dense M:K[:L]`: the dense basis kernels at the shapes of a solve with basis width M, block K and rotation width L
+    (default 3M/4) on N = 98304 rows (config 4): Gram (a5), skinny update (a6), Ritz rotation (a9), and one bse_orth call.
+    CUDA events on the launch stream, 3 warm-ups, 10 timed launches each.  One JSON line (profiles/r2_dense_kernels.md)."""
+    import torch
+    import paper_2504_10096_b200 as b
+    parts = [int(x) for x in spec.split(":")]
+    m, k = parts[0], parts[1]
+    l = parts[2] if len(parts) > 2 else (3 * m) // 4
+    N = 98304
+    torch.cuda.set_device(0)
+    tiles = torch.zeros(b.bse_layout(1024)[2], dtype=torch.uint8, device="cuda")      # the dense kernels never touch the operator
+    h = b.Bse(b.MODE_TDA, N, tiles)                                                     # (handle with N rows; tiles unused)
+    V = torch.randn(m, N, dtype=torch.complex128, device="cuda") / np.sqrt(2 * N)
+    W = torch.randn(k, N, dtype=torch.complex128, device="cuda")
+    hbm, _ = measured_peaks()
+    fp64 = b.selftest_peak(b.PEAK_DMMA, 8, 8)[0]
+    out = {"N": N, "m": m, "k": k, "l": l, "fp64_peak_tflops": fp64, "hbm_peak_GBps": hbm}
+    ms = time_steps(lambda: h.gram(V, W), 10, 3)
+    by = 16.0 * N * (m + k)
+    out["gram"] = {"ms": ms, "GBps": by / ms / 1e6, "frac_hbm": by / ms / 1e6 / hbm, "tflops": 8.0 * N * m * k / ms / 1e9}
+    S = torch.randn(k, m, dtype=torch.complex128, device="cuda")
+    ms = time_steps(lambda: h.update(V, S, W, -1.0, 1.0), 10, 3)
+    by = 16.0 * N * (m + 2 * k)
+    out["update"] = {"ms": ms, "GBps": by / ms / 1e6, "frac_hbm": by / ms / 1e6 / hbm}
+    Sl = torch.randn(l, m, dtype=torch.complex128, device="cuda") / np.sqrt(m)
+    Cout = torch.empty(l, N, dtype=torch.complex128, device="cuda")
+    ms = time_steps(lambda: h.update(V, Sl, Cout), 5, 2)
+    out["rotation"] = {"ms": ms, "tflops": 8.0 * N * m * l / ms / 1e9, "frac_fp64": 8.0 * N * m * l / ms / 1e9 / fp64}
+    Q, _ = torch.linalg.qr(V[:min(m, 256)].T.contiguous())                              # orthonormal basis of the orth timing
+    Vq = Q.T.contiguous()
+    W0 = W.clone()
+
+    def orth():
+        W.copy_(W0)
+        h.orth(Vq, W)
+    ms = time_steps(orth, 10, 3)
+    out["orth_call_m%d" % Vq.shape[0]] = {"ms": ms}
+    print(json.dumps({"dense": out}))
+
+
 def run_slices(args, cfg):
     """`--slices G` -- the G partial handles of a G-way partition of the timed operand, run ONE AFTER
     ANOTHER on this GPU: per-slice apply time (what each of G GPUs would spend in its local kernel, before the all-reduce
@@ -481,11 +571,19 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--solve", default=None, metavar="CFG:K[:NCV[:STORE]]",
                     help="time one bse_solve alone (see run_solve) instead of the apply benchmark")
+    ap.add_argument("--peaks", action="store_true", help="measure the roofline denominators with the library's microbenchmarks")
+    ap.add_argument("--dense", default=None, metavar="M:K[:L]", help="time the dense basis kernels at config-4 shapes")
     ap.add_argument("--slices", type=int, default=0, metavar="G",
                     help="time the G partial handles of a G-way partition one after another on this GPU (see run_slices)")
     args = ap.parse_args()
     if args.solve:
         run_solve(args.solve)
+        return
+    if args.peaks:
+        run_peaks(args)
+        return
+    if args.dense:
+        run_dense(args.dense)
         return
     args.warmup = max(args.warmup, 3)
     global ES

@@ -304,6 +304,20 @@ bse_status_t bse_host_syev(int32_t m, double *hA, int32_t lda, double *hW, doubl
 bse_status_t bse_lanczos_quadrature_static(bse_handle_t h, const void *dStart, int32_t steps, double *hAlpha,
                                            double *hBeta, int32_t *hDone);
 
+/* The two dense basis kernels of the orthogonalisation and the restart on their own (
+ * PAPER.md:71, 67) -- what bse_orth and bse_solve are built from, exported so that they can be driven and timed directly.
+ *   bse_gram  : G = A^H B for A (n x m, lda) and B (n x k, ldb), n = N of the handle.  real_ip = 0: the complex Gram
+ *               matrix, written to dG (m x k complex128, ld = m).  real_ip = 1: Re(A^H B) only -- the real inner product of
+ *               the full-mode iteration (reading S4) -- written as complex128 with zero imaginary parts.  HBM-bound on A.
+ *   bse_update: C = alpha * A S + beta * C for A (n x m, lda), S (m x l complex128 device, ld = m; imaginary parts ignored
+ *               when real_ip = 1) and C (n x l, ldc; must not alias A).  l <= 8: the projection update W -= V h (HBM-bound);
+ *               large l: the Ritz rotation V <- V S (FP64-tensor-bound).
+ * Asynchronous on the handle's stream; dG / dS scratch conversions use the handle's workspace.  Errors: BSE_ERR_INVALID_ARG. */
+bse_status_t bse_gram(bse_handle_t h, const void *dA, int64_t lda, int32_t m, const void *dB, int64_t ldb, int32_t k,
+                      int32_t real_ip, void *dG);
+bse_status_t bse_update(bse_handle_t h, const void *dA, int64_t lda, int32_t m, const void *dS, int32_t l, int32_t real_ip,
+                        void *dC, int64_t ldc, double alpha, double beta);
+
 /* Microbenchmarks behind the roofline denominators (north_star: "achieved HBM GB/s and FP64 pipe utilisation ... against
  * the chip's peaks"; MEASURED_PEAKS.json has no FP64 figure).  Each runs one warm-up and one timed launch of a kernel that
  * does nothing else, on one CTA per SM, timed with CUDA events on `stream`; synchronous.

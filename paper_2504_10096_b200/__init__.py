@@ -67,6 +67,8 @@ _SIGNATURES = {
     "bse_host_syev": [_i32, _vp, _i32, _vp, _vp, _i32, _i32],
     "bse_solve": [_vp, _i32, _i32, _i32, _dbl, _i32, _u64, ctypes.POINTER(_dbl), _vp, _i64, ctypes.POINTER(_dbl),
                   ctypes.POINTER(_Info)],
+    "bse_gram": [_vp, _vp, _i64, _i32, _vp, _i64, _i32, _i32, _vp],
+    "bse_update": [_vp, _vp, _i64, _i32, _vp, _i32, _i32, _vp, _i64, _dbl, _dbl],
     "bse_selftest_peak": [_i32, _i32, _i32, _vp, _i64, _vp, ctypes.POINTER(_dbl), ctypes.POINTER(_dbl)],
 }
 EXPORTS = sorted(list(_SIGNATURES) + ["bse_status_string", "bse_launch_count"])
@@ -271,6 +273,22 @@ class Bse:
                               _ld(BW) if BW is not None else self.N, hcoef.data_ptr(), bfac.data_ptr(),
                               ctypes.byref(rank)), "bse_orth")
         return hcoef[:, :m], bfac, rank.value
+
+    def gram(self, A, B, real_ip: bool = False):
+        """A^H B (bse_gram): A (m, n), B (k, n) torch blocks -> torch (k, m) = column-major m x k."""
+        import torch
+        m, k = A.shape[0], B.shape[0]
+        G = torch.empty((k, m), dtype=torch.complex128, device="cuda")
+        _check(lib().bse_gram(self._h, A.data_ptr(), _ld(A), m, B.data_ptr(), _ld(B), k, 1 if real_ip else 0, G.data_ptr()),
+               "bse_gram")
+        return G
+
+    def update(self, A, S, C, alpha: float = 1.0, beta: float = 0.0, real_ip: bool = False):
+        """C = alpha A S + beta C (bse_update): A (m, n), S (l, m) = column-major m x l, C (l, n)."""
+        m, l = A.shape[0], S.shape[0]
+        _check(lib().bse_update(self._h, A.data_ptr(), _ld(A), m, S.data_ptr(), l, 1 if real_ip else 0, C.data_ptr(), _ld(C),
+                                alpha, beta), "bse_update")
+        return C
 
     def lanczos_quadrature(self, d, steps: int):
         """(alpha[steps'], beta[steps'+1]) of PAPER.md:65's Lanczos-with-quadrature solver; d: torch complex128 (N,)."""

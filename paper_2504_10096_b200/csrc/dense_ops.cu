@@ -142,3 +142,44 @@ bse_status_t assemble_full_vectors(bse_handle_s *h, const void *x, const void *p
 }
 
 }  // namespace bse
+
+namespace bse {
+// S (m x l complex, ld m) -> coefficient layout of gemm_basis (real parts, then imaginary parts, per column)
+__global__ void complex_to_coef_kernel(const double2 *S, int m, int l, int cplx, double *coef)
+{
+    int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= m * l) return;
+    int a = idx % m, col = idx / m;
+    int ldo = cplx ? 2 * m : m;
+    double2 v = S[idx];
+    coef[a + (int64_t)col * ldo] = v.x;
+    if (cplx) coef[a + m + (int64_t)col * ldo] = v.y;
+}
+
+}  // namespace bse
+
+using namespace bse;
+
+extern "C" bse_status_t bse_gram(bse_handle_t h, const void *dA, int64_t lda, int32_t m, const void *dB, int64_t ldb, int32_t k,
+                                 int32_t real_ip, void *dG)
+{
+    if (!h || !dA || !dB || !dG || m < 1 || k < 1 || lda < h->N || ldb < h->N) return BSE_ERR_INVALID_ARG;
+    const bool cplx = !real_ip;
+    bse_status_t st = ensure_ws(h, (size_t)2 * m * k * 8);
+    if (st) return st;
+    if ((st = gram_basis(h, dA, lda, m, dB, ldb, k, cplx, h->N, (double *)h->ws))) return st;
+    return coef_to_complex(h, (const double *)h->ws, nullptr, m, k, cplx, dG);
+}
+
+extern "C" bse_status_t bse_update(bse_handle_t h, const void *dA, int64_t lda, int32_t m, const void *dS, int32_t l,
+                                   int32_t real_ip, void *dC, int64_t ldc, double alpha, double beta)
+{
+    if (!h || !dA || !dS || !dC || m < 1 || l < 1 || lda < h->N || ldc < h->N || dA == dC) return BSE_ERR_INVALID_ARG;
+    const bool cplx = !real_ip;
+    bse_status_t st = ensure_ws(h, (size_t)2 * m * l * 8);
+    if (st) return st;
+    complex_to_coef_kernel<<<(m * l + 255) / 256, 256, 0, h->stream>>>((const double2 *)dS, m, l, cplx ? 1 : 0, (double *)h->ws);
+    count_launch();
+    BSE_CUDA(cudaGetLastError());
+    return gemm_basis(h, dA, lda, m, cplx, (const double *)h->ws, cplx ? 2 * m : m, l, h->N, dC, ldc, alpha, beta);
+}
