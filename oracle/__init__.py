@@ -57,6 +57,10 @@ def _load():
         lib.orc_lanczos_full.argtypes = [_i64, _c128, _c128, ctypes.c_int, ctypes.c_double, ctypes.c_int,
                                          ctypes.c_int, ctypes.c_int, _c128, _f64, _c128, _f64]
         lib.orc_lanczos_full.restype = ctypes.c_int
+        lib.orc_lanczos_full_gruning.argtypes = [_i64, _c128, _c128, ctypes.c_int, ctypes.c_double, ctypes.c_int,
+                                                 ctypes.c_int, ctypes.c_int, _c128, _f64, _c128, _f64, ctypes.c_void_p,
+                                                 ctypes.c_int]
+        lib.orc_lanczos_full_gruning.restype = ctypes.c_int
         lib.orc_tridiag_ql.argtypes = [_i64, _f64, _f64, _f64, ctypes.c_void_p]
         lib.orc_tridiag_ql.restype = ctypes.c_int
         lib.orc_round_c64.argtypes = [_i64, _c128, _c128]
@@ -200,6 +204,22 @@ def lanczos_full(R, C, nev, tol, x0, maxit=None, check=10, minit=0):
     if steps == -1000000:
         raise np.linalg.LinAlgError("Omega is not positive definite")
     return om, Vec, res, steps
+
+
+def lanczos_full_gruning(R, C, nev, tol, x0, maxit=None, check=10, minit=0, n_ritz=0):
+    """The "Gruning" variant (reading R9): Lanczos on H itself in the Omega inner product, T = tridiag(beta, 0, beta).
+    Same outputs as lanczos_full; steps counts Lanczos vectors (one half apply each).  n_ritz > 0: also returns the n_ritz lowest
+    positive Ritz values of the last projected matrix."""
+    R = _c(R); C = _c(C)
+    N = R.shape[0]
+    maxit = 4 * N if maxit is None else maxit
+    om = np.zeros(nev); Vec = np.zeros((2 * N, nev), dtype=np.complex128); res = np.zeros(nev)
+    ritz = np.zeros(max(n_ritz, 1))
+    steps = _load().orc_lanczos_full_gruning(N, R, C, nev, tol, maxit, check, minit, _c(x0).reshape(N), om, Vec, res,
+                                             ritz.ctypes.data if n_ritz > 0 else None, n_ritz)
+    if steps == -1000000:
+        raise np.linalg.LinAlgError("Omega is not positive definite")
+    return (om, Vec, res, steps, ritz[:n_ritz]) if n_ritz > 0 else (om, Vec, res, steps)
 
 
 def lanczos_quadrature(R, d, steps):

@@ -654,6 +654,126 @@ done:
 }
 
 /* ------------------------------------------------------------------------------------------
+ * Second structure-preserving variant ("Gruning": "three variations of a structure-preserving Lanczos
+ * iteration ... very similar in terms of operations"; the recurrence itself is in refs not in the container, DESIGN.md
+ * reading R9, derived from Eq. 1): Lanczos on H ITSELF -- no squaring -- in the inner product of Omega = Sigma H, in which H is
+ * self-adjoint (<u, H v>_Omega = u^H Omega Sigma Omega v; pseudo-Hermitian Lanczos).  Started at u_1 = [z_1; conj z_1], every
+ * Lanczos vector keeps the block structure with alternating sign, u_j = [z_j; s_j conj z_j], s_j = (-1)^(j+1), because
+ *     H [z; s conj z] = [w; -s conj w],   w = R z + s C conj(z)   (= P(z) for s = +1, M(z) for s = -1),
+ * and Omega u_j = [w_j; s_j conj w_j], so that <u_i, u_j>_Omega = 2 Re(w_i^H z_j) for equal signs.  The diagonal recurrence
+ * coefficient alpha_j = <u_j, H u_j>_Omega = |w_j|^2 - |w_j|^2 vanishes identically:
+ *     beta_{j+1} u_{j+1} = H u_j - beta_j u_{j-1}   ->   half vectors:  beta_{j+1} z_{j+1} = w_j - beta_j z_{j-1},
+ * T = tridiag(beta, 0, beta) has the eigenvalues +-theta in pairs and theta_i > 0 approximates omega_i DIRECTLY (one half apply
+ * per Lanczos vector; two of these steps span what one step of orc_lanczos_full spans).  Normalisation <u, u>_Omega = 1:
+ * 2 Re(z^H w) = 1.  Full reorthogonalisation (twice) of the new vector against the stored vectors of ITS OWN sign, with the real
+ * coefficients 2 Re(w_i^H z): vectors of the other sign are Omega-orthogonal to it in exact arithmetic (the coefficient would be
+ * purely imaginary) and are left alone, as the +-i copies are in orc_lanczos_full (reading R1).
+ * Ritz vector for (theta, s): x = sum_{j odd} s_j z_j, y = sum_{j even} s_j z_j, v = [x + y; conj(x - y)], scaled to v^H Sigma v = 1.
+ * Residual estimate |H v - theta v|_2 = beta_{n+1} |s_n| sqrt(2) |z_{n+1}|_2 (times that scale).  Multiplicity as in
+ * orc_lanczos_full (candidates Sigma-orthogonalised against the accepted eigenvectors).  maxit counts Lanczos vectors.
+ * Out: omega (nev ascending), Vec (2N x nev row-major), res (nev).  Returns the number of Lanczos vectors (<0: failed).
+ * Pins (tests/test_oracle_eig.py): bse_direct on the same matrices; Ritz values of 2 m vectors = Ritz values of m steps of
+ * orc_lanczos_full; residuals; Sigma-orthonormality; distinct omega on a run to the whole space.
+ * ------------------------------------------------------------------------------------------ */
+int orc_lanczos_full_gruning(int64_t N, const zc *R, const zc *C, int nev, double tol, int maxit, int check, int minit,
+                             const zc *x0, double *omega, zc *Vec, double *res, double *ritz_out, int n_ritz)
+{
+    if (maxit > 4 * N) maxit = (int)(4 * N);
+    zc *Zb = (zc *)malloc(sizeof(zc) * (size_t)N * (maxit + 1));      /* half vectors z_j            */
+    zc *Wb = (zc *)malloc(sizeof(zc) * (size_t)N * (maxit + 1));      /* images w_j = P / M (z_j)    */
+    double *beta = (double *)calloc(maxit + 2, sizeof(double)), *zero = (double *)calloc(maxit + 2, sizeof(double));
+    zc *zv = (zc *)malloc(sizeof(zc) * N), *cand = (zc *)malloc(sizeof(zc) * 2 * (size_t)N);
+    double *S = NULL, *th = NULL;
+    int result = -1;
+    /* u_1: 2 Re(z^H P z) = 1 */
+    orc_apply_half(N, 1, +1, R, C, x0, Wb);
+    {
+        ld s = 0.0L;
+        for (int64_t i = 0; i < N; ++i) s += (ld)creal(x0[i]) * (ld)creal(Wb[i]) + (ld)cimag(x0[i]) * (ld)cimag(Wb[i]);
+        if (!(s > 0.0L)) { result = -1000000; goto done; }
+        double sc = 1.0 / sqrt(2.0 * (double)s);
+        for (int64_t i = 0; i < N; ++i) { Zb[i] = x0[i] * sc; Wb[i] *= sc; }
+    }
+    for (int j = 0; j < maxit; ++j) {                      /* vector index j (0-based), sign +1 for even j */
+        /* candidate half vector of u_{j+1}: w_j (- beta_j z_{j-1}, covered by the reorthogonalisation) */
+        memcpy(zv, Wb + (size_t)j * N, sizeof(zc) * N);
+        for (int pass = 0; pass < 2; ++pass)
+            for (int p = (j + 1) % 2; p <= j; p += 2) {    /* stored vectors with the sign of u_{j+1} */
+                const zc *wp = Wb + (size_t)p * N, *zp = Zb + (size_t)p * N;
+                ld s = 0.0L;
+                for (int64_t i = 0; i < N; ++i) s += (ld)creal(wp[i]) * (ld)creal(zv[i]) + (ld)cimag(wp[i]) * (ld)cimag(zv[i]);
+                double cf = 2.0 * (double)s;
+                for (int64_t i = 0; i < N; ++i) zv[i] -= cf * zp[i];
+            }
+        zc *wn = Wb + (size_t)(j + 1) * N;
+        orc_apply_half(N, 1, ((j + 1) % 2 == 0) ? +1 : -1, R, C, zv, wn);
+        ld b2 = 0.0L;
+        for (int64_t i = 0; i < N; ++i) b2 += (ld)creal(zv[i]) * (ld)creal(wn[i]) + (ld)cimag(zv[i]) * (ld)cimag(wn[i]);
+        const int n = j + 1;                               /* Lanczos vectors so far */
+        double b = 0.0, zn1 = 0.0;
+        int breakdown = 0;
+        if (b2 > 0.0L) {
+            b = sqrt(2.0 * (double)b2);
+            for (int64_t i = 0; i < N; ++i) { Zb[(size_t)(j + 1) * N + i] = zv[i] / b; wn[i] /= b; }
+            zn1 = nrm2(N, Zb + (size_t)(j + 1) * N);
+        } else if (nrm2(N, zv) > 1e-10) {
+            result = -1000000; break;                      /* Omega not positive definite */
+        } else breakdown = 1;
+        beta[j + 1] = b;
+        const int last = (n == maxit) || breakdown;
+        if (n >= 2 * nev && n >= minit && n % 2 == 0 && (n % check == 0 || last)) {
+            S = (double *)realloc(S, sizeof(double) * n * n);
+            th = (double *)realloc(th, sizeof(double) * n);
+            if (orc_tridiag_ql(n, zero, beta + 1, th, S)) break;          /* T = tridiag(beta, 0, beta) */
+            const int h0 = n / 2;                                         /* th[h0 ...] are the positive eigenvalues, ascending */
+            if (ritz_out) for (int i = 0; i < n_ritz && i < n - h0; ++i) ritz_out[i] = th[h0 + i];
+            const double hn = th[n - 1];
+            int found = 0, all_converged = 1;
+            for (int i = h0; i < n && found < nev; ++i) {
+                const double om = th[i];
+                if (!(om > 0.0)) { all_converged = 0; if (!last) break; else continue; }
+                for (int64_t r = 0; r < N; ++r) {
+                    zc x = 0.0, y = 0.0;
+                    for (int p = 0; p < n; ++p) {
+                        if (p % 2 == 0) x += Zb[(size_t)p * N + r] * S[p * n + i];
+                        else y += Zb[(size_t)p * N + r] * S[p * n + i];
+                    }
+                    cand[r] = x + y;
+                    cand[r + N] = conj(x - y);
+                }
+                double sn = creal(sigma_dot(N, cand, 1, cand, 1));
+                if (!(sn > 0.0)) { all_converged = 0; if (!last) break; else continue; }
+                double sc = 1.0 / sqrt(sn);
+                for (int64_t r = 0; r < 2 * N; ++r) cand[r] *= sc;
+                const double ri = sc * b * fabs(S[(n - 1) * n + i]) * sqrt(2.0) * zn1;
+                if (ri > tol * hn) {
+                    if (!last) break;
+                    all_converged = 0;
+                }
+                for (int pass = 0; pass < 2; ++pass)
+                    for (int q = 0; q < found; ++q) {
+                        zc cf = sigma_dot(N, Vec + q, nev, cand, 1);
+                        for (int64_t r = 0; r < 2 * N; ++r) cand[r] -= Vec[r * nev + q] * cf;
+                    }
+                double left = creal(sigma_dot(N, cand, 1, cand, 1));
+                if (!(left > 1e-4)) continue;                             /* the second copy of an accepted eigenpair */
+                double nrm = 1.0 / sqrt(left);
+                for (int64_t r = 0; r < 2 * N; ++r) Vec[r * nev + found] = cand[r] * nrm;
+                omega[found] = om;
+                res[found] = ri;
+                ++found;
+            }
+            int ok = (found == nev) && all_converged;
+            if (ok || last) { result = ok ? n : -n; break; }
+        }
+        if (last) break;
+    }
+done:
+    free(Zb); free(Wb); free(beta); free(zero); free(zv); free(cand); free(S); free(th);
+    return result;
+}
+
+/* ------------------------------------------------------------------------------------------
  * Lanczos with quadrature rules ("a Lanczos iteration with quadrature rules to obtain the
  * optical absorption spectrum directly, without explicitly computing the eigenpairs"), TDA case.
  * Textbook three-term recurrence on the Hermitian R started at d / |d| (no reorthogonalisation, no stored basis):

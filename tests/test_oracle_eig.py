@@ -182,6 +182,43 @@ def test_lanczos_full_copy_structure(orc):
     assert np.linalg.norm(v2 - 1j * v) < 1e-10
 
 
+def test_gruning_variant_vs_direct_route_and_shao_variant(orc):
+    """The second structure-preserving variant (reading R9: Lanczos on H in the Omega inner product, T = tridiag(beta, 0, beta))
+    against the paper's direct route, and against the first variant: 2 m of its vectors span what m steps of the H^2 recurrence
+    span, so the Ritz values agree long before either has converged ("very similar in terms of operations")."""
+    N, nev = 96, 5
+    R, C = _bse_pair(N, 6)
+    x0 = gen.block_X(N, 1, 97)[:, 0]
+    om, V, res, steps = orc.lanczos_full_gruning(R, C, nev, 1e-10, x0, check=4)
+    assert steps > 0
+    omd, _ = orc.bse_direct(R, C, want_vectors=False)
+    assert np.max(np.abs(om - omd[N:N + nev])) < 1e-10 * omd[-1]
+    H = _H_dense(R, C)
+    r = np.linalg.norm(H @ V - V * om, axis=0)
+    assert np.all(r < 1e-8 * omd[-1]) and np.all(r < 5 * res + 1e-12)
+    Sig = np.concatenate([np.ones(N), -np.ones(N)])
+    assert np.linalg.norm(V.conj().T @ (Sig[:, None] * V) - np.eye(nev)) < 1e-8
+    # one half apply per vector: exactly twice the step count of the H^2 recurrence for the same convergence
+    om_s, _, _, steps_s = orc.lanczos_full(R, C, nev, 1e-10, x0, check=2)
+    assert steps == 2 * steps_s
+    # unconverged Ritz values after m = 30 steps (never-met tolerance, stop at maxit): same Krylov space, same values
+    m = 30
+    a, _, _, sa = orc.lanczos_full(R, C, 4, 1e-30, x0, maxit=m, check=m)
+    b, _, _, sb = orc.lanczos_full_gruning(R, C, 4, 1e-30, x0, maxit=2 * m, check=2 * m)
+    assert sa == -m and sb == -2 * m
+    assert np.max(np.abs(a - b)) < 1e-9 * omd[-1] and np.max(np.abs(a - omd[N:N + 4])) > 1e-6    # equal, and not yet converged
+
+
+def test_gruning_variant_returns_distinct_omega_on_the_whole_space(orc):
+    N, nev = 96, 10
+    R, C = _bse_pair(N, 9)
+    x0 = gen.block_X(N, 1, 95)[:, 0]
+    om, V, res, steps = orc.lanczos_full_gruning(R, C, nev, 1e-11, x0, check=4, minit=4 * N - 8)
+    assert steps >= 4 * N - 8
+    omd, _ = orc.bse_direct(R, C, want_vectors=False)
+    assert np.max(np.abs(om - omd[N:N + nev])) < 1e-10 * omd[-1] and np.min(np.diff(om)) > 1e-6
+
+
 def test_tridiag_ql_closed_form_and_jacobi(orc):
     # Toeplitz tridiag(b, a, b): eigenvalues a + 2 b cos(j pi / (m + 1)), eigenvectors sin(i j pi / (m + 1))
     m, a, b = 60, 1.5, -0.7
