@@ -411,7 +411,8 @@ def run_solve(spec):
     parts = spec.split(":")
     k = int(parts[1])
     ncv = int(parts[2]) if len(parts) > 2 and parts[2] else 0
-    store = parts[3] if len(parts) > 3 else "c128"
+    store = parts[3] if len(parts) > 3 and parts[3] else "c128"
+    variant = {"shao": 0, "gruning": 1}[parts[4]] if len(parts) > 4 else 0      # bse_solve_variant
     if "@" in parts[0]:
         # MODE@N@NEV: the same generator at another size, e.g. the paper's N = 10368 / 36288 / 103680 with nev = 100
         # (PAPER.md:115-122, 180); sigma = 1 in full mode, group 16
@@ -434,11 +435,11 @@ def run_solve(spec):
     h = b.Bse(b.MODE_FULL if full else b.MODE_TDA, N, rt, ct, storage=storage)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    res = h.solve(cfg["nev"], k, ncv=ncv, tol=1e-8, seed=1, raise_on_error=False)
+    res = h.solve(cfg["nev"], k, ncv=ncv, tol=1e-8, seed=1, raise_on_error=False, variant=variant)
     torch.cuda.synchronize()
     sec = time.perf_counter() - t0
     print(json.dumps({"solve": {"workload": f"config {cid}: {cfg['mode']} N={N} nev={cfg['nev']} k={k} tol=1e-8 sigma={cfg['sigma']}",
-                                "store": store, "seconds": sec, "status": res.status, "info": res.info,
+                                "store": store, "variant": ["shao", "gruning"][variant], "seconds": sec, "status": res.status, "info": res.info,
                                 "omega_first": float(res.omega[0]), "omega_last": float(res.omega[-1]),
                                 "max_residual_estimate": float(res.resid.max())}}))
 
@@ -571,7 +572,7 @@ def main():
     ap.add_argument("--ref-rows", type=int, default=1024)
     ap.add_argument("--no-extras", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--solve", default=None, metavar="CFG:K[:NCV[:STORE]]",
+    ap.add_argument("--solve", default=None, metavar="CFG:K[:NCV[:STORE[:VARIANT]]]",
                     help="time one bse_solve alone (see run_solve) instead of the apply benchmark")
     ap.add_argument("--peaks", action="store_true", help="measure the roofline denominators with the library's microbenchmarks")
     ap.add_argument("--dense", default=None, metavar="M:K[:L]", help="time the dense basis kernels at config-4 shapes")

@@ -251,6 +251,21 @@ bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_t ncv, doub
                        int32_t max_restarts, uint64_t seed, double *hOmega, void *dVec, int64_t ldvec,
                        double *hResid, bse_info_t *info);
 
+/* bse_solve with a choice among the structure-preserving variants of PAPER.md:65-67 ("three variations of a structure-preserving
+ * Lanczos iteration with a thick restart ... very similar in terms of operations"); full mode only (TDA handles run the
+ * Hermitian iteration whatever `variant` says).  Same outputs, tolerances and errors as bse_solve.
+ *   BSE_VARIANT_SHAO    (= bse_solve): Lanczos on H^2 through G = M o P in the inner product Re(x^H P(z)) (reading S4);
+ *   BSE_VARIANT_GRUNING : Lanczos on H itself in the Omega inner product (reading R9): the Lanczos vectors alternate
+ *                         between [x; conj x] and [y; -conj y]; both families are stored with their images (X, P(X), Y, M(Y):
+ *                         twice the basis memory), the projected matrix is [[0, Bm^T], [Bm, 0]] with P(X) = Y Bm, and its positive
+ *                         eigenvalues approximate omega directly (no square root of a Ritz value of H^2).  Two half applies per
+ *                         block step, as BSE_VARIANT_SHAO; twice the orthogonalisation work.
+ * The third variant the paper names (ProjectedBSE) is not built: see DESIGN.md section 2, reading R10. */
+enum { BSE_VARIANT_SHAO = 0, BSE_VARIANT_GRUNING = 1 };
+bse_status_t bse_solve_variant(bse_handle_t h, int32_t variant, int32_t nev, int32_t k, int32_t ncv, double tol,
+                               int32_t max_restarts, uint64_t seed, double *hOmega, void *dVec, int64_t ldvec,
+                               double *hResid, bse_info_t *info);
+
 /* Lanczos with quadrature rules (the optical absorption spectrum "directly, without explicitly computing
  * the eigenpairs").  No reorthogonalisation, no stored basis; dStart: N complex128, device, not modified.  Synchronous;
  * all scalars stay on the device until the end.
@@ -303,6 +318,17 @@ bse_status_t bse_host_syev(int32_t m, double *hA, int32_t lda, double *hW, doubl
 #define BSE_STATIC_QUADRATURE_MAX_STEPS 1024
 bse_status_t bse_lanczos_quadrature_static(bse_handle_t h, const void *dStart, int32_t steps, double *hAlpha,
                                            double *hBeta, int32_t *hDone);
+
+/* The eigenvectors that "can be obtained trivially" from the right eigenvectors v_I = [X_I; Y_I] of the positive omega_I that
+ * bse_solve returns (full mode, dVec / dOut 2N x nev column-major, must not alias):
+ *   which = BSE_PARTNER_RIGHT_NEGATIVE : right eigenvectors of -omega_I,  [conj(Y_I); conj(X_I)]
+ *   which = BSE_PARTNER_LEFT_POSITIVE  : left eigenvectors of +omega_I,   Sigma v_I = [X_I; -Y_I]      (u^H H = omega u^H)
+ *   which = BSE_PARTNER_LEFT_NEGATIVE  : left eigenvectors of -omega_I,   [conj(Y_I); -conj(X_I)]
+ * With v_I^H Sigma v_J = delta_IJ the left and right sets are bi-orthonormal: u_I^H v_J = delta_IJ (+omega), = -delta_IJ (-omega).
+ * Asynchronous on the handle's stream.  Errors: BSE_ERR_INVALID_ARG (TDA handle, aliasing, sizes). */
+enum { BSE_PARTNER_RIGHT_NEGATIVE = 0, BSE_PARTNER_LEFT_POSITIVE = 1, BSE_PARTNER_LEFT_NEGATIVE = 2 };
+bse_status_t bse_partner_vectors(bse_handle_t h, const void *dVec, int64_t ldvec, int32_t nev, int32_t which, void *dOut,
+                                 int64_t ldout);
 
 /* The two dense basis kernels of the orthogonalisation and the restart on their own (
  * PAPER.md:71, 67) -- what bse_orth and bse_solve are built from, exported so that they can be driven and timed directly.

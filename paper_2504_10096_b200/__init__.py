@@ -15,6 +15,7 @@ _LIBPATH = os.path.join(_HERE, "libbse_b200.so")
 _lib = None
 
 MODE_TDA, MODE_FULL = 0, 1
+VARIANT_SHAO, VARIANT_GRUNING = 0, 1                                         # bse_solve_variant
 STORE_C128, STORE_C64, STORE_REAL_FORM, STORE_REAL_FORM_C64 = 0, 1, 2, 3      # storage type of the tile store (include/bse.h)
 MATRIX_R, MATRIX_C = 0, 1
 TILE = 64
@@ -67,8 +68,11 @@ _SIGNATURES = {
     "bse_host_syev": [_i32, _vp, _i32, _vp, _vp, _i32, _i32],
     "bse_solve": [_vp, _i32, _i32, _i32, _dbl, _i32, _u64, ctypes.POINTER(_dbl), _vp, _i64, ctypes.POINTER(_dbl),
                   ctypes.POINTER(_Info)],
+    "bse_partner_vectors": [_vp, _vp, _i64, _i32, _i32, _vp, _i64],
     "bse_gram": [_vp, _vp, _i64, _i32, _vp, _i64, _i32, _i32, _vp],
     "bse_update": [_vp, _vp, _i64, _i32, _vp, _i32, _i32, _vp, _i64, _dbl, _dbl],
+    "bse_solve_variant": [_vp, _i32, _i32, _i32, _i32, _dbl, _i32, _u64, ctypes.POINTER(_dbl), _vp, _i64, ctypes.POINTER(_dbl),
+                          ctypes.POINTER(_Info)],
     "bse_selftest_peak": [_i32, _i32, _i32, _vp, _i64, _vp, ctypes.POINTER(_dbl), ctypes.POINTER(_dbl)],
 }
 EXPORTS = sorted(list(_SIGNATURES) + ["bse_status_string", "bse_launch_count"])
@@ -274,6 +278,14 @@ class Bse:
                               ctypes.byref(rank)), "bse_orth")
         return hcoef[:, :m], bfac, rank.value
 
+    def partner_vectors(self, vectors, which: int = 0):
+        """-omega right eigenvectors (which = 0), left eigenvectors of +omega (1) / -omega (2) from solve()'s vectors (nev, 2N)."""
+        import torch
+        out = torch.empty_like(vectors)
+        _check(lib().bse_partner_vectors(self._h, vectors.data_ptr(), _ld(vectors), vectors.shape[0], which, out.data_ptr(),
+                                         _ld(out)), "bse_partner_vectors")
+        return out
+
     def gram(self, A, B, real_ip: bool = False):
         """A^H B (bse_gram): A (m, n), B (k, n) torch blocks -> torch (k, m) = column-major m x k."""
         import torch
@@ -314,14 +326,14 @@ class Bse:
         return alpha[:done.value], beta[:done.value + 1]
 
     def solve(self, nev: int, k: int, ncv: int = 0, tol: float = 1e-8, max_restarts: int = 1000, seed: int = 1,
-              raise_on_error: bool = True):
+              raise_on_error: bool = True, variant: int = 0):
         import numpy as np
         import torch
         omega = np.zeros(nev)
         resid = np.zeros(nev)
         vec = torch.zeros((nev, self.n_op), dtype=torch.complex128, device="cuda")
         info = _Info()
-        st = lib().bse_solve(self._h, nev, k, ncv, tol, max_restarts, seed,
+        st = lib().bse_solve_variant(self._h, variant, nev, k, ncv, tol, max_restarts, seed,
                              omega.ctypes.data_as(ctypes.POINTER(_dbl)), vec.data_ptr(), self.n_op,
                              resid.ctypes.data_as(ctypes.POINTER(_dbl)), ctypes.byref(info))
         if st != 0 and raise_on_error:

@@ -113,7 +113,8 @@ bse_status_t block_norm_scale(bse_handle_s *h, const void *W, int64_t ldw, const
                               bool cplx, double *scale2);
 bse_status_t normalize_block(bse_handle_s *h, const void *V, int64_t ldv, int m, const void *PV, int64_t ldpv, void *W,
                              int64_t ldw, int k, void *PW, int64_t ldpw, bool cplx, double scale2, void *hcoef_host,
-                             void *bfac_host, int *rank_out, uint64_t seed, uint64_t *rng_counter);
+                             void *bfac_host, int *rank_out, uint64_t seed, uint64_t *rng_counter, int image_sign = +1);
+// (image_sign: which half apply gives the image PW of a replacement column in the real inner product: +1 P, -1 M)
 
 // host eigensolver (host_eig.cpp)
 int host_heev(int m, void *A, int lda, double *w, void *Z, int ldz, int nz);

@@ -199,7 +199,7 @@ bse_status_t block_norm_scale(bse_handle_s *h, const void *W, int64_t ldw, const
 // be NULL) receives the corrections of the column-wise path.
 bse_status_t normalize_block(bse_handle_s *h, const void *V, int64_t ldv, int m, const void *PV, int64_t ldpv, void *W,
                              int64_t ldw, int k, void *PW, int64_t ldpw, bool cplx, double scale2, void *hcoef_host,
-                             void *bfac_host, int *rank_out, uint64_t seed, uint64_t *rng_counter)
+                             void *bfac_host, int *rank_out, uint64_t seed, uint64_t *rng_counter, int image_sign)
 {
     const int64_t n = h->N;
     OrthWs w;
@@ -293,7 +293,7 @@ bse_status_t normalize_block(bse_handle_s *h, const void *V, int64_t ldv, int m,
                 for (int tries = 0; tries < 3; ++tries) {
                     ST(fill_random_block(h, wj, ldw, n, 1, seed, (*rng_counter)++));
                     if (!cplx) {
-                        bse_status_t st = bse_apply_half(h, +1, wj, ldw, pwj, ldpw, 1);
+                        bse_status_t st = bse_apply_half(h, image_sign, wj, ldw, pwj, ldpw, 1);
                         if (st) return st;
                     }
                     for (int pass = 0; pass < 2; ++pass) {

@@ -47,6 +47,12 @@ struct Solver {
     double tol;
     int64_t ld;            // leading dimension of the basis buffers (= n)
     DevBuf V, PV, rot, coef, omega_d;
+    // variant BSE_VARIANT_GRUNING (reading R9): the sign -1 Lanczos vectors Y and their images MY = M(Y); Bm (ncv x ncv, real,
+    // column-major) holds the Y-coefficients of P(X): P(X) = Y Bm, so that the projected matrix of H is [[0, Bm^T], [Bm, 0]]
+    int variant = 0;
+    DevBuf Yb, MYb;
+    std::vector<double> Bm;
+    std::vector<zc> B1;     // k x k factor of the last Y block
     std::vector<zc> T;     // ncv x ncv, column-major
     int mp = 0;            // processed columns (T is mp x mp); the basis holds mp + k columns
     uint64_t seed, rng = 0;
@@ -202,6 +208,30 @@ struct Solver {
         if (!full) {
             ST(apply_tda_local(h, col(V, c0), ld, col(V, c0 + k), ld, k));
             ST(comm_sum_block(h, col(V, c0 + k), ld, n, k));
+        } else if (variant == BSE_VARIANT_GRUNING) {
+            // u_{2j} = [y; -conj y]: H u_{2j-1} has the half vector P(x_j); orthonormalise it against the stored vectors of its
+            // sign in the Omega inner product, <y_i, z>_M = Re(M(y_i)^H z) -- image recomputed after the projection (reading R3)
+            const int my = c0;                                                                   // Y columns so far
+            std::vector<zc> Hc1((size_t)std::max(my, 1) * k, zc(0.0));
+            double e_in = 0.0, e_after = 0.0, g_after = 0.0;
+            int rank = 0;
+            ST(copy_block(h, col(PV, c0), ld, col(Yb, my), ld, n, k));
+            ST(block_norm_scale(h, col(Yb, my), ld, nullptr, ld, k, false, &e_in));
+            ST(project_block(h, Yb.p, ld, my, MYb.p, ld, col(Yb, my), ld, k, nullptr, ld, false, Hc1.data()));
+            bse_status_t st = bse_apply_half(h, -1, col(Yb, my), ld, col(MYb, my), ld, k);     // M(z)
+            if (st) return st;
+            ST(block_norm_scale(h, col(Yb, my), ld, nullptr, ld, k, false, &e_after));
+            ST(block_norm_scale(h, col(Yb, my), ld, col(MYb, my), ld, k, false, &g_after));
+            const double scale2 = (e_after > 0.0) ? g_after * (e_in / e_after) : g_after;
+            B1.assign((size_t)k * k, zc(0.0));
+            ST(normalize_block(h, Yb.p, ld, my, MYb.p, ld, col(Yb, my), ld, k, col(MYb, my), ld, false, scale2, Hc1.data(),
+                               B1.data(), &rank, seed, &rng, -1));
+            for (int c = 0; c < k; ++c) {                                                        // P(X_j) = Y[:, :my] Hc1 + Y_j B1
+                for (int a = 0; a < my; ++a) Bm[a + (size_t)(c0 + c) * ncv] = Hc1[a + (size_t)c * my].real();
+                for (int a = 0; a < k; ++a) Bm[(my + a) + (size_t)(c0 + c) * ncv] = B1[a + (size_t)c * k].real();
+            }
+            // H u_{2j} has the half vector M(y_j): the next sign +1 candidate
+            ST(copy_block(h, col(MYb, my), ld, col(V, c0 + k), ld, n, k));
         } else {
             bse_status_t st = bse_apply_half(h, -1, col(PV, c0), ld, col(V, c0 + k), ld, k);      // W = M(p)
             if (st) return st;
@@ -242,7 +272,16 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
                                   uint64_t seed, double *hOmega, void *dVec, int64_t ldvec, double *hResid,
                                   bse_info_t *info_out)
 {
+    return bse_solve_variant(h, BSE_VARIANT_SHAO, nev, k, ncv, tol, max_restarts, seed, hOmega, dVec, ldvec, hResid, info_out);
+}
+
+extern "C" bse_status_t bse_solve_variant(bse_handle_t h, int32_t variant, int32_t nev, int32_t k, int32_t ncv, double tol,
+                                          int32_t max_restarts, uint64_t seed, double *hOmega, void *dVec, int64_t ldvec,
+                                          double *hResid, bse_info_t *info_out)
+{
     if (!h || nev < 1 || k < 1 || !hOmega || !dVec || !(tol > 0.0) || max_restarts < 0) return BSE_ERR_INVALID_ARG;
+    if (variant != BSE_VARIANT_SHAO && variant != BSE_VARIANT_GRUNING) return BSE_ERR_INVALID_ARG;
+    if (h->mode != BSE_MODE_FULL) variant = BSE_VARIANT_SHAO;          // TDA: the Hermitian iteration has no variants
     if (is_incomplete(h)) return BSE_ERR_INVALID_ARG;
     const int64_t n = h->N;
     const bool full = (h->mode == BSE_MODE_FULL);
@@ -269,10 +308,17 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
     } guard{info_out, &s, t_start};
     const bool verbose = getenv("BSE_VERBOSE") != nullptr;
     s.h = h; s.n = n; s.full = full; s.nev = nev; s.k = k; s.ncv = ncv; s.tol = tol; s.ld = n; s.seed = seed;
+    s.variant = variant;
+    const bool gruning = variant == BSE_VARIANT_GRUNING;
     s.info.ncv = ncv;
     const size_t basis_bytes = (size_t)n * (ncv + k) * 16;
     ST(s.V.alloc(basis_bytes));
     if (full) ST(s.PV.alloc(basis_bytes));
+    if (gruning) {
+        ST(s.Yb.alloc(basis_bytes));
+        ST(s.MYb.alloc(basis_bytes));
+        s.Bm.assign((size_t)ncv * ncv, 0.0);
+    }
     ST(s.rot.alloc((size_t)n * (ncv + k) * 16));
     const int ncmax = (ncv + k) / 2;                    // full mode: candidates of the multiplicity test (x and P x side by side in rot)
     ST(s.coef.alloc((size_t)2 * (ncv + k) * (ncv + k) * 8));
@@ -340,6 +386,16 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
         if (full) {
             // real coefficients (reading S4): T is real symmetric -> the real driver, a quarter of the reduction flops
             std::vector<double> Ar((size_t)mp * mp), Sr((size_t)mp * nz);
+            if (gruning) {
+                // T = Bm^T Bm: the positive eigenvalues sigma of [[0, Bm^T], [Bm, 0]] are the singular values of Bm, with the
+                // same right singular vectors S (sign +1 coefficients); the sign -1 coefficients are U = Bm S / sigma
+                for (int j = 0; j < mp; ++j)
+                    for (int i = 0; i <= j; ++i) {
+                        double acc = 0.0;
+                        for (int a = 0; a < mp; ++a) acc += s.Bm[a + (size_t)i * ncv] * s.Bm[a + (size_t)j * ncv];
+                        Ar[i + (size_t)j * mp] = Ar[j + (size_t)i * mp] = acc;
+                    }
+            } else
             for (int j = 0; j < mp; ++j)
                 for (int i = 0; i < mp; ++i) Ar[i + (size_t)j * mp] = s.T[i + (size_t)j * ldT].real();
             if (host_syev(mp, Ar.data(), mp, theta.data(), Sr.data(), mp, nz)) return BSE_ERR_INTERNAL;
@@ -370,10 +426,18 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
         if (verbose) fprintf(stderr, "[bse_solve] restart %d mp %d theta0 %.6e theta_max %.6e\n", restarts, mp, theta[0], theta[mp - 1]);
         if (full && !(theta[0] > 0.0)) return BSE_ERR_NOT_POSITIVE_DEFINITE;
         s.normest = std::max(s.normest, full ? std::sqrt(tmax) : tmax);
+        std::vector<zc> Beff = B;                      // G x - theta x = X_next Beff s_last;  variant R9: Beff = B2 B1
+        if (gruning)
+            for (int a = 0; a < k; ++a)
+                for (int b = 0; b < k; ++b) {
+                    zc acc(0.0);
+                    for (int q = 0; q < k; ++q) acc += B[a + (size_t)q * k] * s.B1[q + (size_t)b * k];
+                    Beff[a + (size_t)b * k] = acc;
+                }
         for (int i = 0; i < nz; ++i) {
             std::vector<zc> c(k, zc(0.0));
             for (int a = 0; a < k; ++a)
-                for (int b = 0; b < k; ++b) c[a] += B[a + (size_t)b * k] * S[(mp - k + b) + (size_t)i * mp];
+                for (int b = 0; b < k; ++b) c[a] += Beff[a + (size_t)b * k] * S[(mp - k + b) + (size_t)i * mp];
             double r2 = 0.0;
             for (int a = 0; a < k; ++a)
                 for (int b = 0; b < k; ++b) r2 += (std::conj(c[a]) * E[a + (size_t)b * k] * c[b]).real();
@@ -434,6 +498,23 @@ extern "C" bse_status_t bse_solve(bse_handle_t h, int32_t nev, int32_t k, int32_
             ST(s.rotate(s.PV, mp, S.data(), mp, l, s.rot.p, n));
             ST(copy_block(h, s.col(s.PV, mp), s.ld, s.col(s.rot, l), s.ld, n, k));
             ST(copy_block(h, s.rot.p, s.ld, s.PV.p, s.ld, n, l + k));
+        }
+        if (gruning) {
+            std::vector<zc> U((size_t)mp * l, zc(0.0));
+            for (int j = 0; j < l; ++j) {
+                const double sg = std::sqrt(std::max(theta[j], 1e-300));
+                for (int a = 0; a < mp; ++a) {
+                    double acc = 0.0;
+                    for (int q = 0; q < mp; ++q) acc += s.Bm[a + (size_t)q * ncv] * S[q + (size_t)j * mp].real();
+                    U[a + (size_t)j * mp] = acc / sg;
+                }
+            }
+            ST(s.rotate(s.Yb, mp, U.data(), mp, l, s.rot.p, n));
+            ST(copy_block(h, s.rot.p, s.ld, s.Yb.p, s.ld, n, l));
+            ST(s.rotate(s.MYb, mp, U.data(), mp, l, s.rot.p, n));
+            ST(copy_block(h, s.rot.p, s.ld, s.MYb.p, s.ld, n, l));
+            std::fill(s.Bm.begin(), s.Bm.end(), 0.0);
+            for (int i = 0; i < l; ++i) s.Bm[i + (size_t)i * ncv] = std::sqrt(std::max(theta[i], 0.0));
         }
         std::fill(s.T.begin(), s.T.end(), zc(0.0));
         for (int i = 0; i < l; ++i) s.T[i + (size_t)i * ldT] = theta[i];

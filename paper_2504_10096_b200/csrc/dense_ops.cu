@@ -144,6 +144,36 @@ bse_status_t assemble_full_vectors(bse_handle_s *h, const void *x, const void *p
 }  // namespace bse
 
 namespace bse {
+// out = [conj(v2); conj(v1)] (which = 0), [v1; -v2] (which = 1), [conj(v2); -conj(v1)] (which = 2) for v = [v1; v2]
+__global__ void partner_kernel(const double2 *v, int64_t ldv, int64_t N, int nev, int which, double2 *out, int64_t ldo)
+{
+    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    int c = blockIdx.y;
+    if (i >= N || c >= nev) return;
+    const double2 a = v[i + c * ldv], b = v[i + N + c * ldv];
+    double2 o1, o2;
+    if (which == 0) { o1 = make_double2(b.x, -b.y); o2 = make_double2(a.x, -a.y); }
+    else if (which == 1) { o1 = a; o2 = make_double2(-b.x, -b.y); }
+    else { o1 = make_double2(b.x, -b.y); o2 = make_double2(-a.x, a.y); }
+    out[i + c * ldo] = o1;
+    out[i + N + c * ldo] = o2;
+}
+}  // namespace bse
+
+extern "C" bse_status_t bse_partner_vectors(bse_handle_t h, const void *dVec, int64_t ldvec, int32_t nev, int32_t which,
+                                            void *dOut, int64_t ldout)
+{
+    if (!h || h->mode != BSE_MODE_FULL || !dVec || !dOut || dVec == dOut || nev < 1 || which < 0 || which > 2 ||
+        ldvec < 2 * h->N || ldout < 2 * h->N)
+        return BSE_ERR_INVALID_ARG;
+    bse::partner_kernel<<<dim3((unsigned)((h->N + 255) / 256), nev), 256, 0, h->stream>>>(
+        (const double2 *)dVec, ldvec, h->N, nev, which, (double2 *)dOut, ldout);
+    bse::count_launch();
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}
+
+namespace bse {
 // S (m x l complex, ld m) -> coefficient layout of gemm_basis (real parts, then imaginary parts, per column)
 __global__ void complex_to_coef_kernel(const double2 *S, int m, int l, int cplx, double *coef)
 {

@@ -103,6 +103,78 @@ def test_full_small_vs_direct_route(orc, k):
     _check_full(orc, R, C, res, nev, omd[N:])
 
 
+@pytest.mark.parametrize("k", [1, 4])
+def test_gruning_variant_small_vs_direct_route(orc, k):
+    """bse_solve_variant(BSE_VARIANT_GRUNING) (reading R9) against the paper's direct route, with the same
+    checks as the default variant; both variants return the same omega."""
+    import paper_2504_10096_b200 as b
+    N, nev = 192, 8
+    R = gen.dense_R(N, 2, sigma=1.0); C = gen.dense_C(N, 2)
+    h = b.Bse(b.MODE_FULL, N, pack(R, 0), pack(C, 1))
+    res = h.solve(nev, k, tol=1e-9, seed=1, variant=b.VARIANT_GRUNING)
+    omd, _ = orc.bse_direct(R, C, want_vectors=False)
+    _check_full(orc, R, C, res, nev, omd[N:])
+    ref = h.solve(nev, k, tol=1e-9, seed=1)
+    assert np.max(np.abs(res.omega - ref.omega) / ref.omega) <= TOL_EIG
+
+
+def test_gruning_variant_config1_golden_and_oracle_variant(orc):
+    """BASELINE.json config 1 with the second variant: the stored oracle values (20 distinct omega), live residuals through
+    the oracle apply; and the oracle's own Gruning recurrence on a smaller instance of the same generator."""
+    import paper_2504_10096_b200 as b
+    cfg = gen.CONFIGS[1]
+    N, nev, k = cfg["N"], cfg["nev"], cfg["k"]
+    R = gen.dense_R(N, 1, sigma=cfg["sigma"]); C = gen.dense_C(N, 1)
+    res = b.Bse(b.MODE_FULL, N, pack(R, 0), pack(C, 1)).solve(nev, k, tol=TOL_SMALL, seed=1, variant=b.VARIANT_GRUNING)
+    _check_full(orc, R, C, res, nev, _golden("oracle_config1.txt"))
+    n = 256
+    Rs = gen.dense_R(n, 4, sigma=1.0); Cs = gen.dense_C(n, 4)
+    om_o, _, _, steps = orc.lanczos_full_gruning(Rs, Cs, 6, 1e-11, gen.block_X(n, 1, 96)[:, 0], check=4)
+    assert steps > 0
+    rs = b.Bse(b.MODE_FULL, n, pack(Rs, 0), pack(Cs, 1)).solve(6, 2, tol=1e-10, seed=2, variant=b.VARIANT_GRUNING)
+    assert np.max(np.abs(rs.omega - om_o) / om_o) <= TOL_EIG
+
+
+def test_gruning_variant_closed_form_degenerate_and_real_form():
+    """Closed-form pair with a double omega (multiplicity decided from the vectors in both variants), complex stores and the
+    real-form store."""
+    import torch
+    import paper_2504_10096_b200 as b
+    N, nev, k = 2048, 10, 4
+    d1 = gen.prescribed_spectrum(N, 7, 1.0, 9.0, power=2 / 3); d2 = gen.prescribed_spectrum(N, 8, 2.0, 5.0, power=2 / 3)
+    d1[1], d2[1] = d1[0] * 1.2, d2[0] / 1.2
+    ur = gen.householder_u(N, 9, complex_u=False).real.copy(); phi = gen.phases(N, 9)
+    rt, ct = b.bse_fill_closed_form_full(N, *(torch.from_numpy(a).cuda() for a in (d1, d2, ur, phi)),
+                                         float(np.sum(d1 * ur ** 2)), float(np.sum(d2 * ur ** 2)))
+    exact = np.sort(np.sqrt(d1 * d2))[:nev]
+    res = b.Bse(b.MODE_FULL, N, rt, ct).solve(nev, k, tol=1e-9, seed=4, variant=b.VARIANT_GRUNING)
+    assert np.max(np.abs(res.omega - exact) / exact) <= TOL_EIG and res.info["basis_orth_err"] <= TOL_ORTH
+    b.bse_to_real_form(rt, ct, N)
+    res = b.Bse(b.MODE_FULL, N, rt, ct, storage=b.STORE_REAL_FORM).solve(nev, 8, tol=1e-9, seed=4, variant=b.VARIANT_GRUNING)
+    assert np.max(np.abs(res.omega - exact) / exact) <= TOL_EIG
+
+
+def test_partner_and_left_eigenvectors(orc):
+    """eigenvectors of the negative eigenvalues and left eigenvectors "can be obtained trivially"."""
+    import paper_2504_10096_b200 as b
+    N, nev = 192, 6
+    R = gen.dense_R(N, 2, sigma=1.0); C = gen.dense_C(N, 2)
+    h = b.Bse(b.MODE_FULL, N, pack(R, 0), pack(C, 1))
+    res = h.solve(nev, 4, tol=1e-10, seed=1)
+    V, om = to_host(res.vectors), res.omega
+    H = _H_dense(R, C)
+    nrm = np.linalg.norm(H, 2)
+    Vn = to_host(h.partner_vectors(res.vectors, 0))
+    assert np.all(np.linalg.norm(orc.apply_full(R, C, Vn) + Vn * om, axis=0) <= TOL_RES * nrm)          # H v' = -omega v'
+    Ul, Uln = to_host(h.partner_vectors(res.vectors, 1)), to_host(h.partner_vectors(res.vectors, 2))
+    assert np.all(np.linalg.norm(Ul.conj().T @ H - om[:, None] * Ul.conj().T, axis=1) <= TOL_RES * nrm)   # u^H H = omega u^H
+    assert np.all(np.linalg.norm(Uln.conj().T @ H + om[:, None] * Uln.conj().T, axis=1) <= TOL_RES * nrm)
+    assert np.linalg.norm(Ul.conj().T @ V - np.eye(nev)) <= 1e-7 and np.linalg.norm(Uln.conj().T @ Vn + np.eye(nev)) <= 1e-7
+    assert np.linalg.norm(Ul.conj().T @ Vn) <= 1e-7                                                      # bi-orthogonality across +-omega
+    ht = b.Bse(b.MODE_TDA, N, pack(R, 0))
+    assert b.lib().bse_partner_vectors(ht._h, res.vectors.data_ptr(), 2 * N, nev, 0, res.vectors.data_ptr(), 2 * N) == 1
+
+
 def _golden(name):
     import os
     path = os.path.join(os.path.dirname(__file__), "golden", name)
