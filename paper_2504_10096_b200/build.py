@@ -11,7 +11,7 @@ LIB = os.path.join(HERE, "libbse_b200.so")
 SOURCES = ["bse_api.cu", "bse_apply.cu", "dense_ops.cu", "bse_orth.cu", "bse_solve.cu", "bse_quadrature.cu", "bse_selftest.cu"]
 HOST_SOURCES = ["host_eig.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
-              "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "-Xcompiler", "-fopenmp", "-Xptxas", "-v"]
 
 
 def _stale() -> bool:

@@ -389,11 +389,14 @@ extern "C" bse_status_t bse_solve_variant(bse_handle_t h, int32_t variant, int32
             if (gruning) {
                 // T = Bm^T Bm: the positive eigenvalues sigma of [[0, Bm^T], [Bm, 0]] are the singular values of Bm, with the
                 // same right singular vectors S (sign +1 coefficients); the sign -1 coefficients are U = Bm S / sigma
+                const double *Bmp = s.Bm.data();
+                double *Arp = Ar.data();
+#pragma omp parallel for schedule(dynamic, 8)
                 for (int j = 0; j < mp; ++j)
                     for (int i = 0; i <= j; ++i) {
                         double acc = 0.0;
-                        for (int a = 0; a < mp; ++a) acc += s.Bm[a + (size_t)i * ncv] * s.Bm[a + (size_t)j * ncv];
-                        Ar[i + (size_t)j * mp] = Ar[j + (size_t)i * mp] = acc;
+                        for (int a = 0; a < mp; ++a) acc += Bmp[a + (size_t)i * ncv] * Bmp[a + (size_t)j * ncv];
+                        Arp[i + (size_t)j * mp] = Arp[j + (size_t)i * mp] = acc;
                     }
             } else
             for (int j = 0; j < mp; ++j)
@@ -501,13 +504,16 @@ extern "C" bse_status_t bse_solve_variant(bse_handle_t h, int32_t variant, int32
         }
         if (gruning) {
             std::vector<zc> U((size_t)mp * l, zc(0.0));
+            const double *Bmp = s.Bm.data();
+#pragma omp parallel for schedule(static)
             for (int j = 0; j < l; ++j) {
-                const double sg = std::sqrt(std::max(theta[j], 1e-300));
-                for (int a = 0; a < mp; ++a) {
-                    double acc = 0.0;
-                    for (int q = 0; q < mp; ++q) acc += s.Bm[a + (size_t)q * ncv] * S[q + (size_t)j * mp].real();
-                    U[a + (size_t)j * mp] = acc / sg;
+                std::vector<double> u(mp, 0.0);
+                for (int q = 0; q < mp; ++q) {
+                    const double sq = S[q + (size_t)j * mp].real();
+                    for (int a = 0; a < mp; ++a) u[a] += Bmp[a + (size_t)q * ncv] * sq;
                 }
+                const double sg = std::sqrt(std::max(theta[j], 1e-300));
+                for (int a = 0; a < mp; ++a) U[a + (size_t)j * mp] = u[a] / sg;
             }
             ST(s.rotate(s.Yb, mp, U.data(), mp, l, s.rot.p, n));
             ST(copy_block(h, s.rot.p, s.ld, s.Yb.p, s.ld, n, l));
