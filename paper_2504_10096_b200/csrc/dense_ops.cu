@@ -68,7 +68,7 @@ bse_status_t gemm_basis(bse_handle_s *h, const void *A, int64_t lda, int m, bool
 {
     if (l <= 0) return BSE_OK;
     if (l <= 8)
-        return launch_gemm<2, 1, 8, 1>(h, (const double *)A, 2 * lda, 2 * n, m, cplx, coef, ldo, l, (double *)C,
+        return launch_gemm<4, 1, 8, 1>(h, (const double *)A, 2 * lda, 2 * n, m, cplx, coef, ldo, l, (double *)C,
                                        2 * ldc, alpha, beta);
     if (l <= 32)
         return launch_gemm<2, 2, 4, 2>(h, (const double *)A, 2 * lda, 2 * n, m, cplx, coef, ldo, l, (double *)C,

@@ -1,7 +1,8 @@
 // C~ = alpha * op(A) * Bm + beta * C~   on the FP64 tensor cores.
 //   A~  : real view (2n x m, leading dimension lda2) of a complex n x m block of basis vectors
 //   op(A) = A~                      (K = m,  real coefficients: full mode)
-//         = [A~ | (iA)~]            (K = 2m, complex coefficients: rows 0..m-1 of Bm = Re(S), rows m..2m-1 = Im(S))
+//         = [A~ | (iA)~]            (K = 2m, complex coefficients: rows 0..m-1 of Bm = Re(S), rows m..2m-1 = Im(S); every
+//                                    chunk of A is brought to shared memory once and used with both halves of Bm)
 //   Bm  : real K x l, column-major (ldb);   C~ : real view 2n x l (ldc2).
 // Used for the Gram-Schmidt update W -= V h (skinny: l = k), the Ritz rotation V <- V S and the eigenvector
 // assembly.  Shared-memory tiled (cp.async double buffering), mma.sync m8n8k4 f64 -> DMMA.8x8x4.
@@ -28,10 +29,11 @@ constexpr int GEMM_KC = 16;
 
 template <int MT, int NT, int WM, int WN>
 struct GemmCfg {
+    static constexpr int NS = 2;   // shared-memory stages: the skinny (HBM-bound) shape keeps 4 chunks in flight
     static constexpr int BM = 8 * MT * WM, BN = 8 * NT * WN, THREADS = 32 * WM * WN;
     static constexpr int LDA_S = BM + 8;          // == 8 (mod 16) doubles: conflict-free A fragments
     static constexpr int LDB_S = GEMM_KC + 4;     // == 4 (mod 16) doubles: conflict-free B fragments
-    static constexpr int SMEM = 2 * (GEMM_KC * LDA_S + BN * LDB_S) * 8;
+    static constexpr int SMEM = NS * (GEMM_KC * LDA_S + 2 * BN * LDB_S) * 8;     // B tile for Re(S) and Im(S)
 };
 
 template <int MT, int NT, int WM, int WN>
@@ -41,10 +43,10 @@ __global__ void __launch_bounds__(32 * WM * WN) gemm_nn_kernel(const double *__r
                                                                int64_t ldc2, double alpha, double beta)
 {
     using Cfg = GemmCfg<MT, NT, WM, WN>;
-    constexpr int BM = Cfg::BM, BN = Cfg::BN, KC = GEMM_KC, LDA_S = Cfg::LDA_S, LDB_S = Cfg::LDB_S;
+    constexpr int BM = Cfg::BM, BN = Cfg::BN, KC = GEMM_KC, LDA_S = Cfg::LDA_S, LDB_S = Cfg::LDB_S, NS = Cfg::NS;
     extern __shared__ __align__(16) double gsm[];
-    double *As = gsm;                                  // [2][KC][LDA_S]
-    double *Bs = gsm + 2 * KC * LDA_S;                 // [2][BN][LDB_S]
+    double *As = gsm;                                  // [NS][KC][LDA_S]
+    double *Bs = gsm + NS * KC * LDA_S;                // [NS][2][BN][LDB_S]: buffer, half (Re S / Im S)
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int g = lane >> 2, t = lane & 3;
@@ -52,24 +54,25 @@ __global__ void __launch_bounds__(32 * WM * WN) gemm_nn_kernel(const double *__r
     const int64_t row0 = (int64_t)blockIdx.x * BM;
     const int col0 = blockIdx.y * BN;
     const int nch = (m + KC - 1) / KC;
-    const int total = cplx ? 2 * nch : nch;
+    const int total = nch;                              // every chunk of A is loaded ONCE and used with Re(S) and with Im(S)
+    const int nhalf = cplx ? 2 : 1;
 
     auto load_chunk = [&](int c, int buf) {
-        const int half = c >= nch ? 1 : 0;
-        const int kk0 = (c - half * nch) * KC;
+        const int kk0 = c * KC;
         double *as = As + buf * KC * LDA_S;
-        double *bs = Bs + buf * BN * LDB_S;
+        double *bs = Bs + buf * 2 * BN * LDB_S;
         for (int idx = tid; idx < KC * (BM / 2); idx += Cfg::THREADS) {
             int kk = idx / (BM / 2), r2 = idx % (BM / 2);
             bool ok = (kk0 + kk) < m && (row0 + 2 * r2) < nr;
             const double *src = ok ? A + (int64_t)(kk0 + kk) * lda2 + row0 + 2 * r2 : A;
             cp_async16(as + kk * LDA_S + 2 * r2, src, ok);
         }
-        for (int idx = tid; idx < BN * KC; idx += Cfg::THREADS) {
-            int col = idx / KC, kk = idx % KC;
+        for (int idx = tid; idx < nhalf * BN * KC; idx += Cfg::THREADS) {
+            int half = idx / (BN * KC), rem = idx % (BN * KC);
+            int col = rem / KC, kk = rem % KC;
             bool ok = (kk0 + kk) < m && (col0 + col) < l;
             const double *src = ok ? Bm + (int64_t)half * m + kk0 + kk + (int64_t)(col0 + col) * ldb : Bm;
-            cp_async8(bs + col * LDB_S + kk, src, ok);
+            cp_async8(bs + half * BN * LDB_S + col * LDB_S + kk, src, ok);
         }
     };
 
@@ -79,33 +82,45 @@ __global__ void __launch_bounds__(32 * WM * WN) gemm_nn_kernel(const double *__r
 #pragma unroll
         for (int j = 0; j < NT; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-    load_chunk(0, 0);
-    cp_async_commit();
-    for (int c = 0; c < total; ++c) {
-        const int buf = c & 1;
-        if (c + 1 < total) load_chunk(c + 1, buf ^ 1);
+#pragma unroll
+    for (int c = 0; c < NS - 1; ++c) {
+        if (c < total) load_chunk(c, c);
         cp_async_commit();
-        cp_async_wait<1>();
+    }
+    for (int c = 0; c < total; ++c) {
+        const int buf = c % NS;
+        if (c + NS - 1 < total) load_chunk(c + NS - 1, (c + NS - 1) % NS);
+        cp_async_commit();
+        cp_async_wait<NS - 1>();
         __syncthreads();
-        const bool rot = c >= nch;
         const double *as = As + buf * KC * LDA_S + wm * 8 * MT;
-        const double *bs = Bs + buf * BN * LDB_S + (wn * 8 * NT) * LDB_S;
+        const double *bs = Bs + buf * 2 * BN * LDB_S + (wn * 8 * NT) * LDB_S;
 #pragma unroll
         for (int ks = 0; ks < KC / 4; ++ks) {
             const int kk = 4 * ks + t;
             double a[MT], b[NT];
 #pragma unroll
-            for (int i = 0; i < MT; ++i) {
-                int r = 8 * i + g;
-                if (!rot) a[i] = as[kk * LDA_S + r];
-                else { double v = as[kk * LDA_S + (r ^ 1)]; a[i] = (r & 1) ? v : -v; }
-            }
+            for (int i = 0; i < MT; ++i) a[i] = as[kk * LDA_S + 8 * i + g];
 #pragma unroll
             for (int j = 0; j < NT; ++j) b[j] = bs[(8 * j + g) * LDB_S + kk];
 #pragma unroll
             for (int i = 0; i < MT; ++i)
 #pragma unroll
                 for (int j = 0; j < NT; ++j) dmma(acc[i][j], a[i], b[j]);
+            if (cplx) {                                  // (iA)~ Im(S): rows (2i, 2i+1) of (iA)~ are (-a_i, a_r)
+#pragma unroll
+                for (int i = 0; i < MT; ++i) {
+                    const int r = 8 * i + g;
+                    const double v = as[kk * LDA_S + (r ^ 1)];
+                    a[i] = (r & 1) ? v : -v;
+                }
+#pragma unroll
+                for (int j = 0; j < NT; ++j) b[j] = bs[BN * LDB_S + (8 * j + g) * LDB_S + kk];
+#pragma unroll
+                for (int i = 0; i < MT; ++i)
+#pragma unroll
+                    for (int j = 0; j < NT; ++j) dmma(acc[i][j], a[i], b[j]);
+            }
         }
         __syncthreads();
     }
