@@ -232,6 +232,15 @@ def test_config3_full_size_half_apply_sampled_rows(orc):
         for sign in (+1, -1):
             Y = to_host(h.apply_half(to_dev(X[:, :k]), sign))
             assert relerr(Y[rows], (RX + sign * CX)[:, :k]) <= TOL_APPLY, (k, sign)
+    # the general apply [Y1; Y2] = H [X1; X2] at the same size (two tile passes with 2k operand columns):
+    # rows of the upper half  R X1 + C X2  and of the lower half  -conj(C) X1 - conj(R) X2  from the same generator rows
+    X2 = gen.block_X(2 * N, 4, 15)
+    Rrows, Crows = gen.rows_R(N, 1, rows, cfg["sigma"], cfg["group"]), gen.rows_C(N, 1, rows)
+    up = orc.rows_times_block(np.hstack([Rrows, Crows]), X2)
+    lo = orc.rows_times_block(np.hstack([-Crows.conj(), -Rrows.conj()]), X2)
+    for k in (1, 3, 4):
+        Y = to_host(h.apply(to_dev(X2[:, :k])))
+        assert relerr(Y[rows], up[:, :k]) <= TOL_APPLY and relerr(Y[N + rows], lo[:, :k]) <= TOL_APPLY, ("general", k)
     # the same stores rewritten as S = R + C, D = R - C (real form of Eq. 3): same operator
     del h
     b.bse_to_real_form(rt, ct, N)
@@ -240,6 +249,9 @@ def test_config3_full_size_half_apply_sampled_rows(orc):
         for sign in (+1, -1):
             Y = to_host(hr.apply_half(to_dev(X[:, :k]), sign))
             assert relerr(Y[rows], (RX + sign * CX)[:, :k]) <= TOL_APPLY, ("real form", k, sign)
+    for k in (1, 4):
+        Y = to_host(hr.apply(to_dev(X2[:, :k])))
+        assert relerr(Y[rows], up[:, :k]) <= TOL_APPLY and relerr(Y[N + rows], lo[:, :k]) <= TOL_APPLY, ("general, real form", k)
 
 
 @pytest.mark.parametrize("N", [1, 2, 63, 65, 127])
