@@ -395,8 +395,11 @@ def run_cuda(args, cfg):
     # ---- CPU baseline: the oracle on this box's host cores, bounded sample
     if not args.no_cpu_baseline:
         sec, threads = cpu_oracle_sample(N, k, cfg["group"], 1, args.ref_rows, 3)
+        # the verification oracle as it stands (dense row-major triple loop, x87 long-double accumulation, no SIMD, no use of
+        # the Hermitian structure): a reported baseline, NOT a performance baseline -- a tuned CPU code would be far faster
         line["cpu_baseline"] = {"value": alg_bytes(N, k) * (args.ref_rows / N) / sec / 1e9, "unit": UNIT,
                                 "cores": threads, "kind": "oracle",
+                                "note": "verification oracle (long-double triple loop), not a tuned CPU implementation",
                                 "sample": f"{args.ref_rows} of {N} rows of Y = R X (k={k}), 3 repetitions"}
     print(json.dumps(line))
 

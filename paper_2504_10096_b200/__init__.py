@@ -227,6 +227,23 @@ class Bse:
                                           _stream_ptr()), "bse_create_shard")
         self._h = h
 
+    # Every call of this handle enqueues on the stream captured at creation.  If the caller's current stream is another
+    # one, order the two: the handle's stream first waits for the work already queued on the caller's stream (the producer
+    # of X, the allocation of Y), and afterwards the caller's stream waits for the handle's.
+    def _enter(self, *tensors):
+        import torch
+        cur = torch.cuda.current_stream()
+        if cur != self._stream:
+            self._stream.wait_stream(cur)
+            for t in tensors:
+                if t is not None:
+                    t.record_stream(self._stream)        # the caching allocator must not recycle it while the handle's stream uses it
+        return cur
+
+    def _exit(self, cur):
+        if cur != self._stream:
+            cur.wait_stream(self._stream)
+
     def close(self):
         if getattr(self, "_h", None):
             lib().bse_destroy(self._h)
@@ -243,14 +260,18 @@ class Bse:
         import torch
         k = X.shape[0] if X.dim() == 2 else 1
         Y = torch.empty_like(X) if Y is None else Y
+        cur = self._enter(X, Y)
         _check(lib().bse_apply(self._h, X.data_ptr(), _ld(X), Y.data_ptr(), _ld(Y), k), "bse_apply")
+        self._exit(cur)
         return Y
 
     def apply_half(self, X, sign: int, Y=None):
         import torch
         k = X.shape[0] if X.dim() == 2 else 1
         Y = torch.empty_like(X) if Y is None else Y
+        cur = self._enter(X, Y)
         _check(lib().bse_apply_half(self._h, sign, X.data_ptr(), _ld(X), Y.data_ptr(), _ld(Y), k), "bse_apply_half")
+        self._exit(cur)
         return Y
 
     def apply_host(self, X_np, Y_np=None):
@@ -332,10 +353,12 @@ class Bse:
         omega = np.zeros(nev)
         resid = np.zeros(nev)
         vec = torch.zeros((nev, self.n_op), dtype=torch.complex128, device="cuda")
+        cur = self._enter(vec)
         info = _Info()
         st = lib().bse_solve_variant(self._h, variant, nev, k, ncv, tol, max_restarts, seed,
                              omega.ctypes.data_as(ctypes.POINTER(_dbl)), vec.data_ptr(), self.n_op,
                              resid.ctypes.data_as(ctypes.POINTER(_dbl)), ctypes.byref(info))
+        self._exit(cur)
         if st != 0 and raise_on_error:
             raise BseError(st, "bse_solve")
         return SolveResult(omega, vec, resid, {f: getattr(info, f) for f, _ in _Info._fields_}, st)
@@ -356,7 +379,8 @@ class ShardedBse:
     (the paper partitions the matrix by rows over MPI ranks).  Rank r holds the slice of
     the packed store that bse_shard_layout assigns to it (contiguous tile rows, equal tile counts); X is replicated;
     apply / apply_half run the local kernels on the slice and sum the partial Y with ONE all-reduce of 16 N k bytes.
-    Apply-level only: the solver calls need the whole operator on one GPU."""
+    After install_comm() the library itself completes every product through the process group, and solve() /
+    lanczos_quadrature() run on the sharded operator with replicated vectors, all ranks in bitwise lock step."""
 
     def __init__(self, mode: int, N: int, r_slice, c_slice=None, rows=None, storage: int = STORE_C128, group=None):
         self.local = Bse(mode, N, r_slice, c_slice, storage=storage, rows=rows)
