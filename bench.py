@@ -408,7 +408,7 @@ def run_solve(spec):
     """`--solve CFG:K[:NCV[:STORE]]` -- time-to-nev of one bse_solve alone (the second half of BASELINE.json's metric), on
     the device-generated synthetic operator of BASELINE.json config CFG (2, 3 or 4; or MODE@N@NEV), block size K, basis size NCV (0 =
     default), STORE in {c128, c64, real, real64} (real*: the real-form store of DESIGN.md 5.5, full mode only).  Prints
-    one JSON line; profiles/r1_solve.md's rows are runs of this command."""
+    one JSON line; profiles/r2_solve.md's rows are runs of this command."""
     import torch
     import paper_2504_10096_b200 as b
     parts = spec.split(":")
