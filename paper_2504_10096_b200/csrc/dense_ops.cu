@@ -14,8 +14,11 @@ bse_status_t gram_basis(bse_handle_s *h, const void *A, int64_t lda, int m, cons
     const int ldo = cplx ? 2 * m : m;
     BSE_CUDA(cudaMemsetAsync(out, 0, sizeof(double) * (size_t)ldo * k, h->stream));
     const int gx = (m + 63) / 64;
-    int ctas_per_sm = 4;
-    if (const char *e = getenv("BSE_GRAM_CTAS")) { int v = atoi(e); if (v >= 1 && v <= 16) ctas_per_sm = v; }
+    static const int ctas_per_sm = [] {                  // BSE_GRAM_CTAS: read once per process
+        int v = 4;
+        if (const char *e = getenv("BSE_GRAM_CTAS")) { int u = atoi(e); if (u >= 1 && u <= 16) v = u; }
+        return v;
+    }();
     int64_t want = ((int64_t)ctas_per_sm * h->num_sms + gx - 1) / gx;             // row chunks so that ~ctas_per_sm CTAs per SM exist
     int64_t rows = (nr + want - 1) / want;
     rows = ((rows + 63) / 64) * 64;
