@@ -18,8 +18,8 @@
  *     (in complex elements);  sizes are int64_t / int32_t;
  *   - all device work is enqueued on the `stream` given to bse_create (a cudaStream_t passed as
  *     void*; NULL = the legacy default stream).  bse_apply / bse_apply_half / bse_gram / bse_update are
- *     asynchronous with respect to the host; bse_orth synchronises the stream several times per call (k x k host
- *     factorisations, rank decisions); bse_solve, bse_lanczos_quadrature and the *_host calls are synchronous;
+ *     asynchronous with respect to the host; bse_orth synchronises the stream once (it returns the rank on the host; the
+ *     k x k factorisations run on the device); bse_solve, bse_lanczos_quadrature and the *_host calls are synchronous;
  *   - bse_apply / bse_apply_half only enqueue kernel launches (and a memset for single columns) into a workspace sized at
  *     bse_create: they allocate nothing, read no environment variable (BSE_APPLY_UNIT, BSE_APPLY_K1 are read once, at
  *     bse_create) and can be captured in a CUDA graph on the handle's stream and replayed, for any mode, store and k

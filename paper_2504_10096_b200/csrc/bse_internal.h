@@ -106,13 +106,18 @@ bse_status_t orth_block(bse_handle_s *h, const void *V, int64_t ldv, int m, cons
                         uint64_t seed, uint64_t *rng_counter);
 
 bse_status_t orth_reserve(bse_handle_s *h, int m_max, int k);
-// the two halves of orth_block, for callers that recompute P(W) between projection and normalisation
+// The pieces of orth_block, for callers that recompute P(W) between projection and normalisation.  All asynchronous on the
+// handle's stream except normalize_block, which ends with the block step's ONE host synchronisation and hands back the
+// projection coefficients h1 + h2 (hcoef_host, m x k, out), the k x k factor and the rank.  Device scalar slots of
+// block_norm_scale: ORTH_E_IN (opens a block step: clears the flags), ORTH_E_AFTER, ORTH_G; normalize_block's scale_mode 0
+// takes the incoming block's norm scale from ORTH_E_IN (same inner product), 1 from ORTH_G * ORTH_E_IN / ORTH_E_AFTER.
+enum { ORTH_E_IN = 0, ORTH_E_AFTER = 1, ORTH_G = 2 };
 bse_status_t project_block(bse_handle_s *h, const void *V, int64_t ldv, int m, const void *PV, int64_t ldpv, void *W,
-                           int64_t ldw, int k, void *PW, int64_t ldpw, bool cplx, void *hcoef_host);
+                           int64_t ldw, int k, void *PW, int64_t ldpw, bool cplx);
 bse_status_t block_norm_scale(bse_handle_s *h, const void *W, int64_t ldw, const void *PW, int64_t ldpw, int k,
-                              bool cplx, double *scale2);
+                              bool cplx, int slot);
 bse_status_t normalize_block(bse_handle_s *h, const void *V, int64_t ldv, int m, const void *PV, int64_t ldpv, void *W,
-                             int64_t ldw, int k, void *PW, int64_t ldpw, bool cplx, double scale2, void *hcoef_host,
+                             int64_t ldw, int k, void *PW, int64_t ldpw, bool cplx, int scale_mode, void *hcoef_host,
                              void *bfac_host, int *rank_out, uint64_t seed, uint64_t *rng_counter, int image_sign = +1);
 // (image_sign: which half apply gives the image PW of a replacement column in the real inner product: +1 P, -1 M)
 

@@ -58,7 +58,11 @@ struct Solver {
     uint64_t seed, rng = 0;
     bse_info_t info{};
     double normest = 0.0;
-    double seconds_apply_in_orth = 0.0;   // full mode: the P(W) apply issued between projection and normalisation
+    // device-side timing of the applies (no host synchronisation for the clock): ev[0..1] around the block apply, ev[2..3]
+    // around the P(W) apply issued between projection and normalisation in full mode
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    bool timed_second_apply = false;
+    ~Solver() { for (auto &e : ev) if (e) cudaEventDestroy(e); }
 
     // || <V, V> - I ||_F over the first mtot basis columns in the active inner product (reading S10)
     bse_status_t basis_orth_error(int mtot, double *err)
@@ -213,18 +217,16 @@ struct Solver {
             // sign in the Omega inner product, <y_i, z>_M = Re(M(y_i)^H z) -- image recomputed after the projection (reading R3)
             const int my = c0;                                                                   // Y columns so far
             std::vector<zc> Hc1((size_t)std::max(my, 1) * k, zc(0.0));
-            double e_in = 0.0, e_after = 0.0, g_after = 0.0;
             int rank = 0;
             ST(copy_block(h, col(PV, c0), ld, col(Yb, my), ld, n, k));
-            ST(block_norm_scale(h, col(Yb, my), ld, nullptr, ld, k, false, &e_in));
-            ST(project_block(h, Yb.p, ld, my, MYb.p, ld, col(Yb, my), ld, k, nullptr, ld, false, Hc1.data()));
+            ST(block_norm_scale(h, col(Yb, my), ld, nullptr, ld, k, false, ORTH_E_IN));
+            ST(project_block(h, Yb.p, ld, my, MYb.p, ld, col(Yb, my), ld, k, nullptr, ld, false));
             bse_status_t st = bse_apply_half(h, -1, col(Yb, my), ld, col(MYb, my), ld, k);     // M(z)
             if (st) return st;
-            ST(block_norm_scale(h, col(Yb, my), ld, nullptr, ld, k, false, &e_after));
-            ST(block_norm_scale(h, col(Yb, my), ld, col(MYb, my), ld, k, false, &g_after));
-            const double scale2 = (e_after > 0.0) ? g_after * (e_in / e_after) : g_after;
+            ST(block_norm_scale(h, col(Yb, my), ld, nullptr, ld, k, false, ORTH_E_AFTER));
+            ST(block_norm_scale(h, col(Yb, my), ld, col(MYb, my), ld, k, false, ORTH_G));
             B1.assign((size_t)k * k, zc(0.0));
-            ST(normalize_block(h, Yb.p, ld, my, MYb.p, ld, col(Yb, my), ld, k, col(MYb, my), ld, false, scale2, Hc1.data(),
+            ST(normalize_block(h, Yb.p, ld, my, MYb.p, ld, col(Yb, my), ld, k, col(MYb, my), ld, false, 1, Hc1.data(),
                                B1.data(), &rank, seed, &rng, -1));
             for (int c = 0; c < k; ++c) {                                                        // P(X_j) = Y[:, :my] Hc1 + Y_j B1
                 for (int a = 0; a < my; ++a) Bm[a + (size_t)(c0 + c) * ncv] = Hc1[a + (size_t)c * my].real();
@@ -246,20 +248,18 @@ struct Solver {
     {
         if (!full)
             return orth_block(h, V.p, ld, m, nullptr, ld, col(V, m), ld, k, nullptr, ld, Hc, B, rank, seed, &rng);
-        double e_in = 0.0, e_after = 0.0, g_after = 0.0;
-        ST(block_norm_scale(h, col(V, m), ld, nullptr, ld, k, false, &e_in));
-        ST(project_block(h, V.p, ld, m, PV.p, ld, col(V, m), ld, k, nullptr, ld, false, Hc));
-        const double ta = now_s();                                                                 // (project_block ends synchronised)
+        // the P-norm scale of the incoming block is estimated through Euclidean norms (device scalars, no host round trip)
+        ST(block_norm_scale(h, col(V, m), ld, nullptr, ld, k, false, ORTH_E_IN));
+        ST(project_block(h, V.p, ld, m, PV.p, ld, col(V, m), ld, k, nullptr, ld, false));
+        BSE_CUDA(cudaEventRecord(ev[2], h->stream));
         bse_status_t st = bse_apply_half(h, +1, col(V, m), ld, col(PV, m), ld, k);                // PW = P(W)
         if (st) return st;
-        BSE_CUDA(cudaStreamSynchronize(h->stream));
-        seconds_apply_in_orth += now_s() - ta;
+        BSE_CUDA(cudaEventRecord(ev[3], h->stream));
+        timed_second_apply = true;
         info.n_apply += 1;
-        ST(block_norm_scale(h, col(V, m), ld, nullptr, ld, k, false, &e_after));
-        ST(block_norm_scale(h, col(V, m), ld, col(PV, m), ld, k, false, &g_after));
-        // scale of the incoming block in the P-norm, estimated through the Euclidean norms
-        double scale2 = (e_after > 0.0) ? g_after * (e_in / e_after) : g_after;
-        return normalize_block(h, V.p, ld, m, PV.p, ld, col(V, m), ld, k, col(PV, m), ld, false, scale2, Hc, B, rank,
+        ST(block_norm_scale(h, col(V, m), ld, nullptr, ld, k, false, ORTH_E_AFTER));
+        ST(block_norm_scale(h, col(V, m), ld, col(PV, m), ld, k, false, ORTH_G));
+        return normalize_block(h, V.p, ld, m, PV.p, ld, col(V, m), ld, k, col(PV, m), ld, false, 1, Hc, B, rank,
                                seed, &rng);
     }
 };
@@ -309,6 +309,7 @@ extern "C" bse_status_t bse_solve_variant(bse_handle_t h, int32_t variant, int32
     const bool verbose = getenv("BSE_VERBOSE") != nullptr;
     s.h = h; s.n = n; s.full = full; s.nev = nev; s.k = k; s.ncv = ncv; s.tol = tol; s.ld = n; s.seed = seed;
     s.variant = variant;
+    for (auto &e : s.ev) BSE_CUDA(cudaEventCreate(&e));
     const bool gruning = variant == BSE_VARIANT_GRUNING;
     s.info.ncv = ncv;
     const size_t basis_bytes = (size_t)n * (ncv + k) * 16;
@@ -351,20 +352,25 @@ extern "C" bse_status_t bse_solve_variant(bse_handle_t h, int32_t variant, int32
     while (true) {
         // ---- one block step: apply (a2 / a3), orthogonalise (a5-a7), extend T
         double t0 = now_s();
+        BSE_CUDA(cudaEventRecord(s.ev[0], h->stream));
         ST(s.apply_block(s.mp));
-        BSE_CUDA(cudaStreamSynchronize(h->stream));
-        double t1 = now_s();
-        s.info.seconds_apply += t1 - t0;
+        BSE_CUDA(cudaEventRecord(s.ev[1], h->stream));
         const int m = s.mp + k;
         int rank = 0;
+        s.timed_second_apply = false;
         {
-            bse_status_t st_o = s.orth_new_block(m, Hc.data(), B.data(), &rank);
+            bse_status_t st_o = s.orth_new_block(m, Hc.data(), B.data(), &rank);      // ends with the step's one synchronisation
             if (verbose && st_o) fprintf(stderr, "[bse_solve] orthogonalisation failed (%d) at m = %d\n", (int)st_o, m);
             if (st_o) return st_o;
         }
-        s.info.seconds_orth += now_s() - t1 - s.seconds_apply_in_orth;
-        s.info.seconds_apply += s.seconds_apply_in_orth;
-        s.seconds_apply_in_orth = 0.0;
+        {
+            float ms_a = 0.f, ms_b = 0.f;
+            BSE_CUDA(cudaEventElapsedTime(&ms_a, s.ev[0], s.ev[1]));
+            if (s.timed_second_apply) BSE_CUDA(cudaEventElapsedTime(&ms_b, s.ev[2], s.ev[3]));
+            const double t_apply = 1e-3 * ((double)ms_a + (double)ms_b);
+            s.info.seconds_apply += t_apply;
+            s.info.seconds_orth += (now_s() - t0) - t_apply;
+        }
         for (int c = 0; c < k; ++c)
             for (int a = 0; a < m; ++a) {
                 zc v = Hc[a + (size_t)c * m];
