@@ -256,8 +256,8 @@ struct Role3M {
     template <int ES> struct P2 {
         using G = TileGeom<ES>;
         double2 z2[8][2];                                    // conj(x_I) (times the pass sign), rows 8 ib + 4 s + t, column g
+        double zs[8][2];                                     // z2r + z2i of the same rows (from the pre-pass: no FP64 add here)
         double Q1[2][2], Q2[2][2], Q3[2][2];
-        const double *zs2;                                   // z2r + z2i of the same rows, read per tile (L1 hits within a unit)
         int frag, r;
         unsigned long long eflip;                            // HERM: the result is conjugated
         __device__ __forceinline__ P2(const TileParams &p, const Lane &l, int r_)
@@ -266,13 +266,14 @@ struct Role3M {
         {
             const unsigned long long flip = p.pass == PASS_HERM ? SIGN_BIT : 0ull;          // img_pair holds x for HERM: conjugate it
             const double2 *zp = p.img_pair + ((int64_t)I * TB + l.t) * IMG_ROW + l.g;
-            zs2 = p.img_a + ((int64_t)I * TB + l.t) * IMG_ROW + l.g;
+            const double *zs2 = p.img_a + ((int64_t)I * TB + l.t) * IMG_ROW + l.g;
 #pragma unroll
             for (int ib = 0; ib < 8; ++ib)
 #pragma unroll
                 for (int s = 0; s < 2; ++s) {
                     const double2 v = __ldg(zp + (ib * 8 + 4 * s) * IMG_ROW);
                     z2[ib][s] = make_double2(v.x, neg_if(v.y, flip));
+                    zs[ib][s] = __ldg(zs2 + (ib * 8 + 4 * s) * IMG_ROW);
                 }
         }
         __device__ __forceinline__ int tile(const TileParams &, const char *stage)
@@ -283,15 +284,12 @@ struct Role3M {
 #pragma unroll
             for (int ib = 0; ib < 8; ib += 2) {
                 double2 b[2][2][2];
-                double zs[2][2];
 #pragma unroll
                 for (int q = 0; q < 2; ++q)
 #pragma unroll
-                    for (int s = 0; s < 2; ++s) {
-                        zs[q][s] = __ldg(zs2 + ((ib + q) * 8 + 4 * s) * IMG_ROW);
+                    for (int s = 0; s < 2; ++s)
 #pragma unroll
                         for (int pc = 0; pc < 2; ++pc) b[q][s][pc] = load_frag<ES>(tp + (pc * 8 + ib + q) * G::PBY + s * G::S2);
-                    }
 #pragma unroll
                 for (int q = 0; q < 2; ++q)
 #pragma unroll
@@ -301,7 +299,7 @@ struct Role3M {
                             const double bs = b[q][s][pc].x + b[q][s][pc].y;
                             dmma(Q1[pc], b[q][s][pc].x, z2[ib + q][s].x);
                             dmma(Q2[pc], b[q][s][pc].y, z2[ib + q][s].y);
-                            dmma(Q3[pc], bs, zs[q][s]);
+                            dmma(Q3[pc], bs, zs[ib + q][s]);
                         }
             }
             int live = 0;
