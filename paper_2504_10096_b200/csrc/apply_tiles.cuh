@@ -49,11 +49,6 @@ template <int ES> __device__ __forceinline__ Lane make_lane(int lane)
     l.offP2 = (((g2 << 1) | t1) * 8 + ((t0 << 2) | (g0 << 1) | (t1 ^ g1))) * ES;   // P2 reads (a = 4 s + t, b = g)
     return l;
 }
-__device__ __forceinline__ double neg_if(double v, unsigned long long mask)       // v or -v without touching the FP64 pipe
-{
-    return __longlong_as_double(__double_as_longlong(v) ^ (long long)mask);
-}
-constexpr unsigned long long SIGN_BIT = 0x8000000000000000ull;
 constexpr int IMG_ROW = 8;                                 // image entries per matrix row
 constexpr int IMG_TILE = TB * IMG_ROW;                     // image entries per tile row
 

@@ -88,6 +88,20 @@ __device__ __forceinline__ void bulk_g2s_hint(void *dst_smem, const void *src_gm
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+__device__ __forceinline__ void cp_async16(void *dst, const void *src, bool valid)
+{
+    int sz = valid ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_u32(dst)), "l"(src), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async8(void *dst, const void *src, bool valid)
+{
+    int sz = valid ? 8 : 0;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(smem_u32(dst)), "l"(src), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 __device__ __forceinline__ double2 lds128(uint32_t addr)
 {
     double2 v;
@@ -113,6 +127,12 @@ __device__ __forceinline__ void dmma(double (&c)[2], double a, double b)
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
                  : "+d"(c[0]), "+d"(c[1])
                  : "d"(a), "d"(b));
+}
+// v or -v (mask = SIGN_BIT) without touching the FP64 pipe, whose instructions share the issue port of the DMMAs
+constexpr unsigned long long SIGN_BIT = 0x8000000000000000ull;
+__device__ __forceinline__ double neg_if(double v, unsigned long long mask)
+{
+    return __longlong_as_double(__double_as_longlong(v) ^ (long long)mask);
 }
 __device__ __forceinline__ void red_add(double *p, double v) { atomicAdd(p, v); }
 

@@ -1,4 +1,6 @@
 // Launch wrappers for the dense basis kernels and a few elementwise kernels.
+#include <algorithm>
+
 #include "bse_internal.h"
 #include "dense_kernels.cuh"
 #include "gemm_kernel.cuh"
@@ -13,16 +15,24 @@ bse_status_t gram_basis(bse_handle_s *h, const void *A, int64_t lda, int m, cons
     const int64_t nr = 2 * n;
     const int ldo = cplx ? 2 * m : m;
     BSE_CUDA(cudaMemsetAsync(out, 0, sizeof(double) * (size_t)ldo * k, h->stream));
-    const int gx = (m + 63) / 64;
+    static std::atomic<uint64_t> attr_devices{0};         // per device (cudaFuncSetAttribute is)
+    int dev = 0;
+    BSE_CUDA(cudaGetDevice(&dev));
+    if (dev >= 64 || !(attr_devices.load(std::memory_order_acquire) & (1ull << dev))) {
+        BSE_CUDA(cudaFuncSetAttribute(gram_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, GRAM_SMEM));
+        BSE_CUDA(cudaFuncSetAttribute(gram_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, GRAM_SMEM));
+        if (dev < 64) attr_devices.fetch_or(1ull << dev, std::memory_order_release);
+    }
+    // one CTA per SM (the rings take the shared memory): 64-column groups x row chunks ~ BSE_GRAM_CTAS x the SM count
+    const int gx = (m + 8 * GRAM_WARPS - 1) / (8 * GRAM_WARPS);
     static const int ctas_per_sm = [] {                  // BSE_GRAM_CTAS: read once per process
-        int v = 4;
+        int v = 1;
         if (const char *e = getenv("BSE_GRAM_CTAS")) { int u = atoi(e); if (u >= 1 && u <= 16) v = u; }
         return v;
     }();
-    int64_t want = ((int64_t)ctas_per_sm * h->num_sms + gx - 1) / gx;             // row chunks so that ~ctas_per_sm CTAs per SM exist
+    const int64_t want = std::max<int64_t>(1, (int64_t)ctas_per_sm * h->num_sms / gx);
     int64_t rows = (nr + want - 1) / want;
-    rows = ((rows + 63) / 64) * 64;
-    if (rows < 256) rows = 256;
+    rows = ((rows + 31) / 32) * 32;
     const int gy = (int)((nr + rows - 1) / rows);
     // up to 8 complex / 16 real columns per launch (two N-tiles); one N-tile when it is enough
     const int step = cplx ? 8 : 16;
@@ -32,10 +42,10 @@ bse_status_t gram_basis(bse_handle_s *h, const void *A, int64_t lda, int m, cons
         const double *Bp = (const double *)B + 2 * (int64_t)c0 * ldb;
         double *op = out + (int64_t)c0 * ldo;
         if (ncols <= 8)
-            gram_kernel<1><<<dim3(gx, gy), 256, 0, h->stream>>>((const double *)A, 2 * lda, m, Bp, 2 * ldb, kc, ncols,
+            gram_kernel<1><<<dim3(gx, gy), 32 * GRAM_WARPS, GRAM_SMEM, h->stream>>>((const double *)A, 2 * lda, m, Bp, 2 * ldb, kc, ncols,
                                                                nr, rows, op, ldo, cplx ? m : 0);
         else
-            gram_kernel<2><<<dim3(gx, gy), 256, 0, h->stream>>>((const double *)A, 2 * lda, m, Bp, 2 * ldb, kc, ncols,
+            gram_kernel<2><<<dim3(gx, gy), 32 * GRAM_WARPS, GRAM_SMEM, h->stream>>>((const double *)A, 2 * lda, m, Bp, 2 * ldb, kc, ncols,
                                                                nr, rows, op, ldo, cplx ? m : 0);
         count_launch();
     }

@@ -11,20 +11,6 @@
 
 namespace bse {
 
-__device__ __forceinline__ void cp_async16(void *dst, const void *src, bool valid)
-{
-    int sz = valid ? 16 : 0;
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_u32(dst)), "l"(src), "r"(sz) : "memory");
-}
-__device__ __forceinline__ void cp_async8(void *dst, const void *src, bool valid)
-{
-    int sz = valid ? 8 : 0;
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(smem_u32(dst)), "l"(src), "r"(sz) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
-
 constexpr int GEMM_KC = 16;
 
 template <int MT, int NT, int WM, int WN>
@@ -76,6 +62,9 @@ __global__ void __launch_bounds__(32 * WM * WN) gemm_nn_kernel(const double *__r
         }
     };
 
+    // (iA)~ Im(S): rows (2i, 2i+1) of (iA)~ are (-a_i, a_r); the sign depends on the parity of the lane's row only and is
+    // flipped with an integer XOR (plain FP64 instructions share the issue port of the DMMAs)
+    const unsigned long long im_flip = (g & 1) ? 0ull : SIGN_BIT;
     double acc[MT][NT][2];
 #pragma unroll
     for (int i = 0; i < MT; ++i)
@@ -107,13 +96,9 @@ __global__ void __launch_bounds__(32 * WM * WN) gemm_nn_kernel(const double *__r
             for (int i = 0; i < MT; ++i)
 #pragma unroll
                 for (int j = 0; j < NT; ++j) dmma(acc[i][j], a[i], b[j]);
-            if (cplx) {                                  // (iA)~ Im(S): rows (2i, 2i+1) of (iA)~ are (-a_i, a_r)
+            if (cplx) {
 #pragma unroll
-                for (int i = 0; i < MT; ++i) {
-                    const int r = 8 * i + g;
-                    const double v = as[kk * LDA_S + (r ^ 1)];
-                    a[i] = (r & 1) ? v : -v;
-                }
+                for (int i = 0; i < MT; ++i) a[i] = neg_if(as[kk * LDA_S + ((8 * i + g) ^ 1)], im_flip);
 #pragma unroll
                 for (int j = 0; j < NT; ++j) b[j] = bs[BN * LDB_S + (8 * j + g) * LDB_S + kk];
 #pragma unroll
