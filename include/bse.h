@@ -321,6 +321,26 @@ bse_status_t bse_host_syev(int32_t m, double *hA, int32_t lda, double *hW, doubl
 bse_status_t bse_lanczos_quadrature_static(bse_handle_t h, const void *dStart, int32_t steps, double *hAlpha,
                                            double *hBeta, int32_t *hDone);
 
+/* The diagonalisation scheme of PAPER.md section 2.1 (Eq. 2-4) on the device, for full-mode handles (any
+ * store): M_r of Eq. (3) from the packed tiles -> real Cholesky M_r = L L^T -> W = L^T J L (real skew-symmetric) -> Householder
+ * tridiagonalisation of W in real arithmetic -> the Hermitian tridiagonal -iT (zero diagonal) solved on the host through its
+ * N x N bidiagonal factor -> back-transformation [X; Y] = Q L^-T z.  "If eigenvectors for more than 5% of the spectrum are
+ * required, direct diagonalization routines are recommended": nev may be anything up to N (the whole positive
+ * spectrum).  O(N^3) work and three real 2N x 2N matrices of device memory, allocated and freed inside the call.
+ *   hOmega  : nev doubles (host): the nev smallest positive omega, ascending;
+ *   dVec    : 2N x nev complex128 (device, column-major, ldvec >= 2N): right eigenvectors [X_I; Y_I] with
+ *             X^H X - Y^H Y = 1; NULL: eigenvalues only (the back-transformation is skipped);
+ *   hSeconds: 6 doubles (host, nullable): Cholesky (with M_r), W, tridiagonalisation, host tridiagonal solve,
+ *             back-transformation, total.
+ * Synchronous.  Errors: BSE_ERR_NOT_POSITIVE_DEFINITE (a Cholesky pivot <= 0: the precondition of PAPER.md:49 fails),
+ * BSE_ERR_INVALID_ARG (TDA or partial handle, nev < 1, nev > N, 2N > BSE_DIRECT_MAX_N), BSE_ERR_ALLOC, BSE_ERR_CUDA. */
+#define BSE_DIRECT_MAX_N 24576
+bse_status_t bse_solve_direct(bse_handle_t h, int32_t nev, double *hOmega, void *dVec, int64_t ldvec, double *hSeconds);
+
+/* Real symmetric tridiagonal eigenproblem on the host (hD: m diagonal, hE: m - 1 sub-diagonal entries; both untouched): all
+ * eigenvalues ascending in hW, eigenvectors of the nz lowest in hZ (m x nz, ldz).  The last stage of bse_solve_direct. */
+bse_status_t bse_host_stev(int32_t m, const double *hD, const double *hE, double *hW, double *hZ, int32_t ldz, int32_t nz);
+
 /* The eigenvectors that "can be obtained trivially" from the right eigenvectors v_I = [X_I; Y_I] of the positive omega_I that
  * bse_solve returns (full mode, dVec / dOut 2N x nev column-major, must not alias):
  *   which = BSE_PARTNER_RIGHT_NEGATIVE : right eigenvectors of -omega_I,  [conj(Y_I); conj(X_I)]

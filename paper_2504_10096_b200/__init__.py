@@ -24,6 +24,7 @@ TILE_BYTES = 65536
 STATUS = {0: "BSE_OK", 1: "BSE_ERR_INVALID_ARG", 2: "BSE_ERR_CUDA", 3: "BSE_ERR_ALLOC", 4: "BSE_ERR_NOT_CONVERGED",
           5: "BSE_ERR_NOT_POSITIVE_DEFINITE", 6: "BSE_ERR_INTERNAL", 7: "BSE_ERR_STATIC_LIMIT"}
 STATIC_QUADRATURE_MAX_N, STATIC_QUADRATURE_MAX_STEPS = 32768, 1024       # include/bse.h
+DIRECT_MAX_N = 24576                                                         # bse_solve_direct: 2N at most
 
 
 class BseError(RuntimeError):
@@ -74,6 +75,8 @@ _SIGNATURES = {
     "bse_solve_variant": [_vp, _i32, _i32, _i32, _i32, _dbl, _i32, _u64, ctypes.POINTER(_dbl), _vp, _i64, ctypes.POINTER(_dbl),
                           ctypes.POINTER(_Info)],
     "bse_selftest_peak": [_i32, _i32, _i32, _vp, _i64, _vp, ctypes.POINTER(_dbl), ctypes.POINTER(_dbl)],
+    "bse_solve_direct": [_vp, _i32, ctypes.POINTER(_dbl), _vp, _i64, ctypes.POINTER(_dbl)],
+    "bse_host_stev": [_i32, _vp, _vp, _vp, _vp, _i32, _i32],
 }
 EXPORTS = sorted(list(_SIGNATURES) + ["bse_status_string", "bse_launch_count"])
 
@@ -364,6 +367,22 @@ class Bse:
         return SolveResult(omega, vec, resid, {f: getattr(info, f) for f, _ in _Info._fields_}, st)
 
 
+    def solve_direct(self, nev: int, vectors: bool = True):
+        """The diagonalisation scheme of PAPER.md section 2.1 on the device (full mode): (omega, vec or None, seconds) with
+        seconds = dict(cholesky, w, tridiag, host_eig, back, total)."""
+        import numpy as np
+        import torch
+        omega = np.zeros(nev)
+        sec = np.zeros(6)
+        vec = torch.zeros((nev, self.n_op), dtype=torch.complex128, device="cuda") if vectors else None
+        cur = self._enter(vec) if vectors else self._enter()
+        st = lib().bse_solve_direct(self._h, nev, omega.ctypes.data_as(ctypes.POINTER(_dbl)),
+                                    vec.data_ptr() if vectors else None, self.n_op, sec.ctypes.data_as(ctypes.POINTER(_dbl)))
+        self._exit(cur)
+        _check(st, "bse_solve_direct")
+        return omega, vec, dict(zip(("cholesky", "w", "tridiag", "host_eig", "back", "total"), sec.tolist()))
+
+
 def sum_partials(Y, group=None):
     """Sum the shards' partial products in place over the process group (one all-reduce of 16 N k bytes; NCCL over
     NVLink on GPUs).  A no-op without an initialised process group or with a single rank."""
@@ -481,6 +500,19 @@ def host_syev(A, nz=None):
     w = np.zeros(m)
     Z = np.zeros((m, max(nz, 1)), dtype=np.float64, order="F")
     _check(lib().bse_host_syev(m, a.ctypes.data, m, w.ctypes.data, Z.ctypes.data, m, nz), "bse_host_syev")
+    return w, Z[:, :nz]
+
+
+def host_stev(d, e, nz=None):
+    """Host utility: eigenvalues (ascending) and first nz eigenvectors of the real symmetric tridiagonal (d, e)."""
+    import numpy as np
+    m = len(d)
+    nz = m if nz is None else nz
+    d = np.ascontiguousarray(d, dtype=np.float64); e = np.ascontiguousarray(e, dtype=np.float64)
+    w = np.zeros(m)
+    Z = np.zeros((m, max(nz, 1)), dtype=np.float64, order="F")
+    _check(lib().bse_host_stev(m, d.ctypes.data, e.ctypes.data if m > 1 else None, w.ctypes.data, Z.ctypes.data, m, nz),
+           "bse_host_stev")
     return w, Z[:, :nz]
 
 

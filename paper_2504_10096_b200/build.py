@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libbse_b200.so")
-SOURCES = ["bse_api.cu", "bse_apply.cu", "dense_ops.cu", "bse_orth.cu", "bse_solve.cu", "bse_quadrature.cu", "bse_selftest.cu"]
+SOURCES = ["bse_api.cu", "bse_apply.cu", "dense_ops.cu", "bse_orth.cu", "bse_solve.cu", "bse_quadrature.cu", "bse_selftest.cu", "bse_direct.cu"]
 HOST_SOURCES = ["host_eig.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "-Xcompiler", "-fopenmp", "-Xptxas", "-v"]

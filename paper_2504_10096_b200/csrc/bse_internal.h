@@ -125,5 +125,7 @@ bse_status_t normalize_block(bse_handle_s *h, const void *V, int64_t ldv, int m,
 int host_heev(int m, void *A, int lda, double *w, void *Z, int ldz, int nz);
 // real symmetric variant (full mode's projected matrix): A, Z real
 int host_syev(int m, double *A, int lda, double *w, double *Z, int ldz, int nz);
+// real symmetric tridiagonal (d, e): all eigenvalues ascending, eigenvectors of the nz lowest
+int host_stev(int m, double *d, double *e, double *w, double *Z, int ldz, int nz);
 
 }  // namespace bse

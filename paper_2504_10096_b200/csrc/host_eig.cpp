@@ -414,4 +414,26 @@ int host_syev(int m, double *A, int lda, double *w, double *Z, int ldz, int nz)
     return fail;
 }
 
+// Real symmetric tridiagonal (d: m diagonal entries, e: m - 1 sub-diagonal entries, both destroyed): all eigenvalues
+// ascending in w and the eigenvectors of the nz lowest in Z (m x nz, column-major, ldz).  The last stage of the direct
+// route (bse_direct.cu).  Returns 0, or >0 if QL failed.
+int host_stev(int m, double *d_in, double *e_in, double *w, double *Z, int ldz, int nz)
+{
+    if (m <= 0) return 0;
+    if (nz > m) nz = m;
+    std::vector<double> d(d_in, d_in + m), e(m, 0.0);
+    for (int i = 0; i + 1 < m; ++i) e[i] = e_in[i];
+    std::vector<double> Zb;
+    std::vector<int> ord;
+    const int fail = tridiag_ql(m, d, e, Zb, ord, w);
+    if (nz <= 0 || !Z) return fail;
+#pragma omp parallel for schedule(static) if ((int64_t)m * nz > 65536)
+    for (int j = 0; j < nz; ++j) {
+        const int src = ord[j];
+        double *z = Z + (int64_t)j * ldz;
+        for (int i = 0; i < m; ++i) z[i] = Zb[((size_t)(i / RP) * m + src) * RP + i % RP];
+    }
+    return fail;
+}
+
 }  // namespace bse

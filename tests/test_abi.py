@@ -130,3 +130,23 @@ def test_quadrature_resolvent_host_utility_matches_oracle(b, orc):
     T = np.diag(rng_a) + np.diag(beta[1:m], 1) + np.diag(beta[1:m], -1)
     direct = np.array([beta[0] ** 2 * np.linalg.inv((w + 0.07j) * np.eye(m) - T)[0, 0] for w in om])
     assert np.max(np.abs(G - direct)) < 1e-11 * np.max(np.abs(direct))
+
+
+def test_host_stev_vs_scipy():
+    """bse_host_stev (last stage of bse_solve_direct): real symmetric tridiagonal, all eigenvalues + the lowest vectors."""
+    import paper_2504_10096_b200 as b
+    from scipy.linalg import eigh_tridiagonal
+    rng = np.random.default_rng(5)
+    for m, nz in [(1, 1), (2, 2), (37, 5), (300, 300), (513, 40)]:
+        d = rng.standard_normal(m) * 3
+        e = rng.standard_normal(max(m - 1, 0))
+        w, Z = b.host_stev(d, e, nz)
+        T = np.diag(d) + np.diag(e, 1) + np.diag(e, -1)
+        wr = eigh_tridiagonal(d, e, eigvals_only=True) if m > 1 else d.copy()
+        assert np.max(np.abs(w - wr)) <= 1e-13 * max(1.0, np.max(np.abs(wr)))
+        assert np.linalg.norm(T @ Z - Z * w[:nz]) <= 1e-12 * np.linalg.norm(T) * np.sqrt(nz)
+        assert np.linalg.norm(Z.T @ Z - np.eye(nz)) <= 1e-12 * np.sqrt(nz)
+    # zero diagonal (the direct route's matrix): eigenvalues in +- pairs
+    e = rng.standard_normal(63)
+    w, _ = b.host_stev(np.zeros(64), e, 0)
+    assert np.max(np.abs(w + w[::-1])) <= 1e-13 * np.max(np.abs(w))
