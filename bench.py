@@ -447,6 +447,45 @@ def run_solve(spec):
                                 "max_residual_estimate": float(res.resid.max())}}))
 
 
+def run_direct(spec):
+    """`--direct N[:NEV[:STORE]]` -- bse_solve_direct (the diagonalisation scheme of PAPER.md section 2.1 on the device) on the
+    synthetic full-mode operator of BASELINE.json's generator at size N (sigma = 1, seed 1), NEV eigenpairs (default: all N,
+    the direct route's use case; 0 = eigenvalues only).  Stage seconds from the library, wall time sync to sync, and the
+    flop / byte counts of the stages.  One JSON line (profiles/r2_direct.md)."""
+    import torch
+    import paper_2504_10096_b200 as b
+    parts = spec.split(":")
+    N = int(parts[0])
+    nev = int(parts[1]) if len(parts) > 1 and parts[1] else N
+    store = parts[2] if len(parts) > 2 else "c128"
+    torch.cuda.set_device(0)
+    rt = b.bse_fill_synthetic(N, b.MATRIX_R, 1, 1.0, 16)
+    ct = b.bse_fill_synthetic(N, b.MATRIX_C, 1, 0.0, 16)
+    storage = b.STORE_C128
+    if store == "real":
+        b.bse_to_real_form(rt, ct, N)
+        storage = b.STORE_REAL_FORM
+    h = b.Bse(b.MODE_FULL, N, rt, ct, storage=storage)
+    h.solve_direct(min(4, N), vectors=False) if N <= 2048 else None          # warm-up (module load, attributes) at small sizes
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    om, vec, sec = h.solve_direct(max(nev, 1), vectors=nev > 0)
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    n = 2 * N
+    out = {"workload": f"full N={N} (operator {n} x {n}) sigma=1.0 seed=1, nev={nev}", "store": store, "seconds_wall": wall,
+           "seconds": sec, "omega_first": float(om[0]), "omega_last": float(om[-1]),
+           "cholesky_tflops": (n ** 3 / 3) / max(sec["cholesky"], 1e-9) / 1e12,
+           "w_tflops": 2.0 * n ** 3 / max(sec["w"], 1e-9) / 1e12,
+           "tridiag_GBps": 8.0 / 3.0 * n ** 3 / max(sec["tridiag"], 1e-9) / 1e9}      # lower triangle read + written once per step
+    if nev > 0:
+        V = vec[: min(nev, 64)]
+        HV = h.apply(V)
+        w = torch.from_numpy(om[: V.shape[0]]).cuda()[:, None]
+        out["max_residual_first_64"] = float((torch.linalg.vector_norm(HV - V * w, dim=1) / torch.linalg.vector_norm(V, dim=1)).max())
+    print(json.dumps({"direct": out}))
+
+
 def measure_peaks(b, sustained_s: float = 0.0):
     """The library's own microbenchmarks (bse_selftest_peak): burst figures from one timed launch each; with
     sustained_s > 0 also the rate of back-to-back launches over that many seconds (power cap reached)."""
@@ -579,11 +618,15 @@ def main():
                     help="time one bse_solve alone (see run_solve) instead of the apply benchmark")
     ap.add_argument("--peaks", action="store_true", help="measure the roofline denominators with the library's microbenchmarks")
     ap.add_argument("--dense", default=None, metavar="M:K[:L]", help="time the dense basis kernels at config-4 shapes")
+    ap.add_argument("--direct", default=None, metavar="N[:NEV[:STORE]]", help="time bse_solve_direct (PAPER.md section 2.1 on the device)")
     ap.add_argument("--slices", type=int, default=0, metavar="G",
                     help="time the G partial handles of a G-way partition one after another on this GPU (see run_slices)")
     args = ap.parse_args()
     if args.solve:
         run_solve(args.solve)
+        return
+    if args.direct:
+        run_direct(args.direct)
         return
     if args.peaks:
         run_peaks(args)

@@ -146,17 +146,29 @@ __global__ void __launch_bounds__(256) jl_kernel(const double *L, int64_t n, int
 }
 
 
-// ---- skew-symmetric Householder tridiagonalisation, step j on the trailing block W22 = W[j+1:, j+1:] (m = n - j - 1 rows)
+// ---- skew-symmetric Householder tridiagonalisation.  Only the strict lower triangle of W is read and written (W[c][r] =
+// -W[r][c]).  Step j works on the trailing block T_j = W[j+1:, j+1:] (m = n - j - 1 rows) with the reflector v_j of column j:
+//     T_j <- H T_j H = T_j + tau (v p^T - p v^T),  p = T_j v      (v^T T_j v = 0 for a skew matrix)
+// and that update is applied lazily: to column j + 1 by the next house_kernel, to the rest, T_{j+1}, by the next
+// skew_fused_kernel in the same pass that forms p_{j+1} = T_{j+1} v_{j+1} -- every step reads and writes the lower triangle
+// once (8/3 n^3 bytes in all).
 
-// x = W[j+1:, j]: beta = -sign(x_0) ||x||, tau = (beta - x_0) / beta, v = (1, x_1.. / (x_0 - beta)) (H = I - tau v v^T, H x =
-// beta e_0); v is written over x (kept for the back-transformation) and to vbuf; p is cleared.  One CTA.
-__global__ void __launch_bounds__(1024) house_kernel(double *W, int64_t n, int64_t j, double *tau, double *beta, double *vbuf,
-                                                     double *p)
+// Reflector of column j: first the pending update of step j - 1 (tau_{j-1}, vp = v_{j-1}, pp = p_{j-1}, both indexed from
+// row j) on x = W[j+1:, j], then beta = -sign(x_0) ||x||, tau = (beta - x_0) / beta, v = (1, x_1.. / (x_0 - beta))
+// (H = I - tau v v^T, H x = beta e_0); v is written over x (kept for the back-transformation) and to vn; pn is cleared.  One CTA.
+__global__ void __launch_bounds__(1024) house_kernel(double *W, int64_t n, int64_t j, double *tau, double *beta,
+                                                     const double *vp, const double *pp, double *vn, double *pn)
 {
     __shared__ double red[32];
     __shared__ double s_scale;
     const int64_t m = n - j - 1;
     double *x = W + (j + 1) + j * n;
+    const double tp = j > 0 ? tau[j - 1] : 0.0;
+    if (tp != 0.0) {
+        const double p0 = pp[0];                                   // v_{j-1}[0] = 1
+        for (int64_t r = threadIdx.x; r < m; r += blockDim.x) x[r] += tp * (vp[r + 1] * p0 - pp[r + 1]);
+        __syncthreads();
+    }
     double acc = 0.0;
     for (int64_t r = 1 + threadIdx.x; r < m; r += blockDim.x) acc += x[r] * x[r];
     for (int o = 16; o; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
@@ -181,51 +193,62 @@ __global__ void __launch_bounds__(1024) house_kernel(double *W, int64_t n, int64
     for (int64_t r = threadIdx.x; r < m; r += blockDim.x) {
         const double v = r == 0 ? 1.0 : x[r] * sc;
         x[r] = v;
-        vbuf[r] = v;
-        p[r] = 0.0;
+        vn[r] = v;
+        pn[r] = 0.0;
     }
 }
 
-// p += W22 v: CTA (bx, by) takes 128 rows and 128 columns, one thread per row (coalesced down the columns)
-__global__ void __launch_bounds__(128) skew_matvec_kernel(const double *W, int64_t n, int64_t j, const double *tau,
-                                                          const double *v, double *p)
+// One 64 x 64 tile (bi >= bj) of the lower triangle of T_j, CTA of 256 threads: w = W[r][c] + tau_{j-1} (vp_r pp_c - pp_r vp_c)
+// (vp, pp: v_{j-1}, p_{j-1} indexed from row j + 1), stored back, and its two contributions to pn = T_j vn:
+// pn_r += w vn_c,  pn_c -= w vn_r.
+__global__ void __launch_bounds__(256) skew_fused_kernel(double *W, int64_t n, int64_t j, const double *tau, const double *vp,
+                                                         const double *pp, const double *vn, double *pn)
 {
-    if (tau[j] == 0.0) return;
-    const int64_t m = n - j - 1;
-    const int64_t r = blockIdx.x * 128ll + threadIdx.x, c0 = blockIdx.y * 128ll;
-    __shared__ double vs[128];
-    vs[threadIdx.x] = (c0 + threadIdx.x < m) ? v[c0 + threadIdx.x] : 0.0;
-    __syncthreads();
-    if (r >= m) return;
-    const double *w = W + (j + 1 + r) + (j + 1 + c0) * n;
-    const int nc = (int)min((int64_t)128, m - c0);
-    double a0 = 0.0, a1 = 0.0;
-    int c = 0;
-    for (; c + 1 < nc; c += 2) {
-        a0 += w[(int64_t)c * n] * vs[c];
-        a1 += w[(int64_t)(c + 1) * n] * vs[c + 1];
+    const int bi = blockIdx.x, bj = blockIdx.y;
+    if (bj > bi) return;
+    __shared__ double tile[64][65];
+    __shared__ double vpr[64], ppr[64], vnr[64], vpc[64], ppc[64], vnc[64];
+    const int64_t m = n - j - 1, r0 = bi * 64ll, c0 = bj * 64ll;
+    const double tp = j > 0 ? tau[j - 1] : 0.0;
+    const int t = threadIdx.x;
+    if (t < 64) {
+        const bool ok = r0 + t < m;
+        vpr[t] = (ok && tp != 0.0) ? vp[r0 + t] : 0.0;
+        ppr[t] = (ok && tp != 0.0) ? pp[r0 + t] : 0.0;
+        vnr[t] = ok ? vn[r0 + t] : 0.0;
+    } else if (t < 128) {
+        const int q = t - 64;
+        const bool ok = c0 + q < m;
+        vpc[q] = (ok && tp != 0.0) ? vp[c0 + q] : 0.0;
+        ppc[q] = (ok && tp != 0.0) ? pp[c0 + q] : 0.0;
+        vnc[q] = ok ? vn[c0 + q] : 0.0;
     }
-    if (c < nc) a0 += w[(int64_t)c * n] * vs[c];
-    atomicAdd(p + r, a0 + a1);
-}
-
-// W22 += tau (v p^T - p v^T)
-__global__ void __launch_bounds__(128) skew_rank2_kernel(double *W, int64_t n, int64_t j, const double *tau, const double *v,
-                                                         const double *p)
-{
-    const double t = tau[j];
-    if (t == 0.0) return;
-    const int64_t m = n - j - 1;
-    const int64_t r = blockIdx.x * 128ll + threadIdx.x, c0 = blockIdx.y * 128ll;
-    __shared__ double vs[128], ps[128];
-    vs[threadIdx.x] = (c0 + threadIdx.x < m) ? v[c0 + threadIdx.x] : 0.0;
-    ps[threadIdx.x] = (c0 + threadIdx.x < m) ? p[c0 + threadIdx.x] : 0.0;
     __syncthreads();
-    if (r >= m) return;
-    const double vr = t * v[r], pr = t * p[r];
-    double *w = W + (j + 1 + r) + (j + 1 + c0) * n;
-    const int nc = (int)min((int64_t)128, m - c0);
-    for (int c = 0; c < nc; ++c) w[(int64_t)c * n] += vr * ps[c] - pr * vs[c];
+    double *w0 = W + (j + 1 + r0) + (j + 1 + c0) * n;
+    const int rr = t & 63;
+    for (int cc = t >> 6; cc < 64; cc += 4) {
+        const int64_t r = r0 + rr, c = c0 + cc;
+        double w = 0.0;
+        if (r < m && c < m && r > c) {
+            w = w0[rr + (int64_t)cc * n];
+            if (tp != 0.0) {
+                w += tp * (vpr[rr] * ppc[cc] - ppr[rr] * vpc[cc]);
+                w0[rr + (int64_t)cc * n] = w;
+            }
+        }
+        tile[cc][rr] = w;
+    }
+    __syncthreads();
+    if (t < 64) {
+        double a0 = 0.0, a1 = 0.0;
+        for (int cc = 0; cc < 64; cc += 2) { a0 += tile[cc][t] * vnc[cc]; a1 += tile[cc + 1][t] * vnc[cc + 1]; }
+        if (r0 + t < m) atomicAdd(pn + r0 + t, a0 + a1);
+    } else if (t < 128) {
+        const int q = t - 64;
+        double a0 = 0.0, a1 = 0.0;
+        for (int r = 0; r < 64; r += 2) { a0 += tile[q][r] * vnr[r]; a1 += tile[q][r + 1] * vnr[r + 1]; }
+        if (c0 + q < m) atomicAdd(pn + c0 + q, -(a0 + a1));
+    }
 }
 
 // z <- H_0 H_1 ... H_{n-3} z for one column of Z per CTA (the column lives in shared memory; the reflectors v_j stream from W's
@@ -343,10 +366,10 @@ extern "C" bse_status_t bse_solve_direct(bse_handle_t h, int32_t nev, double *hO
     const size_t nn = (size_t)n * n * sizeof(double);
     if ((st = A.alloc(nn)) || (st = U.alloc(nn)) || (st = JL.alloc(nn)) ||
         (st = invT.alloc((size_t)(n / DNB) * DNB * DNB * sizeof(double))) || (st = panel.alloc((size_t)n * DNB * sizeof(double))) ||
-        (st = panelT.alloc((size_t)n * DNB * sizeof(double))) || (st = small.alloc((size_t)(4 * n + 64) * sizeof(double))))
+        (st = panelT.alloc((size_t)n * DNB * sizeof(double))) || (st = small.alloc((size_t)(6 * n + 64) * sizeof(double))))
         return st;
-    double *tau = small.d(), *beta = tau + n, *vbuf = beta + n, *pbuf = vbuf + n;
-    int *flag = (int *)(pbuf + n);
+    double *tau = small.d(), *beta = tau + n, *vbuf = beta + n, *pbuf = vbuf + 2 * n;      // v, p: two buffers each
+    int *flag = (int *)(pbuf + 2 * n);
     BSE_CUDA(cudaMemsetAsync(flag, 0, sizeof(int), s));
 
     // ---- 1. M_r
@@ -399,13 +422,13 @@ extern "C" bse_status_t bse_solve_direct(bse_handle_t h, int32_t nev, double *hO
     t1 = now_s();
     for (int64_t j = 0; j + 1 < n; ++j) {
         const int64_t m = n - j - 1;
-        house_kernel<<<1, 1024, 0, s>>>(A.d(), n, j, tau, beta, vbuf, pbuf);
+        double *vp = vbuf + ((j + 1) & 1) * n, *pp = pbuf + ((j + 1) & 1) * n, *vn = vbuf + (j & 1) * n, *pn = pbuf + (j & 1) * n;
+        house_kernel<<<1, 1024, 0, s>>>(A.d(), n, j, tau, beta, vp, pp, vn, pn);
         count_launch();
         if (m < 2) break;                                          // the last entry is its own sub-diagonal (tau = 0)
-        const dim3 grid((unsigned)((m + 127) / 128), (unsigned)((m + 127) / 128));
-        skew_matvec_kernel<<<grid, 128, 0, s>>>(A.d(), n, j, tau, vbuf, pbuf);
-        skew_rank2_kernel<<<grid, 128, 0, s>>>(A.d(), n, j, tau, vbuf, pbuf);
-        count_launch(2);
+        const unsigned nbt = (unsigned)((m + 63) / 64);
+        skew_fused_kernel<<<dim3(nbt, nbt), 256, 0, s>>>(A.d(), n, j, tau, vp + 1, pp + 1, vn, pn);
+        count_launch();
     }
     BSE_CUDA(cudaGetLastError());
     std::vector<double> hb(n), htau(n);

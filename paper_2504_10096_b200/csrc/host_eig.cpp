@@ -134,13 +134,14 @@ BSE_CLONES void reflect_columns(int lo, int m, const double *vi, double taur, do
 // panels of RP rows, Zb[(panel * m + column) * RP + row_in_panel]; eigenvalues sorted ascending into w, ord = the
 // permutation.  Shared by the complex Hermitian and the real symmetric driver.  Returns 0, or >0 if QL failed.
 static int tridiag_ql(int m, std::vector<double> &d, std::vector<double> &e, std::vector<double> &Zb, std::vector<int> &ord,
-                      double *w)
+                      double *w, bool want_z = true)
 {
     // ---- implicit QL on (d, e) with the rotations accumulated in Zr (real m x m), stored in panels of RP rows:
     //      Zb[(panel * m + column) * RP + row_in_panel]
-    const int npan = (m + RP - 1) / RP;
+    const int npan = want_z ? (m + RP - 1) / RP : 0;     // want_z = false: eigenvalues only, O(m^2)
     Zb.assign((size_t)npan * m * RP, 0.0);
-    for (int i = 0; i < m; ++i) Zb[((size_t)(i / RP) * m + i) * RP + i % RP] = 1.0;
+    if (want_z)
+        for (int i = 0; i < m; ++i) Zb[((size_t)(i / RP) * m + i) * RP + i % RP] = 1.0;
     std::vector<double> rc(m), rs(m);
     int fail = 0;
     for (int l = 0; l < m; ++l) {
@@ -175,7 +176,7 @@ static int tridiag_ql(int m, std::vector<double> &d, std::vector<double> &e, std
             const int ilo = under ? i + 1 : l;
             // apply the recorded rotations (q = mm-1 down to ilo) to columns (q, q+1): z[q+1] = s z[q] + c f,
             // z[q] = c z[q] - s f with f the old z[q+1]; the new z[q] is the next step's f and stays in registers
-            if (mm - 1 >= ilo) {
+            if (want_z && mm - 1 >= ilo) {
                 const int64_t work = (int64_t)(mm - ilo) * m;
 #pragma omp parallel for schedule(static) if (work > 32768)
                 for (int pn = 0; pn < npan; ++pn) rotate_panel(&Zb[(size_t)pn * m * RP], mm, ilo, rc.data(), rs.data());
@@ -414,9 +415,132 @@ int host_syev(int m, double *A, int lda, double *w, double *Z, int ldz, int nz)
     return fail;
 }
 
-// Real symmetric tridiagonal (d: m diagonal entries, e: m - 1 sub-diagonal entries, both destroyed): all eigenvalues
+// Eigenvectors of the nz lowest eigenvalues w[0..nz) (ascending, already computed) of the real symmetric tridiagonal (d, e) by
+// inverse iteration: LU with partial pivoting of T - w_j I, a seeded random start, a few solves, and modified Gram-Schmidt
+// against the earlier vectors of the same cluster of close eigenvalues (gaps below 1e-5 ||T||_1) -- the textbook method
+// behind LAPACK's dstein, restated.  O(m) per solve; clusters are independent and run in parallel.  Returns 0, or j + 1 if
+// vector j did not reach a residual of 1e-12 ||T||_1.
+static int tridiag_inverse_iteration(int m, const double *d, const double *e, const double *w, int nz, double *Z, int ldz)
+{
+    const double eps = 2.220446049250313e-16;
+    double onenrm = 0.0;
+    for (int i = 0; i < m; ++i) {
+        const double v = std::fabs(d[i]) + (i > 0 ? std::fabs(e[i - 1]) : 0.0) + (i + 1 < m ? std::fabs(e[i]) : 0.0);
+        onenrm = std::max(onenrm, v);
+    }
+    if (onenrm == 0.0) onenrm = 1.0;
+    // (dstein re-orthogonalises below 1e-3 ||T||; 1e-5 leaves eps ||T|| / gap <= 2e-11 between clusters, far inside the 1e-7
+    //  the eigenvectors of H are held to, and keeps the clusters of a dense spectrum short)
+    const double ortol = 1e-5 * onenrm, tiny = eps * onenrm;
+    // cluster boundaries
+    std::vector<int> start;
+    for (int j = 0; j < nz; ++j)
+        if (j == 0 || w[j] - w[j - 1] > ortol) start.push_back(j);
+    start.push_back(nz);
+    int fail = 0;
+    const int ncl = (int)start.size() - 1;
+    int largest = 0;
+    for (int cl = 0; cl < ncl; ++cl) largest = std::max(largest, start[cl + 1] - start[cl]);
+    // many small clusters: one thread per cluster; a large one: clusters in turn, its Gram-Schmidt sums threaded
+    const bool outer = largest <= 64;
+#pragma omp parallel for schedule(dynamic, 1) if (outer && nz > 8)
+    for (int cl = 0; cl < ncl; ++cl) {
+        std::vector<double> a(m), b(m), b2(m), l(m), x(m), dots(start[cl + 1] - start[cl]);
+        std::vector<char> piv(m);
+        double prev = 0.0;
+        for (int j = start[cl]; j < start[cl + 1]; ++j) {
+            double lam = w[j];
+            if (j > start[cl] && lam - prev < 10.0 * eps * std::fabs(lam) + 10.0 * tiny) lam = prev + 10.0 * eps * std::fabs(lam) + 10.0 * tiny;
+            prev = lam;
+            // ---- P L U = T - lam I
+            for (int i = 0; i < m; ++i) { a[i] = d[i] - lam; b[i] = i + 1 < m ? e[i] : 0.0; b2[i] = 0.0; }
+            for (int k = 0; k + 1 < m; ++k) {
+                const double c = e[k];
+                if (std::fabs(a[k]) >= std::fabs(c)) {
+                    if (std::fabs(a[k]) < tiny) a[k] = std::copysign(tiny, a[k] == 0.0 ? 1.0 : a[k]);
+                    const double mult = c / a[k];
+                    a[k + 1] -= mult * b[k];
+                    l[k] = mult; piv[k] = 0;
+                } else {
+                    const double mult = a[k] / c, t = a[k + 1];
+                    a[k] = c;
+                    a[k + 1] = b[k] - mult * t;
+                    if (k + 2 < m) { b2[k] = b[k + 1]; b[k + 1] = -mult * b2[k]; }
+                    b[k] = t;
+                    l[k] = mult; piv[k] = 1;
+                }
+            }
+            if (std::fabs(a[m - 1]) < tiny) a[m - 1] = std::copysign(tiny, a[m - 1] == 0.0 ? 1.0 : a[m - 1]);
+            // ---- seeded start
+            uint64_t rs = 0x9E3779B97F4A7C15ull * (uint64_t)(j + 1) + 12345u;
+            for (int i = 0; i < m; ++i) {
+                rs = rs * 6364136223846793005ull + 1442695040888963407ull;
+                x[i] = ((double)(rs >> 11) / 9007199254740992.0) - 0.5;
+            }
+            double *zj = Z + (int64_t)j * ldz;
+            bool ok = false;
+            for (int it = 0; it < 8 && !ok; ++it) {
+                for (int k = 0; k + 1 < m; ++k) {                                  // forward
+                    if (piv[k]) std::swap(x[k], x[k + 1]);
+                    x[k + 1] -= l[k] * x[k];
+                }
+                x[m - 1] /= a[m - 1];                                              // backward
+                if (m > 1) x[m - 2] = (x[m - 2] - b[m - 2] * x[m - 1]) / a[m - 2];
+                for (int k = m - 3; k >= 0; --k) x[k] = (x[k] - b[k] * x[k + 1] - b2[k] * x[k + 2]) / a[k];
+                // re-orthogonalise inside the cluster: classical Gram-Schmidt, twice (sums over all earlier vectors at once)
+                const int nq = j - start[cl];
+                const double *Zc = Z + (int64_t)start[cl] * ldz;
+                for (int rep = 0; rep < 2 && nq > 0; ++rep) {
+                    const bool par = !outer && (int64_t)nq * m > 65536;
+#pragma omp parallel for schedule(static) if (par)
+                    for (int q = 0; q < nq; ++q) {
+                        const double *zq = Zc + (int64_t)q * ldz;
+                        double dot = 0.0;
+#pragma omp simd reduction(+ : dot)
+                        for (int i = 0; i < m; ++i) dot += zq[i] * x[i];
+                        dots[q] = dot;
+                    }
+#pragma omp parallel for schedule(static) if (par)
+                    for (int i0 = 0; i0 < m; i0 += 512) {
+                        const int i1 = std::min(m, i0 + 512);
+                        for (int q = 0; q < nq; ++q) {
+                            const double *zq = Zc + (int64_t)q * ldz;
+                            const double dq = dots[q];
+#pragma omp simd
+                            for (int i = i0; i < i1; ++i) x[i] -= dq * zq[i];
+                        }
+                    }
+                }
+                double nrm = 0.0;
+                for (int i = 0; i < m; ++i) nrm += x[i] * x[i];
+                nrm = std::sqrt(nrm);
+                if (!(nrm > 0.0) || !std::isfinite(nrm)) break;
+                for (int i = 0; i < m; ++i) x[i] /= nrm;
+                if (it >= 1) {                                                      // residual of the normalised vector
+                    double r2 = 0.0;
+                    for (int i = 0; i < m; ++i) {
+                        double v = (d[i] - w[j]) * x[i];
+                        if (i > 0) v += e[i - 1] * x[i - 1];
+                        if (i + 1 < m) v += e[i] * x[i + 1];
+                        r2 += v * v;
+                    }
+                    ok = std::sqrt(r2) <= 1e-12 * onenrm;
+                }
+            }
+            for (int i = 0; i < m; ++i) zj[i] = x[i];
+            if (!ok) {
+#pragma omp critical
+                if (!fail) fail = j + 1;
+            }
+        }
+    }
+    return fail;
+}
+
+// Real symmetric tridiagonal (d: m diagonal entries, e: m - 1 sub-diagonal entries, both untouched): all eigenvalues
 // ascending in w and the eigenvectors of the nz lowest in Z (m x nz, column-major, ldz).  The last stage of the direct
-// route (bse_direct.cu).  Returns 0, or >0 if QL failed.
+// route (bse_direct.cu).  A few wanted vectors (nz <= m / 4): eigenvalues by QL without accumulation, O(m^2), then
+// inverse iteration; otherwise QL with the rotations accumulated.  Returns 0, or >0 if an iteration failed.
 int host_stev(int m, double *d_in, double *e_in, double *w, double *Z, int ldz, int nz)
 {
     if (m <= 0) return 0;
@@ -425,8 +549,10 @@ int host_stev(int m, double *d_in, double *e_in, double *w, double *Z, int ldz, 
     for (int i = 0; i + 1 < m; ++i) e[i] = e_in[i];
     std::vector<double> Zb;
     std::vector<int> ord;
-    const int fail = tridiag_ql(m, d, e, Zb, ord, w);
-    if (nz <= 0 || !Z) return fail;
+    const bool few = nz > 0 && Z && 4 * nz <= m;
+    int fail = tridiag_ql(m, d, e, Zb, ord, w, !few && nz > 0 && Z);
+    if (nz <= 0 || !Z || fail) return fail;
+    if (few) return tridiag_inverse_iteration(m, d_in, e_in, w, nz, Z, ldz);
 #pragma omp parallel for schedule(static) if ((int64_t)m * nz > 65536)
     for (int j = 0; j < nz; ++j) {
         const int src = ord[j];

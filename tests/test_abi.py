@@ -137,7 +137,7 @@ def test_host_stev_vs_scipy():
     import paper_2504_10096_b200 as b
     from scipy.linalg import eigh_tridiagonal
     rng = np.random.default_rng(5)
-    for m, nz in [(1, 1), (2, 2), (37, 5), (300, 300), (513, 40)]:
+    for m, nz in [(1, 1), (2, 2), (37, 5), (300, 300), (513, 40), (2000, 150), (64, 16)]:     # nz <= m/4: inverse iteration
         d = rng.standard_normal(m) * 3
         e = rng.standard_normal(max(m - 1, 0))
         w, Z = b.host_stev(d, e, nz)
@@ -150,3 +150,20 @@ def test_host_stev_vs_scipy():
     e = rng.standard_normal(63)
     w, _ = b.host_stev(np.zeros(64), e, 0)
     assert np.max(np.abs(w + w[::-1])) <= 1e-13 * np.max(np.abs(w))
+
+
+def test_host_stev_clusters():
+    """Inverse iteration inside clusters: Wilkinson's W21+ (pairs agreeing to 1e-14) glued three times (a cluster of close
+    triples), and the direct route's own matrix B^T B of a bidiagonal with repeated singular values nearby."""
+    import paper_2504_10096_b200 as b
+    n1 = 21
+    d1 = np.abs(np.arange(n1) - 10.0)
+    d = np.concatenate([d1, d1, d1, d1]); e = np.ones(len(d) - 1); e[n1 - 1::n1] = 1e-9
+    m = len(d)
+    T = np.diag(d) + np.diag(e, 1) + np.diag(e, -1)
+    w_ref = np.linalg.eigvalsh(T)
+    nz = m // 4
+    w, Z = b.host_stev(d, e, nz)
+    assert np.max(np.abs(w - w_ref)) <= 1e-13 * np.max(np.abs(w_ref))
+    assert np.linalg.norm(T @ Z - Z * w[:nz]) <= 1e-11 * np.linalg.norm(T)
+    assert np.linalg.norm(Z.T @ Z - np.eye(nz)) <= 1e-10
