@@ -225,16 +225,21 @@ __global__ void __launch_bounds__(256) skew_fused_kernel(double *W, int64_t n, i
     }
     __syncthreads();
     double *w0 = W + (j + 1 + r0) + (j + 1 + c0) * n;
-    const int rr = t & 63;
-    for (int cc = t >> 6; cc < 64; cc += 4) {
-        const int64_t r = r0 + rr, c = c0 + cc;
-        double w = 0.0;
-        if (r < m && c < m && r > c) {
-            w = w0[rr + (int64_t)cc * n];
-            if (tp != 0.0) {
-                w += tp * (vpr[rr] * ppc[cc] - ppr[rr] * vpc[cc]);
-                w0[rr + (int64_t)cc * n] = w;
-            }
+    const int rr = t & 63, cq = t >> 6;
+    const int64_t r = r0 + rr;
+    double wv[16];
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {                                 // all loads of this thread in flight at once
+        const int cc = cq + 4 * q;
+        wv[q] = (r < m && c0 + cc < m && r > c0 + cc) ? w0[rr + (int64_t)cc * n] : 0.0;
+    }
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+        const int cc = cq + 4 * q;
+        double w = wv[q];
+        if (tp != 0.0 && r < m && c0 + cc < m && r > c0 + cc) {
+            w += tp * (vpr[rr] * ppc[cc] - ppr[rr] * vpc[cc]);
+            w0[rr + (int64_t)cc * n] = w;
         }
         tile[cc][rr] = w;
     }
