@@ -256,38 +256,58 @@ __global__ void __launch_bounds__(256) skew_fused_kernel(double *W, int64_t n, i
     }
 }
 
-// z <- H_0 H_1 ... H_{n-3} z for one column of Z per CTA (the column lives in shared memory; the reflectors v_j stream from W's
-// strict lower triangle, column j rows j+1.., v_0 = 1 stored)
-__global__ void __launch_bounds__(256) reflect_back_kernel(const double *W, int64_t n, const double *tau, double *Z, int64_t ldz)
+// z <- H_0 H_1 ... H_{n-3} z for one column of Z per CTA of 1024 threads.  Thread t owns the absolute rows t + 1024 q
+// (q < PER, n <= 1024 PER) of the column, held in shared memory, for the whole kernel: a step needs one block-wide sum (the
+// dot product; partial sums double-buffered, so one barrier per step) and nothing else crosses threads.  The reflector
+// v_j = W[j+1:, j] (v_0 = 1 stored) is loaded once per step into registers, all loads in flight at once.
+template <int PER>
+__global__ void __launch_bounds__(1024) reflect_back_kernel(const double *W, int64_t n, const double *tau, double *Z, int64_t ldz)
 {
     extern __shared__ double zc[];
-    __shared__ double red[8];
-    __shared__ double s_dot;
+    __shared__ double red[2][32];
     double *z = Z + blockIdx.x * ldz;
-    for (int64_t r = threadIdx.x; r < n; r += blockDim.x) zc[r] = z[r];
-    __syncthreads();
-    for (int64_t j = n - 3; j >= 0; --j) {
-        const double t = tau[j];
-        if (t == 0.0) continue;                                    // uniform
-        const int64_t m = n - j - 1;
-        const double *v = W + (j + 1) + j * n;
-        double *zz = zc + j + 1;
-        double acc = 0.0;
-        for (int64_t r = threadIdx.x; r < m; r += blockDim.x) acc += v[r] * zz[r];
-        for (int o = 16; o; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            double d = 0.0;
-            for (int w = 0; w < 8; ++w) d += red[w];
-            s_dot = t * d;
-        }
-        __syncthreads();
-        const double f = s_dot;
-        for (int64_t r = threadIdx.x; r < m; r += blockDim.x) zz[r] -= f * v[r];
-        __syncthreads();
+    const int t = threadIdx.x, warp = t >> 5;
+#pragma unroll
+    for (int q = 0; q < PER; ++q) {
+        const int64_t a = t + 1024ll * q;
+        if (a < n) zc[a] = z[a];
     }
-    for (int64_t r = threadIdx.x; r < n; r += blockDim.x) z[r] = zc[r];
+    int buf = 0;
+    for (int64_t j = n - 3; j >= 0; --j) {
+        const double tj = tau[j];
+        if (tj == 0.0) continue;                                    // uniform
+        const double *col = W + j * n;
+        double vv[PER];
+        double acc = 0.0;
+#pragma unroll
+        for (int q = 0; q < PER; ++q) {
+            const int64_t a = t + 1024ll * q;
+            vv[q] = (a > j && a < n) ? col[a] : 0.0;
+        }
+#pragma unroll
+        for (int q = 0; q < PER; ++q) {
+            const int64_t a = t + 1024ll * q;
+            if (a > j && a < n) acc += vv[q] * zc[a];
+        }
+        for (int o = 16; o; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if ((t & 31) == 0) red[buf][warp] = acc;
+        __syncthreads();
+        double d = 0.0;
+#pragma unroll
+        for (int w = 0; w < 32; ++w) d += red[buf][w];
+        const double f = tj * d;
+#pragma unroll
+        for (int q = 0; q < PER; ++q) {
+            const int64_t a = t + 1024ll * q;
+            if (a > j && a < n) zc[a] -= f * vv[q];
+        }
+        buf ^= 1;
+    }
+#pragma unroll
+    for (int q = 0; q < PER; ++q) {
+        const int64_t a = t + 1024ll * q;
+        if (a < n) z[a] = zc[a];
+    }
 }
 
 // [X; Y] = Q y, Q = (1/sqrt 2) [[I, -iI], [I, iI]] (Eq. 2), y = Yr + i Yi (n x nev each, real, ld n), then X^H X - Y^H Y = 1.
@@ -486,10 +506,21 @@ extern "C" bse_status_t bse_solve_direct(bse_handle_t h, int32_t nev, double *hO
         BSE_CUDA(cudaMemcpyAsync(Z.d(), hz.data(), hz.size() * 8, cudaMemcpyHostToDevice, s));
         BSE_CUDA(cudaStreamSynchronize(s));
     }
-    BSE_CUDA(cudaFuncSetAttribute(reflect_back_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(n * 8)));
-    reflect_back_kernel<<<l2, 256, (size_t)n * 8, s>>>(A.d(), n, tau, Z.d(), n);
-    count_launch();
-    BSE_CUDA(cudaGetLastError());
+    {
+        const int per = (int)((n + 1023) / 1024);
+        auto launch = [&](auto kern) -> bse_status_t {
+            BSE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(n * 8)));
+            kern<<<l2, 1024, (size_t)n * 8, s>>>(A.d(), n, tau, Z.d(), n);
+            return BSE_OK;
+        };
+        if (per <= 4) st = launch(reflect_back_kernel<4>);
+        else if (per <= 8) st = launch(reflect_back_kernel<8>);
+        else if (per <= 16) st = launch(reflect_back_kernel<16>);
+        else st = launch(reflect_back_kernel<24>);
+        if (st) return st;
+        count_launch();
+        BSE_CUDA(cudaGetLastError());
+    }
     // L^T y = z: U y = z, blocked back substitution from the last block up
     for (int b = nblk - 1; b >= 0; --b) {
         const int64_t k0 = (int64_t)b * DNB;

@@ -539,27 +539,34 @@ static int tridiag_inverse_iteration(int m, const double *d, const double *e, co
 
 // Real symmetric tridiagonal (d: m diagonal entries, e: m - 1 sub-diagonal entries, both untouched): all eigenvalues
 // ascending in w and the eigenvectors of the nz lowest in Z (m x nz, column-major, ldz).  The last stage of the direct
-// route (bse_direct.cu).  A few wanted vectors (nz <= m / 4): eigenvalues by QL without accumulation, O(m^2), then
-// inverse iteration; otherwise QL with the rotations accumulated.  Returns 0, or >0 if an iteration failed.
+// route (bse_direct.cu).  Eigenvalues by QL without accumulation, O(m^2), vectors by inverse iteration, O(m) each plus the
+// Gram-Schmidt sums inside clusters; tiny problems, and any problem on which inverse iteration misses its residual bound,
+// take QL with the rotations accumulated, O(m^3).  Returns 0, or >0 if QL failed.
 int host_stev(int m, double *d_in, double *e_in, double *w, double *Z, int ldz, int nz)
 {
     if (m <= 0) return 0;
     if (nz > m) nz = m;
-    std::vector<double> d(d_in, d_in + m), e(m, 0.0);
-    for (int i = 0; i + 1 < m; ++i) e[i] = e_in[i];
+    const bool want = nz > 0 && Z;
     std::vector<double> Zb;
     std::vector<int> ord;
-    const bool few = nz > 0 && Z && 4 * nz <= m;
-    int fail = tridiag_ql(m, d, e, Zb, ord, w, !few && nz > 0 && Z);
-    if (nz <= 0 || !Z || fail) return fail;
-    if (few) return tridiag_inverse_iteration(m, d_in, e_in, w, nz, Z, ldz);
+    auto ql = [&](bool accumulate) {
+        std::vector<double> d(d_in, d_in + m), e(m, 0.0);
+        for (int i = 0; i + 1 < m; ++i) e[i] = e_in[i];
+        return tridiag_ql(m, d, e, Zb, ord, w, accumulate);
+    };
+    if (!want) return ql(false);
+    if (m > 64) {
+        if (int fail = ql(false)) return fail;
+        if (tridiag_inverse_iteration(m, d_in, e_in, w, nz, Z, ldz) == 0) return 0;
+    }
+    if (int fail = ql(true)) return fail;
 #pragma omp parallel for schedule(static) if ((int64_t)m * nz > 65536)
     for (int j = 0; j < nz; ++j) {
         const int src = ord[j];
         double *z = Z + (int64_t)j * ldz;
         for (int i = 0; i < m; ++i) z[i] = Zb[((size_t)(i / RP) * m + src) * RP + i % RP];
     }
-    return fail;
+    return 0;
 }
 
 }  // namespace bse
