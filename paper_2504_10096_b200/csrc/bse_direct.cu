@@ -201,10 +201,10 @@ __global__ void __launch_bounds__(1024) house_kernel(double *W, int64_t n, int64
 // One 64 x 64 tile (bi >= bj) of the lower triangle of T_j, CTA of 256 threads: w = W[r][c] + tau_{j-1} (vp_r pp_c - pp_r vp_c)
 // (vp, pp: v_{j-1}, p_{j-1} indexed from row j + 1), stored back, and its two contributions to pn = T_j vn:
 // pn_r += w vn_c,  pn_c -= w vn_r.
-__global__ void __launch_bounds__(256) skew_fused_kernel(double *W, int64_t n, int64_t j, const double *tau, const double *vp,
+__global__ void __launch_bounds__(256, 3) skew_fused_kernel(double *W, int64_t n, int64_t j, const double *tau, const double *vp,
                                                          const double *pp, const double *vn, double *pn)
 {
-    const int bi = blockIdx.x, bj = blockIdx.y;
+    const int bi = blockIdx.x, bj = blockIdx.y;                  // (a linear walk of the triangle measured slower: 3.04 vs 2.69 s at n = 16384)
     if (bj > bi) return;
     __shared__ double tile[64][65];
     __shared__ double vpr[64], ppr[64], vnr[64], vpc[64], ppc[64], vnc[64];
