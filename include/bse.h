@@ -195,6 +195,22 @@ typedef int32_t (*bse_comm_fn)(void *user, int32_t op, void *dBuf, int64_t n_dou
 enum { BSE_COMM_SUM = 0, BSE_COMM_BCAST = 1 };
 bse_status_t bse_set_comm(bse_handle_t h, bse_comm_fn fn, void *user);
 
+/* Vectors partitioned by rows as well ("the matrices and vectors are distributed by rows"): after this call the
+ * solver-level calls bse_solve / bse_solve_variant(BSE_VARIANT_SHAO) and bse_orth treat every vector block they are given or
+ * hold as rows [row_begin, row_end) of the full-length block (leading dimensions >= row_end - row_begin).  Needs a hook
+ * (bse_set_comm) and disjoint row ranges that cover [0, N) over the ranks.  Then
+ *   - the Krylov bases, the Gram / update / rotation kernels and the restart work on the local rows only (O(N ncv / G) memory
+ *     and work per rank); every Gram matrix and norm is the SUM over the ranks (one BSE_COMM_SUM of the small matrix);
+ *   - every operator application gathers the operand block (a zero-padded SUM of 16 N k bytes), multiplies it by this rank's
+ *     tile rows, sums the partial results and keeps its own rows (two SUMs of 16 N k bytes per product);
+ *   - start and replacement vectors are functions of the GLOBAL row index (the partitioned block is the slice of the
+ *     replicated one); the projected eigen-decomposition is still rank 0's, broadcast;
+ *   - bse_solve returns the eigenvectors at FULL length on every rank (dVec N x nev / 2N x nev, gathered at the end).
+ * bse_apply / bse_apply_half keep taking full-length blocks.  row_begin = 0, row_end = N restores replicated vectors.
+ * Errors: BSE_ERR_INVALID_ARG (empty or out-of-range rows); the solver calls return BSE_ERR_INVALID_ARG on a row-partitioned
+ * handle without a hook, and bse_lanczos_quadrature*, bse_solve_direct and BSE_VARIANT_GRUNING do not take one. */
+bse_status_t bse_set_row_partition(bse_handle_t h, int64_t row_begin, int64_t row_end);
+
 /* Y = H X for a block of k >= 1 vectors.
  *   TDA : X, Y are N x k;   Y = R X.
  *   FULL: X, Y are 2N x k, rows [X1; X2];  Y1 = R X1 + C X2,  Y2 = -(C^H X1 + R^* X2).

@@ -76,6 +76,7 @@ _SIGNATURES = {
                           ctypes.POINTER(_Info)],
     "bse_selftest_peak": [_i32, _i32, _i32, _vp, _i64, _vp, ctypes.POINTER(_dbl), ctypes.POINTER(_dbl)],
     "bse_solve_direct": [_vp, _i32, ctypes.POINTER(_dbl), _vp, _i64, ctypes.POINTER(_dbl)],
+    "bse_set_row_partition": [_vp, _i64, _i64],
     "bse_host_stev": [_i32, _vp, _vp, _vp, _vp, _i32, _i32],
 }
 EXPORTS = sorted(list(_SIGNATURES) + ["bse_status_string", "bse_launch_count"])
@@ -407,12 +408,19 @@ class ShardedBse:
         self._cb = None
         self.comm_calls = [0, 0]                                 # sums, broadcasts issued through the hook
 
-    def install_comm(self):
+    def install_comm(self, row_partition: bool = False):
         """Give the library the process group (bse_set_comm): its products become complete (local + one all-reduce) and
-        bse_solve / bse_lanczos_quadrature run on the sharded operator with replicated vectors (include/bse.h)."""
+        bse_solve / bse_lanczos_quadrature run on the sharded operator with replicated vectors (include/bse.h).
+        row_partition=True also divides the VECTORS by rows over the ranks (bse_set_row_partition): bases,
+        orthogonalisation and restart then work on N / world rows per rank; solve() still returns full-length vectors."""
         import torch
         import torch.distributed as dist
         group = self.group
+        if row_partition:
+            on = dist.is_available() and dist.is_initialized()
+            world, rank = (dist.get_world_size(group), dist.get_rank(group)) if on else (1, 0)
+            self.vec_rows = (self.N * rank // world, self.N * (rank + 1) // world)
+            _check(lib().bse_set_row_partition(self.local._h, *self.vec_rows), "bse_set_row_partition")
         src = dist.get_global_rank(group, 0) if group is not None else 0
         calls = self.comm_calls
 

@@ -63,6 +63,11 @@ bse_status_t comm_bcast_dev(bse_handle_s *h, void *dBuf, int64_t n_doubles)
     if (!h->comm || n_doubles <= 0) return BSE_OK;
     return h->comm(h->comm_user, BSE_COMM_BCAST, dBuf, n_doubles) ? BSE_ERR_INTERNAL : BSE_OK;
 }
+bse_status_t comm_sum_dev(bse_handle_s *h, void *dBuf, int64_t n_doubles)
+{
+    if (!h->comm || n_doubles <= 0) return BSE_OK;
+    return h->comm(h->comm_user, BSE_COMM_SUM, dBuf, n_doubles) ? BSE_ERR_INTERNAL : BSE_OK;
+}
 bse_status_t comm_bcast_host(bse_handle_s *h, void *hBuf, size_t bytes)
 {
     if (!h->comm || bytes == 0) return BSE_OK;
@@ -267,6 +272,10 @@ bse_status_t bse_create(bse_handle_t *out, int32_t mode, int32_t storage, int64_
     h->comm_user = nullptr;
     h->comm_buf = nullptr;
     h->comm_buf_bytes = 0;
+    h->vr_begin = 0;
+    h->vr_end = N;
+    h->rp_buf = nullptr;
+    h->rp_buf_bytes = 0;
     h->R = (const char *)dRTiles;
     h->C = (mode == BSE_MODE_FULL) ? (const char *)dCTiles : nullptr;
     h->stream = (cudaStream_t)stream;
@@ -357,6 +366,14 @@ bse_status_t bse_set_comm(bse_handle_t h, bse_comm_fn fn, void *user)
     return BSE_OK;
 }
 
+bse_status_t bse_set_row_partition(bse_handle_t h, int64_t row_begin, int64_t row_end)
+{
+    if (!h || row_begin < 0 || row_end <= row_begin || row_end > h->N) return BSE_ERR_INVALID_ARG;
+    h->vr_begin = row_begin;
+    h->vr_end = row_end;
+    return BSE_OK;
+}
+
 bse_status_t bse_destroy(bse_handle_t h)
 {
     if (!h) return BSE_ERR_INVALID_ARG;
@@ -365,6 +382,7 @@ bse_status_t bse_destroy(bse_handle_t h)
     if (h->ws_op) cudaFree(h->ws_op);
     if (h->hpin) cudaFreeHost(h->hpin);
     if (h->comm_buf) cudaFree(h->comm_buf);
+    if (h->rp_buf) cudaFree(h->rp_buf);
     delete h;
     return BSE_OK;
 }

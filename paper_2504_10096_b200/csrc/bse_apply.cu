@@ -353,6 +353,40 @@ static bse_status_t apply_general_local(bse_handle_s *h, const void *dX, int64_t
     return BSE_OK;
 }
 
+bse_status_t apply_vec(bse_handle_s *h, int sign, const void *dX, int64_t ldx, void *dY, int64_t ldy, int32_t k)
+{
+    const int64_t N = h->N;
+    bse_status_t st;
+    if (!is_row_partitioned(h)) {
+        st = sign == 0 ? apply_tda_local(h, dX, ldx, dY, ldy, k) : apply_half_local(h, sign, dX, ldx, dY, ldy, k);
+        if (st) return st;
+        return comm_sum_block(h, dY, ldy, N, k);
+    }
+    // row-partitioned vectors: all-gather of the operand block as a zero-padded sum, product with this rank's tile rows,
+    // sum of the partial results, this rank's rows copied out (2 x 16 N k bytes through the hook per product)
+    if (!h->comm) return BSE_ERR_INVALID_ARG;
+    const size_t need = (size_t)2 * N * k * 16;
+    if (h->rp_buf_bytes < need) {
+        if (h->rp_buf) cudaFree(h->rp_buf);
+        h->rp_buf = nullptr;
+        h->rp_buf_bytes = 0;
+        if (cudaMalloc(&h->rp_buf, need) != cudaSuccess) { cudaGetLastError(); return BSE_ERR_ALLOC; }
+        h->rp_buf_bytes = need;
+    }
+    char *Xf = (char *)h->rp_buf, *Yf = Xf + (size_t)N * k * 16;
+    const int64_t rows = vec_rows(h);
+    BSE_CUDA(cudaMemsetAsync(Xf, 0, (size_t)N * k * 16, h->stream));
+    BSE_CUDA(cudaMemcpy2DAsync(Xf + (size_t)h->vr_begin * 16, (size_t)N * 16, dX, (size_t)ldx * 16, (size_t)rows * 16, (size_t)k,
+                               cudaMemcpyDeviceToDevice, h->stream));
+    if ((st = comm_sum_block(h, Xf, N, N, k))) return st;
+    st = sign == 0 ? apply_tda_local(h, Xf, N, Yf, N, k) : apply_half_local(h, sign, Xf, N, Yf, N, k);
+    if (st) return st;
+    if ((st = comm_sum_block(h, Yf, N, N, k))) return st;
+    BSE_CUDA(cudaMemcpy2DAsync(dY, (size_t)ldy * 16, Yf + (size_t)h->vr_begin * 16, (size_t)N * 16, (size_t)rows * 16, (size_t)k,
+                               cudaMemcpyDeviceToDevice, h->stream));
+    return BSE_OK;
+}
+
 }  // namespace bse
 
 using namespace bse;

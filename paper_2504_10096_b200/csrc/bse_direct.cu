@@ -379,7 +379,7 @@ double now_s()
 extern "C" bse_status_t bse_solve_direct(bse_handle_t h, int32_t nev, double *hOmega, void *dVec, int64_t ldvec,
                                          double *hSeconds)
 {
-    if (!h || h->mode != BSE_MODE_FULL || is_partial(h) || nev < 1 || nev > h->N || !hOmega || (dVec && ldvec < 2 * h->N))
+    if (!h || h->mode != BSE_MODE_FULL || is_partial(h) || is_row_partitioned(h) || nev < 1 || nev > h->N || !hOmega || (dVec && ldvec < 2 * h->N))
         return BSE_ERR_INVALID_ARG;
     const int64_t N = h->N, n = 2 * N;
     if (n > BSE_DIRECT_MAX_N) return BSE_ERR_INVALID_ARG;

@@ -18,6 +18,10 @@ struct bse_handle_s {
     void *comm_user;
     void *comm_buf;      // device staging for host-side broadcasts
     size_t comm_buf_bytes;
+    // bse_set_row_partition: the solver-level calls hold rows [vr_begin, vr_end) of every vector (0, N: replicated vectors)
+    int64_t vr_begin, vr_end;
+    void *rp_buf;        // full-length operand and result blocks of a row-partitioned product
+    size_t rp_buf_bytes;
     int real_form;       // BSE_STORE_REAL_FORM: R holds S = R + C, C holds D = R - C (full mode only, complex128)
     const char *R;
     const char *C;
@@ -48,9 +52,13 @@ namespace bse {
 inline bool is_partial(const bse_handle_s *h) { return h->row_begin != 0 || h->row_end != h->nt; }
 // partial handle that cannot complete its products: the solver-level calls refuse it
 inline bool is_incomplete(const bse_handle_s *h) { return is_partial(h) && !h->comm; }
+// vectors of the solver-level calls partitioned by rows over the ranks behind the hook
+inline bool is_row_partitioned(const bse_handle_s *h) { return h->vr_begin != 0 || h->vr_end != h->N; }
+inline int64_t vec_rows(const bse_handle_s *h) { return h->vr_end - h->vr_begin; }
 // communication through the hook (no-ops without one).  ld, rows in complex elements.
 bse_status_t comm_sum_block(bse_handle_s *h, void *dY, int64_t ld, int64_t rows, int k);
 bse_status_t comm_bcast_dev(bse_handle_s *h, void *dBuf, int64_t n_doubles);
+bse_status_t comm_sum_dev(bse_handle_s *h, void *dBuf, int64_t n_doubles);
 bse_status_t comm_bcast_host(bse_handle_s *h, void *hBuf, size_t bytes);
 
 extern std::atomic<int64_t> g_launches;
@@ -79,6 +87,11 @@ bse_status_t handle_finalize(bse_handle_s *h);
 bse_status_t apply_tda_local(bse_handle_s *h, const void *dX, int64_t ldx, void *dY, int64_t ldy, int32_t k);
 bse_status_t apply_half_local(bse_handle_s *h, int sign, const void *dX, int64_t ldx, void *dY, int64_t ldy, int32_t k);
 bse_status_t zero_block(bse_handle_s *h, void *dY, int64_t ldy, int64_t rows, int32_t k);
+// The COMPLETE product on this handle's vector rows, as the solver-level calls need it: sign = 0: Y = R X (TDA), +-1:
+// Y = R X + sign C conj(X).  Replicated vectors: local product + sum over the slices.  Row-partitioned vectors (X, Y hold
+// rows [vr_begin, vr_end)): the operand block is gathered (zero-padded sum), multiplied by this rank's tile rows, summed, and
+// this rank's rows of the result are copied out.
+bse_status_t apply_vec(bse_handle_s *h, int sign, const void *dX, int64_t ldx, void *dY, int64_t ldy, int32_t k);
 
 
 // ---- dense basis kernels (dense_ops.cu).  Complex blocks are column-major; *_cplx selects complex coefficients.

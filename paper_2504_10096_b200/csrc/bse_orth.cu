@@ -69,7 +69,7 @@ struct OrthWs {
 // scalar slots keep their place while the basis grows (orth_reserve sizes the buffer for the largest m up front).
 static bse_status_t orth_ws(bse_handle_s *h, int m, int k, OrthWs &w)
 {
-    const int64_t n = h->N;
+    const int64_t n = vec_rows(h);
     size_t cm = (size_t)2 * (m > 0 ? m : 1) * k, ck = (size_t)2 * k * k;
     const size_t small = SC_COUNT + F_COUNT + ck;
     size_t doubles = (size_t)4 * n * k + small + 2 * ck + 4 * ck + 2 * cm;
@@ -217,7 +217,7 @@ static bse_status_t fetch_coef(bse_handle_s *h, const double *dev, double *pin, 
 static bse_status_t block_gram(bse_handle_s *h, const void *W, int64_t ldw, const void *PW, int64_t ldpw, int k,
                                bool cplx, OrthWs &w, std::vector<zc> &G)
 {
-    ST(gram_basis(h, W, ldw, k, cplx ? W : PW, cplx ? ldw : ldpw, k, cplx, h->N, w.g));
+    ST(gram_basis(h, W, ldw, k, cplx ? W : PW, cplx ? ldw : ldpw, k, cplx, vec_rows(h), w.g));
     ST(fetch_coef(h, w.g, w.hg, k, k, cplx));
     G.assign((size_t)k * k, zc(0.0));
     coef_to_host(w.hg, k, k, cplx, G.data(), false);
@@ -229,7 +229,7 @@ static bse_status_t project_pass(bse_handle_s *h, const void *V, int64_t ldv, co
                                  void *W, int64_t ldw, void *PW, int64_t ldpw, int kc, bool cplx, double *coef)
 {
     if (m <= 0) return BSE_OK;
-    const int64_t n = h->N;
+    const int64_t n = vec_rows(h);
     const int ldo = cplx ? 2 * m : m;
     ST(gram_basis(h, cplx ? V : PV, cplx ? ldv : ldpv, m, W, ldw, kc, cplx, n, coef));
     ST(gemm_basis(h, V, ldv, m, cplx, coef, ldo, kc, n, W, ldw, -1.0, 1.0));
@@ -268,7 +268,7 @@ bse_status_t block_norm_scale(bse_handle_s *h, const void *W, int64_t ldw, const
     ST(orth_ws(h, 0, k, w));
     if (slot == SC_E_IN) BSE_CUDA(cudaMemsetAsync(w.flags, 0, sizeof(double) * F_COUNT, h->stream));
     const bool euclid = cplx || !PW;
-    ST(gram_basis(h, W, ldw, k, euclid ? W : PW, euclid ? ldw : ldpw, k, euclid, h->N, w.g));
+    ST(gram_basis(h, W, ldw, k, euclid ? W : PW, euclid ? ldw : ldpw, k, euclid, vec_rows(h), w.g));
     diag_stats_kernel<<<1, 32, 0, h->stream>>>(w.g, k, euclid ? 1 : 0, w.scal, slot, w.flags, euclid ? 0 : 1);
     count_launch();
     BSE_CUDA(cudaGetLastError());
@@ -283,7 +283,7 @@ bse_status_t normalize_block(bse_handle_s *h, const void *V, int64_t ldv, int m,
                              int64_t ldw, int k, void *PW, int64_t ldpw, bool cplx, int scale_mode, void *hcoef_host,
                              void *bfac_host, int *rank_out, uint64_t seed, uint64_t *rng_counter, int image_sign)
 {
-    const int64_t n = h->N;
+    const int64_t n = vec_rows(h);
     OrthWs w;
     ST(orth_ws(h, m, k, w));
     std::vector<zc> G, Hc((size_t)(m > 0 ? m : 1) * k, zc(0.0)), B((size_t)k * k, zc(0.0));
@@ -362,7 +362,7 @@ bse_status_t normalize_block(bse_handle_s *h, const void *V, int64_t ldv, int m,
                 for (int tries = 0; tries < 3; ++tries) {
                     ST(fill_random_block(h, wj, ldw, n, 1, seed, (*rng_counter)++));
                     if (!cplx) {
-                        bse_status_t st = bse_apply_half(h, image_sign, wj, ldw, pwj, ldpw, 1);
+                        bse_status_t st = apply_vec(h, image_sign, wj, ldw, pwj, ldpw, 1);
                         if (st) return st;
                     }
                     for (int pass = 0; pass < 2; ++pass) {
@@ -427,10 +427,10 @@ extern "C" bse_status_t bse_orth(bse_handle_t h, const void *dV, int64_t ldv, in
                                  void *dW, int64_t ldw, int32_t k, void *dBW, int64_t ldbw, void *dHcoef, void *dBfac,
                                  int32_t *hRank)
 {
-    if (!h || !dW || k < 1 || m < 0 || ldw < h->N || is_incomplete(h)) return BSE_ERR_INVALID_ARG;
-    if (m > 0 && (!dV || ldv < h->N)) return BSE_ERR_INVALID_ARG;
+    if (!h || !dW || k < 1 || m < 0 || ldw < vec_rows(h) || is_incomplete(h)) return BSE_ERR_INVALID_ARG;
+    if (m > 0 && (!dV || ldv < vec_rows(h))) return BSE_ERR_INVALID_ARG;
     if (dBV || dBW) {
-        if (h->mode != BSE_MODE_FULL || !dBW || ldbw < h->N || (m > 0 && (!dBV || ldbv < h->N))) return BSE_ERR_INVALID_ARG;
+        if (h->mode != BSE_MODE_FULL || !dBW || ldbw < vec_rows(h) || (m > 0 && (!dBV || ldbv < vec_rows(h)))) return BSE_ERR_INVALID_ARG;
     }
     const bool real_ip = (dBW != nullptr);
     // in the real inner product with m == 0 there is no dBV: pass dBW's own pointer as a non-null marker

@@ -117,7 +117,7 @@ static bse_status_t lanczos_quadrature_full(bse_handle_s *h, const void *dStart,
 extern "C" bse_status_t bse_lanczos_quadrature(bse_handle_t h, const void *dStart, int32_t steps, double *hAlpha,
                                                double *hBeta, int32_t *hDone)
 {
-    if (!h || !dStart || steps < 1 || !hAlpha || !hBeta || is_incomplete(h)) return BSE_ERR_INVALID_ARG;
+    if (!h || !dStart || steps < 1 || !hAlpha || !hBeta || is_incomplete(h) || is_row_partitioned(h)) return BSE_ERR_INVALID_ARG;
     if (h->mode == BSE_MODE_FULL) return lanczos_quadrature_full(h, dStart, steps, hAlpha, hBeta, hDone);
     const int64_t n = h->N;
     // workspace: three vectors + alpha[steps] + nrm2[steps + 1]
@@ -238,7 +238,7 @@ static bse_status_t static_scratch_address(char **out)
 extern "C" bse_status_t bse_lanczos_quadrature_static(bse_handle_t h, const void *dStart, int32_t steps, double *hAlpha,
                                                       double *hBeta, int32_t *hDone)
 {
-    if (!h || !dStart || steps < 1 || !hAlpha || !hBeta || is_incomplete(h) || h->mode != BSE_MODE_TDA) return BSE_ERR_INVALID_ARG;
+    if (!h || !dStart || steps < 1 || !hAlpha || !hBeta || is_incomplete(h) || is_row_partitioned(h) || h->mode != BSE_MODE_TDA) return BSE_ERR_INVALID_ARG;
     const int64_t n = h->N;
     if (n > STATIC_MAX_N || steps > STATIC_MAX_STEPS) return BSE_ERR_STATIC_LIMIT;
     char *base = nullptr;

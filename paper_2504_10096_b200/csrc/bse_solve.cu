@@ -210,8 +210,7 @@ struct Solver {
     bse_status_t apply_block(int c0)
     {
         if (!full) {
-            ST(apply_tda_local(h, col(V, c0), ld, col(V, c0 + k), ld, k));
-            ST(comm_sum_block(h, col(V, c0 + k), ld, n, k));
+            ST(apply_vec(h, 0, col(V, c0), ld, col(V, c0 + k), ld, k));
         } else if (variant == BSE_VARIANT_GRUNING) {
             // u_{2j} = [y; -conj y]: H u_{2j-1} has the half vector P(x_j); orthonormalise it against the stored vectors of its
             // sign in the Omega inner product, <y_i, z>_M = Re(M(y_i)^H z) -- image recomputed after the projection (reading R3)
@@ -235,8 +234,7 @@ struct Solver {
             // H u_{2j} has the half vector M(y_j): the next sign +1 candidate
             ST(copy_block(h, col(MYb, my), ld, col(V, c0 + k), ld, n, k));
         } else {
-            bse_status_t st = bse_apply_half(h, -1, col(PV, c0), ld, col(V, c0 + k), ld, k);      // W = M(p)
-            if (st) return st;
+            ST(apply_vec(h, -1, col(PV, c0), ld, col(V, c0 + k), ld, k));                          // W = M(p)
         }
         info.n_apply += 1;
         return BSE_OK;
@@ -252,8 +250,7 @@ struct Solver {
         ST(block_norm_scale(h, col(V, m), ld, nullptr, ld, k, false, ORTH_E_IN));
         ST(project_block(h, V.p, ld, m, PV.p, ld, col(V, m), ld, k, nullptr, ld, false));
         BSE_CUDA(cudaEventRecord(ev[2], h->stream));
-        bse_status_t st = bse_apply_half(h, +1, col(V, m), ld, col(PV, m), ld, k);                // PW = P(W)
-        if (st) return st;
+        ST(apply_vec(h, +1, col(V, m), ld, col(PV, m), ld, k));                                   // PW = P(W)
         BSE_CUDA(cudaEventRecord(ev[3], h->stream));
         timed_second_apply = true;
         info.n_apply += 1;
@@ -283,10 +280,15 @@ extern "C" bse_status_t bse_solve_variant(bse_handle_t h, int32_t variant, int32
     if (variant != BSE_VARIANT_SHAO && variant != BSE_VARIANT_GRUNING) return BSE_ERR_INVALID_ARG;
     if (h->mode != BSE_MODE_FULL) variant = BSE_VARIANT_SHAO;          // TDA: the Hermitian iteration has no variants
     if (is_incomplete(h)) return BSE_ERR_INVALID_ARG;
-    const int64_t n = h->N;
+    // n: rows of every vector held here -- all N, or this rank's rows [vr_begin, vr_end) under bse_set_row_partition (the
+    // dense kernels then work on the local rows, their Gram matrices are summed over the ranks, and apply_vec gathers the
+    // operand block of every product); the returned eigenvectors are gathered to full length on every rank
+    const bool rowpart = is_row_partitioned(h);
+    if (rowpart && (!h->comm || variant == BSE_VARIANT_GRUNING)) return BSE_ERR_INVALID_ARG;
+    const int64_t Nfull = h->N, n = vec_rows(h);
     const bool full = (h->mode == BSE_MODE_FULL);
-    if ((int64_t)nev + k > n || ldvec < (full ? 2 * n : n)) return BSE_ERR_INVALID_ARG;
-    const int64_t dim = full ? 2 * n : n;               // real-linear (full) / complex (TDA) dimension of the space
+    if ((int64_t)nev + k > Nfull || ldvec < (full ? 2 * Nfull : Nfull)) return BSE_ERR_INVALID_ARG;
+    const int64_t dim = full ? 2 * Nfull : Nfull;       // real-linear (full) / complex (TDA) dimension of the space
     const int nwant = full ? 2 * nev : nev;             // Ritz values of G come in pairs in full mode
     if (ncv <= 0) {
         ncv = std::max(2 * nev, nev + 15);
@@ -331,10 +333,7 @@ extern "C" bse_status_t bse_solve_variant(bse_handle_t h, int32_t variant, int32
     // ---- start block: random, orthonormalised in the active inner product
     ST(fill_random_block(h, s.V.p, s.ld, n, k, seed, s.rng));
     s.rng += k;
-    if (full) {
-        bse_status_t st = bse_apply_half(h, +1, s.V.p, s.ld, s.PV.p, s.ld, k);
-        if (st) return st;
-    }
+    if (full) ST(apply_vec(h, +1, s.V.p, s.ld, s.PV.p, s.ld, k));
     {
         int rank = 0;
         ST(orth_block(h, nullptr, s.ld, 0, full ? s.PV.p : nullptr, s.ld, s.V.p, s.ld, k, full ? s.PV.p : nullptr, s.ld,
@@ -551,7 +550,13 @@ extern "C" bse_status_t bse_solve_variant(bse_handle_t h, int32_t variant, int32
         if (hResid) hResid[j] = resid[i];
     }
     if (!full) {
-        ST(s.rotate(s.V, mp, Ssel.data(), mp, nev, dVec, ldvec));
+        if (!rowpart) ST(s.rotate(s.V, mp, Ssel.data(), mp, nev, dVec, ldvec));
+        else {
+            ST(s.rotate(s.V, mp, Ssel.data(), mp, nev, s.rot.p, n));
+            ST(zero_block(h, dVec, ldvec, Nfull, nev));
+            ST(copy_block(h, s.rot.p, n, (char *)dVec + (size_t)h->vr_begin * 16, ldvec, n, nev));
+            ST(comm_sum_block(h, dVec, ldvec, Nfull, nev));
+        }
     } else {
         // candidates (left in rot by select_distinct): x = X s, p = PX s;  v = [x + p/w; conj(x - p/w)] sqrt(w)/2, assembled
         // into the storage of X (no longer needed), then the returned vectors are their combinations Cm
@@ -560,7 +565,16 @@ extern "C" bse_status_t bse_solve_variant(bse_handle_t h, int32_t variant, int32
         BSE_CUDA(cudaMemcpyAsync(s.omega_d.p, wc.data(), sizeof(double) * ncand, cudaMemcpyHostToDevice, h->stream));
         ST(assemble_full_vectors(h, s.rot.p, s.col(s.rot, ncand), n, ncand, (const double *)s.omega_d.p, s.V.p, 2 * n));
         ST(s.upload_coef(Cm.data(), ncand, ncand, nev, true));
-        ST(gemm_basis(h, s.V.p, 2 * n, ncand, true, (const double *)s.coef.p, 2 * ncand, nev, 2 * n, dVec, ldvec, 1.0, 0.0));
+        if (!rowpart)
+            ST(gemm_basis(h, s.V.p, 2 * n, ncand, true, (const double *)s.coef.p, 2 * ncand, nev, 2 * n, dVec, ldvec, 1.0, 0.0));
+        else {
+            // local rows of [X; Y] (2 n x nev) -> their places in the full-length vectors, summed over the ranks
+            ST(gemm_basis(h, s.V.p, 2 * n, ncand, true, (const double *)s.coef.p, 2 * ncand, nev, 2 * n, s.rot.p, 2 * n, 1.0, 0.0));
+            ST(zero_block(h, dVec, ldvec, 2 * Nfull, nev));
+            ST(copy_block(h, s.rot.p, 2 * n, (char *)dVec + (size_t)h->vr_begin * 16, ldvec, n, nev));
+            ST(copy_block(h, (char *)s.rot.p + (size_t)n * 16, 2 * n, (char *)dVec + (size_t)(Nfull + h->vr_begin) * 16, ldvec, n, nev));
+            ST(comm_sum_block(h, dVec, ldvec, 2 * Nfull, nev));
+        }
     }
     BSE_CUDA(cudaStreamSynchronize(h->stream));
     return result;

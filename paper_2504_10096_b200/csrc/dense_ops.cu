@@ -50,7 +50,9 @@ bse_status_t gram_basis(bse_handle_s *h, const void *A, int64_t lda, int m, cons
         count_launch();
     }
     BSE_CUDA(cudaGetLastError());
-    // the partial sums were combined with floating-point atomics: on a sharded operator rank 0's result is everyone's
+    // row-partitioned vectors: every rank holds part of the rows, the Gram matrix is the sum over the ranks.  Replicated
+    // vectors: the partial sums were combined with floating-point atomics, so on a sharded operator rank 0's result is everyone's
+    if (is_row_partitioned(h)) return comm_sum_dev(h, out, (int64_t)ldo * k);
     return comm_bcast_dev(h, out, (int64_t)ldo * k);
 }
 
@@ -90,15 +92,17 @@ bse_status_t gemm_basis(bse_handle_s *h, const void *A, int64_t lda, int m, bool
                                    alpha, beta);
 }
 
-__global__ void fill_random_kernel(double2 *W, int64_t ldw, int64_t n, int k, uint64_t h0, uint64_t counter)
+__global__ void fill_random_kernel(double2 *W, int64_t ldw, int64_t n, int64_t row0, int k, uint64_t h0, uint64_t counter)
 {
     int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     int c = blockIdx.y;
-    if (i < n && c < k) W[i + c * ldw] = normal_pair(h0, (uint64_t)i, counter + (uint64_t)c);
+    if (i < n && c < k) W[i + c * ldw] = normal_pair(h0, (uint64_t)(row0 + i), counter + (uint64_t)c);
 }
+// n rows starting at this handle's first vector row (the entries are a function of the GLOBAL row index, so a row-partitioned
+// block is the slice of the replicated one)
 bse_status_t fill_random_block(bse_handle_s *h, void *W, int64_t ldw, int64_t n, int k, uint64_t seed, uint64_t counter)
 {
-    fill_random_kernel<<<dim3((unsigned)((n + 255) / 256), k), 256, 0, h->stream>>>((double2 *)W, ldw, n, k,
+    fill_random_kernel<<<dim3((unsigned)((n + 255) / 256), k), 256, 0, h->stream>>>((double2 *)W, ldw, n, h->vr_begin, k,
                                                                                     stream_key(seed, 6), counter);
     count_launch();
     BSE_CUDA(cudaGetLastError());

@@ -295,3 +295,93 @@ def test_unit_length_and_slices_every_kernel(orc, L, monkeypatch):
         for sign in (+1, -1):
             Y = sum(h.apply_half(to_dev(X), sign) for h in hs)
             assert relerr(to_host(Y), orc.apply_half(R, C, X, sign)) <= 1e-12, (G, sign)
+
+
+# ------------------------------------------------- GPU: vectors partitioned by rows as well, two host processes
+def _rowpart_worker(rank, world, port, q):
+    try:
+        import torch
+        import torch.distributed as dist
+        os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        torch.cuda.set_device(0)
+        dist.init_process_group("gloo", rank=rank, world_size=world)
+        import paper_2504_10096_b200 as b
+        from gpu_util import pack, to_host
+        out = {}
+        N, k, nev = 448, 4, 6                                  # 7 tile rows: unequal tile slices; 224 vector rows per rank
+        R = gen.dense_R(N, 3, sigma=1.0)
+        C = gen.dense_C(N, 3)
+
+        def sliced(tiles):
+            rb, re, ft, n, by = b.bse_shard_layout(N, world, rank)
+            return (rb, re), tiles[ft * 65536: ft * 65536 + by]
+        rows, sl = sliced(pack(R, 0))
+        h = b.ShardedBse(b.MODE_TDA, N, sl, None, rows).install_comm(row_partition=True)
+        out["vec_rows"] = h.vec_rows
+        res = h.solve(nev, k, tol=1e-9, seed=1)
+        out["tda_omega"], out["tda_vec"], out["tda_info"] = res.omega, to_host(res.vectors), res.info
+        out["tda_calls"] = list(h.comm_calls)
+        (rows, sr), (_, sc) = sliced(pack(R, 0)), sliced(pack(C, 1))
+        hf = b.ShardedBse(b.MODE_FULL, N, sr, sc, rows).install_comm(row_partition=True)
+        resf = hf.solve(5, k, tol=1e-9, seed=2)
+        out["full_omega"], out["full_vec"], out["full_info"] = resf.omega, to_host(resf.vectors), resf.info
+        # what a row-partitioned handle does not take
+        try:
+            hf.solve(5, k, variant=b.VARIANT_GRUNING)
+            out["gruning_refused"] = False
+        except b.BseError as e:
+            out["gruning_refused"] = e.status == 1
+        dist.barrier()
+        dist.destroy_process_group()
+        q.put((rank, out))
+    except Exception:
+        import traceback
+        q.put((rank, {"error": traceback.format_exc()}))
+
+
+@pytest.mark.gpu
+def test_solver_with_row_partitioned_vectors_two_ranks(orc):
+    """bse_set_row_partition: each rank holds half of the rows of every basis vector and its own slice of the tile store; the
+    eigenpairs (gathered to full length) are certified by the oracle on both ranks, and agree with the replicated-vector
+    solve of one process to the solver's accuracy (the Gram sums are split differently, so not bitwise)."""
+    import torch.multiprocessing as mp
+    import paper_2504_10096_b200 as b
+    from gpu_util import pack
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 31700 + os.getpid() % 2000
+    ps = [ctx.Process(target=_rowpart_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in ps: p.start()
+    got = dict(q.get(timeout=600) for _ in ps)
+    for p in ps: p.join(120)
+    for r in (0, 1):
+        assert "error" not in got[r], got[r].get("error")
+    N, nev = 448, 6
+    R, C = gen.dense_R(N, 3, sigma=1.0), gen.dense_C(N, 3)
+    assert got[0]["vec_rows"] == (0, 224) and got[1]["vec_rows"] == (224, 448)
+    wj, _ = orc.jacobi_herm(R)
+    omd, _ = orc.bse_direct(R, C, want_vectors=False)
+    for r in (0, 1):
+        o = got[r]
+        assert np.max(np.abs(o["tda_omega"] - wj[:nev]) / np.abs(wj[:nev])) <= 1e-10
+        V = o["tda_vec"]
+        assert V.shape == (N, nev)
+        assert np.linalg.norm(V.conj().T @ V - np.eye(nev)) <= 1e-12
+        assert np.max(np.linalg.norm(orc.apply_tda(R, V) - V * o["tda_omega"], axis=0)) <= 1e-8 * 12
+        assert o["tda_info"]["basis_orth_err"] <= 1e-12
+        assert np.max(np.abs(o["full_omega"] - omd[N:N + 5]) / omd[N:N + 5]) <= 1e-10
+        Vf = o["full_vec"]
+        assert Vf.shape == (2 * N, 5)
+        rr = np.linalg.norm(orc.apply_full(R, C, Vf) - Vf * o["full_omega"], axis=0) / np.linalg.norm(Vf, axis=0)
+        assert np.all(rr <= 1e-8 * 12)
+        Sig = np.concatenate([np.ones(N), -np.ones(N)])
+        assert np.max(np.abs(np.sum(Sig[:, None] * np.abs(Vf) ** 2, axis=0) - 1)) <= 1e-10
+        assert o["full_info"]["basis_orth_err"] <= 1e-12
+        assert o["gruning_refused"]
+    # both ranks hold the same gathered result and took the same path
+    assert np.array_equal(got[0]["tda_omega"], got[1]["tda_omega"]) and np.array_equal(got[0]["tda_vec"], got[1]["tda_vec"])
+    assert np.array_equal(got[0]["full_vec"], got[1]["full_vec"])
+    assert got[0]["tda_info"]["n_apply"] == got[1]["tda_info"]["n_apply"]
+    # and agree with the replicated-vector solve of a single handle
+    ref = b.Bse(b.MODE_TDA, N, pack(R, 0)).solve(nev, 4, tol=1e-9, seed=1)
+    assert np.max(np.abs(ref.omega - got[0]["tda_omega"]) / np.abs(ref.omega)) <= 1e-10
