@@ -27,6 +27,11 @@ typedef std::complex<double> zc;
 namespace {
 constexpr int RP = 8;       // rows per panel of the rotation accumulator
 constexpr int JB = 8;       // eigenvector columns per back-transformation task
+inline int max_threads();
+// threads worth starting for an m x m problem: the parallel regions of a step are short (a mat-vec, a rank-2 update, a
+// panel sweep), and with more than one thread per ~64 rows the fork / barrier costs more than it saves (m = 200 on
+// 8 cores: 11.1 ms with 8 threads, 7.1 ms with 4)
+inline int threads_for(int m);
 inline int max_threads()
 {
 #ifdef _OPENMP
@@ -35,6 +40,7 @@ inline int max_threads()
     return 1;
 #endif
 }
+inline int threads_for(int m) { return std::max(1, std::min(max_threads(), m / 64)); }
 
 // The four hot loops, in explicit real arithmetic on interleaved (re, im) doubles (std::complex multiplication does
 // not vectorise without -ffast-math) and compiled for SSE2 / AVX2+FMA / AVX-512 with run-time dispatch, so that the
@@ -178,7 +184,7 @@ static int tridiag_ql(int m, std::vector<double> &d, std::vector<double> &e, std
             // z[q] = c z[q] - s f with f the old z[q+1]; the new z[q] is the next step's f and stays in registers
             if (want_z && mm - 1 >= ilo) {
                 const int64_t work = (int64_t)(mm - ilo) * m;
-#pragma omp parallel for schedule(static) if (work > 32768)
+#pragma omp parallel for schedule(static) num_threads(threads_for(m)) if (work > 32768)
                 for (int pn = 0; pn < npan; ++pn) rotate_panel(&Zb[(size_t)pn * m * RP], mm, ilo, rc.data(), rs.data());
             }
             if (under) continue;
@@ -207,7 +213,7 @@ int host_heev(int m, void *A_, int lda, double *w, void *Z_, int ldz, int nz)
     auto a = [&](int i, int j) -> zc & { return A[i + (int64_t)j * lda]; };
 
     // ---- Householder tridiagonalisation, lower variant:  A = Q T Q^H,  Q = H_0 H_1 ... H_{m-2},  H_i = I - tau v v^H
-    const int nth = max_threads();
+    const int nth = threads_for(m);
     std::vector<zc> x(m), v(m), xt((size_t)nth * m);
     for (int i = 0; i < m - 1; ++i) {
         const int n = m - i - 1;                  // length of the column below the diagonal
@@ -255,7 +261,7 @@ int host_heev(int m, void *A_, int lda, double *w, void *Z_, int ldz, int nz)
             zc al = -0.5 * t * dot;
             for (int r = 0; r < n; ++r) x[r] += al * v[r];                 // w
             // A22 -= v w^H + w v^H   (lower triangle)
-#pragma omp parallel for schedule(static, 1) if (par)
+#pragma omp parallel for schedule(static, 1) num_threads(nth) if (par)
             for (int c0 = 0; c0 < n; c0 += 4)
                 rank2_update_columns(n, reinterpret_cast<double *>(&a(i + 1, i + 1)), lda,
                                      reinterpret_cast<const double *>(v.data()), reinterpret_cast<const double *>(x.data()),
@@ -272,7 +278,7 @@ int host_heev(int m, void *A_, int lda, double *w, void *Z_, int ldz, int nz)
 
     // ---- Z = Q * Zr[:, ord[0..nz)]:  start from the real eigenvectors and apply H_{m-2} ... H_0 from the left,
     //      each reflector to JB columns at a time (the reflector is read once per block, not once per column)
-#pragma omp parallel for schedule(dynamic, 1) if (m > 64)
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nth) if (m > 64)
     for (int j0 = 0; j0 < nz; j0 += JB) {
         const int nb = std::min(JB, nz - j0);
         zc *zcol[JB];
@@ -344,7 +350,7 @@ int host_syev(int m, double *A, int lda, double *w, double *Z, int ldz, int nz)
     if (nz > m) nz = m;
     std::vector<double> d(m), e(m, 0.0), tau(m, 0.0);
     auto a = [&](int i, int j) -> double & { return A[i + (int64_t)j * lda]; };
-    const int nth = max_threads();
+    const int nth = threads_for(m);
     std::vector<double> x(m), v(m), xt((size_t)nth * m);
     for (int i = 0; i < m - 1; ++i) {
         const int n = m - i - 1;
@@ -386,7 +392,7 @@ int host_syev(int m, double *A, int lda, double *w, double *Z, int ldz, int nz)
             }
             const double al = -0.5 * t * dot;
             for (int r = 0; r < n; ++r) x[r] += al * v[r];
-#pragma omp parallel for schedule(static, 1) if (par)
+#pragma omp parallel for schedule(static, 1) num_threads(nth) if (par)
             for (int c0 = 0; c0 < n; c0 += 8)
                 rank2_update_columns_real(n, &a(i + 1, i + 1), lda, v.data(), x.data(), c0, std::min(c0 + 8, n));
         }
@@ -398,7 +404,7 @@ int host_syev(int m, double *A, int lda, double *w, double *Z, int ldz, int nz)
     std::vector<int> ord;
     const int fail = tridiag_ql(m, d, e, Zb, ord, w);
     if (nz <= 0 || !Z) return fail;
-#pragma omp parallel for schedule(dynamic, 1) if (m > 64)
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nth) if (m > 64)
     for (int j0 = 0; j0 < nz; j0 += JB) {
         const int nb = std::min(JB, nz - j0);
         double *zcol[JB];
