@@ -14,6 +14,7 @@
 //   6. back-transformation (Eq. 4): z = H_0 ... H_{n-3} D s,  L^T y = z,  [X; Y] = Q y with Q of Eq. (2),
 //      normalised X^H X - Y^H Y = 1
 // Everything O(n^3) runs on the device; the host sequences kernels and solves the tridiagonal problem.
+#include <algorithm>
 #include <cmath>
 #include <ctime>
 #include <vector>
@@ -310,6 +311,21 @@ __global__ void __launch_bounds__(1024) reflect_back_kernel(const double *W, int
     }
 }
 
+// Reflector panel of the blocked back-transformation: Vp (m x nb, ld m) = the reflectors j0 .. j0 + nbk - 1 restricted to rows
+// j0 .. n - 1 (m = n - j0, even; row 0 is zero, column c starts at row c + 1; columns >= nbk are zero), and VpT (nb x m, ld nb)
+// its transpose.
+__global__ void __launch_bounds__(256) reflector_panel_kernel(const double *W, int64_t n, int64_t j0, int nbk, int nb, double *Vp,
+                                                              double *VpT)
+{
+    const int64_t m = n - j0;
+    const int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const int c = blockIdx.y;
+    if (r >= m) return;
+    const double v = (c < nbk && r >= c + 1) ? W[(j0 + r) + (j0 + c) * n] : 0.0;
+    Vp[r + (int64_t)c * m] = v;
+    VpT[c + r * (int64_t)nb] = v;
+}
+
 // [X; Y] = Q y, Q = (1/sqrt 2) [[I, -iI], [I, iI]] (Eq. 2), y = Yr + i Yi (n x nev each, real, ld n), then X^H X - Y^H Y = 1.
 // One CTA per eigenvector.  sig[c] receives the Sigma-norm before scaling (must be positive for a positive omega).
 __global__ void __launch_bounds__(256) assemble_direct_kernel(const double *Yr, const double *Yi, int64_t n, int64_t N,
@@ -483,6 +499,15 @@ extern "C" bse_status_t bse_solve_direct(bse_handle_t h, int32_t nev, double *hO
 
     // ---- 6. back-transformation.  z_T = D s with D = diag((-i)^j): Z = [Re | Im], n x 2 nev real
     t1 = now_s();
+    const bool verbose = getenv("BSE_VERBOSE") != nullptr;
+    double t_lap = t1;
+    auto lap = [&](const char *what) {
+        if (!verbose) return;
+        cudaStreamSynchronize(s);
+        const double t = now_s();
+        fprintf(stderr, "[bse_solve_direct] %s: %.3f s\n", what, t - t_lap);
+        t_lap = t;
+    };
     DevBuf Z, Ytmp;
     const int l2 = 2 * nev;
     if ((st = Z.alloc((size_t)n * l2 * sizeof(double))) || (st = Ytmp.alloc((size_t)DNB * l2 * sizeof(double)))) return st;
@@ -503,10 +528,56 @@ extern "C" bse_status_t bse_solve_direct(bse_handle_t h, int32_t nev, double *hO
                 zi[2 * o + 1] = -sg * odd;
             }
         }
+        lap("host Z");
         BSE_CUDA(cudaMemcpyAsync(Z.d(), hz.data(), hz.size() * 8, cudaMemcpyHostToDevice, s));
         BSE_CUDA(cudaStreamSynchronize(s));
+        lap("upload Z");
     }
-    {
+    constexpr int RNB = 32;                                        // reflectors per block of the compact WY form
+    if (l2 >= 64 && n > 2 * RNB) {
+        // Blocked: H_j0 ... H_j0+nb-1 = I - V T V^T (forward, columnwise: T upper triangular, T_ii = tau_i,
+        // T[0:i, i] = -tau_i T[0:i, 0:i] (V^T V)[0:i, i]); on the transposed block ZT = Z^T (2 nev x n) the update is three
+        // row-rich real GEMMs on the tensor cores:  ZT[:, rows] -= ((ZT[:, rows] V) T^T) V^T.
+        DevBuf ZT, Vp, VpT, W1, W2, Gd;
+        if ((st = ZT.alloc((size_t)n * l2 * 8)) || (st = Vp.alloc((size_t)n * RNB * 8)) || (st = VpT.alloc((size_t)n * RNB * 8)) ||
+            (st = W1.alloc((size_t)l2 * RNB * 8)) || (st = W2.alloc((size_t)l2 * RNB * 8)) || (st = Gd.alloc((size_t)2 * RNB * RNB * 8)))
+            return st;
+        transpose_kernel<<<dim3((unsigned)((n + 31) / 32), (unsigned)((l2 + 31) / 32)), 256, 0, s>>>(Z.d(), n, n, l2, ZT.d(), l2, 0);
+        count_launch();
+        std::vector<double> htau(n, 0.0), G((size_t)RNB * RNB), TT((size_t)RNB * RNB);
+        BSE_CUDA(cudaMemcpyAsync(htau.data(), tau, (size_t)(n - 1) * 8, cudaMemcpyDeviceToHost, s));
+        BSE_CUDA(cudaStreamSynchronize(s));
+        const int64_t nref = n - 2;                               // reflectors j = 0 .. n - 3
+        for (int64_t j0 = ((nref - 1) / RNB) * RNB; j0 >= 0; j0 -= RNB) {
+            const int nbk = (int)std::min<int64_t>(RNB, nref - j0);
+            const int64_t m = n - j0;                              // rows j0 .. n - 1 (even; the first row of the panel is zero)
+            reflector_panel_kernel<<<dim3((unsigned)((m + 255) / 256), RNB), 256, 0, s>>>(A.d(), n, j0, nbk, RNB, Vp.d(), VpT.d());
+            count_launch();
+            // G = V^T V (nb x nb) with the Gram kernel of the basis (real inner product over the m rows = m / 2 complex rows)
+            if ((st = gram_basis(h, Vp.d(), m / 2, RNB, Vp.d(), m / 2, RNB, false, m / 2, Gd.d()))) return st;
+            BSE_CUDA(cudaMemcpyAsync(G.data(), Gd.d(), (size_t)RNB * RNB * 8, cudaMemcpyDeviceToHost, s));
+            BSE_CUDA(cudaStreamSynchronize(s));
+            std::fill(TT.begin(), TT.end(), 0.0);                 // TT = T^T, column-major: TT[i + a * nb] = T[a, i]
+            for (int i = 0; i < nbk; ++i) {
+                const double ti = htau[j0 + i];
+                TT[i + (size_t)i * RNB] = ti;
+                for (int a = 0; a < i; ++a) {
+                    double acc = 0.0;
+                    for (int q = a; q < i; ++q) acc += TT[q + (size_t)a * RNB] * G[q + (size_t)i * RNB];      // T[a, q] G[q, i]
+                    TT[i + (size_t)a * RNB] = -ti * acc;
+                }
+            }
+            BSE_CUDA(cudaMemcpyAsync(Gd.d() + RNB * RNB, TT.data(), (size_t)RNB * RNB * 8, cudaMemcpyHostToDevice, s));
+            double *Zr = ZT.d() + (size_t)j0 * l2;                // columns j0 .. n - 1 of ZT
+            if ((st = rgemm(h, l2, RNB, (int)m, 1.0, Zr, l2, Vp.d(), m, 0.0, W1.d(), l2))) return st;
+            if ((st = rgemm(h, l2, RNB, RNB, 1.0, W1.d(), l2, Gd.d() + RNB * RNB, RNB, 0.0, W2.d(), l2))) return st;
+            if ((st = rgemm(h, l2, (int)m, RNB, -1.0, W2.d(), l2, VpT.d(), RNB, 1.0, Zr, l2))) return st;
+            BSE_CUDA(cudaStreamSynchronize(s));                   // TT and G are reused by the next block
+        }
+        transpose_kernel<<<dim3((unsigned)((l2 + 31) / 32), (unsigned)((n + 31) / 32)), 256, 0, s>>>(ZT.d(), l2, l2, n, Z.d(), n, 0);
+        count_launch();
+        BSE_CUDA(cudaGetLastError());
+    } else {
         const int per = (int)((n + 1023) / 1024);
         auto launch = [&](auto kern) -> bse_status_t {
             BSE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(n * 8)));
@@ -521,6 +592,7 @@ extern "C" bse_status_t bse_solve_direct(bse_handle_t h, int32_t nev, double *hO
         count_launch();
         BSE_CUDA(cudaGetLastError());
     }
+    lap("reflectors");
     // L^T y = z: U y = z, blocked back substitution from the last block up
     for (int b = nblk - 1; b >= 0; --b) {
         const int64_t k0 = (int64_t)b * DNB;
@@ -529,6 +601,7 @@ extern "C" bse_status_t bse_solve_direct(bse_handle_t h, int32_t nev, double *hO
         BSE_CUDA(cudaMemcpy2DAsync(Z.d() + k0, (size_t)n * 8, Ytmp.d(), (size_t)DNB * 8, (size_t)DNB * 8, l2, cudaMemcpyDeviceToDevice, s));
         if (k0 > 0 && (st = rgemm(h, k0, l2, DNB, -1.0, U.d() + k0 * n, n, Ytmp.d(), DNB, 1.0, Z.d(), n))) return st;
     }
+    lap("triangular solve");
     double *sig = pbuf;
     assemble_direct_kernel<<<nev, 256, 0, s>>>(Z.d(), Z.d() + (size_t)nev * n, n, N, (double2 *)dVec, ldvec, sig);
     count_launch();
