@@ -534,7 +534,9 @@ extern "C" bse_status_t bse_solve_direct(bse_handle_t h, int32_t nev, double *hO
         lap("upload Z");
     }
     constexpr int RNB = 32;                                        // reflectors per block of the compact WY form
-    if (l2 >= 64 && n > 2 * RNB) {
+    // (per block: a panel kernel, a Gram, one host round trip for T, three GEMMs -- n / 32 of them; below ~256 vectors the
+    //  one-CTA-per-column kernel, whose cost grows with the number of columns, is faster: 0.15 vs 0.28 s at n = 16384, nev = 100)
+    if (l2 >= 512 && n > 2 * RNB) {
         // Blocked: H_j0 ... H_j0+nb-1 = I - V T V^T (forward, columnwise: T upper triangular, T_ii = tau_i,
         // T[0:i, i] = -tau_i T[0:i, 0:i] (V^T V)[0:i, i]); on the transposed block ZT = Z^T (2 nev x n) the update is three
         // row-rich real GEMMs on the tensor cores:  ZT[:, rows] -= ((ZT[:, rows] V) T^T) V^T.
