@@ -356,6 +356,9 @@ bse_status_t bse_solve_direct(bse_handle_t h, int32_t nev, double *hOmega, void 
 /* Real symmetric tridiagonal eigenproblem on the host (hD: m diagonal, hE: m - 1 sub-diagonal entries; both untouched): all
  * eigenvalues ascending in hW, eigenvectors of the nz lowest in hZ (m x nz, ldz).  The last stage of bse_solve_direct. */
 bse_status_t bse_host_stev(int32_t m, const double *hD, const double *hE, double *hW, double *hZ, int32_t ldz, int32_t nz);
+/* The nz lowest eigenpairs only (hW: nz values, hZ nullable): a small part of the spectrum (8 nz <= m) is found by bisection on
+ * the Sturm count plus inverse iteration, O(m nz), without the O(m^2) sweep over the whole matrix; otherwise as bse_host_stev. */
+bse_status_t bse_host_stev_lowest(int32_t m, const double *hD, const double *hE, int32_t nz, double *hW, double *hZ, int32_t ldz);
 
 /* The eigenvectors that "can be obtained trivially" from the right eigenvectors v_I = [X_I; Y_I] of the positive omega_I that
  * bse_solve returns (full mode, dVec / dOut 2N x nev column-major, must not alias):

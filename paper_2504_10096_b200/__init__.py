@@ -78,6 +78,7 @@ _SIGNATURES = {
     "bse_solve_direct": [_vp, _i32, ctypes.POINTER(_dbl), _vp, _i64, ctypes.POINTER(_dbl)],
     "bse_set_row_partition": [_vp, _i64, _i64],
     "bse_host_stev": [_i32, _vp, _vp, _vp, _vp, _i32, _i32],
+    "bse_host_stev_lowest": [_i32, _vp, _vp, _i32, _vp, _vp, _i32],
 }
 EXPORTS = sorted(list(_SIGNATURES) + ["bse_status_string", "bse_launch_count"])
 
@@ -522,6 +523,18 @@ def host_stev(d, e, nz=None):
     _check(lib().bse_host_stev(m, d.ctypes.data, e.ctypes.data if m > 1 else None, w.ctypes.data, Z.ctypes.data, m, nz),
            "bse_host_stev")
     return w, Z[:, :nz]
+
+
+def host_stev_lowest(d, e, nz, vectors: bool = True):
+    """Host utility: the nz lowest eigenvalues (and eigenvectors) of the real symmetric tridiagonal (d, e)."""
+    import numpy as np
+    m = len(d)
+    d = np.ascontiguousarray(d, dtype=np.float64); e = np.ascontiguousarray(e, dtype=np.float64)
+    w = np.zeros(nz)
+    Z = np.zeros((m, nz), dtype=np.float64, order="F") if vectors else None
+    _check(lib().bse_host_stev_lowest(m, d.ctypes.data, e.ctypes.data if m > 1 else None, nz, w.ctypes.data,
+                                      Z.ctypes.data if vectors else None, m), "bse_host_stev_lowest")
+    return w, Z
 
 
 def quadrature_resolvent(alpha, beta, omega, eta: float):

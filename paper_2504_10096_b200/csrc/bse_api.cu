@@ -127,6 +127,12 @@ bse_status_t bse_host_stev(int32_t m, const double *hD, const double *hE, double
     return host_stev(m, const_cast<double *>(hD), const_cast<double *>(hE), hW, hZ, ldz, nz) ? BSE_ERR_INTERNAL : BSE_OK;
 }
 
+bse_status_t bse_host_stev_lowest(int32_t m, const double *hD, const double *hE, int32_t nz, double *hW, double *hZ, int32_t ldz)
+{
+    if (m < 1 || !hD || (m > 1 && !hE) || !hW || nz < 1 || nz > m || (hZ && ldz < m)) return BSE_ERR_INVALID_ARG;
+    return host_stev_lowest(m, const_cast<double *>(hD), const_cast<double *>(hE), nz, hW, hZ, ldz) ? BSE_ERR_INTERNAL : BSE_OK;
+}
+
 static inline bool storage_ok(int32_t storage) { return storage == BSE_STORE_C128 || storage == BSE_STORE_C64; }
 static inline bool storage_real_form(int32_t storage) { return storage == BSE_STORE_REAL_FORM || storage == BSE_STORE_REAL_FORM_C64; }
 static inline int storage_es(int32_t storage)

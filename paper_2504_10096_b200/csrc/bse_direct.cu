@@ -311,6 +311,28 @@ __global__ void __launch_bounds__(1024) reflect_back_kernel(const double *W, int
     }
 }
 
+// z_T = D s for every wanted eigenvector, D = diag((-i)^j): from the even half s_E (SE, N x nev) of the unit eigenvector of the
+// zero-diagonal tridiagonal S = tridiag(b, 0, b), its odd half s_O = B s_E / omega (B upper bidiagonal: B[o][o] = b_{2o},
+// B[o][o+1] = b_{2o+1}), both scaled by 1/sqrt 2:  Z = [Re | Im] (n x 2 nev, ld n): Re z_{2o} = (-1)^o s_E[o], Im z_{2o+1} = -(-1)^o s_O[o]
+__global__ void __launch_bounds__(256) build_z_kernel(const double *SE, const double *b, const double *omega, int64_t N, int nev,
+                                                      double *Z)
+{
+    const int64_t o = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const int c = blockIdx.y;
+    if (o >= N) return;
+    const int64_t n = 2 * N;
+    const double *se = SE + (int64_t)c * N;
+    const double r2 = 0.70710678118654752440;
+    const double even = se[o] * r2;
+    const double odd = (b[2 * o] * se[o] + (o + 1 < N ? b[2 * o + 1] * se[o + 1] : 0.0)) / omega[c] * r2;
+    const double sg = (o & 1) ? -1.0 : 1.0;
+    double *zr = Z + (int64_t)c * n, *zi = Z + (int64_t)(nev + c) * n;
+    zr[2 * o] = sg * even;
+    zr[2 * o + 1] = 0.0;
+    zi[2 * o] = 0.0;
+    zi[2 * o + 1] = -sg * odd;
+}
+
 // Reflector panel of the blocked back-transformation: Vp (m x nb, ld m) = the reflectors j0 .. j0 + nbk - 1 restricted to rows
 // j0 .. n - 1 (m = n - j0, even; row 0 is zero, column c starts at row c + 1; columns >= nbk are zero), and VpT (nb x m, ld nb)
 // its transpose.
@@ -480,13 +502,13 @@ extern "C" bse_status_t bse_solve_direct(bse_handle_t h, int32_t nev, double *hO
     // ---- 5. S = tridiag(b, 0, b) (n x n) = perfect shuffle of [[0, B^T], [B, 0]], B upper bidiagonal N x N with
     //         B[o][o] = b_{2o}, B[o][o+1] = b_{2o+1}:  B^T B s_E = omega^2 s_E,  s_O = B s_E / omega
     t1 = now_s();
-    std::vector<double> dE(N), eE(N, 0.0), w2(N), ZE((size_t)N * nev);
+    std::vector<double> dE(N), eE(N, 0.0), w2(nev), ZE(dVec ? (size_t)N * nev : 0);
     for (int64_t e = 0; e < N; ++e) {
         const double bd = hb[2 * e], bu = e > 0 ? hb[2 * e - 1] : 0.0;
         dE[e] = bd * bd + bu * bu;
         if (e + 1 < N) eE[e] = hb[2 * e] * hb[2 * e + 1];
     }
-    if (host_stev((int)N, dE.data(), eE.data(), w2.data(), ZE.data(), (int)N, nev)) return BSE_ERR_INTERNAL;
+    if (host_stev_lowest((int)N, dE.data(), eE.data(), nev, w2.data(), dVec ? ZE.data() : nullptr, (int)N)) return BSE_ERR_INTERNAL;
     for (int c = 0; c < nev; ++c) {
         if (!(w2[c] > 0.0)) return BSE_ERR_NOT_POSITIVE_DEFINITE;
         hOmega[c] = std::sqrt(w2[c]);
@@ -512,26 +534,16 @@ extern "C" bse_status_t bse_solve_direct(bse_handle_t h, int32_t nev, double *hO
     const int l2 = 2 * nev;
     if ((st = Z.alloc((size_t)n * l2 * sizeof(double))) || (st = Ytmp.alloc((size_t)DNB * l2 * sizeof(double)))) return st;
     {
-        std::vector<double> hz((size_t)n * l2, 0.0);
-        const double r2 = std::sqrt(0.5);
-#pragma omp parallel for schedule(static)
-        for (int c = 0; c < nev; ++c) {
-            const double *se = &ZE[(size_t)c * N];
-            double *zr = &hz[(size_t)c * n], *zi = &hz[(size_t)(nev + c) * n];
-            const double om = hOmega[c];
-            for (int64_t o = 0; o < N; ++o) {
-                const double even = se[o] * r2;
-                const double odd = (hb[2 * o] * se[o] + (o + 1 < N ? hb[2 * o + 1] * se[o + 1] : 0.0)) / om * r2;
-                // (-i)^j: j = 2o -> (-1)^o;  j = 2o + 1 -> -i (-1)^o
-                const double sg = (o & 1) ? -1.0 : 1.0;
-                zr[2 * o] = sg * even;
-                zi[2 * o + 1] = -sg * odd;
-            }
-        }
-        lap("host Z");
-        BSE_CUDA(cudaMemcpyAsync(Z.d(), hz.data(), hz.size() * 8, cudaMemcpyHostToDevice, s));
-        BSE_CUDA(cudaStreamSynchronize(s));
-        lap("upload Z");
+        // s_E, omega to the device (the sub-diagonal b is still there): the start vectors are formed by a kernel
+        DevBuf SE, omd;
+        if ((st = SE.alloc((size_t)N * nev * 8)) || (st = omd.alloc((size_t)nev * 8))) return st;
+        BSE_CUDA(cudaMemcpyAsync(SE.d(), ZE.data(), (size_t)N * nev * 8, cudaMemcpyHostToDevice, s));
+        BSE_CUDA(cudaMemcpyAsync(omd.d(), hOmega, (size_t)nev * 8, cudaMemcpyHostToDevice, s));
+        build_z_kernel<<<dim3((unsigned)((N + 255) / 256), nev), 256, 0, s>>>(SE.d(), beta, omd.d(), N, nev, Z.d());
+        count_launch();
+        BSE_CUDA(cudaGetLastError());
+        BSE_CUDA(cudaStreamSynchronize(s));                        // SE, omd are freed here
+        lap("start vectors");
     }
     constexpr int RNB = 32;                                        // reflectors per block of the compact WY form
     // (per block: a panel kernel, a Gram, one host round trip for T, three GEMMs -- n / 32 of them; below ~256 vectors the

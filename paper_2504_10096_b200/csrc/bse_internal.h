@@ -140,5 +140,7 @@ int host_heev(int m, void *A, int lda, double *w, void *Z, int ldz, int nz);
 int host_syev(int m, double *A, int lda, double *w, double *Z, int ldz, int nz);
 // real symmetric tridiagonal (d, e): all eigenvalues ascending, eigenvectors of the nz lowest
 int host_stev(int m, double *d, double *e, double *w, double *Z, int ldz, int nz);
+// the nz lowest eigenpairs only (w: nz values; Z nullable): bisection + inverse iteration when nz is a small part of m
+int host_stev_lowest(int m, double *d, double *e, int nz, double *w, double *Z, int ldz);
 
 }  // namespace bse

@@ -575,4 +575,61 @@ int host_stev(int m, double *d_in, double *e_in, double *w, double *Z, int ldz, 
     return 0;
 }
 
+// The nz lowest eigenvalues of the real symmetric tridiagonal (d, e) by bisection on the Sturm count (number of negative
+// pivots of the LDL^T factorisation of T - x I), each to the last bit the count can resolve (absolute accuracy ~ eps ||T||, as
+// QL); O(m) per count, ~60 counts per eigenvalue, eigenvalues in parallel.
+static void tridiag_bisect_lowest(int m, const double *d, const double *e, int nz, double *w)
+{
+    const double eps = 2.220446049250313e-16;
+    double lo0 = d[0], hi0 = d[0], tnorm = 0.0;
+    for (int i = 0; i < m; ++i) {
+        const double r = (i > 0 ? std::fabs(e[i - 1]) : 0.0) + (i + 1 < m ? std::fabs(e[i]) : 0.0);
+        lo0 = std::min(lo0, d[i] - r);
+        hi0 = std::max(hi0, d[i] + r);
+        tnorm = std::max(tnorm, std::fabs(d[i]) + r);
+    }
+    const double pivmin = std::max(eps * tnorm * eps, 1e-300);
+    auto count_below = [&](double x) {                      // number of eigenvalues < x
+        int c = 0;
+        double q = d[0] - x;
+        if (std::fabs(q) < pivmin) q = -pivmin;
+        if (q < 0.0) ++c;
+        for (int i = 1; i < m; ++i) {
+            q = d[i] - x - e[i - 1] * e[i - 1] / q;
+            if (std::fabs(q) < pivmin) q = -pivmin;
+            if (q < 0.0) ++c;
+        }
+        return c;
+    };
+    lo0 -= 2.0 * eps * tnorm + pivmin;
+    hi0 += 2.0 * eps * tnorm + pivmin;
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int i = 0; i < nz; ++i) {
+        double lo = lo0, hi = hi0;                          // invariant: count(lo) <= i < count(hi)
+        for (int it = 0; it < 200; ++it) {
+            const double mid = 0.5 * (lo + hi);
+            if (!(mid > lo && mid < hi)) break;            // adjacent doubles
+            if (count_below(mid) <= i) lo = mid; else hi = mid;
+            if (hi - lo <= 2.0 * eps * std::max(std::fabs(lo), std::fabs(hi))) break;
+        }
+        w[i] = 0.5 * (lo + hi);
+    }
+}
+
+// The nz lowest eigenpairs only (w: nz values).  A small part of the spectrum (8 nz <= m): bisection + inverse iteration, no
+// O(m^2) sweep over the whole matrix; otherwise host_stev.
+int host_stev_lowest(int m, double *d, double *e, int nz, double *w, double *Z, int ldz)
+{
+    if (m <= 0 || nz <= 0) return 0;
+    if (nz > m) nz = m;
+    if (m > 64 && 8 * nz <= m) {
+        tridiag_bisect_lowest(m, d, e, nz, w);
+        if (!Z || tridiag_inverse_iteration(m, d, e, w, nz, Z, ldz) == 0) return 0;
+    }
+    std::vector<double> wall(m);
+    const int fail = host_stev(m, d, e, wall.data(), Z, ldz, Z ? nz : 0);
+    for (int i = 0; i < nz; ++i) w[i] = wall[i];
+    return fail;
+}
+
 }  // namespace bse

@@ -167,3 +167,26 @@ def test_host_stev_clusters():
     assert np.max(np.abs(w - w_ref)) <= 1e-13 * np.max(np.abs(w_ref))
     assert np.linalg.norm(T @ Z - Z * w[:nz]) <= 1e-11 * np.linalg.norm(T)
     assert np.linalg.norm(Z.T @ Z - np.eye(nz)) <= 1e-10
+
+
+def test_host_stev_lowest_bisection_vs_scipy():
+    """A few lowest eigenpairs by bisection + inverse iteration (8 nz <= m), and the fall-through to the full solver."""
+    import paper_2504_10096_b200 as b
+    from scipy.linalg import eigh_tridiagonal
+    rng = np.random.default_rng(9)
+    for m, nz in [(1000, 25), (1000, 125), (300, 100), (65, 8), (2048, 1)]:
+        d = rng.uniform(0.3, 150.0, m)
+        e = rng.standard_normal(m - 1) * 2
+        wr = eigh_tridiagonal(d, e, eigvals_only=True)
+        w, Z = b.host_stev_lowest(d, e, nz)
+        assert np.max(np.abs(w - wr[:nz])) <= 2e-14 * np.max(np.abs(wr))
+        T = np.diag(d) + np.diag(e, 1) + np.diag(e, -1)
+        assert np.linalg.norm(T @ Z - Z * w) <= 1e-11 * np.linalg.norm(T)
+        assert np.linalg.norm(Z.T @ Z - np.eye(nz)) <= 1e-10
+        w2, none = b.host_stev_lowest(d, e, nz, vectors=False)
+        assert none is None and np.array_equal(w2, w) or np.max(np.abs(w2 - w)) <= 2e-14 * np.max(np.abs(wr))
+    # a zero-diagonal matrix (pairs +-sigma): the lowest are the most negative
+    e = rng.standard_normal(511)
+    w, _ = b.host_stev_lowest(np.zeros(512), e, 10, vectors=False)
+    wr = eigh_tridiagonal(np.zeros(512), e, eigvals_only=True)
+    assert np.max(np.abs(w - wr[:10])) <= 2e-14 * np.max(np.abs(wr))
