@@ -390,7 +390,20 @@ def run_cuda(args, cfg):
         line["lanczos_time_to_nev_config3"] = {
             "workload": f"config 3: full N={N3} nev={c3['nev']} k=8 tol=1e-8, real-form store", "seconds": time.perf_counter() - t0,
             "status": res.status, "info": res.info}
-        del h3
+        del h3, r3, c3t
+        torch.cuda.empty_cache()
+        # the paper's direct route (section 2.1) on the device at config 1's size: every positive eigenpair of the 4096 x 4096 operator
+        c1 = gen.CONFIGS[1]
+        h1 = b.Bse(b.MODE_FULL, c1["N"], b.bse_fill_synthetic(c1["N"], b.MATRIX_R, 1, c1["sigma"], c1["group"]),
+                   b.bse_fill_synthetic(c1["N"], b.MATRIX_C, 1, 0.0, c1["group"]))
+        h1.solve_direct(4, vectors=False)                       # warm-up
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        om1, _, sec1 = h1.solve_direct(c1["N"])
+        torch.cuda.synchronize()
+        line["direct_route_config1"] = {"workload": f"config 1 operator: full N={c1['N']}, all {c1['N']} positive eigenpairs (bse_solve_direct)",
+                                        "seconds": time.perf_counter() - t0, "stage_seconds": sec1, "omega_first": float(om1[0])}
+        del h1
 
     # ---- CPU baseline: the oracle on this box's host cores, bounded sample
     if not args.no_cpu_baseline:
