@@ -392,10 +392,10 @@ namespace {
 // C (nr x l, ldc) = alpha A (nr x K, lda) B (K x l, ldb) + beta C, all real column-major; nr, lda, ldc even, A and C
 // 16-byte aligned (every caller passes multiples of the 64-row block)
 bse_status_t rgemm(bse_handle_s *h, int64_t nr, int l, int K, double alpha, const double *A, int64_t lda, const double *B,
-                   int64_t ldb, double beta, double *C, int64_t ldc)
+                   int64_t ldb, double beta, double *C, int64_t ldc, bool a_upper = false, bool c_lower = false)
 {
     if (nr <= 0 || l <= 0 || K <= 0) return BSE_OK;
-    return gemm_basis(h, A, lda / 2, K, false, B, ldb, l, nr / 2, C, ldc / 2, alpha, beta);
+    return gemm_basis(h, A, lda / 2, K, false, B, ldb, l, nr / 2, C, ldc / 2, alpha, beta, a_upper, c_lower);
 }
 
 struct DevBuf {
@@ -462,8 +462,8 @@ extern "C" bse_status_t bse_solve_direct(bse_handle_t h, int32_t nev, double *hO
         BSE_CUDA(cudaMemcpy2DAsync(A21, (size_t)n * 8, panel.d(), (size_t)n * 8, (size_t)rows * 8, DNB, cudaMemcpyDeviceToDevice, s));
         transpose_kernel<<<dim3((unsigned)((rows + 31) / 32), DNB / 32), 256, 0, s>>>(panel.d(), n, rows, DNB, panelT.d(), DNB, 0);
         count_launch();
-        // A22 -= L21 L21^T (the whole square: the upper half is never used)
-        if ((st = rgemm(h, rows, (int)rows, DNB, -1.0, panel.d(), n, panelT.d(), DNB, 1.0, A22, n))) return st;
+        // A22 -= L21 L21^T (tiles on and below the diagonal: the upper triangle is never used)
+        if ((st = rgemm(h, rows, (int)rows, DNB, -1.0, panel.d(), n, panelT.d(), DNB, 1.0, A22, n, false, true))) return st;
     }
     BSE_CUDA(cudaGetLastError());
     int hflag = 0;
@@ -477,7 +477,7 @@ extern "C" bse_status_t bse_solve_direct(bse_handle_t h, int32_t nev, double *hO
     transpose_kernel<<<dim3((unsigned)((n + 31) / 32), (unsigned)((n + 31) / 32)), 256, 0, s>>>(A.d(), n, n, n, U.d(), n, 1);
     jl_kernel<<<dim3((unsigned)((n + 255) / 256), (unsigned)n), 256, 0, s>>>(A.d(), n, N, JL.d());
     count_launch(2);
-    if ((st = rgemm(h, n, (int)n, (int)n, 1.0, U.d(), n, JL.d(), n, 0.0, A.d(), n))) return st;
+    if ((st = rgemm(h, n, (int)n, (int)n, 1.0, U.d(), n, JL.d(), n, 0.0, A.d(), n, true))) return st;      // U upper triangular
     BSE_CUDA(cudaStreamSynchronize(s));
     t_w = now_s() - t1;
 

@@ -100,8 +100,11 @@ bse_status_t apply_vec(bse_handle_s *h, int sign, const void *dX, int64_t ldx, v
 bse_status_t gram_basis(bse_handle_s *h, const void *A, int64_t lda, int m, const void *B, int64_t ldb, int k,
                         bool cplx, int64_t n, double *out);
 // C(n x l) = alpha * A(n x m) * S + beta * C,  S given as coefficient matrix `coef` (layout above, ld = ldo).
+// a_upper: A~ (real view) is upper triangular, A~[row, col] = 0 for col < row: the zero part of the contraction is skipped;
+// c_lower: only the lower triangle of the (square) C~ is wanted: tiles above the diagonal are left alone
 bse_status_t gemm_basis(bse_handle_s *h, const void *A, int64_t lda, int m, bool cplx, const double *coef,
-                        int64_t ldo, int l, int64_t n, void *C, int64_t ldc, double alpha, double beta);
+                        int64_t ldo, int l, int64_t n, void *C, int64_t ldc, double alpha, double beta, bool a_upper = false,
+                        bool c_lower = false);
 bse_status_t fill_random_block(bse_handle_s *h, void *W, int64_t ldw, int64_t n, int k, uint64_t seed,
                                uint64_t counter);
 bse_status_t copy_block(bse_handle_s *h, const void *src, int64_t lds, void *dst, int64_t ldd, int64_t n, int k);

@@ -78,10 +78,11 @@ static bse_status_t launch_gemm(bse_handle_s *h, const double *A, int64_t lda2, 
     return BSE_OK;
 }
 
-bse_status_t gemm_basis(bse_handle_s *h, const void *A, int64_t lda, int m, bool cplx, const double *coef, int64_t ldo,
-                        int l, int64_t n, void *C, int64_t ldc, double alpha, double beta)
+bse_status_t gemm_basis(bse_handle_s *h, const void *A, int64_t lda, int m, bool cplx_, const double *coef, int64_t ldo,
+                        int l, int64_t n, void *C, int64_t ldc, double alpha, double beta, bool a_upper, bool c_lower)
 {
     if (l <= 0) return BSE_OK;
+    const int cplx = (cplx_ ? 1 : 0) | (a_upper ? 2 : 0) | (c_lower ? 4 : 0);          // kernel flags
     if (l <= 8)
         return launch_gemm<4, 1, 8, 1>(h, (const double *)A, 2 * lda, 2 * n, m, cplx, coef, ldo, l, (double *)C,
                                        2 * ldc, alpha, beta);

@@ -24,7 +24,7 @@ struct GemmCfg {
 
 template <int MT, int NT, int WM, int WN>
 __global__ void __launch_bounds__(32 * WM * WN) gemm_nn_kernel(const double *__restrict__ A, int64_t lda2, int64_t nr,
-                                                               int m, int cplx, const double *__restrict__ Bm,
+                                                               int m, int flags, const double *__restrict__ Bm,
                                                                int64_t ldb, int l, double *__restrict__ C,
                                                                int64_t ldc2, double alpha, double beta)
 {
@@ -39,8 +39,15 @@ __global__ void __launch_bounds__(32 * WM * WN) gemm_nn_kernel(const double *__r
     const int wm = warp % WM, wn = warp / WM;
     const int64_t row0 = (int64_t)blockIdx.x * BM;
     const int col0 = blockIdx.y * BN;
+    // flags & 4: only the lower triangle of a square C is wanted (the trailing update of the Cholesky factorisation): tiles
+    // entirely above the diagonal do nothing
+    if ((flags & 4) && (int64_t)col0 >= row0 + BM) return;
     const int nch = (m + KC - 1) / KC;
     const int total = nch;                              // every chunk of A is loaded ONCE and used with Re(S) and with Im(S)
+    // flags & 2: A is upper triangular (A[row, kk] = 0 for kk < row, the L^T of the direct route): the chunks left of this
+    // row tile's diagonal are skipped
+    const int c_begin = (flags & 2) ? (int)min((int64_t)nch, row0 / KC) : 0;
+    const int cplx = flags & 1;
     const int nhalf = cplx ? 2 : 1;
 
     auto load_chunk = [&](int c, int buf) {
@@ -73,12 +80,12 @@ __global__ void __launch_bounds__(32 * WM * WN) gemm_nn_kernel(const double *__r
 
 #pragma unroll
     for (int c = 0; c < NS - 1; ++c) {
-        if (c < total) load_chunk(c, c);
+        if (c_begin + c < total) load_chunk(c_begin + c, c);
         cp_async_commit();
     }
-    for (int c = 0; c < total; ++c) {
-        const int buf = c % NS;
-        if (c + NS - 1 < total) load_chunk(c + NS - 1, (c + NS - 1) % NS);
+    for (int c = c_begin; c < total; ++c) {
+        const int buf = (c - c_begin) % NS;
+        if (c + NS - 1 < total) load_chunk(c + NS - 1, (c - c_begin + NS - 1) % NS);
         cp_async_commit();
         cp_async_wait<NS - 1>();
         __syncthreads();
