@@ -82,13 +82,13 @@ __global__ void __launch_bounds__(256) build_mr_real_form_kernel(const char *S, 
 // row r.  Writes L (lower; the strict upper part is zeroed) back and inv(L)^T, column-major 64 x 64, to invT (the B operand
 // of the panel GEMM A21 inv(L)^T and, as inv(L^T), of the triangular solve).  A pivot <= 0 sets *flag (PAPER.md:49:
 // "If M is positive definite ... we can perform a Cholesky decomposition").
-__global__ void __launch_bounds__(DNB) potrf_diag_kernel(double *A, int64_t lda, double *invT, int *flag)
+__global__ void __launch_bounds__(DNB) potrf_diag_kernel(double *A, int64_t lda, int nb, double *invT, int *flag)
 {
     __shared__ double a[DNB][DNB + 1];
-    const int r = threadIdx.x;
-    for (int c = 0; c < DNB; ++c) a[r][c] = A[r + c * lda];
+    const int r = threadIdx.x;                                  // nb <= DNB rows are active (the last block of a ragged n)
+    for (int c = 0; c < DNB; ++c) a[r][c] = (r < nb && c < nb) ? A[r + c * lda] : (r == c ? 1.0 : 0.0);
     __syncthreads();
-    for (int j = 0; j < DNB; ++j) {
+    for (int j = 0; j < nb; ++j) {
         const double d = a[j][j];
         if (!(d > 0.0)) {
             if (r == 0) *flag = 1;
@@ -104,7 +104,7 @@ __global__ void __launch_bounds__(DNB) potrf_diag_kernel(double *A, int64_t lda,
         __syncthreads();
     }
     // thread r: column r of X = inv(L) by forward substitution L x = e_r; X[i][r] lives at invT[r + i * DNB], which is
-    // entry (r, i) of (inv L)^T in column-major order (written and read back by this thread only)
+    // entry (r, i) of (inv L)^T in column-major order (written and read back by this thread only); identity beyond nb
     for (int i = 0; i < DNB; ++i) {
         double v = 0.0;
         if (i >= r) {
@@ -114,7 +114,8 @@ __global__ void __launch_bounds__(DNB) potrf_diag_kernel(double *A, int64_t lda,
         }
         invT[r + i * DNB] = v;
     }
-    for (int c = 0; c < DNB; ++c) A[r + c * lda] = (c <= r) ? a[r][c] : 0.0;
+    if (r < nb)
+        for (int c = 0; c < nb; ++c) A[r + c * lda] = (c <= r) ? a[r][c] : 0.0;
 }
 
 // dst (cols x rows, ldd) = src (rows x cols, lds)^T, with `lower_only`: entries of src above its diagonal read as zero
@@ -428,7 +429,7 @@ extern "C" bse_status_t bse_solve_direct(bse_handle_t h, int32_t nev, double *hO
     DevBuf A, U, JL, invT, panel, panelT, small;
     const size_t nn = (size_t)n * n * sizeof(double);
     if ((st = A.alloc(nn)) || (st = U.alloc(nn)) || (st = JL.alloc(nn)) ||
-        (st = invT.alloc((size_t)(n / DNB) * DNB * DNB * sizeof(double))) || (st = panel.alloc((size_t)n * DNB * sizeof(double))) ||
+        (st = invT.alloc((size_t)((n + DNB - 1) / DNB) * DNB * DNB * sizeof(double))) || (st = panel.alloc((size_t)n * DNB * sizeof(double))) ||
         (st = panelT.alloc((size_t)n * DNB * sizeof(double))) || (st = small.alloc((size_t)(6 * n + 64) * sizeof(double))))
         return st;
     double *tau = small.d(), *beta = tau + n, *vbuf = beta + n, *pbuf = vbuf + 2 * n;      // v, p: two buffers each
@@ -449,11 +450,13 @@ extern "C" bse_status_t bse_solve_direct(bse_handle_t h, int32_t nev, double *hO
         BSE_CUDA(cudaGetLastError());
     }
     // ---- 2. blocked Cholesky, lower: A <- L (the strict upper triangle keeps entries of M_r; never read as L)
-    const int nblk = (int)(n / DNB);
+    const int nblk = (int)((n + DNB - 1) / DNB);                  // the last block of a ragged n is shorter (n is even, so is it)
     for (int b = 0; b < nblk; ++b) {
-        const int64_t k0 = (int64_t)b * DNB, rows = n - k0 - DNB;
+        const int64_t k0 = (int64_t)b * DNB;
+        const int nb = (int)std::min<int64_t>(DNB, n - k0);
+        const int64_t rows = n - k0 - nb;
         double *Akk = A.d() + k0 + k0 * n, *inv_b = invT.d() + (size_t)b * DNB * DNB;
-        potrf_diag_kernel<<<1, DNB, 0, s>>>(Akk, n, inv_b, flag);
+        potrf_diag_kernel<<<1, DNB, 0, s>>>(Akk, n, nb, inv_b, flag);
         count_launch();
         if (rows <= 0) break;
         double *A21 = Akk + DNB, *A22 = Akk + DNB + DNB * n;
@@ -610,10 +613,11 @@ extern "C" bse_status_t bse_solve_direct(bse_handle_t h, int32_t nev, double *hO
     // L^T y = z: U y = z, blocked back substitution from the last block up
     for (int b = nblk - 1; b >= 0; --b) {
         const int64_t k0 = (int64_t)b * DNB;
-        const double *inv_b = invT.d() + (size_t)b * DNB * DNB;             // inv(L_bb)^T = inv(U_bb)
-        if ((st = rgemm(h, DNB, l2, DNB, 1.0, inv_b, DNB, Z.d() + k0, n, 0.0, Ytmp.d(), DNB))) return st;
-        BSE_CUDA(cudaMemcpy2DAsync(Z.d() + k0, (size_t)n * 8, Ytmp.d(), (size_t)DNB * 8, (size_t)DNB * 8, l2, cudaMemcpyDeviceToDevice, s));
-        if (k0 > 0 && (st = rgemm(h, k0, l2, DNB, -1.0, U.d() + k0 * n, n, Ytmp.d(), DNB, 1.0, Z.d(), n))) return st;
+        const int nb = (int)std::min<int64_t>(DNB, n - k0);
+        const double *inv_b = invT.d() + (size_t)b * DNB * DNB;             // inv(L_bb)^T = inv(U_bb) (identity beyond nb)
+        if ((st = rgemm(h, nb, l2, nb, 1.0, inv_b, DNB, Z.d() + k0, n, 0.0, Ytmp.d(), DNB))) return st;
+        BSE_CUDA(cudaMemcpy2DAsync(Z.d() + k0, (size_t)n * 8, Ytmp.d(), (size_t)DNB * 8, (size_t)nb * 8, l2, cudaMemcpyDeviceToDevice, s));
+        if (k0 > 0 && (st = rgemm(h, k0, l2, nb, -1.0, U.d() + k0 * n, n, Ytmp.d(), DNB, 1.0, Z.d(), n))) return st;
     }
     lap("triangular solve");
     double *sig = pbuf;

@@ -115,3 +115,40 @@ def test_config1_stored_oracle_values_and_iterative_solver(orc):
     _check_vectors(orc, R, C, om, to_host(vec), 12.0)
     it = h.solve(nev, cfg["k"], tol=1e-10, seed=1)
     assert np.max(np.abs(it.omega - om) / om) <= TOL_EIG
+
+
+@pytest.mark.parametrize("seed", range(14))
+def test_random_sizes_and_stores_vs_oracle_direct_route(orc, seed):
+    """Seeded sweep: N below one tile, ragged last tiles and last Cholesky blocks, every store; all eigenpairs against the
+    oracle's section-2.1 route on the operator the store defines."""
+    import paper_2504_10096_b200 as b
+    from gpu_util import to_dev
+    rng = np.random.default_rng(4000 + seed)
+    N = int(rng.choice([1, 2, 7, 31, 33, 63, 65, 100, 129, 200, 257]))
+    store = str(rng.choice(["c128", "c64", "real", "real64"]))
+    Np = N if N % 16 == 0 else N + 16 - N % 16
+    R = gen.dense_R(Np, 300 + seed, sigma=1.0)[:N, :N]
+    C = gen.dense_C(Np, 300 + seed)[:N, :N]
+    base = b.STORE_C64 if store in ("c64", "real64") else b.STORE_C128
+    rt = b.bse_pack_from_dense(to_dev(R), N, 0, storage=base)
+    ct = b.bse_pack_from_dense(to_dev(C), N, 1, storage=base)
+    if base == b.STORE_C64:
+        R, C = orc.round_c64(R), orc.round_c64(C)
+    storage = base
+    if store.startswith("real"):
+        b.bse_to_real_form(rt, ct, N, storage=base)
+        storage = b.STORE_REAL_FORM if base == b.STORE_C128 else b.STORE_REAL_FORM_C64
+        if base == b.STORE_C64:                                # the operator the rounded planes define (include/bse.h)
+            S32, D32 = orc.round_c64(R + C), orc.round_c64(R - C)
+            R, C = (S32 + D32) / 2, (S32 - D32) / 2
+    h = b.Bse(b.MODE_FULL, N, rt, ct, storage=storage)
+    om_o, _ = orc.bse_direct(R, C, want_vectors=False)
+    nev = N if seed % 3 else max(1, N // 5)
+    om, vec, _ = h.solve_direct(nev)
+    assert np.max(np.abs(om - om_o[N:N + nev]) / om_o[N:N + nev]) <= TOL_EIG, (N, store)
+    nrm = np.linalg.norm(np.block([[R, C], [-C.conj().T, -R.conj()]]), 2)
+    V = to_host(vec)
+    r = np.linalg.norm(orc.apply_full(R, C, V) - V * om, axis=0) / np.linalg.norm(V, axis=0)
+    assert np.all(r <= TOL_RES * nrm), (N, store, r.max())
+    Sig = np.concatenate([np.ones(N), -np.ones(N)])
+    assert np.max(np.abs(np.sum(Sig[:, None] * np.abs(V) ** 2, axis=0) - 1)) <= 1e-10
