@@ -312,3 +312,25 @@ def test_config0_other_matrix_seeds(orc, seed):
     _check_tda(orc, R, res, cfg["nev"], np.linalg.eigvalsh(R))
     w_o, _, _, steps = orc.lanczos_tda(R, cfg["nev"], 1e-10, gen.block_X(cfg["N"], 1, 90 + seed)[:, 0], check=20)
     assert steps > 0 and np.max(np.abs(res.omega - w_o) / np.abs(w_o)) <= TOL_EIG
+
+
+def test_tda_locking_returns_the_same_pairs(orc, monkeypatch):
+    """Converged leading Ritz pairs are locked at restarts (Rayleigh-Ritz on the active columns only): same eigenpairs as
+    without locking, ascending order, residuals through the oracle apply; many restarts (small basis) so that pairs are
+    locked long before the end."""
+    import paper_2504_10096_b200 as b
+    N, nev, k = 1024, 40, 4
+    R = gen.dense_R(N, 6, sigma=0.0)
+    h = b.Bse(b.MODE_TDA, N, pack(R, 0))
+    res = h.solve(nev, k, ncv=96, tol=1e-10, seed=5)
+    monkeypatch.setenv("BSE_SOLVE_LOCK", "0")
+    ref = h.solve(nev, k, ncv=96, tol=1e-10, seed=5)
+    monkeypatch.delenv("BSE_SOLVE_LOCK")
+    assert res.info["n_restart"] >= 5
+    w = np.linalg.eigvalsh(R)[:nev]
+    for r_ in (res, ref):
+        assert np.all(np.diff(r_.omega) > 0)
+        assert np.max(np.abs(r_.omega - w) / np.abs(w)) <= TOL_EIG
+    _check_tda(orc, R, res, nev, w)
+    assert abs(res.info["n_apply"] - ref.info["n_apply"]) <= max(8, ref.info["n_apply"] // 10)
+    assert res.info["seconds_project"] <= ref.info["seconds_project"] * 1.5 + 0.05
