@@ -260,7 +260,9 @@ bse_status_t bse_orth(bse_handle_t h, const void *dV, int64_t ldv, int32_t m, co
  *   k    : block size (>= 1; >= 2 recommended in full mode);  ncv: maximum basis
  *          size, 0 -> default max(2 nev, nev + 15) (doubled in full mode) and at least (wanted Ritz values) + 8 k,
  *          rounded up to a multiple of k;
- *   tol  : a Ritz pair is converged when ||H v - w v||_2 <= tol * ||H||_est * ||v||_2;
+ *   tol  : a Ritz pair is converged when ||H v - w v||_2 <= tol * ||H||_est * ||v||_2 (accepted at 0.9 of that: ||H||_est is a
+ *          lower bound of ||H||; reading S7).  TDA: converged leading pairs are locked at restarts (kept in the basis,
+ *          left out of the projected eigenproblem);
  *   hOmega: nev doubles (host);  hResid: nev doubles (host, nullable): the residual estimates;
  *   info : nullable.
  * Synchronous.  Errors: BSE_ERR_NOT_CONVERGED after max_restarts, BSE_ERR_NOT_POSITIVE_DEFINITE,
